@@ -1,0 +1,256 @@
+"""Pins for the oracle: each checks oracle/ against something other than
+itself -- the Kronecker-sum Hamiltonian, brute-force projection in the full Hilbert space, exact
+propagation e^{-iHt}, scipy's dense expm, conservation laws, and the paper's statements that
+TDVP-MU preserves the gauge (Eq. 34) and agrees with TDVP-PS."""
+import dataclasses
+
+import numpy as np
+import pytest
+import scipy.linalg
+
+import synthetic_inputs as si
+from oracle import contractions as oc
+from oracle import exact, lanczos, model, observables as obs, tdvp_mu, tdvp_ps
+
+
+def _small_params(layout="A", n_el=3, n_modes=1, n_ph=3, seed=11):
+    cfg = dataclasses.replace(si.CONFIGS["tiny"], model_seed=seed, n_el=n_el, n_modes=n_modes,
+                              n_ph=n_ph, nearest_neighbour=False, layout=layout)
+    return si.draw_vibronic_params(cfg)
+
+
+# ---------------------------------------------------------------- p1: MPO (Eq. 11, Eq. 45)
+@pytest.mark.parametrize("layout", ["A", "B"])
+def test_p1_mpo_equals_kronecker_sum(layout):
+    p = _small_params(layout, n_el=3, n_modes=2, n_ph=2)
+    H, dims = model.kronecker_sum_hamiltonian(p)
+    Hd = model.mpo_to_dense(model.build_mpo(p))
+    assert Hd.shape == H.shape
+    assert np.abs(Hd - H.toarray()).max() < 1e-15
+    assert np.abs(Hd - Hd.conj().T).max() == 0.0
+
+
+def test_p1_mpo_bond_dimensions(tiny_model):
+    cfg, params, mpo, dims, occ = tiny_model
+    assert [W.shape[3] for W in mpo] == [5, 5, 4, 4, 3, 3, 1]
+    assert [W.shape[1] for W in mpo] == dims == [3, 4, 4, 4, 4, 4, 4]
+
+
+def test_p1_layout_a_and_b_same_physics():
+    pa = _small_params("A")
+    pb = dataclasses.replace(pa, layout="B")
+    pops = []
+    for p in (pa, pb):
+        H, dims = model.kronecker_sum_hamiltonian(p)
+        occ = si.initial_occupations(p)
+        psi0 = np.zeros(int(np.prod(dims)), dtype=np.complex128)
+        psi0[np.ravel_multi_index(occ, dims)] = 1.0
+        psi = list(exact.propagate(H, psi0, 10.0, 5))[-1]
+        if p.layout == "A":
+            pops.append(exact.site_populations(psi, dims, 0))
+        else:
+            el = [m * (1 + p.n_modes) for m in range(p.n_el)]
+            pops.append(np.array([exact.site_populations(psi, dims, s)[1] for s in el]))
+    assert np.abs(pops[0] - pops[1]).max() < 1e-13
+    assert abs(pops[0].sum() - 1.0) < 1e-13
+
+
+# ---------------------------------------------------------------- p2: contractions (Eq. 29-32, 44)
+def _mixed_canonical(mps_right_canonical, centre):
+    out = [A.copy() for A in mps_right_canonical]
+    for i in range(centre):
+        Ml, d, Mr = out[i].shape
+        Q, D = np.linalg.qr(out[i].reshape(Ml * d, Mr))
+        out[i] = Q.reshape(Ml, d, -1)
+        out[i + 1] = np.einsum("ab,bsc->asc", D, out[i + 1])
+    return out
+
+
+def _left_basis(mps, centre):
+    P = np.ones((1, 1), dtype=np.complex128)                 # [sigma_left, a]
+    for A in mps[:centre]:
+        P = np.einsum("pa,asb->psb", P, A).reshape(-1, A.shape[2])
+    return P
+
+
+def _right_basis(mps, centre):
+    P = np.ones((1, 1), dtype=np.complex128)                 # [b, sigma_right]
+    for A in reversed(mps[centre + 1:]):
+        P = np.einsum("asb,bq->asq", A, P).reshape(A.shape[0], -1)
+    return P
+
+
+def test_p2_staged_equals_definition():
+    L, W, A, R = si.random_site_problem(5, 7, 3, 4, 6, 0.4, seed=3)
+    assert np.abs(oc.heff(L, W, A, R) - oc.heff_definition(L, W, A, R)).max() < 1e-12
+    assert np.abs(oc.envL(L, W, A) - oc.envL_definition(L, W, A)).max() < 1e-12
+    assert np.abs(oc.envR(R, W, A) - oc.envR_definition(R, W, A)).max() < 1e-12
+    D = si.complex_normal(np.random.default_rng(4), (5, 7))
+    L2, _, _, R2 = si.random_site_problem(5, 7, 3, 4, 4, 0.4, seed=5)
+    assert np.abs(oc.bond(L2, D, R2) - oc.bond_definition(L2, D, R2)).max() < 1e-12
+
+
+@pytest.mark.parametrize("centre", [0, 1, 2, 3])
+def test_p2_heff_is_projected_hamiltonian(centre):
+    """H_eff[i] = P^dagger H P with P = P[1:i-1] (x) I_i (x) P[i+1:N] (Eq. 29, 43), brute force."""
+    p = _small_params("A")
+    H, dims = model.kronecker_sum_hamiltonian(p)
+    H = H.toarray()
+    mpo = model.build_mpo(p)
+    mps = _mixed_canonical(si.random_right_canonical_mps(dims, 4, seed=2), centre)
+    Lenv = oc.boundary_env()
+    for i in range(centre):
+        Lenv = oc.envL(Lenv, mpo[i], mps[i])
+    Renv = oc.boundary_env()
+    for i in range(len(mps) - 1, centre, -1):
+        Renv = oc.envR(Renv, mpo[i], mps[i])
+    PL, PR = _left_basis(mps, centre), _right_basis(mps, centre)
+    d = dims[centre]
+    P = np.einsum("pa,su,bq->psqaub", PL, np.eye(d), PR).reshape(H.shape[0], -1)
+    assert np.abs(P.conj().T @ P - np.eye(P.shape[1])).max() < 1e-13      # Eq. 7, 8
+    C = mps[centre]
+    brute = (P.conj().T @ H @ P @ C.reshape(-1)).reshape(C.shape)
+    got = oc.heff(Lenv, mpo[centre], C, Renv)
+    assert np.abs(got - brute).max() < 1e-13
+    psi = obs.mps_to_vector(mps)
+    assert abs(np.vdot(C, got) - np.vdot(psi, H @ psi)) < 1e-13
+    assert abs(obs.energy(mpo, mps) - np.vdot(psi, H @ psi).real) < 1e-13
+    if centre < len(mps) - 1:
+        # bond operator K = P[1:i] (x) P[i+1:N] projected H (Eq. 44)
+        Ml, dd, Mr = C.shape
+        Q, D = np.linalg.qr(C.reshape(Ml * dd, Mr))
+        Lnext = oc.envL(Lenv, mpo[centre], Q.reshape(Ml, dd, -1))
+        PL2 = np.einsum("pa,asb->psb", PL, Q.reshape(Ml, dd, -1)).reshape(-1, Q.shape[1])
+        P2 = np.einsum("pa,bq->pqab", PL2, PR).reshape(H.shape[0], -1)
+        brute = (P2.conj().T @ H @ P2 @ D.reshape(-1)).reshape(D.shape)
+        assert np.abs(oc.bond(Lnext, D, Renv) - brute).max() < 1e-13
+
+
+# ---------------------------------------------------------------- p8: Lanczos vs dense expm
+@pytest.mark.parametrize("z", [-0.7j, +0.35j])
+def test_p8_lanczos_full_dimension_is_exact(z):
+    rng = np.random.default_rng(8)
+    n = 12
+    G = si.complex_normal(rng, (n, n))
+    Hm = (G + G.conj().T) / 2
+    v = si.complex_normal(rng, (3, 4))
+    y, m = lanczos.lanczos_expm(lambda x: (Hm @ x.reshape(-1)).reshape(x.shape), v, z, 40)
+    assert m == n                                            # Krylov space exhausted -> breakdown rule
+    ref = scipy.linalg.expm(z * Hm) @ v.reshape(-1)
+    assert np.abs(y.reshape(-1) - ref).max() < 1e-12
+
+
+def test_p8_lanczos_truncated_is_unitary_and_accurate():
+    rng = np.random.default_rng(9)
+    n = 60
+    G = si.complex_normal(rng, (n, n))
+    Hm = (G + G.conj().T) / 2 / np.sqrt(n)
+    v = si.complex_normal(rng, (n,))
+    y, m = lanczos.lanczos_expm(lambda x: Hm @ x, v, -0.5j, 10)
+    assert m == 10
+    assert abs(np.linalg.norm(y) - np.linalg.norm(v)) < 1e-13 * np.linalg.norm(v)   # T7
+    ref = scipy.linalg.expm(-0.5j * Hm) @ v
+    assert np.abs(y - ref).max() < 1e-9
+
+
+# ---------------------------------------------------------------- p3: TDVP-PS closed form
+def test_p3_ps_untruncated_equals_exact_propagation(tiny_model):
+    """With complete bonds every backward step cancels a forward step and Eq. 42 reduces to
+    e^{-iH tau} exactly, for ANY tau (derivation: SURVEY.md 8(c) 'Why p3 holds')."""
+    cfg, params, mpo, dims, occ = tiny_model
+    H, _ = model.kronecker_sum_hamiltonian(params)
+    mps = si.padded_product_mps(dims, occ, 64, cfg.pad_seed)
+    assert [A.shape[2] for A in mps] == [3, 12, 48, 64, 16, 4, 1]
+    st = tdvp_ps.PSState(mpo, mps)
+    ex = exact.propagate(H, obs.mps_to_vector(mps), 25.0, 3)
+    for _ in range(3):
+        tdvp_ps.step_ps(st, 25.0, 40)
+        psi = next(ex)
+    assert np.linalg.norm(obs.mps_to_vector(st.mps) - psi) < 2e-12
+    assert np.abs(obs.populations(st.mps) - exact.site_populations(psi, dims)).max() < 1e-12
+
+
+# ---------------------------------------------------------------- p4, p5, p9: config 1 as stated
+def test_p4_p5_p9_config1_vs_exact(tiny_model):
+    cfg, params, mpo, dims, occ = tiny_model
+    H, _ = model.kronecker_sum_hamiltonian(params)
+    mps = si.padded_product_mps(dims, occ, cfg.M, cfg.pad_seed)
+    for A in mps[1:]:                                         # Eq. 8
+        m = A.reshape(A.shape[0], -1)
+        assert np.abs(m @ m.conj().T - np.eye(A.shape[0])).max() < 1e-14
+    st = tdvp_ps.PSState(mpo, mps)
+    e0 = obs.energy(mpo, mps)
+    ex = exact.propagate(H, obs.mps_to_vector(mps), cfg.dt_fs, cfg.n_steps)
+    worst = 0.0
+    traj = []
+    for _ in range(cfg.n_steps):
+        tdvp_ps.step_ps(st, cfg.dt_fs, cfg.krylov_dim)
+        pops = obs.populations(st.mps)
+        traj.append(pops)
+        worst = max(worst, np.abs(pops - exact.site_populations(next(ex), dims)).max())
+        assert abs(pops.sum() - 1.0) < 1e-13                   # p9
+    assert worst < 1e-5                                        # p5 (truncation + k = 10)
+    assert abs(obs.norm_sq(st.mps) - 1.0) < 1e-13              # p4 / T7
+    assert abs(obs.energy(mpo, st.mps) - e0) < 1e-13 * max(1.0, abs(e0)) * 10
+    golden = np.loadtxt("tests/golden/tiny_ps_populations.txt")
+    assert np.abs(np.array(traj) - golden).max() < 1e-10       # regression of the stored values
+
+
+# ---------------------------------------------------------------- p6, p7, T4: TDVP-MU
+@pytest.fixture(scope="module")
+def warmed_up(tiny_model):
+    cfg, params, mpo, dims, occ = tiny_model
+    st = tdvp_ps.PSState(mpo, si.padded_product_mps(dims, occ, cfg.M, cfg.pad_seed))
+    for _ in range(3):
+        tdvp_ps.step_ps(st, 10.0, 30)
+    return mpo, [A.copy() for A in st.mps]
+
+
+def test_p7_mu_gauge_condition(warmed_up):
+    """Eq. 34: L^dagger dL/dt = 0."""
+    mpo, warm = warmed_up
+    lc = tdvp_mu.to_left_canonical(warm)
+    assert abs(abs(np.vdot(obs.mps_to_vector(lc), obs.mps_to_vector(warm))) - 1.0) < 1e-13   # T2
+    deriv = tdvp_mu.mu_derivative(mpo, lc)
+    for L, dL in zip(lc[:-1], deriv[:-1]):
+        assert np.abs(np.einsum("asb,asc->bc", L.conj(), dL)).max() < 1e-12
+
+
+def test_t4_unfolded_form_equals_overlap_inverse_form(tiny_model):
+    """Eq. 37 with eps -> 0 equals Eq. 28 written with S[i+1:N]^{-1}; checked on
+    a random full-rank state so that S is well conditioned."""
+    cfg, params, mpo, dims, occ = tiny_model
+    lc = tdvp_mu.to_left_canonical(si.random_right_canonical_mps(dims, 6, seed=13))
+    n = len(lc)
+    deriv = tdvp_mu.mu_derivative(mpo, lc, eps=1e-30)
+    Lenv = [oc.boundary_env()]
+    for i in range(n - 1):
+        Lenv.append(oc.envL(Lenv[i], mpo[i], lc[i]))
+    Renv = oc.boundary_env()                                  # built from the RAW (non-orthonormal) basis
+    S = np.ones((1, 1), dtype=np.complex128)                  # S[l', l] = <l'|l>, Eq. 5
+    checked = 0
+    for i in range(n - 1, 0, -1):
+        Renv = oc.envR(Renv, mpo[i], lc[i])
+        S = np.einsum("asb,xsy,by->ax", lc[i].conj(), lc[i], S)
+        assert np.linalg.cond(S) < 1e6
+        HL = oc.heff(Lenv[i - 1], mpo[i - 1], lc[i - 1], Renv)
+        G = np.einsum("asl,ml->asm", HL, np.linalg.inv(S))
+        a, s, l = G.shape
+        Lm, Gm = lc[i - 1].reshape(a * s, l), G.reshape(a * s, l)
+        direct = (-1j * (Gm - Lm @ (Lm.conj().T @ Gm))).reshape(a, s, l)
+        assert np.abs(direct - deriv[i - 1]).max() < 1e-9 * np.abs(G).max()
+        checked += np.abs(direct).max() > 1e-3 * np.abs(G).max()
+    assert checked >= 3                                       # not only trivially-zero derivatives
+
+
+def test_p6_mu_agrees_with_ps(warmed_up):
+    """both schemes give the same |Psi(t)> up to numerical error."""
+    mpo, warm = warmed_up
+    st = tdvp_ps.PSState(mpo, warm)
+    for _ in range(4):
+        tdvp_ps.step_ps(st, 1.25, 30)
+    y = tdvp_mu.to_left_canonical(warm)
+    for _ in range(20):
+        y, err = tdvp_mu.step_mu(mpo, y, 0.25)
+    assert np.abs(obs.populations(y) - obs.populations(st.mps)).max() < 1e-8
+    assert err < 1e-3
