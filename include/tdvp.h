@@ -1,0 +1,189 @@
+/*
+ * tdvp.h -- C ABI of libtdvp.so: the data-parallel hot path of TDVP time evolution of a matrix
+ * product state (MPS) under a matrix product operator (MPO), arXiv:1907.12044, written for one
+ * NVIDIA B200 (sm_100a).  Every operation below runs in hand-written CUDA kernels; there is no CPU
+ * fallback.  Citations are PAPER.md:<line> plus the equation / section the line falls in.
+ *
+ * Conventions (BASELINE.json north_star)
+ *   complex128 everywhere, interleaved (re, im), C-contiguous arrays (last index fastest):
+ *     L[a, w, x]   left  environment block h[1:i-1]  (Eq. 30-32), [Ml, Dl, Ml]
+ *     R[b, v, y]   right environment block h[i+1:N]                                , [Mr, Dr, Mr]
+ *                  first bond index = bra (conjugated) side, last = ket side
+ *     W[w, s, t, v] MPO site tensor (Eq. 11), [Dl, d, d, Dr], s = bra/output
+ *                  physical index, t = ket/input physical index
+ *     A[x, t, y]   MPS site tensor (Eq. 1), [Ml, d, Mr]
+ *   hbar = 1; dt is in the inverse of the MPO's energy unit (the caller converts units).
+ *
+ * Pointers: every argument says HOST or DEVICE.  The library copies what it keeps; the caller
+ * keeps ownership of everything it passes in.  One handle = one CUDA stream = not thread safe;
+ * several handles may coexist.  No call blocks on the stream unless it says so.
+ *
+ * Errors: every int-returning call returns TDVP_OK (0) or a negative TDVP_E* code and stores a
+ * message retrievable with tdvp_last_error(h) (h may be NULL: the last error of the calling
+ * thread's handle-less calls).  No exceptions or signals cross the boundary.
+ */
+#ifndef TDVP_H
+#define TDVP_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TDVP_OK        0
+#define TDVP_EINVAL   -1   /* bad shape, null pointer, non-canonical MPS, unsupported size        */
+#define TDVP_ENOMEM   -2   /* device or host allocation failed                                   */
+#define TDVP_ECUDA    -3   /* a CUDA call failed; tdvp_last_error has the CUDA error string      */
+#define TDVP_ESTATE   -4   /* call not valid in the handle's current gauge / state               */
+
+#define TDVP_MAX_KRYLOV 64
+
+typedef struct tdvp_handle tdvp_handle;            /* opaque; owns all device state             */
+typedef struct { double re, im; } tdvp_c128;       /* interleaved complex128                    */
+
+typedef struct {
+  int    krylov_dim;   /* k of the Lanczos exponential; default 10; <= 64     */
+  double krylov_tol;   /* reserved for the adaptive rule (paper gives no formula); must be 0     */
+  double mu_eps;       /* epsilon of Eq. 38; default 1e-10                    */
+  double w_zero_tol;   /* |W| <= tol is a structural zero of the MPO; default 0 (exact zeros)    */
+  int    flags;        /* TDVP_FLAG_* below                                                      */
+} tdvp_options;
+
+#define TDVP_FLAG_SKIP_CANONICAL_CHECK 1  /* tdvp_create / tdvp_set_mps do not verify Eq. 8      */
+#define TDVP_FLAG_NO_GRAPH             2  /* step drivers enqueue kernels directly (no CUDA graph)*/
+
+void tdvp_default_options(tdvp_options *opt);
+
+/* ---- handles ---------------------------------------------------------------------------- */
+
+/* A handle without a chain: stream + workspace for the stateless calls below.
+   cuda_stream: a cudaStream_t (NULL = the legacy default stream). */
+int tdvp_create_context(tdvp_handle **out, const tdvp_options *opt /*HOST, nullable*/,
+                        void *cuda_stream);
+
+/* tdvp_create(mpo, mps): the paper's problem statement -- an MPO H (Eq. 11 / Eq. 45) and an MPS
+   (Eq. 1) to be evolved.
+     n_sites            number of sites N
+     phys_dim[N]        HOST, d_i
+     mpo_bond[N+1]      HOST, MPO bond dimensions, mpo_bond[0] = mpo_bond[N] = 1
+     mpo[N]             HOST array of pointers; mpo[i] -> W_i[mpo_bond[i], d_i, d_i, mpo_bond[i+1]]
+     mps_bond[N+1]      HOST, MPS bond dimensions, mps_bond[0] = mps_bond[N] = 1, and every
+                        bond must satisfy M_i <= d_i * M_{i+1} and M_{i+1} <= M_i * d_i (so that
+                        each gauge move is a tall-or-square QR)
+     mps[N]             HOST array of pointers; mps[i] -> A_i[mps_bond[i], d_i, mps_bond[i+1]]
+     on_device          0: the tensors pointed to are in HOST memory; 1: in DEVICE memory
+   The MPS must be right-canonical (Eq. 8) on sites 1..N-1 with the gauge centre
+   at site 0; this is checked to 1e-10 (TDVP_EINVAL) unless TDVP_FLAG_SKIP_CANONICAL_CHECK.
+   All tensors are copied into device memory owned by the handle; all right environment blocks
+   h[i+1:N] (Eq. 31-32) are built and kept resident.  Blocks on the stream before returning. */
+int tdvp_create(tdvp_handle **out, int n_sites, const int *phys_dim,
+                const int *mpo_bond, const tdvp_c128 *const *mpo,
+                const int *mps_bond, const tdvp_c128 *const *mps,
+                int on_device, const tdvp_options *opt /*HOST, nullable*/, void *cuda_stream);
+int tdvp_destroy(tdvp_handle *h);
+
+/* ---- stateless contractions on caller-provided DEVICE buffers ---------------------------- */
+/* h may be NULL (legacy default stream, a library-owned workspace) or any handle (its stream
+   and workspace).  Buffers must not overlap.  Enqueue only.                                   */
+
+/* out[a,s,b] = sum_{w,x,t,v,y} L[a,w,x] W[w,s,t,v] A[x,t,y] R[b,v,y]
+   (H[i] applied to a site tensor: Eq. 29, used as in Eq. 43). */
+int tdvp_apply_heff(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr,
+                    const tdvp_c128 *L /*DEVICE [Ml,Dl,Ml]*/, const tdvp_c128 *W /*DEVICE [Dl,d,d,Dr]*/,
+                    const tdvp_c128 *A /*DEVICE [Ml,d,Mr]*/,  const tdvp_c128 *R /*DEVICE [Mr,Dr,Mr]*/,
+                    tdvp_c128 *out /*DEVICE [Ml,d,Mr]*/);
+
+/* Environment update (Eq. 30-32).
+   side = 0: env_in = L[Ml,Dl,Ml], env_out = L'[b,v,y] = sum conj(A[a,s,b]) L[a,w,x] W[w,s,t,v] A[x,t,y]   ([Mr,Dr,Mr])
+   side = 1: env_in = R[Mr,Dr,Mr], env_out = R'[a,w,x] = sum conj(A[a,s,b]) W[w,s,t,v] A[x,t,y] R[b,v,y]   ([Ml,Dl,Ml]) */
+int tdvp_update_env(tdvp_handle *h, int side, int Ml, int Mr, int d, int Dl, int Dr,
+                    const tdvp_c128 *env_in /*DEVICE*/, const tdvp_c128 *W /*DEVICE [Dl,d,d,Dr]*/,
+                    const tdvp_c128 *A /*DEVICE [Ml,d,Mr]*/, tdvp_c128 *env_out /*DEVICE*/);
+
+/* Bond (zero-site) operator of the backward step (Eq. 44):
+   out[a,b] = sum_{w,x,y} L[a,w,x] D[x,y] R[b,w,y];  L[Ml,Dw,Ml], R[Mr,Dw,Mr], D and out [Ml,Mr]. */
+int tdvp_apply_bond(tdvp_handle *h, int Ml, int Mr, int Dw,
+                    const tdvp_c128 *L /*DEVICE*/, const tdvp_c128 *D /*DEVICE*/,
+                    const tdvp_c128 *R /*DEVICE*/, tdvp_c128 *out /*DEVICE*/);
+
+/* y = exp(z * H[i]) v by the Lanczos / Krylov method with fixed dimension k = opt.krylov_dim,
+   full re-orthogonalisation, real alpha_j, breakdown rule beta_j < 1e-14 * max(1, |alpha_j|)
+   (SURVEY.md 8(c) O3/c11).  H[i] is the (Hermitian) operator of
+   tdvp_apply_heff with the given L, W, R.  All scalars of the recurrence stay on the device.
+   krylov_used: HOST, nullable; if non-NULL the call blocks on the stream and returns the Krylov
+   dimension actually used. */
+int tdvp_expm_heff(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr,
+                   const tdvp_c128 *L, const tdvp_c128 *W, const tdvp_c128 *R /*DEVICE, as above*/,
+                   double z_re, double z_im, const tdvp_c128 *v /*DEVICE [Ml,d,Mr]*/,
+                   tdvp_c128 *y /*DEVICE [Ml,d,Mr]*/, int *krylov_used);
+/* Same for the bond operator of tdvp_apply_bond. */
+int tdvp_expm_bond(tdvp_handle *h, int Ml, int Mr, int Dw,
+                   const tdvp_c128 *L, const tdvp_c128 *R, double z_re, double z_im,
+                   const tdvp_c128 *v /*DEVICE [Ml,Mr]*/, tdvp_c128 *y /*DEVICE [Ml,Mr]*/,
+                   int *krylov_used);
+
+/* QR gauge move (Eq. 9), Householder, on the device.
+   side = 0: C[Ml,d,Mr] viewed as (Ml*d) x Mr = Q D,  Q[Ml,d,Mr] left-canonical (Eq. 7), D[Mr,Mr]
+   side = 1: C viewed as Ml x (d*Mr) = D Q,  Q[Ml,d,Mr] right-canonical (Eq. 8), D[Ml,Ml]
+   Requires Ml*d >= Mr (side 0) or d*Mr >= Ml (side 1).  Q and D are unique only up to a unitary
+   on the bond (the paper does not distinguish QR from RQ); the product is exact. */
+int tdvp_qr_gauge(tdvp_handle *h, int side, int Ml, int d, int Mr,
+                  const tdvp_c128 *C /*DEVICE*/, tdvp_c128 *Q /*DEVICE*/, tdvp_c128 *D /*DEVICE*/);
+
+/* ---- stateful calls on the handle's resident MPS / environment cache ---------------------- */
+
+/* H[site] applied to A_dev using the cached L[site], R[site] (valid when the gauge centre is at
+   `site`).  A_dev, out_dev: DEVICE [Ml_site, d_site, Mr_site]. */
+int tdvp_apply_heff_site(tdvp_handle *h, int site, const tdvp_c128 *A_dev, tdvp_c128 *out_dev);
+/* Rebuild one cached block from its neighbour and the resident site tensor:
+   side = 0: L[site+1] from L[site], W_site, A_site;  side = 1: R[site-1] from R[site], W_site, A_site. */
+int tdvp_update_env_site(tdvp_handle *h, int site, int side);
+
+/* One TDVP-PS step of length dt (Eq. 42-44): left-to-right sweep with dt/2
+   (forward Eq. 43, QR Eq. 9, environment Eq. 30-32, backward Eq. 44), the last site evolved once
+   by dt, and the mirror sweep.  Needs the PS gauge (centre at site 0); leaves it there.
+   Enqueue only: no host round trip inside the step. */
+int tdvp_step_ps(tdvp_handle *h, double dt);
+
+/* One Dormand-Prince 5(4) step of length dt of the TDVP-MU equations of motion
+   (Eq. 27, 33, 36-38) in the left-canonical gauge (centre at site N-1).  If the
+   handle is in the PS gauge it is first moved by a QR sweep (no time evolution).
+   err_est: HOST, nullable; if non-NULL the call blocks and returns the Euclidean norm of the
+   embedded (5th - 4th order) difference. */
+int tdvp_step_mu(tdvp_handle *h, double dt, double *err_est);
+
+/* Move the gauge centre by QR / RQ sweeps without time evolution and rebuild the environment
+   cache: centre = 0 (PS gauge) or centre = N-1 (MU gauge). */
+int tdvp_set_gauge(tdvp_handle *h, int centre);
+
+/* <psi| op_site |psi> / <psi|psi> is NOT normalised here: out = <psi| op |psi>.
+   op: HOST [d,d] (row = bra).  Blocks on the stream.  Gauge-agnostic (identity transfer matrices
+   from both ends). */
+int tdvp_observe(tdvp_handle *h, int site, const tdvp_c128 *op, tdvp_c128 *out /*HOST*/);
+/* Diagonal of the one-site reduced density matrix at `site` (site populations P^(n)(t),
+   PAPER.md:335).  out: HOST [d_site].  Blocks on the stream. */
+int tdvp_populations(tdvp_handle *h, int site, double *out);
+/* <psi|psi> and <psi|H|psi>.  HOST outputs, either may be NULL.  Blocks on the stream. */
+int tdvp_norm_energy(tdvp_handle *h, double *norm_sq, double *energy);
+
+/* Copy site tensor out (HOST [Ml,d,Mr]); Ml/Mr nullable.  Blocks on the stream. */
+int tdvp_get_mps(tdvp_handle *h, int site, tdvp_c128 *out_host, int *Ml, int *Mr);
+/* Replace the MPS (same bond dimensions as at creation).  mps_host[N]: HOST pointers to HOST
+   tensors.  centre must be 0 (right-canonical) or N-1 (left-canonical); environments are rebuilt. */
+int tdvp_set_mps(tdvp_handle *h, const tdvp_c128 *const *mps_host, int centre);
+int tdvp_get_centre(tdvp_handle *h);               /* current gauge centre, or a negative error  */
+int tdvp_sync(tdvp_handle *h);                     /* block until the handle's stream is idle    */
+const char *tdvp_last_error(const tdvp_handle *h);
+
+/* ---- measurement helpers ------------------------------------------------------------------- */
+/* Issue-rate probe of the FP64 tensor pipe (DMMA m8n8k4 in registers, no memory traffic): runs on
+   the legacy default stream, blocks, returns TFLOP/s.  This is the denominator bench.py uses for
+   "fraction of FP64 tensor peak". */
+int tdvp_probe_fp64_tensor_peak(int iters, double *tflops /*HOST*/);
+/* Number of kernel launches this library has enqueued since load (for bench.py's gpu_launches;
+   launches replayed from a captured CUDA graph are counted when the graph is launched). */
+long long tdvp_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TDVP_H */

@@ -1,0 +1,266 @@
+// api.cu -- C ABI entry points that work on caller-provided device buffers (include/tdvp.h),
+// handle bookkeeping, error reporting and the FP64 tensor-pipe probe.
+#include <mutex>
+
+#include "handle.cuh"
+
+std::atomic<long long> g_launch_count{0};
+thread_local long long *g_capture_tally = nullptr;
+static thread_local std::string g_null_err;
+
+int set_err(tdvp_handle *h, int code, const std::string &msg) {
+  if (h) h->err = msg; else g_null_err = msg;
+  return code;
+}
+int check_cuda(tdvp_handle *h, cudaError_t e, const char *what) {
+  if (e == cudaSuccess) return TDVP_OK;
+  return set_err(h, e == cudaErrorMemoryAllocation ? TDVP_ENOMEM : TDVP_ECUDA,
+                 std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+cudaError_t Arena::reserve(size_t bytes, cudaStream_t st) {
+  if (bytes <= cap) return cudaSuccess;
+  if (base) {                                   // kernels in flight may still use the old arena
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return e;
+    cudaFree(base); base = nullptr; cap = 0;
+  }
+  size_t want = bytes + bytes / 4 + (1 << 20);
+  cudaError_t e = cudaMalloc(&base, want);
+  if (e != cudaSuccess) { base = nullptr; cap = 0; return e; }
+  cap = want; off = 0;
+  return cudaSuccess;
+}
+void Arena::release() { if (base) cudaFree(base); base = nullptr; cap = 0; off = 0; }
+
+void configure_kernels_once() {
+  static std::once_flag once;
+  std::call_once(once, [] { zgemm_configure(); wstage_configure(); qr_configure(); });
+}
+
+tdvp_handle *default_handle() {
+  configure_kernels_once();
+  static tdvp_handle *h = nullptr;
+  static std::mutex mu;
+  std::lock_guard<std::mutex> g(mu);
+  if (!h) { h = new tdvp_handle(); tdvp_default_options(&h->opt); h->stream = nullptr; }
+  return h;
+}
+
+static int check_opts(tdvp_handle *h, const tdvp_options &o) {
+  if (o.krylov_dim < 1 || o.krylov_dim > TDVP_MAX_KRYLOV)
+    return set_err(h, TDVP_EINVAL, "krylov_dim must be in [1, 64]");
+  if (o.krylov_tol != 0.0) return set_err(h, TDVP_EINVAL, "krylov_tol must be 0 (fixed-k contract mode)");
+  if (!(o.mu_eps > 0.0)) return set_err(h, TDVP_EINVAL, "mu_eps must be > 0");
+  if (o.w_zero_tol < 0.0) return set_err(h, TDVP_EINVAL, "w_zero_tol must be >= 0");
+  return TDVP_OK;
+}
+
+extern "C" {
+
+void tdvp_default_options(tdvp_options *opt) {
+  if (!opt) return;
+  opt->krylov_dim = 10;
+  opt->krylov_tol = 0.0;
+  opt->mu_eps = 1e-10;
+  opt->w_zero_tol = 0.0;
+  opt->flags = 0;
+}
+
+int tdvp_create_context(tdvp_handle **out, const tdvp_options *opt, void *cuda_stream) {
+  if (!out) return set_err(nullptr, TDVP_EINVAL, "out is NULL");
+  tdvp_handle *h = new (std::nothrow) tdvp_handle();
+  if (!h) return set_err(nullptr, TDVP_ENOMEM, "host allocation failed");
+  if (opt) h->opt = *opt; else tdvp_default_options(&h->opt);
+  int rc = check_opts(nullptr, h->opt);
+  if (rc) { delete h; return rc; }
+  h->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  configure_kernels_once();
+  *out = h;
+  return TDVP_OK;
+}
+
+const char *tdvp_last_error(const tdvp_handle *h) { return h ? h->err.c_str() : g_null_err.c_str(); }
+
+long long tdvp_launch_count(void) { return g_launch_count.load(); }
+
+int tdvp_sync(tdvp_handle *h) {
+  tdvp_handle *hh = h ? h : default_handle();
+  return check_cuda(h, cudaStreamSynchronize(hh->stream), "tdvp_sync");
+}
+
+static int bad_dims(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr) {
+  if (Ml < 1 || Mr < 1 || d < 1 || Dl < 1 || Dr < 1) return set_err(h, TDVP_EINVAL, "dimensions must be >= 1");
+  const double lim = 2.0e9;
+  if ((double)Ml * Dl * d * Mr > lim || (double)Ml * Dr * d * Mr > lim || (double)Ml * Ml * Dl > lim ||
+      (double)Mr * Mr * Dr > lim)
+    return set_err(h, TDVP_EINVAL, "problem too large (an intermediate exceeds 2e9 elements)");
+  return 0;
+}
+
+int tdvp_apply_heff(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr, const tdvp_c128 *L,
+                    const tdvp_c128 *W, const tdvp_c128 *A, const tdvp_c128 *R, tdvp_c128 *out) {
+  tdvp_handle *hh = h ? h : default_handle();
+  if (!L || !W || !A || !R || !out) return set_err(h, TDVP_EINVAL, "null pointer");
+  if (int rc = bad_dims(h, Ml, Mr, d, Dl, Dr)) return rc;
+  size_t wb = wsparse_bytes(Dl, d, Dr), hb = heff_ws_bytes(Ml, Mr, d, Dl, Dr);
+  if (int rc = check_cuda(h, hh->arena.reserve(wb + hb + 1024, hh->stream), "workspace")) return rc;
+  hh->arena.reset();
+  void *wmem = hh->arena.take(wb);
+  void *ws = hh->arena.take(hb);
+  WSparse wsp;
+  wsparse_build(hh->stream, wsp, wmem, Dl, d, Dr, reinterpret_cast<const c128 *>(W), hh->opt.w_zero_tol);
+  heff_apply(hh->stream, Ml, Mr, d, Dl, Dr, reinterpret_cast<const c128 *>(L), wsp,
+             reinterpret_cast<const c128 *>(A), reinterpret_cast<const c128 *>(R),
+             reinterpret_cast<c128 *>(out), ws);
+  return check_cuda(h, cudaGetLastError(), "tdvp_apply_heff");
+}
+
+int tdvp_update_env(tdvp_handle *h, int side, int Ml, int Mr, int d, int Dl, int Dr,
+                    const tdvp_c128 *env_in, const tdvp_c128 *W, const tdvp_c128 *A,
+                    tdvp_c128 *env_out) {
+  tdvp_handle *hh = h ? h : default_handle();
+  if (!env_in || !W || !A || !env_out) return set_err(h, TDVP_EINVAL, "null pointer");
+  if (side != 0 && side != 1) return set_err(h, TDVP_EINVAL, "side must be 0 or 1");
+  if (int rc = bad_dims(h, Ml, Mr, d, Dl, Dr)) return rc;
+  size_t wb = wsparse_bytes(Dl, d, Dr), eb = env_ws_bytes(Ml, Mr, d, Dl, Dr);
+  if (int rc = check_cuda(h, hh->arena.reserve(wb + eb + 1024, hh->stream), "workspace")) return rc;
+  hh->arena.reset();
+  void *wmem = hh->arena.take(wb);
+  void *ws = hh->arena.take(eb);
+  WSparse wsp;
+  wsparse_build(hh->stream, wsp, wmem, Dl, d, Dr, reinterpret_cast<const c128 *>(W), hh->opt.w_zero_tol);
+  env_update(hh->stream, side, Ml, Mr, d, Dl, Dr, reinterpret_cast<const c128 *>(env_in), wsp,
+             reinterpret_cast<const c128 *>(A), reinterpret_cast<c128 *>(env_out), ws);
+  return check_cuda(h, cudaGetLastError(), "tdvp_update_env");
+}
+
+int tdvp_apply_bond(tdvp_handle *h, int Ml, int Mr, int Dw, const tdvp_c128 *L,
+                    const tdvp_c128 *D, const tdvp_c128 *R, tdvp_c128 *out) {
+  tdvp_handle *hh = h ? h : default_handle();
+  if (!L || !D || !R || !out) return set_err(h, TDVP_EINVAL, "null pointer");
+  if (int rc = bad_dims(h, Ml, Mr, 1, Dw, Dw)) return rc;
+  size_t bb = bond_ws_bytes(Ml, Mr, Dw);
+  if (int rc = check_cuda(h, hh->arena.reserve(bb + 1024, hh->stream), "workspace")) return rc;
+  hh->arena.reset();
+  void *ws = hh->arena.take(bb);
+  bond_apply(hh->stream, Ml, Mr, Dw, reinterpret_cast<const c128 *>(L),
+             reinterpret_cast<const c128 *>(D), reinterpret_cast<const c128 *>(R),
+             reinterpret_cast<c128 *>(out), ws);
+  return check_cuda(h, cudaGetLastError(), "tdvp_apply_bond");
+}
+
+int tdvp_expm_heff(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr, const tdvp_c128 *L,
+                   const tdvp_c128 *W, const tdvp_c128 *R, double z_re, double z_im,
+                   const tdvp_c128 *v, tdvp_c128 *y, int *krylov_used) {
+  tdvp_handle *hh = h ? h : default_handle();
+  if (!L || !W || !R || !v || !y) return set_err(h, TDVP_EINVAL, "null pointer");
+  if (int rc = bad_dims(h, Ml, Mr, d, Dl, Dr)) return rc;
+  LanczosOp op{0, Ml, Mr, d, Dl, Dr, reinterpret_cast<const c128 *>(L), reinterpret_cast<const c128 *>(R), nullptr};
+  const int k = hh->opt.krylov_dim;
+  size_t wb = wsparse_bytes(Dl, d, Dr), lb = lanczos_ws_bytes(op, k);
+  if (int rc = check_cuda(h, hh->arena.reserve(wb + lb + 2048, hh->stream), "workspace")) return rc;
+  hh->arena.reset();
+  void *wmem = hh->arena.take(wb);
+  void *ws = hh->arena.take(lb);
+  int *m_dev = reinterpret_cast<int *>(hh->arena.take(256));
+  WSparse wsp;
+  wsparse_build(hh->stream, wsp, wmem, Dl, d, Dr, reinterpret_cast<const c128 *>(W), hh->opt.w_zero_tol);
+  op.W = &wsp;
+  lanczos_expm(hh->stream, op, k, z_re, z_im, reinterpret_cast<const c128 *>(v),
+               reinterpret_cast<c128 *>(y), ws, m_dev);
+  if (int rc = check_cuda(h, cudaGetLastError(), "tdvp_expm_heff")) return rc;
+  if (krylov_used) {
+    if (int rc = check_cuda(h, cudaMemcpyAsync(krylov_used, m_dev, sizeof(int), cudaMemcpyDeviceToHost, hh->stream), "memcpy")) return rc;
+    return check_cuda(h, cudaStreamSynchronize(hh->stream), "tdvp_expm_heff sync");
+  }
+  return TDVP_OK;
+}
+
+int tdvp_expm_bond(tdvp_handle *h, int Ml, int Mr, int Dw, const tdvp_c128 *L, const tdvp_c128 *R,
+                   double z_re, double z_im, const tdvp_c128 *v, tdvp_c128 *y, int *krylov_used) {
+  tdvp_handle *hh = h ? h : default_handle();
+  if (!L || !R || !v || !y) return set_err(h, TDVP_EINVAL, "null pointer");
+  if (int rc = bad_dims(h, Ml, Mr, 1, Dw, Dw)) return rc;
+  LanczosOp op{1, Ml, Mr, 1, Dw, Dw, reinterpret_cast<const c128 *>(L), reinterpret_cast<const c128 *>(R), nullptr};
+  const int k = hh->opt.krylov_dim;
+  size_t lb = lanczos_ws_bytes(op, k);
+  if (int rc = check_cuda(h, hh->arena.reserve(lb + 2048, hh->stream), "workspace")) return rc;
+  hh->arena.reset();
+  void *ws = hh->arena.take(lb);
+  int *m_dev = reinterpret_cast<int *>(hh->arena.take(256));
+  lanczos_expm(hh->stream, op, k, z_re, z_im, reinterpret_cast<const c128 *>(v),
+               reinterpret_cast<c128 *>(y), ws, m_dev);
+  if (int rc = check_cuda(h, cudaGetLastError(), "tdvp_expm_bond")) return rc;
+  if (krylov_used) {
+    if (int rc = check_cuda(h, cudaMemcpyAsync(krylov_used, m_dev, sizeof(int), cudaMemcpyDeviceToHost, hh->stream), "memcpy")) return rc;
+    return check_cuda(h, cudaStreamSynchronize(hh->stream), "tdvp_expm_bond sync");
+  }
+  return TDVP_OK;
+}
+
+int tdvp_qr_gauge(tdvp_handle *h, int side, int Ml, int d, int Mr, const tdvp_c128 *C,
+                  tdvp_c128 *Q, tdvp_c128 *D) {
+  tdvp_handle *hh = h ? h : default_handle();
+  if (!C || !Q || !D) return set_err(h, TDVP_EINVAL, "null pointer");
+  if (side != 0 && side != 1) return set_err(h, TDVP_EINVAL, "side must be 0 or 1");
+  if (Ml < 1 || d < 1 || Mr < 1) return set_err(h, TDVP_EINVAL, "dimensions must be >= 1");
+  long long tall = side == 0 ? (long long)Ml * d : (long long)d * Mr;
+  int thin = side == 0 ? Mr : Ml;
+  if (tall < thin) return set_err(h, TDVP_EINVAL, "gauge move needs a tall or square matrix");
+  size_t qb = qr_ws_bytes((int)tall, thin);
+  if (int rc = check_cuda(h, hh->arena.reserve(qb + 1024, hh->stream), "workspace")) return rc;
+  hh->arena.reset();
+  void *ws = hh->arena.take(qb);
+  qr_gauge(hh->stream, side, Ml, d, Mr, reinterpret_cast<const c128 *>(C),
+           reinterpret_cast<c128 *>(Q), reinterpret_cast<c128 *>(D), ws);
+  return check_cuda(h, cudaGetLastError(), "tdvp_qr_gauge");
+}
+
+// ---- FP64 tensor-pipe issue-rate probe ------------------------------------------------------
+__global__ void dmma_probe_kernel(double *out, int iters, double a, double b) {
+  double c0[8], c1[8];
+#pragma unroll
+  for (int i = 0; i < 8; i++) { c0[i] = threadIdx.x; c1[i] = i; }
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int i = 0; i < 8; i++)
+      asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                   : "+d"(c0[i]), "+d"(c1[i]) : "d"(a), "d"(b));
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; i++) s += c0[i] + c1[i];
+  if (s == 1.2345) out[0] = s;
+}
+
+int tdvp_probe_fp64_tensor_peak(int iters, double *tflops) {
+  if (!tflops || iters < 1) return set_err(nullptr, TDVP_EINVAL, "bad arguments");
+  int dev = 0, nsm = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  double *out = nullptr;
+  if (int rc = check_cuda(nullptr, cudaMalloc(&out, 8), "cudaMalloc")) return rc;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int blocks = 2 * nsm, threads = 256;
+  dmma_probe_kernel<<<blocks, threads>>>(out, iters / 10 + 1, 1.0000001, 1e-9);
+  float best = 1e30f;
+  for (int r = 0; r < 3; r++) {
+    cudaEventRecord(e0);
+    dmma_probe_kernel<<<blocks, threads>>>(out, iters, 1.0000001, 1e-9);
+    cudaEventRecord(e1);
+    cudaEventSynchronize(e1);
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (ms < best) best = ms;
+  }
+  cudaError_t e = cudaGetLastError();
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out);
+  if (e != cudaSuccess) return check_cuda(nullptr, e, "probe");
+  double fma = 256.0 * 8 * (double)iters * (threads / 32) * blocks;
+  *tflops = 2.0 * fma / (best * 1e-3) / 1e12;
+  return TDVP_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,136 @@
+// common.cuh -- shared declarations of libtdvp.so (CUDA path; shares nothing with oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <atomic>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+
+#include "../../include/tdvp.h"
+
+typedef double2 c128;  // (x = re, y = im), same memory layout as tdvp_c128
+
+extern std::atomic<long long> g_launch_count;   // kernels enqueued (tdvp_launch_count)
+// While a stream capture is recording, launches are counted into the graph's own tally instead.
+extern thread_local long long *g_capture_tally;
+
+static inline void count_launch() {
+  if (g_capture_tally) ++*g_capture_tally; else g_launch_count.fetch_add(1, std::memory_order_relaxed);
+}
+
+// Launch wrapper: counts the launch; errors are picked up by the API layer via cudaGetLastError.
+#define TDVP_LAUNCH(kernel, grid, block, smem, stream, ...)              \
+  do {                                                                   \
+    kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);          \
+    count_launch();                                                      \
+  } while (0)
+
+__host__ __device__ static inline c128 cmul(c128 a, c128 b) {
+  return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__host__ __device__ static inline c128 cconj(c128 a) { return make_double2(a.x, -a.y); }
+
+// One-time kernel attribute setup (dynamic shared memory limits); called when a handle is made.
+void zgemm_configure();
+void wstage_configure();
+void qr_configure();
+void configure_kernels_once();
+
+static inline long long ceil_div_ll(long long a, long long b) { return (a + b - 1) / b; }
+
+// ---------------------------------------------------------------------------------------------
+// zgemm.cu : complex128 GEMM on the FP64 tensor pipe (DMMA m8n8k4), batched, split-K.
+// C[bi](m,n) = sum_k opA[bi](m,k) * opB[bi](k,n),  m < M, n < N, k < K
+//   opA(m,k) = conjA ? conj(A[m*a_ms + k*a_ks]) : A[m*a_ms + k*a_ks]   (one of a_ms, a_ks is 1)
+//   opB(k,n) = conjB ? conj(B[k*b_ks + n*b_ns]) : B[k*b_ks + n*b_ns]   (one of b_ks, b_ns is 1)
+//   C(m,n)   = C[m*ldc + n]
+// batch index bi = bo*batch_inner + bin; each operand has an (outer, inner) pair of strides.
+struct ZGemm {
+  const c128 *A; const c128 *B; c128 *C;
+  int M, N, K;
+  long long a_ms, a_ks, b_ks, b_ns, ldc;
+  int batch_inner = 1, batch_outer = 1;
+  long long a_bsi = 0, b_bsi = 0, c_bsi = 0;   // inner batch strides
+  long long a_bso = 0, b_bso = 0, c_bso = 0;   // outer batch strides
+  int conjA = 0, conjB = 0;
+  int splitk = 0;                               // 0 = choose
+};
+// ws: split-K workspace of at least zgemm_ws_elems(p) complex numbers (may be NULL if 0).
+size_t zgemm_ws_elems(const ZGemm &p);          // upper bound for any split the heuristic may pick
+void zgemm(cudaStream_t st, const ZGemm &p, c128 *ws);
+
+// ---------------------------------------------------------------------------------------------
+// wstage.cu : sparse MPO stage.
+// Device CSR of a dense W[Dl,d,d,Dr], rows r = s*Dr + v (heff order) and columns c = w*d + t.
+struct WSparse {
+  int Dl, d, Dr;
+  int *rowptr;      // DEVICE [d*Dr + 1]
+  int *col;         // DEVICE [capacity]
+  c128 *val;        // DEVICE [capacity]
+  // transposed-role CSR used by the right-to-left order: rows r = w*d + s, columns c = t*Dr + v
+  int *rowptr_r; int *col_r; c128 *val_r;
+  int capacity;
+};
+size_t wsparse_bytes(int Dl, int d, int Dr);
+// carve a WSparse out of `mem` (DEVICE, wsparse_bytes) and build both CSRs from dense W (DEVICE)
+void wsparse_build(cudaStream_t st, WSparse &ws, void *mem, int Dl, int d, int Dr,
+                   const c128 *W, double zero_tol);
+// T2[a,s,v,y] = sum_{w,t} W[w,s,t,v] T1[a,w,t,y];  T1 [Ml,Dl,d,Mr] -> T2 [Ml,d,Dr,Mr]
+void wstage_left(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2);
+// T2[w,x,s,b] = sum_{t,v} W[w,s,t,v] T1[x,t,v,b];  T1 [Ml,d,Dr,Mr] -> T2 [Dl,Ml,d,Mr]
+void wstage_right(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2);
+
+// ---------------------------------------------------------------------------------------------
+// Workspace: one growable device arena per handle (cudaMalloc only when it has to grow).
+struct Arena {
+  char *base = nullptr; size_t cap = 0; size_t off = 0;
+  cudaError_t reserve(size_t bytes, cudaStream_t st);
+  void reset() { off = 0; }
+  void *take(size_t bytes) {
+    size_t a = (off + 255) & ~size_t(255);
+    if (a + bytes > cap) return nullptr;
+    off = a + bytes; return base + a;
+  }
+  void release();
+};
+
+// ---------------------------------------------------------------------------------------------
+// contract.cu : the local contractions on explicit device pointers.
+size_t heff_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr);
+void heff_apply(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c128 *L,
+                const WSparse &W, const c128 *A, const c128 *R, c128 *out, void *ws);
+size_t env_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr);
+void env_update(cudaStream_t st, int side, int Ml, int Mr, int d, int Dl, int Dr,
+                const c128 *env_in, const WSparse &W, const c128 *A, c128 *env_out, void *ws);
+size_t bond_ws_bytes(int Ml, int Mr, int Dw);
+void bond_apply(cudaStream_t st, int Ml, int Mr, int Dw, const c128 *L, const c128 *D,
+                const c128 *R, c128 *out, void *ws);
+
+// ---------------------------------------------------------------------------------------------
+// lanczos.cu : Krylov exponential with all scalars on the device.
+struct LanczosOp {           // which operator: heff (site) or bond
+  int kind;                  // 0 = heff, 1 = bond
+  int Ml, Mr, d, Dl, Dr;     // bond: d = 1, Dl = Dr = Dw
+  const c128 *L; const c128 *R; const WSparse *W;
+};
+size_t lanczos_ws_bytes(const LanczosOp &op, int k);
+// y = exp(z H) v.  m_used_dev: DEVICE int (nullable) receiving the Krylov dimension used.
+void lanczos_expm(cudaStream_t st, const LanczosOp &op, int k, double z_re, double z_im,
+                  const c128 *v, c128 *y, void *ws, int *m_used_dev);
+
+// ---------------------------------------------------------------------------------------------
+// qr.cu : Householder QR gauge move on the device.
+size_t qr_ws_bytes(int rows, int cols);
+// side 0: C (rows x cols, row-major, rows = Ml*d, cols = Mr) = Q D, Q rows x cols, D cols x cols
+// side 1: C (Ml x (d*Mr)) = D Q, i.e. QR of C^T: tall = d*Mr, thin = Ml; Q [Ml, d*Mr], D [Ml, Ml]
+void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c128 *Q, c128 *D,
+              void *ws);
+
+// ---------------------------------------------------------------------------------------------
+// small vector kernels shared by the drivers (vecops.cu)
+void vec_copy(cudaStream_t st, c128 *dst, const c128 *src, long long n);
+void vec_zero(cudaStream_t st, c128 *dst, long long n);
+// partial-free deterministic reductions: out_dev[0] = sum |x|^2 ; uses scratch of vec_red_scratch()
+size_t vec_red_scratch_bytes();
+void vec_norm_sq(cudaStream_t st, const c128 *x, long long n, double *out_dev, void *scratch);
+void vec_dotc(cudaStream_t st, const c128 *x, const c128 *y, long long n, c128 *out_dev, void *scratch);

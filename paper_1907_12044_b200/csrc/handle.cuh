@@ -1,0 +1,46 @@
+// handle.cuh -- the opaque tdvp_handle: stream, options, scratch arena, resident chain state.
+#pragma once
+#include <vector>
+
+#include "common.cuh"
+
+struct StepGraph {                 // a captured TDVP step (CUDA graph), keyed by dt
+  cudaGraphExec_t exec = nullptr;
+  double dt = 0.0;
+  long long launches = 0;          // kernels inside the graph (for tdvp_launch_count)
+};
+
+struct tdvp_handle {
+  cudaStream_t stream = nullptr;
+  tdvp_options opt;
+  std::string err;
+  Arena arena;                     // scratch for the current call (reset per call)
+
+  // ---- resident chain state (n == 0 for a context-only handle) ----
+  int n = 0;
+  std::vector<int> d;              // physical dims [n]
+  std::vector<int> Dw;             // MPO bonds [n+1]
+  std::vector<int> M;              // MPS bonds [n+1]
+  std::vector<c128 *> W;           // dense MPO tensors (DEVICE)
+  std::vector<WSparse> Wsp;        // their CSR forms (DEVICE)
+  std::vector<void *> Wsp_mem;
+  std::vector<c128 *> A;           // MPS tensors (DEVICE)
+  std::vector<c128 *> Lenv;        // Lenv[i]: sites < i contracted, [M[i], Dw[i], M[i]]
+  std::vector<c128 *> Renv;        // Renv[i]: sites > i contracted, [M[i+1], Dw[i+1], M[i+1]]
+  int centre = 0;                  // gauge centre; sites < centre left-canonical, > centre right-canonical
+  c128 *tmpA = nullptr;            // scratch site tensors (largest site)
+  c128 *tmpB = nullptr;
+  c128 *bondD = nullptr;           // bond matrix D and its evolved copy
+  c128 *bondD2 = nullptr;
+  void *step_ws = nullptr;         // persistent workspace for the step drivers
+  size_t step_ws_bytes = 0;
+  // TDVP-MU state (allocated on first use)
+  std::vector<c128 *> mu_k[7];     // Dormand-Prince stage derivatives
+  std::vector<c128 *> mu_y;        // stage states
+  double *mu_err_dev = nullptr;
+  StepGraph ps_graph, mu_graph;
+};
+
+int set_err(tdvp_handle *h, int code, const std::string &msg);
+int check_cuda(tdvp_handle *h, cudaError_t e, const char *what);
+tdvp_handle *default_handle();

@@ -1,0 +1,268 @@
+// lanczos.cu -- y = exp(z H) v by the Lanczos / Krylov method (SURVEY.md 8(a) a6,
+// 8(c) O3/c11): fixed Krylov dimension k, alpha_j = Re<q_j, H q_j>, full re-orthogonalisation (two
+// classical Gram-Schmidt passes against all previous vectors), breakdown rule
+// beta_j < 1e-14 * max(1, |alpha_j|).
+//
+// The paper attributes a large share of its GPU step time to this sub-step because every alpha and
+// beta crossed PCIe.  Here every scalar of the recurrence lives in device
+// memory: reductions finish in the last CTA to arrive (fixed summation order: deterministic), the
+// breakdown decision is a device flag that turns the remaining iterations into no-ops (q = 0), and
+// the k x k tridiagonal eigenproblem runs in one warp.  Nothing is read back by the host.
+#include "common.cuh"
+#include "tridiag.cuh"
+
+namespace {
+
+constexpr int VT = 256;                 // threads per CTA of the vector kernels
+constexpr int MAXG = 296;               // max CTAs of a vector kernel (2 per SM)
+constexpr double BREAKDOWN_TOL = 1e-14;
+
+struct LzState {
+  int m;            // Krylov dimension used (valid once done)
+  int done;
+  double beta0;
+  double inv_beta;  // 1/beta_j of the current iteration, 0 after breakdown
+};
+
+struct LzBuffers {
+  c128 *Q;          // [(k+1)][n]
+  c128 *dots;       // [k+1]
+  c128 *coef;       // [k]
+  double *alpha;    // [k]
+  double *beta;     // [k]
+  LzState *state;
+  unsigned *counter;
+  c128 *partial;    // [MAXG][k+1]
+  double *npartial; // [MAXG]
+  void *apply_ws;
+};
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// True in exactly one CTA: the last one to arrive.  Resets the counter for the next kernel.
+__device__ __forceinline__ bool last_block(unsigned *counter) {
+  __shared__ bool is_last;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned t = atomicAdd(counter, 1u);
+    is_last = (t == gridDim.x - 1);
+    if (is_last) *counter = 0u;
+  }
+  __syncthreads();
+  if (is_last) __threadfence();
+  return is_last;
+}
+
+__device__ __forceinline__ void chunk_of(long long n, long long &e0, long long &e1) {
+  long long per = (n + gridDim.x - 1) / gridDim.x;
+  e0 = (long long)blockIdx.x * per;
+  e1 = e0 + per; if (e1 > n) e1 = n;
+}
+
+// beta0 = ||v||, state reset.
+__global__ void __launch_bounds__(VT) lz_init_kernel(const c128 *v, long long n, LzBuffers b) {
+  long long e0, e1; chunk_of(n, e0, e1);
+  double s = 0.0;
+  for (long long e = e0 + threadIdx.x; e < e1; e += VT) { c128 x = v[e]; s += x.x * x.x + x.y * x.y; }
+  __shared__ double red[VT / 32];
+  s = warp_sum(s);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) { double t = 0; for (int i = 0; i < VT / 32; i++) t += red[i]; b.npartial[blockIdx.x] = t; }
+  if (last_block(b.counter) && threadIdx.x < 32) {
+    double t = 0.0;
+    for (int g = threadIdx.x; g < gridDim.x; g += 32) t += b.npartial[g];
+    t = warp_sum(t);
+    if (threadIdx.x == 0) {
+      double beta0 = sqrt(t);
+      b.state->beta0 = beta0;
+      b.state->inv_beta = beta0 > 0.0 ? 1.0 / beta0 : 0.0;
+      b.state->done = 0;
+      b.state->m = 0;
+    }
+  }
+}
+
+// dst = src * state.inv_beta
+__global__ void __launch_bounds__(VT) lz_scale_kernel(c128 *dst, const c128 *src, long long n, const LzState *st) {
+  const double f = st->inv_beta;
+  for (long long e = blockIdx.x * (long long)VT + threadIdx.x; e < n; e += (long long)gridDim.x * VT) {
+    c128 x = src[e];
+    dst[e] = make_double2(x.x * f, x.y * f);
+  }
+}
+
+// dots[i] = <q_i, w> for i < nd (conjugate on q).  first_pass: alpha[j] = Re dots[j].
+__global__ void __launch_bounds__(VT) lz_dots_kernel(long long n, int nd, int j, int first_pass, LzBuffers b) {
+  const c128 *w = b.Q + (long long)(j + 1) * n;
+  long long e0, e1; chunk_of(n, e0, e1);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int i = warp; i < nd; i += VT / 32) {
+    const c128 *q = b.Q + (long long)i * n;
+    double sx = 0.0, sy = 0.0;
+    for (long long e = e0 + lane; e < e1; e += 32) {
+      c128 a = q[e], x = w[e];
+      sx += a.x * x.x + a.y * x.y;
+      sy += a.x * x.y - a.y * x.x;
+    }
+    sx = warp_sum(sx); sy = warp_sum(sy);
+    if (lane == 0) b.partial[(long long)blockIdx.x * nd + i] = make_double2(sx, sy);
+  }
+  if (last_block(b.counter)) {
+    for (int i = warp; i < nd; i += VT / 32) {
+      double sx = 0.0, sy = 0.0;
+      for (int g = lane; g < gridDim.x; g += 32) { c128 p = b.partial[(long long)g * nd + i]; sx += p.x; sy += p.y; }
+      sx = warp_sum(sx); sy = warp_sum(sy);
+      if (lane == 0) {
+        b.dots[i] = make_double2(sx, sy);
+        if (first_pass && i == j && !b.state->done) b.alpha[j] = sx;
+      }
+    }
+  }
+}
+
+// w -= sum_{i<nd} dots[i] q_i.  If with_norm: beta_j = ||w|| and the breakdown decision.
+__global__ void __launch_bounds__(VT) lz_update_kernel(long long n, int nd, int j, int k, int with_norm, LzBuffers b) {
+  c128 *w = b.Q + (long long)(j + 1) * n;
+  long long e0, e1; chunk_of(n, e0, e1);
+  __shared__ c128 cs[TDVP_MAX_KRYLOV + 1];
+  for (int i = threadIdx.x; i < nd; i += VT) cs[i] = b.dots[i];
+  __syncthreads();
+  double s = 0.0;
+  for (long long e = e0 + threadIdx.x; e < e1; e += VT) {
+    c128 x = w[e];
+    for (int i = 0; i < nd; i++) {
+      c128 q = b.Q[(long long)i * n + e], c = cs[i];
+      x.x -= c.x * q.x - c.y * q.y;
+      x.y -= c.x * q.y + c.y * q.x;
+    }
+    w[e] = x;
+    s += x.x * x.x + x.y * x.y;
+  }
+  if (!with_norm) return;
+  __shared__ double red[VT / 32];
+  s = warp_sum(s);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) { double t = 0; for (int i = 0; i < VT / 32; i++) t += red[i]; b.npartial[blockIdx.x] = t; }
+  if (last_block(b.counter) && threadIdx.x < 32) {
+    double t = 0.0;
+    for (int g = threadIdx.x; g < gridDim.x; g += 32) t += b.npartial[g];
+    t = warp_sum(t);
+    if (threadIdx.x == 0) {
+      LzState *st = b.state;
+      double beta = sqrt(t);
+      if (!st->done) {
+        double aj = fabs(b.alpha[j]);
+        if (j == k - 1 || beta < BREAKDOWN_TOL * (aj > 1.0 ? aj : 1.0)) {
+          st->done = 1; st->m = j + 1; st->inv_beta = 0.0;
+        } else {
+          b.beta[j] = beta; st->inv_beta = 1.0 / beta;
+        }
+      } else {
+        st->inv_beta = 0.0;
+      }
+    }
+  }
+}
+
+// One warp: coef = beta0 * V exp(z Lambda) V^T e_1 for the m x m tridiagonal (alpha, beta).
+__global__ void lz_coef_kernel(int k, double zr, double zi, LzBuffers b, int *m_out) {
+  __shared__ double V[TDVP_MAX_KRYLOV * TDVP_MAX_KRYLOV];
+  double a[TDVP_MAX_KRYLOV], off[TDVP_MAX_KRYLOV];
+  const int lane = threadIdx.x;
+  const int m = b.state->m;
+  if (lane == 0 && m_out) *m_out = m;
+  for (int i = 0; i < m; i++) { a[i] = b.alpha[i]; off[i] = (i < m - 1) ? b.beta[i] : 0.0; }
+  for (int r = lane; r < m; r += 32)
+    for (int c = 0; c < m; c++) V[r * m + c] = (r == c) ? 1.0 : 0.0;
+  tridiag_qr_eig(m, a, off, V, m, lane, 32);
+  __syncwarp();
+  const double beta0 = b.state->beta0;
+  for (int r = lane; r < k; r += 32) {
+    double cx = 0.0, cy = 0.0;
+    if (r < m) {
+      for (int i = 0; i < m; i++) {
+        double mag = exp(zr * a[i]), sn, cn;
+        sincos(zi * a[i], &sn, &cn);
+        double wgt = V[r * m + i] * V[i] * mag;      // V[0][i] = V[i]
+        cx += wgt * cn; cy += wgt * sn;
+      }
+    }
+    b.coef[r] = make_double2(beta0 * cx, beta0 * cy);
+  }
+}
+
+// y = sum_{j<k} coef[j] q_j
+__global__ void __launch_bounds__(VT) lz_combine_kernel(long long n, int k, LzBuffers b, c128 *y) {
+  __shared__ c128 cs[TDVP_MAX_KRYLOV];
+  for (int i = threadIdx.x; i < k; i += VT) cs[i] = b.coef[i];
+  __syncthreads();
+  for (long long e = blockIdx.x * (long long)VT + threadIdx.x; e < n; e += (long long)gridDim.x * VT) {
+    double sx = 0.0, sy = 0.0;
+    for (int i = 0; i < k; i++) {
+      c128 q = b.Q[(long long)i * n + e], c = cs[i];
+      sx += c.x * q.x - c.y * q.y;
+      sy += c.x * q.y + c.y * q.x;
+    }
+    y[e] = make_double2(sx, sy);
+  }
+}
+
+inline size_t up256(size_t x) { return (x + 255) & ~size_t(255); }
+
+size_t apply_ws_bytes(const LanczosOp &op) {
+  return op.kind == 0 ? heff_ws_bytes(op.Ml, op.Mr, op.d, op.Dl, op.Dr) : bond_ws_bytes(op.Ml, op.Mr, op.Dl);
+}
+
+}  // namespace
+
+size_t lanczos_ws_bytes(const LanczosOp &op, int k) {
+  size_t n = (size_t)op.Ml * (op.kind == 0 ? op.d : 1) * op.Mr;
+  return up256((k + 1) * n * 16) + up256((k + 1) * 16) + up256(k * 16) + 2 * up256(k * 8) +
+         up256(sizeof(LzState)) + 256 + up256((size_t)MAXG * (k + 1) * 16) + up256(MAXG * 8) +
+         apply_ws_bytes(op) + 512;
+}
+
+void lanczos_expm(cudaStream_t st, const LanczosOp &op, int k, double z_re, double z_im,
+                  const c128 *v, c128 *y, void *ws, int *m_used_dev) {
+  const long long n = (long long)op.Ml * (op.kind == 0 ? op.d : 1) * op.Mr;
+  char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
+  LzBuffers b;
+  b.Q = reinterpret_cast<c128 *>(p); p += up256((k + 1) * n * 16);
+  b.dots = reinterpret_cast<c128 *>(p); p += up256((k + 1) * 16);
+  b.coef = reinterpret_cast<c128 *>(p); p += up256(k * 16);
+  b.alpha = reinterpret_cast<double *>(p); p += up256(k * 8);
+  b.beta = reinterpret_cast<double *>(p); p += up256(k * 8);
+  b.state = reinterpret_cast<LzState *>(p); p += up256(sizeof(LzState));
+  b.counter = reinterpret_cast<unsigned *>(p); p += 256;
+  b.partial = reinterpret_cast<c128 *>(p); p += up256((size_t)MAXG * (k + 1) * 16);
+  b.npartial = reinterpret_cast<double *>(p); p += up256(MAXG * 8);
+  b.apply_ws = p;
+
+  int G = (int)((n + VT - 1) / VT);
+  if (G > MAXG) G = MAXG;
+  if (G < 1) G = 1;
+  cudaMemsetAsync(b.counter, 0, sizeof(unsigned), st);
+  TDVP_LAUNCH(lz_init_kernel, G, VT, 0, st, v, n, b);
+  TDVP_LAUNCH(lz_scale_kernel, G, VT, 0, st, b.Q, v, n, b.state);
+  for (int j = 0; j < k; j++) {
+    c128 *qj = b.Q + (long long)j * n, *w = b.Q + (long long)(j + 1) * n;
+    if (op.kind == 0)
+      heff_apply(st, op.Ml, op.Mr, op.d, op.Dl, op.Dr, op.L, *op.W, qj, op.R, w, b.apply_ws);
+    else
+      bond_apply(st, op.Ml, op.Mr, op.Dl, op.L, qj, op.R, w, b.apply_ws);
+    TDVP_LAUNCH(lz_dots_kernel, G, VT, 0, st, n, j + 1, j, 1, b);
+    TDVP_LAUNCH(lz_update_kernel, G, VT, 0, st, n, j + 1, j, k, 0, b);
+    TDVP_LAUNCH(lz_dots_kernel, G, VT, 0, st, n, j + 1, j, 0, b);
+    TDVP_LAUNCH(lz_update_kernel, G, VT, 0, st, n, j + 1, j, k, 1, b);
+    if (j < k - 1) TDVP_LAUNCH(lz_scale_kernel, G, VT, 0, st, w, w, n, b.state);
+  }
+  TDVP_LAUNCH(lz_coef_kernel, 1, 32, 0, st, k, z_re, z_im, b, m_used_dev);
+  TDVP_LAUNCH(lz_combine_kernel, G, VT, 0, st, n, k, b, y);
+}

@@ -1,0 +1,370 @@
+// qr.cu -- QR gauge move C = Q D (Eq. 9) by blocked Householder reflections, on
+// the device.  The paper runs this on one CPU core with a PCIe copy each way
+// and names the transfer overhead; here the matrix never leaves HBM.
+//
+// Householder (not Cholesky-QR): centre tensors of a padded / delta-seeded MPS are numerically
+// rank deficient (relative singular values down to 1e-8 and below), and Q must still be an exact
+// isometry (Eq. 7/8).
+//
+// Layout: the tall matrix (rows x cols, rows >= cols) is held column-major in a workspace X (every
+// column contiguous), so all passes are coalesced.  side 1 (RQ = QR of the plain transpose,
+// SURVEY.md 8(c) c9) is natively that layout; side 0 is transposed on the way in and out.
+//   panel kernel : one CTA keeps an nb-column panel in shared memory, factors it column by column
+//                  (zlarfg-style reflectors), builds the compact-WY factor T, emits R entries
+//   trail kernel : X[:, c] <- (I - V T^H V^H) X[:, c] for the trailing columns (a few columns/CTA)
+//   the same kernel with T instead of T^H applied to identity columns, panels in reverse, forms Q.
+#include "common.cuh"
+
+namespace {
+
+constexpr int NB_MAX = 8;
+constexpr int PANEL_THREADS = 1024;
+constexpr int TRAIL_THREADS = 256;
+constexpr int CB = 4;   // columns per CTA in the trailing update
+
+inline size_t up256(size_t x) { return (x + 255) & ~size_t(255); }
+
+__device__ __forceinline__ double warp_sum_d(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// X[j][i] (column-major, ld = rows) <- C[i*cols + j]     (tiled transpose)
+__global__ void transpose_in_kernel(const c128 *C, c128 *X, int rows, int cols) {
+  __shared__ c128 t[32][33];
+  int i0 = blockIdx.y * 32, j0 = blockIdx.x * 32;
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    int i = i0 + r, j = j0 + threadIdx.x;
+    if (i < rows && j < cols) t[r][threadIdx.x] = C[(long long)i * cols + j];
+  }
+  __syncthreads();
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    int j = j0 + r, i = i0 + threadIdx.x;
+    if (i < rows && j < cols) X[(long long)j * rows + i] = t[threadIdx.x][r];
+  }
+}
+// Q[i*cols + j] <- Y[j][i]
+__global__ void transpose_out_kernel(const c128 *Y, c128 *Q, int rows, int cols) {
+  __shared__ c128 t[32][33];
+  int i0 = blockIdx.y * 32, j0 = blockIdx.x * 32;
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    int j = j0 + r, i = i0 + threadIdx.x;
+    if (i < rows && j < cols) t[r][threadIdx.x] = Y[(long long)j * rows + i];
+  }
+  __syncthreads();
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    int i = i0 + r, j = j0 + threadIdx.x;
+    if (i < rows && j < cols) Q[(long long)i * cols + j] = t[threadIdx.x][r];
+  }
+}
+
+__global__ void copy_kernel(c128 *dst, const c128 *src, long long n) {
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x)
+    dst[e] = src[e];
+}
+// Y[c][i] = delta(i, c)
+__global__ void identity_kernel(c128 *Y, int rows, int cols) {
+  long long n = (long long)rows * cols;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
+    int i = e % rows, c = e / rows;
+    Y[e] = make_double2(i == c ? 1.0 : 0.0, 0.0);
+  }
+}
+// D out: transpose_d = 0: D[i][j] = R[i][j]; 1: D[i][j] = R[j][i]
+__global__ void store_d_kernel(const c128 *Rm, c128 *D, int cols, int transpose_d) {
+  int n = cols * cols;
+  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
+    int i = e / cols, j = e % cols;
+    D[e] = transpose_d ? Rm[j * cols + i] : Rm[e];
+  }
+}
+
+// Factor the panel of columns [j0, j0+w) on rows [j0, rows).  Writes reflectors back into X (unit
+// diagonal explicit, zeros above it inside the panel rows), R entries of these columns into Rm
+// (row-major cols x cols, zeros below the diagonal), tau and the w x w upper-triangular T.
+__global__ void __launch_bounds__(PANEL_THREADS) qr_panel_kernel(c128 *X, int rows, int cols, int j0, int w,
+                                                                  c128 *Rm, c128 *Tm /*[NB_MAX][NB_MAX]*/) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int len = rows - j0;
+  c128 *P = reinterpret_cast<c128 *>(smem_raw);                // [w][len]
+  __shared__ double red[PANEL_THREADS / 32];
+  __shared__ c128 wdot[NB_MAX];
+  __shared__ c128 tau_s[NB_MAX];
+  __shared__ c128 gram[NB_MAX][NB_MAX];
+  __shared__ c128 scal_s;
+  __shared__ double beta_s;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  constexpr int NW = PANEL_THREADS / 32;
+
+  for (int e = tid; e < w * len; e += PANEL_THREADS) {
+    int c = e / len, i = e % len;
+    P[e] = X[(long long)(j0 + c) * rows + j0 + i];
+  }
+  // R entries above the panel rows are final already
+  for (int e = tid; e < w * j0; e += PANEL_THREADS) {
+    int c = e / j0, i = e % j0;
+    Rm[(long long)i * cols + j0 + c] = X[(long long)(j0 + c) * rows + i];
+  }
+  // zeros below the diagonal of R in these columns
+  for (int e = tid; e < w * cols; e += PANEL_THREADS) {
+    int c = e / cols, i = e % cols;
+    if (i > j0 + c) Rm[(long long)i * cols + j0 + c] = make_double2(0.0, 0.0);
+  }
+  __syncthreads();
+
+  for (int jj = 0; jj < w; jj++) {
+    c128 *x = P + (long long)jj * len;
+    // ---- reflector for x[jj..len) ----
+    double s = 0.0;
+    for (int i = jj + 1 + tid; i < len; i += PANEL_THREADS) { c128 v = x[i]; s += v.x * v.x + v.y * v.y; }
+    s = warp_sum_d(s);
+    if (lane == 0) red[warp] = s;
+    __syncthreads();
+    if (tid == 0) {
+      double xn2 = 0.0;
+      for (int i = 0; i < NW; i++) xn2 += red[i];
+      c128 alpha = x[jj];
+      c128 tau, scal;
+      double beta;
+      if (xn2 == 0.0 && alpha.y == 0.0) {
+        tau = make_double2(0.0, 0.0); scal = make_double2(0.0, 0.0); beta = alpha.x;
+      } else {
+        double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xn2);
+        beta = alpha.x >= 0.0 ? -nrm : nrm;
+        tau = make_double2((beta - alpha.x) / beta, -alpha.y / beta);
+        // scal = 1 / (alpha - beta)
+        double dr = alpha.x - beta, di = alpha.y, dn = dr * dr + di * di;
+        scal = make_double2(dr / dn, -di / dn);
+      }
+      tau_s[jj] = tau; scal_s = scal; beta_s = beta;
+    }
+    __syncthreads();
+    {
+      const c128 scal = scal_s;
+      for (int i = jj + 1 + tid; i < len; i += PANEL_THREADS) x[i] = cmul(x[i], scal);
+      if (tid == 0) {
+        Rm[(long long)(j0 + jj) * cols + j0 + jj] = make_double2(beta_s, 0.0);
+        x[jj] = make_double2(1.0, 0.0);
+      }
+      for (int i = tid; i < jj; i += PANEL_THREADS) {       // entries above the diagonal -> R, then 0
+        Rm[(long long)(j0 + i) * cols + j0 + jj] = x[i];
+        x[i] = make_double2(0.0, 0.0);
+      }
+    }
+    __syncthreads();
+    // ---- apply H^H = I - conj(tau) v v^H to the remaining panel columns ----
+    const int nrem = w - jj - 1;
+    if (nrem > 0) {
+      // each remaining column gets NW / nrem warps (at least one)
+      const int wpc = NW / nrem > 0 ? NW / nrem : 1;
+      const int cc = warp / wpc, part = warp % wpc;
+      if (warp < wpc * nrem) {
+        const c128 *y = P + (long long)(jj + 1 + cc) * len;
+        double sx = 0.0, sy = 0.0;
+        for (int i = jj + part * 32 + lane; i < len; i += wpc * 32) {
+          c128 v = x[i], u = y[i];
+          sx += v.x * u.x + v.y * u.y;
+          sy += v.x * u.y - v.y * u.x;
+        }
+        sx = warp_sum_d(sx); sy = warp_sum_d(sy);
+        if (lane == 0) { red[warp] = sx; }
+        // second array for imaginary parts: reuse gram storage rows as scratch
+        if (lane == 0) reinterpret_cast<double *>(&gram[0][0])[warp] = sy;
+      }
+      __syncthreads();
+      if (tid < nrem) {
+        double sx = 0.0, sy = 0.0;
+        for (int pz = 0; pz < wpc; pz++) {
+          sx += red[tid * wpc + pz];
+          sy += reinterpret_cast<double *>(&gram[0][0])[tid * wpc + pz];
+        }
+        // coefficient conj(tau) * (v^H y)
+        c128 ct = cconj(tau_s[jj]);
+        wdot[tid] = cmul(ct, make_double2(sx, sy));
+      }
+      __syncthreads();
+      for (int e = tid; e < nrem * (len - jj); e += PANEL_THREADS) {
+        int c2 = e / (len - jj), i = jj + e % (len - jj);
+        c128 *y = P + (long long)(jj + 1 + c2) * len;
+        c128 t = cmul(wdot[c2], x[i]);
+        y[i].x -= t.x; y[i].y -= t.y;
+      }
+      __syncthreads();
+    }
+  }
+  // ---- compact WY factor: T upper triangular with H_1...H_w = I - V T V^H ----
+  for (int pr = warp; pr < w * w; pr += NW) {
+    int a = pr / w, bq = pr % w;
+    double sx = 0.0, sy = 0.0;
+    if (a < bq) {
+      const c128 *va = P + (long long)a * len, *vb = P + (long long)bq * len;
+      for (int i = lane; i < len; i += 32) {
+        c128 v = va[i], u = vb[i];
+        sx += v.x * u.x + v.y * u.y;
+        sy += v.x * u.y - v.y * u.x;
+      }
+      sx = warp_sum_d(sx); sy = warp_sum_d(sy);
+    }
+    if (lane == 0) gram[a][bq] = make_double2(sx, sy);      // v_a^H v_b
+  }
+  __syncthreads();
+  if (tid == 0) {
+    c128 T[NB_MAX][NB_MAX];
+    for (int a = 0; a < NB_MAX; a++) for (int c = 0; c < NB_MAX; c++) T[a][c] = make_double2(0.0, 0.0);
+    for (int c = 0; c < w; c++) {
+      T[c][c] = tau_s[c];
+      // T[0:c, c] = -tau_c * T[0:c, 0:c] * (V[:, 0:c]^H v_c)
+      for (int a = 0; a < c; a++) {
+        c128 acc = make_double2(0.0, 0.0);
+        for (int q = a; q < c; q++) { c128 t = cmul(T[a][q], gram[q][c]); acc.x += t.x; acc.y += t.y; }
+        c128 t = cmul(tau_s[c], acc);
+        T[a][c] = make_double2(-t.x, -t.y);
+      }
+    }
+    for (int a = 0; a < NB_MAX; a++) for (int c = 0; c < NB_MAX; c++) Tm[a * NB_MAX + c] = T[a][c];
+  }
+  for (int e = tid; e < w * len; e += PANEL_THREADS) {
+    int c = e / len, i = e % len;
+    X[(long long)(j0 + c) * rows + j0 + i] = P[e];
+  }
+}
+
+// For columns c in [c_begin, c_end): Y[c][j0:rows) <- (I - V Top V^H) Y[c][j0:rows) with
+// Top = T (adjoint = 0) or T^H (adjoint = 1); V = X[j0 .. j0+w)[j0:rows).
+__global__ void __launch_bounds__(TRAIL_THREADS) qr_apply_kernel(const c128 *X, c128 *Y, int rows, int j0, int w,
+                                                                  const c128 *Tm, int adjoint, int c_begin, int c_end) {
+  const int len = rows - j0;
+  const int c0 = c_begin + blockIdx.x * CB;
+  const int nc = (c_end - c0) < CB ? (c_end - c0) : CB;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  constexpr int NW = TRAIL_THREADS / 32;
+  __shared__ c128 part[NW][CB][NB_MAX];
+  __shared__ c128 Wc[CB][NB_MAX];
+  c128 acc[CB][NB_MAX];
+#pragma unroll
+  for (int c = 0; c < CB; c++)
+#pragma unroll
+    for (int q = 0; q < NB_MAX; q++) acc[c][q] = make_double2(0.0, 0.0);
+  for (int i = tid; i < len; i += TRAIL_THREADS) {
+    c128 yv[CB];
+#pragma unroll
+    for (int c = 0; c < CB; c++) yv[c] = c < nc ? Y[(long long)(c0 + c) * rows + j0 + i] : make_double2(0.0, 0.0);
+#pragma unroll
+    for (int q = 0; q < NB_MAX; q++) {
+      if (q < w) {
+        c128 v = X[(long long)(j0 + q) * rows + j0 + i];
+#pragma unroll
+        for (int c = 0; c < CB; c++) {
+          acc[c][q].x += v.x * yv[c].x + v.y * yv[c].y;
+          acc[c][q].y += v.x * yv[c].y - v.y * yv[c].x;
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < CB; c++)
+#pragma unroll
+    for (int q = 0; q < NB_MAX; q++) {
+      double sx = warp_sum_d(acc[c][q].x), sy = warp_sum_d(acc[c][q].y);
+      if (lane == 0) part[warp][c][q] = make_double2(sx, sy);
+    }
+  __syncthreads();
+  if (tid < CB * NB_MAX) {
+    int c = tid / NB_MAX, q = tid % NB_MAX;
+    double sx = 0.0, sy = 0.0;
+    for (int ww = 0; ww < NW; ww++) { sx += part[ww][c][q].x; sy += part[ww][c][q].y; }
+    part[0][c][q] = make_double2(sx, sy);               // V^H y
+  }
+  __syncthreads();
+  if (tid < CB * NB_MAX) {
+    int c = tid / NB_MAX, q = tid % NB_MAX;
+    c128 s = make_double2(0.0, 0.0);
+    if (q < w) {
+      for (int r = 0; r < w; r++) {
+        c128 t = adjoint ? cconj(Tm[r * NB_MAX + q]) : Tm[q * NB_MAX + r];
+        c128 pr = cmul(t, part[0][c][r]);
+        s.x += pr.x; s.y += pr.y;
+      }
+    }
+    Wc[c][q] = s;
+  }
+  __syncthreads();
+  for (int i = tid; i < len; i += TRAIL_THREADS) {
+    c128 d[CB];
+#pragma unroll
+    for (int c = 0; c < CB; c++) d[c] = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int q = 0; q < NB_MAX; q++) {
+      if (q < w) {
+        c128 v = X[(long long)(j0 + q) * rows + j0 + i];
+#pragma unroll
+        for (int c = 0; c < CB; c++) { c128 t = cmul(v, Wc[c][q]); d[c].x += t.x; d[c].y += t.y; }
+      }
+    }
+#pragma unroll
+    for (int c = 0; c < CB; c++)
+      if (c < nc) {
+        c128 *dst = Y + (long long)(c0 + c) * rows + j0 + i;
+        c128 o = *dst;
+        *dst = make_double2(o.x - d[c].x, o.y - d[c].y);
+      }
+  }
+}
+
+int panel_width(int rows) {
+  long long budget = 200 * 1024;
+  int nb = (int)(budget / ((long long)rows * 16));
+  if (nb > NB_MAX) nb = NB_MAX;
+  return nb;
+}
+
+}  // namespace
+
+void qr_configure() {
+  cudaFuncSetAttribute(qr_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024 + 1024);
+}
+
+size_t qr_ws_bytes(int rows, int cols) {
+  size_t mat = up256((size_t)rows * cols * 16);
+  int nb = panel_width(rows);
+  if (nb < 1) nb = 1;
+  size_t npanels = (cols + nb - 1) / nb;
+  return 2 * mat + up256((size_t)cols * cols * 16) + up256(npanels * NB_MAX * NB_MAX * 16) + 512;
+}
+
+void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c128 *Q, c128 *D, void *ws) {
+  const int rows = side == 0 ? Ml * d : d * Mr;
+  const int cols = side == 0 ? Mr : Ml;
+  const int nb = panel_width(rows);
+  char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
+  size_t mat = up256((size_t)rows * cols * 16);
+  c128 *X = reinterpret_cast<c128 *>(p); p += mat;
+  c128 *Y = reinterpret_cast<c128 *>(p); p += mat;
+  c128 *Rm = reinterpret_cast<c128 *>(p); p += up256((size_t)cols * cols * 16);
+  c128 *Tm = reinterpret_cast<c128 *>(p);
+  const long long n = (long long)rows * cols;
+  const int gcopy = (int)((n + 255) / 256 > 592 ? 592 : (n + 255) / 256);
+  dim3 tb(32, 8), tg((cols + 31) / 32, (rows + 31) / 32);
+  if (side == 0) TDVP_LAUNCH(transpose_in_kernel, tg, tb, 0, st, C, X, rows, cols);
+  else TDVP_LAUNCH(copy_kernel, gcopy, 256, 0, st, X, C, n);
+  const int npanels = (cols + nb - 1) / nb;
+  for (int pz = 0; pz < npanels; pz++) {
+    int j0 = pz * nb, w = cols - j0 < nb ? cols - j0 : nb;
+    size_t smem = (size_t)w * (rows - j0) * 16;
+    TDVP_LAUNCH(qr_panel_kernel, 1, PANEL_THREADS, smem, st, X, rows, cols, j0, w, Rm, Tm + (size_t)pz * NB_MAX * NB_MAX);
+    int c_begin = j0 + w;
+    if (c_begin < cols)
+      TDVP_LAUNCH(qr_apply_kernel, (cols - c_begin + CB - 1) / CB, TRAIL_THREADS, 0, st, X, X, rows, j0, w,
+                  Tm + (size_t)pz * NB_MAX * NB_MAX, 1, c_begin, cols);
+  }
+  TDVP_LAUNCH(identity_kernel, gcopy, 256, 0, st, Y, rows, cols);
+  for (int pz = npanels - 1; pz >= 0; pz--) {
+    int j0 = pz * nb, w = cols - j0 < nb ? cols - j0 : nb;
+    TDVP_LAUNCH(qr_apply_kernel, (cols - j0 + CB - 1) / CB, TRAIL_THREADS, 0, st, X, Y, rows, j0, w,
+                Tm + (size_t)pz * NB_MAX * NB_MAX, 0, j0, cols);
+  }
+  if (side == 0) TDVP_LAUNCH(transpose_out_kernel, tg, tb, 0, st, Y, Q, rows, cols);
+  else TDVP_LAUNCH(copy_kernel, gcopy, 256, 0, st, Q, Y, n);
+  TDVP_LAUNCH(store_d_kernel, (cols * cols + 255) / 256 > 296 ? 296 : (cols * cols + 255) / 256, 256, 0, st, Rm, D, cols, side);
+}

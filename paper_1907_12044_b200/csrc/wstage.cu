@@ -1,0 +1,168 @@
+// wstage.cu -- the MPO ("W") stage of H_eff / environment updates as a sparse-aware contraction
+// (the M_S^2 M_O^2 d^2 term of Table I, with the zeros of W
+// skipped: vibronic MPO tensors are ~3 % dense, Eq. 45 / SURVEY.md 8(c) c3).
+//
+// For every bond-index pair the stage is a sparse (rows x cols) matrix applied to a dense
+// cols x Mr panel whose rows are contiguous in y.  One CTA owns (batch index a, 32 consecutive y):
+// it stages the panel T1[a, :, y0:y0+32] in shared memory with 16 B cp.async copies, then each
+// warp produces output rows r = warp, warp + 8, ... with lane = y (coalesced 512 B row writes,
+// conflict-free LDS.128), walking the row's CSR entries (warp-uniform loads).  HBM/L2 traffic is
+// exactly one read of T1 and one write of T2.
+#include "common.cuh"
+
+namespace {
+
+constexpr int YT = 32;          // y per CTA (one lane each)
+constexpr int WS_THREADS = 256;
+
+// Build CSR of the (nrows x ncols) matrix view of W.  which = 0: rows (s,v), cols (w,t) ["left"];
+// which = 1: rows (w,s), cols (t,v) ["right"].
+__global__ void csr_build_kernel(const c128 *W, int Dl, int d, int Dr, double tol,
+                                 int *rowptr0, int *col0, c128 *val0,
+                                 int *rowptr1, int *col1, c128 *val1) {
+  extern __shared__ int counts[];
+  const int which = blockIdx.x;
+  const int nrows = which == 0 ? d * Dr : Dl * d;
+  const int ncols = which == 0 ? Dl * d : d * Dr;
+  int *rowptr = which == 0 ? rowptr0 : rowptr1;
+  int *col = which == 0 ? col0 : col1;
+  c128 *val = which == 0 ? val0 : val1;
+  auto widx = [&](int r, int c) -> long long {
+    if (which == 0) { int s = r / Dr, v = r % Dr, w = c / d, t = c % d;
+                      return (((long long)w * d + s) * d + t) * Dr + v; }
+    return (long long)r * ncols + c;
+  };
+  for (int r = threadIdx.x; r < nrows; r += blockDim.x) {
+    int n = 0;
+    for (int c = 0; c < ncols; c++) {
+      c128 x = W[widx(r, c)];
+      n += (fabs(x.x) > tol || fabs(x.y) > tol) ? 1 : 0;
+    }
+    counts[r] = n;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int acc = 0;
+    for (int r = 0; r < nrows; r++) { int n = counts[r]; counts[r] = acc; rowptr[r] = acc; acc += n; }
+    rowptr[nrows] = acc;
+  }
+  __syncthreads();
+  for (int r = threadIdx.x; r < nrows; r += blockDim.x) {
+    int o = counts[r];
+    for (int c = 0; c < ncols; c++) {
+      c128 x = W[widx(r, c)];
+      if (fabs(x.x) > tol || fabs(x.y) > tol) { col[o] = c; val[o] = x; o++; }
+    }
+  }
+}
+
+struct WStageParams {
+  const c128 *in; c128 *out;
+  int nrows, ncols, Mr;
+  long long in_bs;                 // input batch stride (per a); input row stride is Mr
+  int rdiv; long long o_s1, o_s2;  // output offset of row r: (r / rdiv) * o_s1 + (r % rdiv) * o_s2
+  long long o_bs;                  // output batch stride
+  const int *rowptr; const int *col; const c128 *val;
+};
+
+template <bool STAGE_SMEM>
+__global__ void __launch_bounds__(WS_THREADS) wstage_kernel(WStageParams p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  c128 *tile = reinterpret_cast<c128 *>(smem_raw);      // [ncols][YT]
+  const int a = blockIdx.y;
+  const int y0 = blockIdx.x * YT;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const c128 *in = p.in + a * p.in_bs;
+  const int y = y0 + lane;
+  const bool yok = y < p.Mr;
+  if (STAGE_SMEM) {
+    for (int e = threadIdx.x; e < p.ncols * YT; e += WS_THREADS) {
+      int c = e / YT, yy = e % YT;
+      bool ok = (y0 + yy) < p.Mr;
+      const c128 *src = ok ? in + (long long)c * p.Mr + y0 + yy : in;
+      unsigned s = (unsigned)__cvta_generic_to_shared(tile + e);
+      int sz = ok ? 16 : 0;
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(src), "r"(sz));
+    }
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::);
+    __syncthreads();
+  }
+  c128 *out = p.out + a * p.o_bs;
+  for (int r = warp; r < p.nrows; r += WS_THREADS / 32) {
+    const int e0 = p.rowptr[r], e1 = p.rowptr[r + 1];
+    double sx = 0.0, sy = 0.0;
+    for (int e = e0; e < e1; e++) {
+      const int c = __ldg(p.col + e);
+      const c128 w = __ldg(p.val + e);
+      c128 t;
+      if (STAGE_SMEM) t = tile[c * YT + lane];
+      else t = yok ? __ldg(in + (long long)c * p.Mr + y) : make_double2(0.0, 0.0);
+      sx = fma(w.x, t.x, sx); sx = fma(-w.y, t.y, sx);
+      sy = fma(w.x, t.y, sy); sy = fma(w.y, t.x, sy);
+    }
+    if (yok) out[(r / p.rdiv) * p.o_s1 + (r % p.rdiv) * p.o_s2 + y] = make_double2(sx, sy);
+  }
+}
+
+void launch_wstage(cudaStream_t st, const WStageParams &p, int nbatch) {
+  dim3 grid((p.Mr + YT - 1) / YT, nbatch);
+  size_t smem = (size_t)p.ncols * YT * 16;
+  if (smem <= 200 * 1024) {
+    TDVP_LAUNCH(wstage_kernel<true>, grid, WS_THREADS, smem, st, p);
+  } else {
+    TDVP_LAUNCH(wstage_kernel<false>, grid, WS_THREADS, 0, st, p);
+  }
+}
+
+}  // namespace
+
+void wstage_configure() {
+  cudaFuncSetAttribute(wstage_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+}
+
+size_t wsparse_bytes(int Dl, int d, int Dr) {
+  size_t cap = (size_t)Dl * d * d * Dr;
+  size_t rows0 = (size_t)d * Dr + 1, rows1 = (size_t)Dl * d + 1;
+  auto up = [](size_t x) { return (x + 255) & ~size_t(255); };
+  return up(rows0 * 4) + up(rows1 * 4) + 2 * up(cap * 4) + 2 * up(cap * 16) + 256;
+}
+
+void wsparse_build(cudaStream_t st, WSparse &ws, void *mem, int Dl, int d, int Dr, const c128 *W,
+                   double zero_tol) {
+  size_t cap = (size_t)Dl * d * d * Dr;
+  auto up = [](size_t x) { return (x + 255) & ~size_t(255); };
+  char *p = reinterpret_cast<char *>(mem);
+  p = reinterpret_cast<char *>(up(reinterpret_cast<size_t>(p)));
+  ws.Dl = Dl; ws.d = d; ws.Dr = Dr; ws.capacity = (int)cap;
+  ws.val = reinterpret_cast<c128 *>(p); p += up(cap * 16);
+  ws.val_r = reinterpret_cast<c128 *>(p); p += up(cap * 16);
+  ws.col = reinterpret_cast<int *>(p); p += up(cap * 4);
+  ws.col_r = reinterpret_cast<int *>(p); p += up(cap * 4);
+  ws.rowptr = reinterpret_cast<int *>(p); p += up(((size_t)d * Dr + 1) * 4);
+  ws.rowptr_r = reinterpret_cast<int *>(p);
+  int maxrows = (d * Dr > Dl * d ? d * Dr : Dl * d);
+  TDVP_LAUNCH(csr_build_kernel, 2, 256, maxrows * sizeof(int), st, W, Dl, d, Dr, zero_tol,
+              ws.rowptr, ws.col, ws.val, ws.rowptr_r, ws.col_r, ws.val_r);
+}
+
+void wstage_left(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2) {
+  WStageParams p;
+  p.in = T1; p.out = T2;
+  p.nrows = ws.d * ws.Dr; p.ncols = ws.Dl * ws.d; p.Mr = Mr;
+  p.in_bs = (long long)ws.Dl * ws.d * Mr;
+  p.rdiv = p.nrows > 0 ? p.nrows : 1; p.o_s1 = 0; p.o_s2 = Mr;
+  p.o_bs = (long long)ws.d * ws.Dr * Mr;
+  p.rowptr = ws.rowptr; p.col = ws.col; p.val = ws.val;
+  launch_wstage(st, p, Ml);
+}
+
+void wstage_right(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2) {
+  WStageParams p;
+  p.in = T1; p.out = T2;
+  p.nrows = ws.Dl * ws.d; p.ncols = ws.d * ws.Dr; p.Mr = Mr;
+  p.in_bs = (long long)ws.d * ws.Dr * Mr;
+  p.rdiv = ws.d; p.o_s1 = (long long)Ml * ws.d * Mr; p.o_s2 = Mr;
+  p.o_bs = (long long)ws.d * Mr;
+  p.rowptr = ws.rowptr_r; p.col = ws.col_r; p.val = ws.val_r;
+  launch_wstage(st, p, Ml);
+}
