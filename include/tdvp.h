@@ -92,6 +92,13 @@ int tdvp_apply_heff(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr,
                     const tdvp_c128 *A /*DEVICE [Ml,d,Mr]*/,  const tdvp_c128 *R /*DEVICE [Mr,Dr,Mr]*/,
                     tdvp_c128 *out /*DEVICE [Ml,d,Mr]*/);
 
+/* Same operation with HOST buffers (all five pointers HOST, pageable or pinned): copies L, W, A, R
+   to the device on the handle's stream, applies H[i], copies `out` back and BLOCKS until it has
+   arrived.  This is the end-to-end entry bench.py times (h2d + kernels + d2h). */
+int tdvp_apply_heff_host(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr,
+                         const tdvp_c128 *L, const tdvp_c128 *W, const tdvp_c128 *A,
+                         const tdvp_c128 *R, tdvp_c128 *out);
+
 /* Environment update (Eq. 30-32).
    side = 0: env_in = L[Ml,Dl,Ml], env_out = L'[b,v,y] = sum conj(A[a,s,b]) L[a,w,x] W[w,s,t,v] A[x,t,y]   ([Mr,Dr,Mr])
    side = 1: env_in = R[Mr,Dr,Mr], env_out = R'[a,w,x] = sum conj(A[a,s,b]) W[w,s,t,v] A[x,t,y] R[b,v,y]   ([Ml,Dl,Ml]) */
@@ -129,6 +136,15 @@ int tdvp_expm_bond(tdvp_handle *h, int Ml, int Mr, int Dw,
 int tdvp_qr_gauge(tdvp_handle *h, int side, int Ml, int d, int Mr,
                   const tdvp_c128 *C /*DEVICE*/, tdvp_c128 *Q /*DEVICE*/, tdvp_c128 *D /*DEVICE*/);
 
+/* Matrix unfolding of a bond (Eq. 36): C[Ml,d,Mr] viewed as Ml x (d*Mr) with
+   Ml <= d*Mr is factored as U diag(lam) Vh on the device (Householder QR of C^T, then one-sided
+   Jacobi on the Ml x Ml triangular factor).  U: DEVICE [Ml,Ml] unitary; lam: DEVICE double[Ml],
+   non-negative, descending; Vh: DEVICE [Ml,d,Mr] with orthonormal rows (a right-canonical site,
+   Eq. 8).  Singular vectors are unique only up to phases / rotations inside degenerate
+   subspaces; the product is exact. */
+int tdvp_svd_bond(tdvp_handle *h, int Ml, int d, int Mr, const tdvp_c128 *C /*DEVICE*/,
+                  tdvp_c128 *U /*DEVICE*/, double *lam /*DEVICE*/, tdvp_c128 *Vh /*DEVICE*/);
+
 /* ---- stateful calls on the handle's resident MPS / environment cache ---------------------- */
 
 /* H[site] applied to A_dev using the cached L[site], R[site] (valid when the gauge centre is at
@@ -150,6 +166,11 @@ int tdvp_step_ps(tdvp_handle *h, double dt);
    err_est: HOST, nullable; if non-NULL the call blocks and returns the Euclidean norm of the
    embedded (5th - 4th order) difference. */
 int tdvp_step_mu(tdvp_handle *h, double dt, double *err_est);
+
+/* One evaluation of the TDVP-MU right-hand side (Eq. 27 and Eq. 37-38) on the resident MPS, which
+   must be in the MU gauge (centre N-1; else TDVP_ESTATE).  out_host[N]: HOST pointers to HOST
+   buffers [Ml_i, d_i, Mr_i] receiving dL_i/dt (i < N-1) and dC_N/dt.  Blocks on the stream. */
+int tdvp_mu_derivative(tdvp_handle *h, tdvp_c128 *const *out_host);
 
 /* Move the gauge centre by QR / RQ sweeps without time evolution and rebuild the environment
    cache: centre = 0 (PS gauge) or centre = N-1 (MU gauge). */

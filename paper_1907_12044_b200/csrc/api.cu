@@ -116,6 +116,36 @@ int tdvp_apply_heff(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr, const
   return check_cuda(h, cudaGetLastError(), "tdvp_apply_heff");
 }
 
+int tdvp_apply_heff_host(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr, const tdvp_c128 *L,
+                         const tdvp_c128 *W, const tdvp_c128 *A, const tdvp_c128 *R, tdvp_c128 *out) {
+  tdvp_handle *hh = h ? h : default_handle();
+  if (!L || !W || !A || !R || !out) return set_err(h, TDVP_EINVAL, "null pointer");
+  if (int rc = bad_dims(h, Ml, Mr, d, Dl, Dr)) return rc;
+  const size_t nL = (size_t)Ml * Dl * Ml * 16, nW = (size_t)Dl * d * d * Dr * 16, nA = (size_t)Ml * d * Mr * 16,
+               nR = (size_t)Mr * Dr * Mr * 16;
+  auto up = [](size_t x) { return (x + 255) & ~size_t(255); };
+  size_t wb = wsparse_bytes(Dl, d, Dr), hb = heff_ws_bytes(Ml, Mr, d, Dl, Dr);
+  size_t io = up(nL) + up(nW) + 2 * up(nA) + up(nR);
+  if (int rc = check_cuda(h, hh->arena.reserve(io + wb + hb + 4096, hh->stream), "workspace")) return rc;
+  hh->arena.reset();
+  c128 *dL = reinterpret_cast<c128 *>(hh->arena.take(nL)), *dW = reinterpret_cast<c128 *>(hh->arena.take(nW));
+  c128 *dA = reinterpret_cast<c128 *>(hh->arena.take(nA)), *dR = reinterpret_cast<c128 *>(hh->arena.take(nR));
+  c128 *dO = reinterpret_cast<c128 *>(hh->arena.take(nA));
+  void *wmem = hh->arena.take(wb);
+  void *ws = hh->arena.take(hb);
+  cudaStream_t st = hh->stream;
+  if (int rc = check_cuda(h, cudaMemcpyAsync(dL, L, nL, cudaMemcpyHostToDevice, st), "h2d L")) return rc;
+  if (int rc = check_cuda(h, cudaMemcpyAsync(dW, W, nW, cudaMemcpyHostToDevice, st), "h2d W")) return rc;
+  if (int rc = check_cuda(h, cudaMemcpyAsync(dA, A, nA, cudaMemcpyHostToDevice, st), "h2d A")) return rc;
+  if (int rc = check_cuda(h, cudaMemcpyAsync(dR, R, nR, cudaMemcpyHostToDevice, st), "h2d R")) return rc;
+  WSparse wsp;
+  wsparse_build(st, wsp, wmem, Dl, d, Dr, dW, hh->opt.w_zero_tol);
+  heff_apply(st, Ml, Mr, d, Dl, Dr, dL, wsp, dA, dR, dO, ws);
+  if (int rc = check_cuda(h, cudaGetLastError(), "tdvp_apply_heff_host")) return rc;
+  if (int rc = check_cuda(h, cudaMemcpyAsync(out, dO, nA, cudaMemcpyDeviceToHost, st), "d2h out")) return rc;
+  return check_cuda(h, cudaStreamSynchronize(st), "tdvp_apply_heff_host sync");
+}
+
 int tdvp_update_env(tdvp_handle *h, int side, int Ml, int Mr, int d, int Dl, int Dr,
                     const tdvp_c128 *env_in, const tdvp_c128 *W, const tdvp_c128 *A,
                     tdvp_c128 *env_out) {

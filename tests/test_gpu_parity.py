@@ -1,0 +1,284 @@
+"""Parity of the CUDA path (through the C ABI of include/tdvp.h) against oracle/ on the same seeded
+inputs.  Tolerances (BASELINE.json north_star): relative Frobenius error <= 1e-11 for one complex128
+contraction; site populations within 1e-8 absolute after 20 steps."""
+import dataclasses
+import os
+
+import numpy as np
+import pytest
+
+import synthetic_inputs as si
+from oracle import contractions as oc
+from oracle import lanczos, model, observables as obs, tdvp_ps
+
+pytestmark = pytest.mark.gpu
+
+REL_TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def T():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1907_12044_b200 as t
+    t.library_path()
+    return t
+
+
+def dev(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def host(x):
+    return x.cpu().numpy()
+
+
+def rel(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+# ---- single contractions --------------------------------------------------------------------
+SITE_CASES = [
+    # Ml, Mr, d, Dl, Dr, density
+    (1, 3, 3, 1, 5, 0.5),        # left chain end
+    (3, 1, 4, 4, 1, 0.5),        # right chain end
+    (1, 1, 2, 1, 1, 1.0),        # degenerate 1-site chain
+    (12, 16, 4, 5, 4, 0.3),
+    (37, 29, 5, 7, 3, 0.2),      # ragged, several tiles with tails
+    (64, 64, 10, 9, 9, 0.04),    # real-MPO-like density
+    (70, 130, 3, 6, 11, 0.15),   # more than one 64-tile in both bonds, ragged
+]
+
+
+@pytest.mark.parametrize("case", SITE_CASES)
+def test_apply_heff_ragged(T, case):
+    Ml, Mr, d, Dl, Dr, dens = case
+    L, W, A, R = si.random_site_problem(Ml, Mr, d, Dl, Dr, dens, seed=100 + Ml + Mr)
+    want = oc.heff_definition(L, W, A, R) if Ml * Mr <= 600 else oc.heff(L, W, A, R)
+    got = host(T.tdvp_apply_heff(dev(L), dev(W), dev(A), dev(R)))
+    assert rel(got, want) <= REL_TOL
+
+
+@pytest.mark.parametrize("M", [32, 64, 128])
+def test_apply_heff_microbench_config(T, M):
+    """BASELINE.json configs[1]: d = 10, D_W = 20, 6000 non-zeros of W."""
+    L, W, A, R = si.microbench_tensors(M)
+    want = oc.heff(L, W, A, R)
+    got = host(T.tdvp_apply_heff(dev(L), dev(W), dev(A), dev(R)))
+    assert rel(got, want) <= REL_TOL
+
+
+def test_apply_heff_host_entry(T):
+    L, W, A, R = si.microbench_tensors(32)
+    out = np.empty_like(A)
+    T.tdvp_apply_heff_host(L, W, A, R, out)
+    assert rel(out, oc.heff(L, W, A, R)) <= REL_TOL
+
+
+@pytest.mark.parametrize("case", SITE_CASES)
+@pytest.mark.parametrize("side", [0, 1])
+def test_update_env_ragged(T, case, side):
+    Ml, Mr, d, Dl, Dr, dens = case
+    L, W, A, R = si.random_site_problem(Ml, Mr, d, Dl, Dr, dens, seed=200 + Ml + Mr)
+    if side == 0:
+        want = oc.envL(L, W, A)
+        got = host(T.tdvp_update_env(0, dev(L), dev(W), dev(A)))
+    else:
+        want = oc.envR(R, W, A)
+        got = host(T.tdvp_update_env(1, dev(R), dev(W), dev(A)))
+    assert got.shape == want.shape
+    assert rel(got, want) <= REL_TOL
+
+
+@pytest.mark.parametrize("M", [32, 128])
+def test_update_env_microbench_config(T, M):
+    L, W, A, R = si.microbench_tensors(M)
+    assert rel(host(T.tdvp_update_env(0, dev(L), dev(W), dev(A))), oc.envL(L, W, A)) <= REL_TOL
+    assert rel(host(T.tdvp_update_env(1, dev(R), dev(W), dev(A))), oc.envR(R, W, A)) <= REL_TOL
+
+
+@pytest.mark.parametrize("dims", [(1, 1, 1), (5, 3, 4), (40, 72, 9), (128, 128, 20)])
+def test_apply_bond(T, dims):
+    Ml, Mr, Dw = dims
+    rng = np.random.default_rng(300 + Ml)
+    L = si.complex_normal(rng, (Ml, Dw, Ml))
+    R = si.complex_normal(rng, (Mr, Dw, Mr))
+    D = si.complex_normal(rng, (Ml, Mr))
+    got = host(T.tdvp_apply_bond(dev(L), dev(D), dev(R)))
+    assert rel(got, oc.bond(L, D, R)) <= REL_TOL
+
+
+# ---- QR gauge move (Eq. 9) ------------------------------------------------------------------
+@pytest.mark.parametrize("shape", [(1, 3, 3), (3, 4, 12), (16, 4, 16), (37, 5, 29), (64, 10, 64), (130, 3, 70)])
+@pytest.mark.parametrize("side", [0, 1])
+def test_qr_gauge(T, shape, side):
+    Ml, d, Mr = shape
+    if side == 0 and Ml * d < Mr:
+        pytest.skip("not tall")
+    if side == 1 and d * Mr < Ml:
+        pytest.skip("not tall")
+    rng = np.random.default_rng(400 + Ml + Mr)
+    C = si.complex_normal(rng, shape)
+    # make it numerically rank deficient like a padded centre: scale trailing columns / rows down
+    if side == 0:
+        C = C * np.logspace(0, -9, Mr)[None, None, :]
+    else:
+        C = C * np.logspace(0, -9, Ml)[:, None, None]
+    Q, D = T.tdvp_qr_gauge(side, dev(C))
+    Q, D = host(Q), host(D)
+    if side == 0:
+        Qm = Q.reshape(Ml * d, Mr)
+        assert np.abs(Qm.conj().T @ Qm - np.eye(Mr)).max() < 1e-13 * max(Mr, 8)      # Eq. 7
+        assert rel((Qm @ D).reshape(shape), C) < 1e-13
+    else:
+        Qm = Q.reshape(Ml, d * Mr)
+        assert np.abs(Qm @ Qm.conj().T - np.eye(Ml)).max() < 1e-13 * max(Ml, 8)      # Eq. 8
+        assert rel((D @ Qm).reshape(shape), C) < 1e-13
+
+
+# ---- Lanczos exponential on a Hermitian H_eff of a real chain ---------------------------------
+def _tiny_state(n_warm=1):
+    cfg = si.CONFIGS["tiny"]
+    params = si.draw_vibronic_params(cfg)
+    mpo = model.build_mpo(params)
+    mps = si.padded_product_mps(si.site_dims(params), si.initial_occupations(params), cfg.M, cfg.pad_seed)
+    st = tdvp_ps.PSState(mpo, mps)
+    for _ in range(n_warm):
+        tdvp_ps.step_ps(st, cfg.dt_fs, cfg.krylov_dim)
+    return cfg, mpo, st
+
+
+def test_expm_heff_and_bond(T):
+    cfg, mpo, st = _tiny_state()
+    # move the centre two sites to the right by hand so that L and R are both non-trivial
+    for i in range(2):
+        C = st.mps[i]
+        Ml, d, Mr = C.shape
+        Q, D = np.linalg.qr(C.reshape(Ml * d, Mr))
+        st.mps[i] = Q.reshape(Ml, d, Mr)
+        st.Lenv[i + 1] = oc.envL(st.Lenv[i], mpo[i], st.mps[i])
+        st.mps[i + 1] = np.einsum("ab,bsc->asc", D, st.mps[i + 1])
+    i = 2
+    L, W, R, v = st.Lenv[i], mpo[i], st.Renv[i], st.mps[i]
+    for k in (10, 4):
+        ctx = T.tdvp_create_context(T.make_options(krylov_dim=k))
+        z = -0.5j * cfg.dt_fs
+        want, m = lanczos.lanczos_expm(lambda x: oc.heff(L, W, x, R), v, z, k)
+        got, mg = T.tdvp_expm_heff(dev(L), dev(W), dev(R), z, dev(v), handle=ctx, want_dim=True)
+        assert mg == m
+        assert rel(host(got), want) <= REL_TOL
+        # bond operator between sites 1 and 2
+        Lb, Rb = st.Lenv[2], st.Renv[1]
+        rng = np.random.default_rng(5)
+        Dm = si.complex_normal(rng, (Lb.shape[0], Rb.shape[0]))
+        want, m = lanczos.lanczos_expm(lambda x: oc.bond(Lb, x, Rb), Dm, -z, k)
+        got, mg = T.tdvp_expm_bond(dev(Lb), dev(Rb), -z, dev(Dm), handle=ctx, want_dim=True)
+        assert mg == m
+        assert rel(host(got), want) <= REL_TOL
+        ctx.close()
+
+
+def test_expm_breakdown_small_space(T):
+    """Krylov space exhausted (1-dimensional bond at a chain end): m < k on both sides."""
+    cfg, mpo, st = _tiny_state(0)
+    L, W, R, v = st.Lenv[0], mpo[0], st.Renv[0], st.mps[0]       # dimension 1*3*3 = 9 < k = 10
+    z = -0.5j * cfg.dt_fs
+    want, m = lanczos.lanczos_expm(lambda x: oc.heff(L, W, x, R), v, z, 10)
+    got, mg = T.tdvp_expm_heff(dev(L), dev(W), dev(R), z, dev(v), want_dim=True)
+    assert mg == m and m < 10
+    assert rel(host(got), want) <= 1e-10
+
+
+# ---- whole trajectories ---------------------------------------------------------------------
+@pytest.mark.parametrize("graph", [True, False])
+def test_tiny_chain_20_steps(T, graph):
+    """BASELINE.json configs[0]: populations within 1e-8 of the oracle after each of 20 steps."""
+    cfg = si.CONFIGS["tiny"]
+    params = si.draw_vibronic_params(cfg)
+    mpo = model.build_mpo(params)
+    mps = si.padded_product_mps(si.site_dims(params), si.initial_occupations(params), cfg.M, cfg.pad_seed)
+    golden = np.loadtxt(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "tiny_ps_populations.txt"))
+    ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=cfg.krylov_dim, flags=0 if graph else T.TDVP_FLAG_NO_GRAPH))
+    n0, e0 = ch.tdvp_norm_energy()
+    assert abs(n0 - 1.0) < 1e-12
+    assert abs(e0 - obs.energy(mpo, mps)) < 1e-12 * max(1.0, abs(e0))
+    worst = 0.0
+    for s in range(cfg.n_steps):
+        ch.tdvp_step_ps(cfg.dt_fs)
+        p = ch.tdvp_populations(0)
+        worst = max(worst, np.abs(p - golden[s]).max())
+    assert worst <= 1e-8
+    n1, e1 = ch.tdvp_norm_energy()
+    assert abs(n1 - 1.0) < 1e-11 and abs(e1 - e0) < 1e-11 * max(1.0, abs(e0))
+    assert ch.tdvp_get_centre() == 0
+    ch.close()
+
+
+def test_fmo_like_chain_delta_seeded(T):
+    """A short FMO-like chain (layout A, d = 10 phonon sites) at M = 12, delta-seeded start
+    (SURVEY.md 8(c) c8): free-running parity over 4 steps, plus observables."""
+    cfg = dataclasses.replace(si.CONFIGS["fmo64"], n_el=4, n_modes=2, n_ph=6, M=12, dt_fs=5.0)
+    params = si.draw_vibronic_params(cfg)
+    mpo = model.build_mpo(params)
+    dims = si.site_dims(params)
+    mps = si.padded_product_mps(dims, si.initial_occupations(params), cfg.M, cfg.pad_seed, cfg.delta, cfg.delta_seed)
+    st = tdvp_ps.PSState(mpo, mps)
+    ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=cfg.krylov_dim))
+    for s in range(4):
+        tdvp_ps.step_ps(st, cfg.dt_fs, cfg.krylov_dim)
+        ch.tdvp_step_ps(cfg.dt_fs)
+        assert np.abs(ch.tdvp_populations(0) - obs.populations(st.mps, 0)).max() <= 1e-8
+    # a phonon-site observable: <n> at site 3 through tdvp_observe
+    num = np.diag(np.arange(dims[3], dtype=np.float64)).astype(np.complex128)
+    want = np.trace(num @ obs.one_site_rdm(st.mps, 3))
+    assert abs(ch.tdvp_observe(3, num) - want) <= 1e-8
+    # state overlap |<psi_oracle|psi_gpu>| = 1 (gauge invariant)
+    got = ch.tdvp_get_mps()
+    E = np.ones((1, 1), dtype=np.complex128)
+    for A, B in zip(st.mps, got):
+        E = np.einsum("ax,asb,xsy->by", E, A.conj(), B)
+    assert abs(abs(E[0, 0]) - 1.0) <= 1e-9
+    ch.close()
+
+
+def test_teacher_forced_step(T):
+    """tdvp_set_mps with the oracle's tensors, one step, compare."""
+    cfg, mpo, st = _tiny_state(3)
+    ch = T.tdvp_create(mpo, st.mps, T.make_options(krylov_dim=cfg.krylov_dim))
+    for _ in range(2):
+        ch.tdvp_set_mps(st.mps, 0)
+        tdvp_ps.step_ps(st, cfg.dt_fs, cfg.krylov_dim)
+        ch.tdvp_step_ps(cfg.dt_fs)
+        assert np.abs(ch.tdvp_populations(0) - obs.populations(st.mps, 0)).max() <= 1e-10
+    ch.close()
+
+
+def test_gauge_sweep_and_site_calls(T):
+    cfg, mpo, st = _tiny_state(2)
+    ch = T.tdvp_create(mpo, st.mps)
+    p0 = ch.tdvp_populations(0)
+    n0, e0 = ch.tdvp_norm_energy()
+    ch.tdvp_set_gauge(ch.n - 1)
+    assert ch.tdvp_get_centre() == ch.n - 1
+    assert np.abs(ch.tdvp_populations(0) - p0).max() < 1e-12
+    n1, e1 = ch.tdvp_norm_energy()
+    assert abs(n1 - n0) < 1e-12 and abs(e1 - e0) < 1e-12 * max(1, abs(e0))
+    # energy = <C, H_eff C> at the centre
+    C = ch.tdvp_get_mps(ch.n - 1)
+    HC = host(ch.tdvp_apply_heff_site(ch.n - 1, dev(C)))
+    assert abs(np.vdot(C, HC).real - e0) < 1e-11 * max(1, abs(e0))
+    ch.tdvp_set_gauge(0)
+    assert np.abs(ch.tdvp_populations(0) - p0).max() < 1e-12
+    ch.close()
+
+
+def test_errors_are_reported(T):
+    with pytest.raises(T.TdvpError):
+        T.make_options(krylov_dim=0) and T.tdvp_create_context(T.make_options(krylov_dim=0))
+    cfg, mpo, st = _tiny_state(0)
+    bad = [A.copy() for A in st.mps]
+    bad[3] = bad[3] * 1.5                               # not right-canonical
+    with pytest.raises(T.TdvpError):
+        T.tdvp_create(mpo, bad)
