@@ -1,0 +1,386 @@
+"""bench.py -- headline benchmark of the B200-native TDVP hot path (BASELINE.json metric:
+"H_eff.A applies/s and TDVP-PS step time at M=128; % FP64 tensor-core peak").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+One "step" = APPLIES_PER_STEP H_eff applies of BASELINE.json configs[1] at
+M = 128 (d = 10, D_W = 20, 6000 non-zeros of W), each on the next of N_SETS resident input sets
+(total > L2, so L, A, R are L2-cold), through the C ABI (tdvp_apply_heff).  `value` = applies/s with
+inputs resident in HBM; `e2e` = the same through tdvp_apply_heff_host (HOST buffers, h2d + d2h
+inside the timed region).  Also reported on the same JSON line: the M sweep, the environment update
+(a4), one TDVP-PS step (a5-a8, a10) of the M = 128 FMO-like chain (configs[3]), the roofline of the
+dominant kernel (DMMA complex GEMM) from live CUDA-event brackets, and the oracle timed on the
+host cores (cpu_baseline).  Multi-GPU: the path does not shard -- "replicas only":
+every rank runs the same workload, `value` is the sum over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import synthetic_inputs as si  # noqa: E402
+
+M_HEADLINE, D_PHYS, D_W, NNZ = 128, 10, 20, 6000
+APPLIES_PER_STEP = 24
+N_SETS = 12                      # 12 x (L 5.2 + A 2.6 + R 5.2 + out 2.6 MB) = 188 MB > 126 MB L2
+METRIC, UNIT = "heff_applies_per_s_M128", "applies/s"
+WORKLOAD = "configs[1]: isolated H_eff.A, complex128, M=128, d=10, D_W=20, W 15% dense (6000 nnz)"
+
+
+def heff_flops(M, d=D_PHYS, Dw=D_W, nnz=NNZ):
+    """Algorithmic flops of one apply: two GEMM stages 8 M^3 D_W d each + W stage 8 M^2 nnz."""
+    return 16.0 * M ** 3 * Dw * d + 8.0 * M ** 2 * nnz
+
+
+def gemm_stage_flops(M, d=D_PHYS, Dw=D_W):
+    return 8.0 * M ** 3 * Dw * d
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_cores():
+    try:
+        from threadpoolctl import threadpool_info
+        n = max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
+        return int(n)
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def time_oracle_heff(M, min_seconds=10.0, max_applies=200):
+    """The oracle's heff, as it stands, on the host cores: applies/s over a bounded sample."""
+    from oracle import contractions as oc
+    L, W, A, R = si.microbench_tensors(M)
+    oc.heff(L, W, A, R)
+    n, t0 = 0, time.perf_counter()
+    while True:
+        oc.heff(L, W, A, R)
+        n += 1
+        el = time.perf_counter() - t0
+        if el >= min_seconds or n >= max_applies:
+            break
+    return n / el, n, el
+
+
+def run_reference(args):
+    """--impl reference: the oracle (oracle/contractions.py heff) on the host cores, same metric
+    and config; each step is ONE apply (a bounded sample of the APPLIES_PER_STEP-apply step)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import contractions as oc
+    L, W, A, R = si.microbench_tensors(M_HEADLINE)
+    for _ in range(max(1, min(args.warmup, 3))):
+        oc.heff(L, W, A, R)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oc.heff(L, W, A, R)
+    el = time.perf_counter() - t0
+    val = args.steps / el
+    cores = oracle_cores()
+    sample = "1 oracle heff apply per step (of the %d-apply step), %d steps, numpy tensordot" % (APPLIES_PER_STEP, args.steps)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "c128", "data": "synthetic", "config": {"workload": WORKLOAD},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def make_sets(torch, M, n_sets):
+    """n_sets independent resident input sets of configs[1] at bond dimension M (seeded)."""
+    sets = []
+    for s in range(n_sets):
+        L, W, A, R = si.microbench_tensors(M, seed=1000 + M + 7919 * s)
+        sets.append([torch.from_numpy(x).cuda() for x in (L, W, A, R)] +
+                    [torch.empty((M, D_PHYS, M), dtype=torch.complex128, device="cuda")])
+    return sets
+
+
+def time_applies(torch, T, ctx, sets, n_applies):
+    """CUDA-event time (ms) of n_applies back-to-back calls on torch's current stream."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for i in range(n_applies):
+        L, W, A, R, out = sets[i % len(sets)]
+        T.tdvp_apply_heff(L, W, A, R, out=out, handle=ctx)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1)
+
+
+def sweep_point(torch, T, M, peak_tflops):
+    """applies/s and fraction of the FP64 tensor peak at one M of the configs[1] sweep."""
+    per_set = 16.0 * M * M * (2 * D_W + 2 * D_PHYS)
+    n_sets = int(max(2, min(16, np.ceil(1.5 * 126e6 / per_set)))) if M < 512 else 2
+    sets = make_sets(torch, M, n_sets)
+    ctx = T.tdvp_create_context()
+    n = int(max(4, min(200, 2e11 / heff_flops(M))))
+    time_applies(torch, T, ctx, sets, max(3, n // 4))
+    ms = time_applies(torch, T, ctx, sets, n)
+    env_out = torch.empty((M, D_W, M), dtype=torch.complex128, device="cuda")
+    for _ in range(3):
+        T.tdvp_update_env(0, sets[0][0], sets[0][1], sets[0][2], env_out=env_out, handle=ctx)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for i in range(n):
+        s = sets[i % len(sets)]
+        T.tdvp_update_env(0, s[0], s[1], s[2], env_out=env_out, handle=ctx)
+    e1.record()
+    torch.cuda.synchronize()
+    ms_env = e0.elapsed_time(e1)
+    ctx.close()
+    aps = n / (ms * 1e-3)
+    return {"M": M, "applies_per_s": aps, "us_per_apply": 1e3 * ms / n, "tflops": aps * heff_flops(M) / 1e12,
+            "frac_fp64_tensor_peak": aps * heff_flops(M) / 1e12 / peak_tflops,
+            "env_updates_per_s": n / (ms_env * 1e-3), "input_sets": n_sets}
+
+
+def build_chain(name, M=None):
+    """MPO (built by the oracle's model builder: host-side input construction) and the
+    seeded delta-padded initial MPS of one of BASELINE.json's chain configs."""
+    import dataclasses
+    from oracle import model
+    cfg = si.CONFIGS[name]
+    if M is not None:
+        cfg = dataclasses.replace(cfg, M=M)
+    params = si.draw_vibronic_params(cfg)
+    mpo = model.build_mpo(params)
+    dims = si.site_dims(params)
+    mps = si.padded_product_mps(dims, si.initial_occupations(params), cfg.M, cfg.pad_seed, cfg.delta, cfg.delta_seed)
+    return cfg, mpo, mps
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import paper_1907_12044_b200 as T
+    T.library_path()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    peak = T.tdvp_probe_fp64_tensor_peak(20000)        # DMMA issue-rate ceiling, measured live
+    M = M_HEADLINE
+    sets = make_sets(torch, M, N_SETS)
+    ctx = T.tdvp_create_context()
+    launches0 = T.tdvp_launch_count()
+
+    # ---- resident-input arm: W warm-up steps, then exactly K timed steps ----
+    for _ in range(args.warmup):
+        time_applies(torch, T, ctx, sets, APPLIES_PER_STEP)
+    sampler = ClockSampler(local)
+    sampler.start()
+    T.tdvp_profile_enable(True)
+    T.tdvp_profile_read()
+    barrier()
+    l0 = T.tdvp_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for s in range(args.steps):
+        for i in range(APPLIES_PER_STEP):
+            L, W, A, R, out = sets[(s * APPLIES_PER_STEP + i) % N_SETS]
+            T.tdvp_apply_heff(L, W, A, R, out=out, handle=ctx)
+    e1.record()
+    barrier()
+    ms_total = max_over_ranks(e0.elapsed_time(e1))
+    gpu_launches = T.tdvp_launch_count() - l0
+    prof = T.tdvp_profile_read()
+    T.tdvp_profile_enable(False)
+    clocks = sampler.stop()
+    n_applies = args.steps * APPLIES_PER_STEP
+    value = world * n_applies / (ms_total * 1e-3)
+
+    # ---- roofline of the dominant kernel (DMMA complex GEMM): live event brackets above ----
+    zg_ms, zg_n = prof["zgemm"]
+    ws_ms, ws_n = prof["wstage"]
+    sk_ms, sk_n = prof["splitk_reduce"]
+    flops_per_launch = gemm_stage_flops(M)             # each of the 2 GEMM launches of an apply
+    achieved = flops_per_launch / (zg_ms / max(zg_n, 1) * 1e-3) / 1e12 if zg_n else None
+    roofline = {"bound": "tensor", "kernel": "zgemm_kernel (FP64 DMMA m8n8k4, complex128)",
+                "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": (achieved / peak) if achieved else None, "traffic": None,
+                "peak_source": "tdvp_probe_fp64_tensor_peak: DMMA m8n8k4 issue rate measured in this run "
+                               "(MEASURED_PEAKS.json has no FP64 figure; cuBLAS ZGEMM 4096^3 measured 36.85 TFLOP/s)",
+                "flops_per_launch": flops_per_launch, "avg_launch_us": 1e3 * zg_ms / max(zg_n, 1), "launches": zg_n,
+                "share_of_step": {"zgemm": zg_ms / ms_total, "wstage": ws_ms / ms_total, "splitk_reduce": sk_ms / ms_total},
+                "wstage": {"bound": "hbm", "algorithmic_bytes": 2 * 16.0 * M * M * D_W * D_PHYS,
+                           "achieved_gbs": (2 * 16.0 * M * M * D_W * D_PHYS / (ws_ms / max(ws_n, 1) * 1e-3) / 1e9) if ws_n else None,
+                           "avg_launch_us": 1e3 * ws_ms / max(ws_n, 1)}}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        roofline["wstage"]["peak_gbs"] = peaks.get("hbm_gbs")
+        if roofline["wstage"]["achieved_gbs"] and peaks.get("hbm_gbs"):
+            roofline["wstage"]["frac"] = roofline["wstage"]["achieved_gbs"] / peaks["hbm_gbs"]
+    except OSError:
+        roofline["wstage"]["peak_gbs"] = 6650.0
+        roofline["wstage"]["peak_source"] = "fallback"
+
+    # ---- end-to-end arm: HOST (pinned) buffers through tdvp_apply_heff_host ----
+    hsets = []
+    for s in range(3):
+        arrs = []
+        for x in si.microbench_tensors(M, seed=1000 + M + 7919 * s) + (np.empty((M, D_PHYS, M), np.complex128),):
+            t = torch.empty(x.shape, dtype=torch.complex128).pin_memory()
+            t.numpy()[...] = x
+            arrs.append(t.numpy())
+        hsets.append(arrs)
+    h2d = sum(a.nbytes for a in hsets[0][:4])
+    d2h = hsets[0][4].nbytes
+    e2e_applies = max(4, min(n_applies, 40))
+    for i in range(3):
+        T.tdvp_apply_heff_host(*hsets[i % 3], handle=ctx)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(e2e_applies):
+        T.tdvp_apply_heff_host(*hsets[i % 3], handle=ctx)
+    torch.cuda.synchronize()
+    el = max_over_ranks(time.perf_counter() - t0)
+    e2e = {"value": world * e2e_applies / el, "unit": UNIT, "h2d_bytes_per_step": h2d * APPLIES_PER_STEP,
+           "d2h_bytes_per_step": d2h * APPLIES_PER_STEP, "applies_timed": e2e_applies,
+           "api": "tdvp_apply_heff_host (pinned host buffers; h2d L,W,A,R + kernels + d2h out per apply)"}
+    ctx.close()
+    del sets
+    torch.cuda.empty_cache()
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "c128", "data": "synthetic",
+           "config": {"workload": WORKLOAD, "applies_per_step": APPLIES_PER_STEP, "input_sets": N_SETS,
+                      "l2": "inputs rotate over %d resident sets (188 MB > 126 MB L2); T1/T2 intermediates 52 MB each" % N_SETS,
+                      "multi_gpu": "replicas only (SURVEY.md 8(e))", "seed": "1000+M+7919*set"},
+           "us_per_apply": 1e3 * ms_total / n_applies, "tflops": value / world * heff_flops(M) / 1e12,
+           "frac_fp64_tensor_peak": value / world * heff_flops(M) / 1e12 / peak,
+           "roofline": roofline, "e2e": e2e, "gpu_launches": int(gpu_launches), "clocks": clocks}
+
+    if rank == 0 and not args.no_extras:
+        # M sweep of configs[1]
+        out["sweep"] = [sweep_point(torch, T, m, peak) for m in (32, 64, 128, 256, 512)]
+        torch.cuda.empty_cache()
+        # one TDVP-PS step of the FMO-like chain at M = 128 (configs[3]; k = 10, dt = 5 fs)
+        cfg, mpo, mps = build_chain("fmo128")
+        ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=cfg.krylov_dim))
+        for _ in range(2):
+            ch.tdvp_step_ps(cfg.dt_fs)
+        ch.tdvp_sync()
+        l0 = T.tdvp_launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        n_ps = 3
+        for _ in range(n_ps):
+            ch.tdvp_step_ps(cfg.dt_fs)
+        e1.record()
+        ch.tdvp_sync()
+        torch.cuda.synchronize()
+        nrm, en = ch.tdvp_norm_energy()
+        out["ps_step"] = {"workload": "configs[3]: FMO-like chain, 71 sites, M=128, D_W<=9 (real MPO), k=10, dt=5 fs, CUDA graph",
+                          "ms_per_step": e0.elapsed_time(e1) / n_ps, "steps_timed": n_ps,
+                          "launches_per_step": (T.tdvp_launch_count() - l0) // n_ps,
+                          "norm_sq": nrm, "energy": en, "populations": ch.tdvp_populations(0).tolist()}
+        ch.close()
+        # the oracle as it stands on the host cores, bounded sample
+        v, n, el = time_oracle_heff(M, min_seconds=10.0)
+        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": oracle_cores(), "kind": "oracle",
+                               "sample": "%d oracle heff applies (numpy tensordot) of the same M=128 workload in %.1f s" % (n, el)}
+    elif rank == 0:
+        out["cpu_baseline"] = None
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-extras", action="store_true", help="skip the M sweep, the PS step and the CPU baseline")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -200,6 +200,14 @@ const char *tdvp_last_error(const tdvp_handle *h);
    the legacy default stream, blocks, returns TFLOP/s.  This is the denominator bench.py uses for
    "fraction of FP64 tensor peak". */
 int tdvp_probe_fp64_tensor_peak(int iters, double *tflops /*HOST*/);
+/* Phase profiler: when enabled, launches of the dominant kernel classes are bracketed by CUDA events
+   on the launching stream (not inside a captured step).  tdvp_profile_read blocks on the device,
+   returns the summed elapsed milliseconds and bracket counts per phase since the last read and
+   resets them.  Phases: 0 complex GEMM (DMMA), 1 split-K reduce, 2 MPO (W) stage, 3 Lanczos /
+   vector kernels, 4 QR, 5 SVD.  ms, count: HOST arrays of TDVP_PROFILE_PHASES entries. */
+#define TDVP_PROFILE_PHASES 6
+int tdvp_profile_enable(int on);
+int tdvp_profile_read(double *ms, long long *count);
 /* Number of kernel launches this library has enqueued since load (for bench.py's gpu_launches;
    launches replayed from a captured CUDA graph are counted when the graph is launched). */
 long long tdvp_launch_count(void);

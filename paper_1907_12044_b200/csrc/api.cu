@@ -1,12 +1,36 @@
 // api.cu -- C ABI entry points that work on caller-provided device buffers (include/tdvp.h),
 // handle bookkeeping, error reporting and the FP64 tensor-pipe probe.
 #include <mutex>
+#include <vector>
 
 #include "handle.cuh"
 
 std::atomic<long long> g_launch_count{0};
 thread_local long long *g_capture_tally = nullptr;
 static thread_local std::string g_null_err;
+
+// ---- phase profiler ---------------------------------------------------------------------------
+bool g_prof_on = false;
+namespace {
+struct ProfRec { cudaEvent_t e0, e1; int phase; };
+std::vector<ProfRec> g_prof_recs;
+size_t g_prof_used = 0;
+constexpr size_t PROF_MAX = 1 << 16;
+}
+void prof_begin(cudaStream_t st, int phase) {
+  if (g_prof_used >= PROF_MAX) return;
+  if (g_prof_used == g_prof_recs.size()) {
+    ProfRec r; cudaEventCreate(&r.e0); cudaEventCreate(&r.e1); r.phase = phase;
+    g_prof_recs.push_back(r);
+  }
+  g_prof_recs[g_prof_used].phase = phase;
+  cudaEventRecord(g_prof_recs[g_prof_used].e0, st);
+}
+void prof_end(cudaStream_t st) {
+  if (g_prof_used >= PROF_MAX) return;
+  cudaEventRecord(g_prof_recs[g_prof_used].e1, st);
+  g_prof_used++;
+}
 
 int set_err(tdvp_handle *h, int code, const std::string &msg) {
   if (h) h->err = msg; else g_null_err = msg;
@@ -83,6 +107,23 @@ int tdvp_create_context(tdvp_handle **out, const tdvp_options *opt, void *cuda_s
 const char *tdvp_last_error(const tdvp_handle *h) { return h ? h->err.c_str() : g_null_err.c_str(); }
 
 long long tdvp_launch_count(void) { return g_launch_count.load(); }
+
+int tdvp_profile_enable(int on) { g_prof_on = on != 0; return TDVP_OK; }
+
+int tdvp_profile_read(double *ms, long long *count) {
+  if (!ms || !count) return set_err(nullptr, TDVP_EINVAL, "null pointer");
+  for (int i = 0; i < TDVP_PROFILE_PHASES; i++) { ms[i] = 0.0; count[i] = 0; }
+  if (int rc = check_cuda(nullptr, cudaDeviceSynchronize(), "tdvp_profile_read")) return rc;
+  for (size_t i = 0; i < g_prof_used; i++) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, g_prof_recs[i].e0, g_prof_recs[i].e1) == cudaSuccess) {
+      ms[g_prof_recs[i].phase] += t; count[g_prof_recs[i].phase]++;
+    }
+  }
+  g_prof_used = 0;
+  cudaGetLastError();
+  return TDVP_OK;
+}
 
 int tdvp_sync(tdvp_handle *h) {
   tdvp_handle *hh = h ? h : default_handle();

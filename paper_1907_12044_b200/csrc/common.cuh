@@ -14,6 +14,18 @@ extern std::atomic<long long> g_launch_count;   // kernels enqueued (tdvp_launch
 // While a stream capture is recording, launches are counted into the graph's own tally instead.
 extern thread_local long long *g_capture_tally;
 
+// Phase profiler (tdvp_profile_enable / tdvp_profile_read): CUDA-event pairs around the launches
+// of a kernel class, recorded on the launching stream; off by default, skipped during capture.
+enum { PH_ZGEMM = 0, PH_SPLITK = 1, PH_WSTAGE = 2, PH_VEC = 3, PH_QR = 4, PH_SVD = 5, PH_COUNT = 6 };
+void prof_begin(cudaStream_t st, int phase);
+void prof_end(cudaStream_t st);
+extern bool g_prof_on;
+struct ProfScope {
+  cudaStream_t st; bool live;
+  ProfScope(cudaStream_t s, int phase) : st(s), live(g_prof_on && !g_capture_tally) { if (live) prof_begin(st, phase); }
+  ~ProfScope() { if (live) prof_end(st); }
+};
+
 static inline void count_launch() {
   if (g_capture_tally) ++*g_capture_tally; else g_launch_count.fetch_add(1, std::memory_order_relaxed);
 }

@@ -107,6 +107,7 @@ __global__ void __launch_bounds__(WS_THREADS) wstage_kernel(WStageParams p) {
 void launch_wstage(cudaStream_t st, const WStageParams &p, int nbatch) {
   dim3 grid((p.Mr + YT - 1) / YT, nbatch);
   size_t smem = (size_t)p.ncols * YT * 16;
+  ProfScope ps(st, PH_WSTAGE);
   if (smem <= 200 * 1024) {
     TDVP_LAUNCH(wstage_kernel<true>, grid, WS_THREADS, smem, st, p);
   } else {

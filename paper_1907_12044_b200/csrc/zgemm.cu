@@ -274,11 +274,15 @@ void zgemm(cudaStream_t st, const ZGemm &p, c128 *ws) {
   kp.partial_split_stride = batch * p.M * p.N;
   dim3 grid((unsigned)(kp.tiles_m * kp.tiles_n), (unsigned)s, (unsigned)batch);
   const bool ak = (p.a_ks == 1), bk = (p.b_ks == 1);
-  if (ak && bk) launch<true, true>(st, kp, grid);
-  else if (ak && !bk) launch<true, false>(st, kp, grid);
-  else if (!ak && bk) launch<false, true>(st, kp, grid);
-  else launch<false, false>(st, kp, grid);
+  {
+    ProfScope ps(st, PH_ZGEMM);
+    if (ak && bk) launch<true, true>(st, kp, grid);
+    else if (ak && !bk) launch<true, false>(st, kp, grid);
+    else if (!ak && bk) launch<false, true>(st, kp, grid);
+    else launch<false, false>(st, kp, grid);
+  }
   if (s > 1) {
+    ProfScope ps(st, PH_SPLITK);
     long long total = batch * p.M * p.N;
     TDVP_LAUNCH(splitk_reduce_kernel, (unsigned)ceil_div_ll(total, 256), 256, 0, st, ws,
                 kp.partial_split_stride, s, p.C, p.M, p.N, p.ldc, p.batch_inner, p.c_bsi, p.c_bso, total);
