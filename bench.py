@@ -355,6 +355,23 @@ def run_ours(args):
                           "launches_per_step": (T.tdvp_launch_count() - l0) // n_ps,
                           "norm_sq": nrm, "energy": en, "populations": ch.tdvp_populations(0).tolist()}
         ch.close()
+        # phase breakdown of one step (direct enqueue, event brackets per kernel class; the graph replay above is the timed number)
+        ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=cfg.krylov_dim, flags=T.TDVP_FLAG_NO_GRAPH))
+        ch.tdvp_step_ps(cfg.dt_fs)
+        ch.tdvp_sync()
+        T.tdvp_profile_enable(True)
+        T.tdvp_profile_read()
+        e0.record()
+        ch.tdvp_step_ps(cfg.dt_fs)
+        e1.record()
+        ch.tdvp_sync()
+        torch.cuda.synchronize()
+        ph = T.tdvp_profile_read()
+        T.tdvp_profile_enable(False)
+        out["ps_step"]["no_graph_ms"] = e0.elapsed_time(e1)
+        out["ps_step"]["phase_ms"] = {k: round(v[0], 3) for k, v in ph.items()}
+        out["ps_step"]["phase_brackets"] = {k: v[1] for k, v in ph.items()}
+        ch.close()
         # the oracle as it stands on the host cores, bounded sample
         v, n, el = time_oracle_heff(M, min_seconds=10.0)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": oracle_cores(), "kind": "oracle",

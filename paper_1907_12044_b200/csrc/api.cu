@@ -11,6 +11,7 @@ static thread_local std::string g_null_err;
 
 // ---- phase profiler ---------------------------------------------------------------------------
 bool g_prof_on = false;
+int g_prof_depth = 0;
 namespace {
 struct ProfRec { cudaEvent_t e0, e1; int phase; };
 std::vector<ProfRec> g_prof_recs;

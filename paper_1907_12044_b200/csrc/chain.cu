@@ -55,6 +55,7 @@ size_t chain_step_ws_bytes(const tdvp_handle *h) {
     if (i > 0) {
       need = std::max(need, qr_ws_bytes(h->d[i] * h->M[i + 1], h->M[i]));
       need = std::max(need, lanczos_ws_bytes(bond_op(h, i), k));
+      need = std::max(need, svd_ws_bytes(h->M[i], h->d[i], h->M[i + 1]));
     }
   }
   return need + 4096;
@@ -107,7 +108,7 @@ static void free_chain(tdvp_handle *h) {
   for (auto p : h->Renv) fr(p);
   for (int s = 0; s < 7; s++) for (auto p : h->mu_k[s]) fr(p);
   for (auto p : h->mu_y) fr(p);
-  fr(h->tmpA); fr(h->tmpB); fr(h->bondD); fr(h->bondD2); fr(h->step_ws); fr(h->mu_err_dev);
+  fr(h->tmpA); fr(h->tmpB); fr(h->bondD); fr(h->bondD2); fr(h->step_ws); fr(h->mu_err_dev); fr(h->mu_scratch);
   if (h->ps_graph.exec) cudaGraphExecDestroy(h->ps_graph.exec);
   if (h->mu_graph.exec) cudaGraphExecDestroy(h->mu_graph.exec);
   h->arena.release();

@@ -20,10 +20,13 @@ enum { PH_ZGEMM = 0, PH_SPLITK = 1, PH_WSTAGE = 2, PH_VEC = 3, PH_QR = 4, PH_SVD
 void prof_begin(cudaStream_t st, int phase);
 void prof_end(cudaStream_t st);
 extern bool g_prof_on;
+extern int g_prof_depth;          // nested scopes: only the outermost one records
 struct ProfScope {
-  cudaStream_t st; bool live;
-  ProfScope(cudaStream_t s, int phase) : st(s), live(g_prof_on && !g_capture_tally) { if (live) prof_begin(st, phase); }
-  ~ProfScope() { if (live) prof_end(st); }
+  cudaStream_t st; bool counted, live;
+  ProfScope(cudaStream_t s, int phase) : st(s), counted(g_prof_on && !g_capture_tally), live(false) {
+    if (counted) { live = (g_prof_depth++ == 0); if (live) prof_begin(st, phase); }
+  }
+  ~ProfScope() { if (counted) { g_prof_depth--; if (live) prof_end(st); } }
 };
 
 static inline void count_launch() {
@@ -137,6 +140,11 @@ size_t qr_ws_bytes(int rows, int cols);
 // side 1: C (Ml x (d*Mr)) = D Q, i.e. QR of C^T: tall = d*Mr, thin = Ml; Q [Ml, d*Mr], D [Ml, Ml]
 void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c128 *Q, c128 *D,
               void *ws);
+
+// ---------------------------------------------------------------------------------------------
+// svd.cu : matrix unfolding C[Ml, d*Mr] = U diag(lam) Vh (Eq. 36) on the device, Ml <= d*Mr.
+size_t svd_ws_bytes(int Ml, int d, int Mr);
+void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, double *lam, c128 *Vh, void *ws);
 
 // ---------------------------------------------------------------------------------------------
 // small vector kernels shared by the drivers (vecops.cu)

@@ -38,6 +38,7 @@ struct tdvp_handle {
   std::vector<c128 *> mu_k[7];     // Dormand-Prince stage derivatives
   std::vector<c128 *> mu_y;        // stage states
   double *mu_err_dev = nullptr;
+  void *mu_scratch = nullptr;      // U, Lambda, V^dagger, centre forms ... of one derivative evaluation
   StepGraph ps_graph, mu_graph;
 };
 

@@ -248,21 +248,26 @@ void lanczos_expm(cudaStream_t st, const LanczosOp &op, int k, double z_re, doub
   int G = (int)((n + VT - 1) / VT);
   if (G > MAXG) G = MAXG;
   if (G < 1) G = 1;
-  cudaMemsetAsync(b.counter, 0, sizeof(unsigned), st);
-  TDVP_LAUNCH(lz_init_kernel, G, VT, 0, st, v, n, b);
-  TDVP_LAUNCH(lz_scale_kernel, G, VT, 0, st, b.Q, v, n, b.state);
+  {
+    ProfScope ps(st, PH_VEC);
+    cudaMemsetAsync(b.counter, 0, sizeof(unsigned), st);
+    TDVP_LAUNCH(lz_init_kernel, G, VT, 0, st, v, n, b);
+    TDVP_LAUNCH(lz_scale_kernel, G, VT, 0, st, b.Q, v, n, b.state);
+  }
   for (int j = 0; j < k; j++) {
     c128 *qj = b.Q + (long long)j * n, *w = b.Q + (long long)(j + 1) * n;
     if (op.kind == 0)
       heff_apply(st, op.Ml, op.Mr, op.d, op.Dl, op.Dr, op.L, *op.W, qj, op.R, w, b.apply_ws);
     else
       bond_apply(st, op.Ml, op.Mr, op.Dl, op.L, qj, op.R, w, b.apply_ws);
+    ProfScope ps(st, PH_VEC);
     TDVP_LAUNCH(lz_dots_kernel, G, VT, 0, st, n, j + 1, j, 1, b);
     TDVP_LAUNCH(lz_update_kernel, G, VT, 0, st, n, j + 1, j, k, 0, b);
     TDVP_LAUNCH(lz_dots_kernel, G, VT, 0, st, n, j + 1, j, 0, b);
     TDVP_LAUNCH(lz_update_kernel, G, VT, 0, st, n, j + 1, j, k, 1, b);
     if (j < k - 1) TDVP_LAUNCH(lz_scale_kernel, G, VT, 0, st, w, w, n, b.state);
   }
+  ProfScope ps(st, PH_VEC);
   TDVP_LAUNCH(lz_coef_kernel, 1, 32, 0, st, k, z_re, z_im, b, m_used_dev);
   TDVP_LAUNCH(lz_combine_kernel, G, VT, 0, st, n, k, b, y);
 }

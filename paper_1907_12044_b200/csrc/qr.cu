@@ -337,6 +337,7 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
   const int rows = side == 0 ? Ml * d : d * Mr;
   const int cols = side == 0 ? Mr : Ml;
   const int nb = panel_width(rows);
+  ProfScope ps(st, PH_QR);
   char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
   size_t mat = up256((size_t)rows * cols * 16);
   c128 *X = reinterpret_cast<c128 *>(p); p += mat;

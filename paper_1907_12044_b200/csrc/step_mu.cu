@@ -1,16 +1,252 @@
-// step_mu.cu -- TDVP-MU step driver.  Placeholder until the SVD path lands.
+// step_mu.cu -- TDVP-MU: the right-hand side of the
+// equations of motion in the left-canonical gauge and one Dormand-Prince 5(4) step of it.
+//   Eq. 27:        i dC_N/dt = H[N] C_N
+//   Eq. 37:    i dL_i/dt = (1 - p[i]) H[i](L_i U Lambda) Lambda~^{-1} U^dagger
+//   Eq. 33:        p[i] = L_i L_i^dagger, applied as G - L (L^dagger G)
+//   Eq. 36:    the centre of site i+1 unfolded by SVD, U Lambda R
+//   Eq. 38:    Lambda~ = Lambda + eps^{1/2} exp(-Lambda / eps^{1/2})
+// Reading c13: G = H_eff(C_i) Lambda~^{-1} U^dagger with C_i = L_i U Lambda; only the
+// inverse factor is regularised.  Reading c12: one call = one fixed Dormand-Prince step (the
+// paper's VMF integrator); step-size control is the caller's loop.
+// Everything is enqueued on the handle's stream; the SVDs run on the device (svd.cu).
+#include <algorithm>
+#include <cmath>
+
 #include "handle.cuh"
+
+int move_gauge(tdvp_handle *h, int centre);
+
+namespace {
+
+constexpr int VT = 256;
+inline int grid_for(long long n) { long long g = (n + VT - 1) / VT; return (int)(g > 1184 ? 1184 : (g < 1 ? 1 : g)); }
+inline size_t up256(size_t x) { return (x + 255) & ~size_t(255); }
+long long site_elems(const tdvp_handle *h, int i) { return (long long)h->M[i] * h->d[i] * h->M[i + 1]; }
+
+// X[row][c] *= f(lam[c]);  mode 0: f = lam (U Lambda); mode 1: f = 1 / (lam + sq exp(-lam / sq))  (Eq. 38)
+__global__ void scale_cols_kernel(c128 *X, long long rows, int n, const double *lam, int mode, double sq) {
+  const long long total = rows * n;
+  for (long long e = blockIdx.x * (long long)VT + threadIdx.x; e < total; e += (long long)gridDim.x * VT) {
+    const double l = lam[e % n];
+    const double f = mode == 0 ? l : 1.0 / (l + sq * exp(-l / sq));
+    c128 v = X[e];
+    X[e] = make_double2(v.x * f, v.y * f);
+  }
+}
+// out = -i (G - T)   (T may be NULL: out = -i G)
+__global__ void minus_i_diff_kernel(c128 *out, const c128 *G, const c128 *T, long long n) {
+  for (long long e = blockIdx.x * (long long)VT + threadIdx.x; e < n; e += (long long)gridDim.x * VT) {
+    c128 g = G[e];
+    if (T) { c128 t = T[e]; g.x -= t.x; g.y -= t.y; }
+    out[e] = make_double2(g.y, -g.x);
+  }
+}
+struct Comb { const c128 *k[7]; double c[7]; int n; };
+// out = base + sum_j c_j k_j   (base may be NULL)
+__global__ void lincomb_kernel(c128 *out, const c128 *base, Comb cb, long long n) {
+  for (long long e = blockIdx.x * (long long)VT + threadIdx.x; e < n; e += (long long)gridDim.x * VT) {
+    c128 v = base ? base[e] : make_double2(0.0, 0.0);
+    for (int j = 0; j < cb.n; j++) { c128 k = cb.k[j][e]; v.x += cb.c[j] * k.x; v.y += cb.c[j] * k.y; }
+    out[e] = v;
+  }
+}
+// out[0] = sqrt(sum_i parts[i])
+__global__ void err_final_kernel(const double *parts, int n, double *out) {
+  double s = 0.0;
+  for (int i = 0; i < n; i++) s += parts[i];
+  out[0] = sqrt(s);
+}
+
+struct MuScratch {
+  c128 *U, *UL, *P, *Vh, *C0, *C1, *HC, *G, *T;
+  double *lam;
+};
+
+MuScratch mu_scratch(tdvp_handle *h) {
+  long long ms = 0; int mm = 1;
+  for (int i = 0; i < h->n; i++) { ms = std::max(ms, site_elems(h, i)); mm = std::max(mm, h->M[i + 1]); }
+  const size_t sb = up256(ms * 16), bb = up256((size_t)mm * mm * 16);
+  if (!h->mu_scratch) {
+    if (cudaMalloc(&h->mu_scratch, 6 * sb + 3 * bb + up256(mm * 8) + 1024) != cudaSuccess) { h->mu_scratch = nullptr; }
+  }
+  MuScratch s{};
+  char *p = reinterpret_cast<char *>(h->mu_scratch);
+  if (!p) return s;
+  s.Vh = reinterpret_cast<c128 *>(p); p += sb;
+  s.C0 = reinterpret_cast<c128 *>(p); p += sb;
+  s.C1 = reinterpret_cast<c128 *>(p); p += sb;
+  s.HC = reinterpret_cast<c128 *>(p); p += sb;
+  s.G = reinterpret_cast<c128 *>(p); p += sb;
+  s.T = reinterpret_cast<c128 *>(p); p += sb;
+  s.U = reinterpret_cast<c128 *>(p); p += bb;
+  s.UL = reinterpret_cast<c128 *>(p); p += bb;
+  s.P = reinterpret_cast<c128 *>(p); p += bb;
+  s.lam = reinterpret_cast<double *>(p);
+  return s;
+}
+
+void gemm1(cudaStream_t st, ZGemm g) { g.splitk = 1; zgemm(st, g, nullptr); }
+
+// K = F(Y): the TDVP-MU right-hand side.  Uses the handle's Lenv / Renv storage as scratch caches.
+int mu_rhs(tdvp_handle *h, const std::vector<c128 *> &Y, const std::vector<c128 *> &K) {
+  cudaStream_t st = h->stream;
+  const int n = h->n;
+  MuScratch s = mu_scratch(h);
+  if (!s.U) return set_err(h, TDVP_ENOMEM, "TDVP-MU scratch allocation failed");
+  void *ws = h->step_ws;
+  const double sq = std::sqrt(h->opt.mu_eps);
+  for (int i = 0; i < n - 1; i++)                                                        // "Get Env"
+    env_update(st, 0, h->M[i], h->M[i + 1], h->d[i], h->Dw[i], h->Dw[i + 1], h->Lenv[i], h->Wsp[i], Y[i],
+               h->Lenv[i + 1], ws);
+  {                                                                                      // Eq. 27
+    const int i = n - 1;
+    heff_apply(st, h->M[i], h->M[i + 1], h->d[i], h->Dw[i], h->Dw[i + 1], h->Lenv[i], h->Wsp[i], Y[i], h->Renv[i],
+               s.HC, ws);
+    TDVP_LAUNCH(minus_i_diff_kernel, grid_for(site_elems(h, i)), VT, 0, st, K[i], s.HC, (const c128 *)nullptr,
+                site_elems(h, i));
+  }
+  const c128 *C = Y[n - 1];
+  c128 *Cnext = s.C0;
+  for (int i = n - 1; i >= 1; i--) {
+    const int Ml = h->M[i], Mr = h->M[i + 1], d = h->d[i];
+    svd_bond(st, Ml, d, Mr, C, s.U, s.lam, s.Vh, ws);                                    // Eq. 36
+    env_update(st, 1, Ml, Mr, d, h->Dw[i], h->Dw[i + 1], h->Renv[i], h->Wsp[i], s.Vh, h->Renv[i - 1], ws);
+    // site i-1: centre form C' = L (U Lambda)
+    const int j = i - 1, Jl = h->M[j], Jr = h->M[j + 1], dj = h->d[j];                    // Jr == Ml
+    const long long ne = site_elems(h, j), rows = (long long)Jl * dj;
+    vec_copy(st, s.UL, s.U, (long long)Jr * Jr);
+    TDVP_LAUNCH(scale_cols_kernel, grid_for((long long)Jr * Jr), VT, 0, st, s.UL, (long long)Jr, Jr, s.lam, 0, sq);
+    ZGemm g{};
+    g.A = Y[j]; g.B = s.UL; g.C = Cnext;                    // C'[(a,s)][r] = sum_l L[(a,s)][l] UL[l][r]
+    g.M = (int)rows; g.K = Jr; g.N = Jr; g.a_ms = Jr; g.a_ks = 1; g.b_ks = Jr; g.b_ns = 1; g.ldc = Jr;
+    gemm1(st, g);
+    heff_apply(st, Jl, Jr, dj, h->Dw[j], h->Dw[j + 1], h->Lenv[j], h->Wsp[j], Cnext, h->Renv[j], s.HC, ws);
+    TDVP_LAUNCH(scale_cols_kernel, grid_for(ne), VT, 0, st, s.HC, rows, Jr, s.lam, 1, sq);  // Lambda~^{-1}, Eq. 38
+    ZGemm g2{};
+    g2.A = s.HC; g2.B = s.U; g2.C = s.G;                    // G[(a,s)][l] = sum_r HC[(a,s)][r] conj(U[l][r])
+    g2.M = (int)rows; g2.K = Jr; g2.N = Jr; g2.a_ms = Jr; g2.a_ks = 1; g2.b_ns = Jr; g2.b_ks = 1; g2.conjB = 1; g2.ldc = Jr;
+    gemm1(st, g2);
+    ZGemm g3{};
+    g3.A = Y[j]; g3.B = s.G; g3.C = s.P;                    // P[b][l] = sum_{(a,s)} conj(L[(a,s)][b]) G[(a,s)][l]
+    g3.M = Jr; g3.N = Jr; g3.K = (int)rows; g3.a_ms = 1; g3.a_ks = Jr; g3.conjA = 1; g3.b_ks = Jr; g3.b_ns = 1; g3.ldc = Jr;
+    gemm1(st, g3);
+    ZGemm g4{};
+    g4.A = Y[j]; g4.B = s.P; g4.C = s.T;                    // T = L P
+    g4.M = (int)rows; g4.K = Jr; g4.N = Jr; g4.a_ms = Jr; g4.a_ks = 1; g4.b_ks = Jr; g4.b_ns = 1; g4.ldc = Jr;
+    gemm1(st, g4);
+    TDVP_LAUNCH(minus_i_diff_kernel, grid_for(ne), VT, 0, st, K[j], s.G, s.T, ne);         // -i (1 - p) G, Eq. 33/37
+    C = Cnext;
+    Cnext = (Cnext == s.C0) ? s.C1 : s.C0;
+  }
+  return check_cuda(h, cudaGetLastError(), "TDVP-MU derivative");
+}
+
+int mu_alloc(tdvp_handle *h) {
+  if (!h->mu_y.empty()) return TDVP_OK;
+  std::vector<c128 *> tmp;
+  for (int sidx = 0; sidx < 8; sidx++) {
+    std::vector<c128 *> v(h->n, nullptr);
+    for (int i = 0; i < h->n; i++)
+      if (int rc = check_cuda(h, cudaMalloc(&v[i], site_elems(h, i) * 16), "cudaMalloc TDVP-MU stage")) return rc;
+    if (sidx < 7) h->mu_k[sidx] = v; else h->mu_y = v;
+  }
+  if (int rc = check_cuda(h, cudaMalloc(&h->mu_err_dev, (h->n + 1) * sizeof(double)), "cudaMalloc")) return rc;
+  return TDVP_OK;
+}
+
+// Dormand-Prince 5(4) Butcher tableau (the RK45 of PAPER.md:224)
+const double DP_A[7][6] = {
+    {0, 0, 0, 0, 0, 0},
+    {1.0 / 5, 0, 0, 0, 0, 0},
+    {3.0 / 40, 9.0 / 40, 0, 0, 0, 0},
+    {44.0 / 45, -56.0 / 15, 32.0 / 9, 0, 0, 0},
+    {19372.0 / 6561, -25360.0 / 2187, 64448.0 / 6561, -212.0 / 729, 0, 0},
+    {9017.0 / 3168, -355.0 / 33, 46732.0 / 5247, 49.0 / 176, -5103.0 / 18656, 0},
+    {35.0 / 384, 0.0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84}};
+const double DP_B5[7] = {35.0 / 384, 0.0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84, 0.0};
+const double DP_B4[7] = {5179.0 / 57600, 0.0, 7571.0 / 16695, 393.0 / 640, -92097.0 / 339200, 187.0 / 2100, 1.0 / 40};
+
+int enqueue_mu_step(tdvp_handle *h, double dt) {
+  cudaStream_t st = h->stream;
+  const int n = h->n;
+  for (int sidx = 0; sidx < 7; sidx++) {
+    const std::vector<c128 *> *Y = &h->A;
+    if (sidx > 0) {
+      for (int i = 0; i < n; i++) {
+        Comb cb{}; cb.n = 0;
+        for (int j = 0; j < sidx; j++)
+          if (DP_A[sidx][j] != 0.0) { cb.k[cb.n] = h->mu_k[j][i]; cb.c[cb.n] = dt * DP_A[sidx][j]; cb.n++; }
+        TDVP_LAUNCH(lincomb_kernel, grid_for(site_elems(h, i)), VT, 0, st, h->mu_y[i], (const c128 *)h->A[i], cb,
+                    site_elems(h, i));
+      }
+      Y = &h->mu_y;
+    }
+    if (int rc = mu_rhs(h, *Y, h->mu_k[sidx])) return rc;
+  }
+  void *scratch = h->step_ws;
+  for (int i = 0; i < n; i++) {
+    Comb ce{}; ce.n = 0;
+    for (int j = 0; j < 7; j++)
+      if (DP_B5[j] - DP_B4[j] != 0.0) { ce.k[ce.n] = h->mu_k[j][i]; ce.c[ce.n] = dt * (DP_B5[j] - DP_B4[j]); ce.n++; }
+    TDVP_LAUNCH(lincomb_kernel, grid_for(site_elems(h, i)), VT, 0, st, h->mu_y[i], (const c128 *)nullptr, ce, site_elems(h, i));
+    vec_norm_sq(st, h->mu_y[i], site_elems(h, i), h->mu_err_dev + 1 + i, scratch);
+    Comb cb{}; cb.n = 0;
+    for (int j = 0; j < 7; j++)
+      if (DP_B5[j] != 0.0) { cb.k[cb.n] = h->mu_k[j][i]; cb.c[cb.n] = dt * DP_B5[j]; cb.n++; }
+    TDVP_LAUNCH(lincomb_kernel, grid_for(site_elems(h, i)), VT, 0, st, h->A[i], (const c128 *)h->A[i], cb, site_elems(h, i));
+  }
+  TDVP_LAUNCH(err_final_kernel, 1, 1, 0, st, h->mu_err_dev + 1, n, h->mu_err_dev);
+  return check_cuda(h, cudaGetLastError(), "tdvp_step_mu");
+}
+
+int prepare_mu(tdvp_handle *h) {
+  if (!h || h->n < 1) return set_err(h, TDVP_EINVAL, "handle has no chain");
+  if (h->n < 2) return set_err(h, TDVP_EINVAL, "TDVP-MU needs at least two sites");
+  if (int rc = mu_alloc(h)) return rc;
+  return TDVP_OK;
+}
+
+}  // namespace
+
 extern "C" {
+
 int tdvp_step_mu(tdvp_handle *h, double dt, double *err_est) {
-  (void)dt; (void)err_est;
-  return set_err(h, TDVP_ESTATE, "tdvp_step_mu: not built yet in this revision");
+  if (int rc = prepare_mu(h)) return rc;
+  if (h->centre != h->n - 1) {
+    if (int rc = move_gauge(h, h->n - 1)) return rc;
+  }
+  if (int rc = enqueue_mu_step(h, dt)) return rc;
+  if (err_est) {
+    if (int rc = check_cuda(h, cudaMemcpyAsync(err_est, h->mu_err_dev, sizeof(double), cudaMemcpyDeviceToHost, h->stream), "memcpy")) return rc;
+    return check_cuda(h, cudaStreamSynchronize(h->stream), "tdvp_step_mu sync");
+  }
+  return TDVP_OK;
 }
+
 int tdvp_mu_derivative(tdvp_handle *h, tdvp_c128 *const *out_host) {
-  (void)out_host;
-  return set_err(h, TDVP_ESTATE, "tdvp_mu_derivative: not built yet in this revision");
+  if (int rc = prepare_mu(h)) return rc;
+  if (!out_host) return set_err(h, TDVP_EINVAL, "null pointer");
+  if (h->centre != h->n - 1) return set_err(h, TDVP_ESTATE, "tdvp_mu_derivative needs the MU gauge (centre N-1): call tdvp_set_gauge");
+  if (int rc = mu_rhs(h, h->A, h->mu_k[0])) return rc;
+  for (int i = 0; i < h->n; i++) {
+    if (!out_host[i]) return set_err(h, TDVP_EINVAL, "null output tensor");
+    if (int rc = check_cuda(h, cudaMemcpyAsync(out_host[i], h->mu_k[0][i], site_elems(h, i) * 16, cudaMemcpyDeviceToHost, h->stream), "memcpy")) return rc;
+  }
+  return check_cuda(h, cudaStreamSynchronize(h->stream), "tdvp_mu_derivative");
 }
+
 int tdvp_svd_bond(tdvp_handle *h, int Ml, int d, int Mr, const tdvp_c128 *C, tdvp_c128 *U, double *lam, tdvp_c128 *Vh) {
-  (void)Ml; (void)d; (void)Mr; (void)C; (void)U; (void)lam; (void)Vh;
-  return set_err(h, TDVP_ESTATE, "tdvp_svd_bond: not built yet in this revision");
+  tdvp_handle *hh = h ? h : default_handle();
+  if (!C || !U || !lam || !Vh) return set_err(h, TDVP_EINVAL, "null pointer");
+  if (Ml < 1 || d < 1 || Mr < 1) return set_err(h, TDVP_EINVAL, "dimensions must be >= 1");
+  if ((long long)d * Mr < Ml) return set_err(h, TDVP_EINVAL, "matrix unfolding needs Ml <= d*Mr");
+  size_t sb = svd_ws_bytes(Ml, d, Mr);
+  if (int rc = check_cuda(h, hh->arena.reserve(sb + 1024, hh->stream), "workspace")) return rc;
+  hh->arena.reset();
+  void *ws = hh->arena.take(sb);
+  svd_bond(hh->stream, Ml, d, Mr, reinterpret_cast<const c128 *>(C), reinterpret_cast<c128 *>(U), lam,
+           reinterpret_cast<c128 *>(Vh), ws);
+  return check_cuda(h, cudaGetLastError(), "tdvp_svd_bond");
 }
-}
+
+}  // extern "C"

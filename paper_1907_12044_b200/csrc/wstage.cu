@@ -5,7 +5,7 @@
 // For every bond-index pair the stage is a sparse (rows x cols) matrix applied to a dense
 // cols x Mr panel whose rows are contiguous in y.  One CTA owns (batch index a, 32 consecutive y):
 // it stages the panel T1[a, :, y0:y0+32] in shared memory with 16 B cp.async copies, then each
-// warp produces output rows r = warp, warp + 8, ... with lane = y (coalesced 512 B row writes,
+// warp produces output rows r = warp, warp + 16, ... with lane = y (coalesced 512 B row writes,
 // conflict-free LDS.128), walking the row's CSR entries (warp-uniform loads).  HBM/L2 traffic is
 // exactly one read of T1 and one write of T2.
 #include "common.cuh"
@@ -13,46 +13,61 @@
 namespace {
 
 constexpr int YT = 32;          // y per CTA (one lane each)
-constexpr int WS_THREADS = 256;
+constexpr int WS_THREADS = 512;
 
-// Build CSR of the (nrows x ncols) matrix view of W.  which = 0: rows (s,v), cols (w,t) ["left"];
-// which = 1: rows (w,s), cols (t,v) ["right"].
-__global__ void csr_build_kernel(const c128 *W, int Dl, int d, int Dr, double tol,
-                                 int *rowptr0, int *col0, c128 *val0,
-                                 int *rowptr1, int *col1, c128 *val1) {
-  extern __shared__ int counts[];
-  const int which = blockIdx.x;
-  const int nrows = which == 0 ? d * Dr : Dl * d;
-  const int ncols = which == 0 ? Dl * d : d * Dr;
+// CSR of the (nrows x ncols) matrix view of W.  which = 0: rows (s,v), cols (w,t) ["left"];
+// which = 1: rows (w,s), cols (t,v) ["right"].  One warp per row; blockIdx.y = which.
+// Pass 1 counts the non-zeros of every row, pass 2 sums the counts of the rows before its own
+// (a few hundred integers) and writes the row's entries in column order (ballot prefix).
+constexpr int CSR_WARPS = 8;
+
+__device__ __forceinline__ long long csr_widx(int which, int r, int c, int Dl, int d, int Dr, int ncols) {
+  if (which == 0) { int s = r / Dr, v = r % Dr, w = c / d, t = c % d;
+                    return (((long long)w * d + s) * d + t) * Dr + v; }
+  return (long long)r * ncols + c;
+}
+
+__global__ void __launch_bounds__(CSR_WARPS * 32) csr_count_kernel(const c128 *W, int Dl, int d, int Dr, double tol,
+                                                                    int *cnt0, int *cnt1) {
+  const int which = blockIdx.y;
+  const int nrows = which == 0 ? d * Dr : Dl * d, ncols = which == 0 ? Dl * d : d * Dr;
+  const int lane = threadIdx.x & 31, r = blockIdx.x * CSR_WARPS + (threadIdx.x >> 5);
+  if (r >= nrows) return;
+  int n = 0;
+  for (int c0 = 0; c0 < ncols; c0 += 32) {
+    int c = c0 + lane;
+    bool nz = false;
+    if (c < ncols) { c128 x = W[csr_widx(which, r, c, Dl, d, Dr, ncols)]; nz = fabs(x.x) > tol || fabs(x.y) > tol; }
+    n += __popc(__ballot_sync(0xffffffffu, nz));
+  }
+  if (lane == 0) (which == 0 ? cnt0 : cnt1)[r] = n;
+}
+
+__global__ void __launch_bounds__(CSR_WARPS * 32) csr_fill_kernel(const c128 *W, int Dl, int d, int Dr, double tol,
+                                                                   const int *cnt0, const int *cnt1,
+                                                                   int *rowptr0, int *col0, c128 *val0,
+                                                                   int *rowptr1, int *col1, c128 *val1) {
+  const int which = blockIdx.y;
+  const int nrows = which == 0 ? d * Dr : Dl * d, ncols = which == 0 ? Dl * d : d * Dr;
+  const int *cnt = which == 0 ? cnt0 : cnt1;
   int *rowptr = which == 0 ? rowptr0 : rowptr1;
   int *col = which == 0 ? col0 : col1;
   c128 *val = which == 0 ? val0 : val1;
-  auto widx = [&](int r, int c) -> long long {
-    if (which == 0) { int s = r / Dr, v = r % Dr, w = c / d, t = c % d;
-                      return (((long long)w * d + s) * d + t) * Dr + v; }
-    return (long long)r * ncols + c;
-  };
-  for (int r = threadIdx.x; r < nrows; r += blockDim.x) {
-    int n = 0;
-    for (int c = 0; c < ncols; c++) {
-      c128 x = W[widx(r, c)];
-      n += (fabs(x.x) > tol || fabs(x.y) > tol) ? 1 : 0;
-    }
-    counts[r] = n;
-  }
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    int acc = 0;
-    for (int r = 0; r < nrows; r++) { int n = counts[r]; counts[r] = acc; rowptr[r] = acc; acc += n; }
-    rowptr[nrows] = acc;
-  }
-  __syncthreads();
-  for (int r = threadIdx.x; r < nrows; r += blockDim.x) {
-    int o = counts[r];
-    for (int c = 0; c < ncols; c++) {
-      c128 x = W[widx(r, c)];
-      if (fabs(x.x) > tol || fabs(x.y) > tol) { col[o] = c; val[o] = x; o++; }
-    }
+  const int lane = threadIdx.x & 31, r = blockIdx.x * CSR_WARPS + (threadIdx.x >> 5);
+  if (r >= nrows) return;
+  int o = 0;
+  for (int i = lane; i < r; i += 32) o += cnt[i];
+#pragma unroll
+  for (int k = 16; k > 0; k >>= 1) o += __shfl_xor_sync(0xffffffffu, o, k);
+  if (lane == 0) { rowptr[r] = o; if (r == nrows - 1) rowptr[nrows] = o + cnt[r]; }
+  for (int c0 = 0; c0 < ncols; c0 += 32) {
+    int c = c0 + lane;
+    bool nz = false;
+    c128 x = make_double2(0.0, 0.0);
+    if (c < ncols) { x = W[csr_widx(which, r, c, Dl, d, Dr, ncols)]; nz = fabs(x.x) > tol || fabs(x.y) > tol; }
+    unsigned m = __ballot_sync(0xffffffffu, nz);
+    if (nz) { int q = o + __popc(m & ((1u << lane) - 1u)); col[q] = c; val[q] = x; }
+    o += __popc(m);
   }
 }
 
@@ -65,14 +80,22 @@ struct WStageParams {
   const int *rowptr; const int *col; const c128 *val;
 };
 
+__device__ __forceinline__ void cfma(double &sx, double &sy, c128 w, c128 t) {
+  sx = fma(w.x, t.x, sx); sx = fma(-w.y, t.y, sx);
+  sy = fma(w.x, t.y, sy); sy = fma(w.y, t.x, sy);
+}
+
+// 16 warps per CTA and two CTAs per SM keep 8 warps per scheduler in flight; the entry loop is
+// unrolled by four with all index / value / panel loads issued before the FMAs, so that the DFMA
+// pipe (4 per entry and lane), not load latency, sets the pace at 15 % density, and HBM at ~3 %.
 template <bool STAGE_SMEM>
-__global__ void __launch_bounds__(WS_THREADS) wstage_kernel(WStageParams p) {
+__global__ void __launch_bounds__(WS_THREADS, 2) wstage_kernel(WStageParams p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   c128 *tile = reinterpret_cast<c128 *>(smem_raw);      // [ncols][YT]
   const int a = blockIdx.y;
   const int y0 = blockIdx.x * YT;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const c128 *in = p.in + a * p.in_bs;
+  const c128 *__restrict__ in = p.in + a * p.in_bs;
   const int y = y0 + lane;
   const bool yok = y < p.Mr;
   if (STAGE_SMEM) {
@@ -87,20 +110,26 @@ __global__ void __launch_bounds__(WS_THREADS) wstage_kernel(WStageParams p) {
     asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::);
     __syncthreads();
   }
+  const int *__restrict__ colp = p.col;
+  const c128 *__restrict__ valp = p.val;
+  const long long yc = yok ? y : 0;
+  auto panel = [&](int c) -> c128 {
+    if (STAGE_SMEM) return tile[c * YT + lane];
+    return __ldg(in + (long long)c * p.Mr + yc);
+  };
   c128 *out = p.out + a * p.o_bs;
   for (int r = warp; r < p.nrows; r += WS_THREADS / 32) {
-    const int e0 = p.rowptr[r], e1 = p.rowptr[r + 1];
-    double sx = 0.0, sy = 0.0;
-    for (int e = e0; e < e1; e++) {
-      const int c = __ldg(p.col + e);
-      const c128 w = __ldg(p.val + e);
-      c128 t;
-      if (STAGE_SMEM) t = tile[c * YT + lane];
-      else t = yok ? __ldg(in + (long long)c * p.Mr + y) : make_double2(0.0, 0.0);
-      sx = fma(w.x, t.x, sx); sx = fma(-w.y, t.y, sx);
-      sy = fma(w.x, t.y, sy); sy = fma(w.y, t.x, sy);
+    const int e0 = __ldg(p.rowptr + r), e1 = __ldg(p.rowptr + r + 1);
+    double sx0 = 0.0, sy0 = 0.0, sx1 = 0.0, sy1 = 0.0;
+    int e = e0;
+    for (; e + 4 <= e1; e += 4) {
+      const int c0 = __ldg(colp + e), c1 = __ldg(colp + e + 1), c2 = __ldg(colp + e + 2), c3 = __ldg(colp + e + 3);
+      const c128 w0 = __ldg(valp + e), w1 = __ldg(valp + e + 1), w2 = __ldg(valp + e + 2), w3 = __ldg(valp + e + 3);
+      const c128 t0 = panel(c0), t1 = panel(c1), t2 = panel(c2), t3 = panel(c3);
+      cfma(sx0, sy0, w0, t0); cfma(sx1, sy1, w1, t1); cfma(sx0, sy0, w2, t2); cfma(sx1, sy1, w3, t3);
     }
-    if (yok) out[(r / p.rdiv) * p.o_s1 + (r % p.rdiv) * p.o_s2 + y] = make_double2(sx, sy);
+    for (; e < e1; e++) cfma(sx0, sy0, __ldg(valp + e), panel(__ldg(colp + e)));
+    if (yok) out[(r / p.rdiv) * p.o_s1 + (r % p.rdiv) * p.o_s2 + y] = make_double2(sx0 + sx1, sy0 + sy1);
   }
 }
 
@@ -125,7 +154,7 @@ size_t wsparse_bytes(int Dl, int d, int Dr) {
   size_t cap = (size_t)Dl * d * d * Dr;
   size_t rows0 = (size_t)d * Dr + 1, rows1 = (size_t)Dl * d + 1;
   auto up = [](size_t x) { return (x + 255) & ~size_t(255); };
-  return up(rows0 * 4) + up(rows1 * 4) + 2 * up(cap * 4) + 2 * up(cap * 16) + 256;
+  return 2 * up(rows0 * 4) + 2 * up(rows1 * 4) + 2 * up(cap * 4) + 2 * up(cap * 16) + 256;
 }
 
 void wsparse_build(cudaStream_t st, WSparse &ws, void *mem, int Dl, int d, int Dr, const c128 *W,
@@ -141,8 +170,13 @@ void wsparse_build(cudaStream_t st, WSparse &ws, void *mem, int Dl, int d, int D
   ws.col_r = reinterpret_cast<int *>(p); p += up(cap * 4);
   ws.rowptr = reinterpret_cast<int *>(p); p += up(((size_t)d * Dr + 1) * 4);
   ws.rowptr_r = reinterpret_cast<int *>(p);
+  p += up(((size_t)Dl * d + 1) * 4);
+  int *cnt0 = reinterpret_cast<int *>(p); p += up(((size_t)d * Dr + 1) * 4);
+  int *cnt1 = reinterpret_cast<int *>(p);
   int maxrows = (d * Dr > Dl * d ? d * Dr : Dl * d);
-  TDVP_LAUNCH(csr_build_kernel, 2, 256, maxrows * sizeof(int), st, W, Dl, d, Dr, zero_tol,
+  dim3 grid((maxrows + CSR_WARPS - 1) / CSR_WARPS, 2);
+  TDVP_LAUNCH(csr_count_kernel, grid, CSR_WARPS * 32, 0, st, W, Dl, d, Dr, zero_tol, cnt0, cnt1);
+  TDVP_LAUNCH(csr_fill_kernel, grid, CSR_WARPS * 32, 0, st, W, Dl, d, Dr, zero_tol, cnt0, cnt1,
               ws.rowptr, ws.col, ws.val, ws.rowptr_r, ws.col_r, ws.val_r);
 }
 

@@ -282,3 +282,81 @@ def test_errors_are_reported(T):
     bad[3] = bad[3] * 1.5                               # not right-canonical
     with pytest.raises(T.TdvpError):
         T.tdvp_create(mpo, bad)
+
+
+# ---- TDVP-MU: matrix unfolding (Eq. 36), derivative (Eq. 27, 37, 38), Dormand-Prince step ------
+@pytest.mark.parametrize("shape", [(1, 3, 4), (4, 3, 4), (12, 4, 16), (37, 5, 29), (64, 10, 64), (70, 3, 130)])
+@pytest.mark.parametrize("deficient", [False, True])
+def test_svd_bond(T, shape, deficient):
+    Ml, d, Mr = shape
+    rng = np.random.default_rng(500 + Ml + Mr)
+    C = si.complex_normal(rng, shape)
+    if deficient and Ml > 2:                       # graded singular values and an exact null space
+        Um, _ = np.linalg.qr(si.complex_normal(rng, (Ml, Ml)))
+        Vm, _ = np.linalg.qr(si.complex_normal(rng, (d * Mr, Ml)))
+        sv = np.logspace(0, -10, Ml)
+        sv[-2:] = 0.0
+        C = ((Um * sv[None, :]) @ Vm.conj().T).reshape(shape)
+    U, lam, Vh = [host(x) for x in T.tdvp_svd_bond(dev(C))]
+    Vm = Vh.reshape(Ml, d * Mr)
+    tol = 1e-13 * max(Ml, 8)
+    assert np.abs(U.conj().T @ U - np.eye(Ml)).max() < tol
+    assert np.abs(Vm @ Vm.conj().T - np.eye(Ml)).max() < tol              # Eq. 8
+    assert np.all(np.diff(lam) <= 0) and np.all(lam >= 0)
+    want = np.linalg.svd(C.reshape(Ml, d * Mr), compute_uv=False)
+    assert np.abs(lam - want).max() <= 1e-13 * want[0]
+    assert rel(((U * lam[None, :]) @ Vm).reshape(shape), C) < 1e-13
+
+
+def _warm_left_canonical(n_warm=3):
+    from oracle import tdvp_mu
+    cfg, mpo, st = _tiny_state(n_warm)
+    return cfg, mpo, tdvp_mu.to_left_canonical(st.mps)
+
+
+def test_mu_derivative(T):
+    from oracle import tdvp_mu
+    cfg, mpo, mpsL = _warm_left_canonical()
+    want = tdvp_mu.mu_derivative(mpo, mpsL)
+    ch = T.tdvp_create(mpo, tdvp_mu.to_right_canonical(mpsL))
+    ch.tdvp_set_mps(mpsL, centre=ch.n - 1)
+    got = ch.tdvp_mu_derivative()
+    scale = max(np.linalg.norm(w) for w in want)         # complete bonds have (1 - p) = 0: dL/dt = round-off there
+    for g, w in zip(got, want):
+        assert np.linalg.norm(g - w) <= 1e-8 * scale
+    for g, Lsite in zip(got[:-1], mpsL[:-1]):                              # Eq. 34: L^dagger dL/dt = 0
+        a, s, b = Lsite.shape
+        assert np.abs(Lsite.reshape(a * s, b).conj().T @ g.reshape(a * s, b)).max() < 1e-9
+    ch.close()
+
+
+def test_mu_step_matches_oracle_and_ps(T):
+    """Dormand-Prince steps of h = 0.1 fs after a shared PS warm-up."""
+    from oracle import tdvp_mu
+    cfg, mpo, mpsL = _warm_left_canonical()
+    ch = T.tdvp_create(mpo, tdvp_mu.to_right_canonical(mpsL))
+    ch.tdvp_set_mps(mpsL, centre=ch.n - 1)
+    cur = mpsL
+    for s in range(4):
+        cur, err_want = tdvp_mu.step_mu(mpo, cur, 0.1)
+        err_got = ch.tdvp_step_mu(0.1, want_err=True)
+        assert abs(err_got - err_want) <= 1e-6 * max(err_want, 1e-12) + 1e-14
+        assert np.abs(ch.tdvp_populations(0) - obs.populations(cur, 0)).max() <= 1e-8
+    nrm, en = ch.tdvp_norm_energy()
+    assert abs(nrm - obs.norm_sq(cur)) < 1e-10 and abs(en - obs.energy(mpo, cur)) < 1e-9
+    # switching back to the PS gauge leaves the state unchanged
+    p = ch.tdvp_populations(0)
+    ch.tdvp_set_gauge(0)
+    assert np.abs(ch.tdvp_populations(0) - p).max() < 1e-12
+    ch.close()
+
+
+def test_mu_step_from_ps_gauge(T):
+    """tdvp_step_mu on a handle in the PS gauge first moves the centre (no time evolution)."""
+    cfg, mpo, st = _tiny_state(3)
+    ch = T.tdvp_create(mpo, st.mps)
+    p0 = ch.tdvp_populations(0)
+    ch.tdvp_step_mu(1e-6)
+    assert ch.tdvp_get_centre() == ch.n - 1
+    assert np.abs(ch.tdvp_populations(0) - p0).max() < 1e-6
+    ch.close()
