@@ -133,10 +133,91 @@ __global__ void __launch_bounds__(WS_THREADS, 2) wstage_kernel(WStageParams p) {
   }
 }
 
+// Persistent variant: one CTA of 32 warps per SM walks over (a, y-tile) work items.  The CSR of W
+// (values, columns, row pointers) is staged ONCE per CTA in shared memory when it fits beside the
+// panel (it does for every MPO of the paper's workloads and for the 15 % microbench), so the entry
+// loop issues shared-memory loads only.  At 15 % density the loop is bound by the shared-memory
+// crossbar (16 B of panel per 4 DFMA and lane); at the ~3 % density of real MPOs by HBM.
+constexpr int WP_THREADS = 1024;
+constexpr int WP_SMEM = 227 * 1024;
+
+template <bool CSR_SMEM>
+__device__ __forceinline__ void wp_rows(const WStageParams &p, const c128 *tile, const c128 *__restrict__ gval,
+                                        const int *__restrict__ gcol, const int *__restrict__ grow, c128 *out,
+                                        int y, int lane, int warp, int split, int nsplit) {
+  for (int r = split + nsplit * warp; r < p.nrows; r += nsplit * (WP_THREADS / 32)) {
+    const int e0 = grow[r], e1 = grow[r + 1];
+    double sx0 = 0.0, sy0 = 0.0, sx1 = 0.0, sy1 = 0.0;
+    int e = e0;
+    for (; e + 4 <= e1; e += 4) {
+      const int c0 = gcol[e], c1 = gcol[e + 1], c2 = gcol[e + 2], c3 = gcol[e + 3];
+      const c128 w0 = gval[e], w1 = gval[e + 1], w2 = gval[e + 2], w3 = gval[e + 3];
+      const c128 t0 = tile[c0 * YT + lane], t1 = tile[c1 * YT + lane], t2 = tile[c2 * YT + lane], t3 = tile[c3 * YT + lane];
+      cfma(sx0, sy0, w0, t0); cfma(sx1, sy1, w1, t1); cfma(sx0, sy0, w2, t2); cfma(sx1, sy1, w3, t3);
+    }
+    for (; e < e1; e++) cfma(sx0, sy0, gval[e], tile[gcol[e] * YT + lane]);
+    if (y < p.Mr) out[(r / p.rdiv) * p.o_s1 + (r % p.rdiv) * p.o_s2 + y] = make_double2(sx0 + sx1, sy0 + sy1);
+  }
+}
+
+__global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStageParams p, int ntile, int nitems, int nsplit) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  c128 *tile = reinterpret_cast<c128 *>(smem_raw);                        // [ncols][YT]
+  const int tile_elems = p.ncols * YT;
+  const int nnz = __ldg(p.rowptr + p.nrows);
+  const size_t csr_off = (size_t)tile_elems * 16;
+  const bool csr_smem = csr_off + (size_t)nnz * 20 + (size_t)(p.nrows + 1) * 4 + 64 <= (size_t)WP_SMEM;
+  c128 *sval = reinterpret_cast<c128 *>(smem_raw + csr_off);
+  int *scol = reinterpret_cast<int *>(smem_raw + csr_off + (size_t)nnz * 16);
+  int *srow = scol + nnz;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (csr_smem) {
+    for (int e = threadIdx.x; e < nnz; e += WP_THREADS) { sval[e] = __ldg(p.val + e); scol[e] = __ldg(p.col + e); }
+    for (int e = threadIdx.x; e <= p.nrows; e += WP_THREADS) srow[e] = __ldg(p.rowptr + e);
+  }
+  for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+    const int split = item % nsplit, panel = item / nsplit;
+    const int a = panel / ntile, y0 = (panel % ntile) * YT;
+    const c128 *in = p.in + a * p.in_bs;
+    __syncthreads();                                   // previous item's readers are done with the panel
+    for (int e = threadIdx.x; e < tile_elems; e += WP_THREADS) {
+      const int c = e / YT, yy = e % YT;
+      const bool ok = (y0 + yy) < p.Mr;
+      const c128 *src = ok ? in + (long long)c * p.Mr + y0 + yy : in;
+      unsigned sa = (unsigned)__cvta_generic_to_shared(tile + e);
+      int sz = ok ? 16 : 0;
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(src), "r"(sz));
+    }
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::);
+    __syncthreads();
+    c128 *out = p.out + a * p.o_bs;
+    if (csr_smem) wp_rows<true>(p, tile, sval, scol, srow, out, y0 + lane, lane, warp, split, nsplit);
+    else wp_rows<false>(p, tile, p.val, p.col, p.rowptr, out, y0 + lane, lane, warp, split, nsplit);
+  }
+}
+
+int g_num_sms = 0;
+
 void launch_wstage(cudaStream_t st, const WStageParams &p, int nbatch) {
-  dim3 grid((p.Mr + YT - 1) / YT, nbatch);
+  const int ntile = (p.Mr + YT - 1) / YT;
   size_t smem = (size_t)p.ncols * YT * 16;
   ProfScope ps(st, PH_WSTAGE);
+  if (smem + 4096 <= (size_t)WP_SMEM) {
+    if (!g_num_sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev); }
+    // split the rows of a panel over several work items when the panels alone balance badly
+    int nsplit = 1;
+    while (nsplit < 4 && p.nrows >= 64 * nsplit) {
+      const long long it = (long long)nbatch * ntile * nsplit;
+      const long long rounds = (it + g_num_sms - 1) / g_num_sms;
+      if (it >= g_num_sms && (double)it / (double)(rounds * g_num_sms) > 0.93) break;
+      nsplit *= 2;
+    }
+    const int nitems = nbatch * ntile * nsplit;
+    const int grid = nitems < g_num_sms ? nitems : g_num_sms;
+    TDVP_LAUNCH(wstage_persistent_kernel, grid, WP_THREADS, WP_SMEM, st, p, ntile, nitems, nsplit);
+    return;
+  }
+  dim3 grid(ntile, nbatch);
   if (smem <= 200 * 1024) {
     TDVP_LAUNCH(wstage_kernel<true>, grid, WS_THREADS, smem, st, p);
   } else {
@@ -148,6 +229,7 @@ void launch_wstage(cudaStream_t st, const WStageParams &p, int nbatch) {
 
 void wstage_configure() {
   cudaFuncSetAttribute(wstage_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  cudaFuncSetAttribute(wstage_persistent_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, WP_SMEM);
 }
 
 size_t wsparse_bytes(int Dl, int d, int Dr) {
