@@ -80,6 +80,185 @@ __global__ void store_d_kernel(const c128 *Rm, c128 *D, int cols, int transpose_
   }
 }
 
+// ---- register-resident panel factorisation ---------------------------------------------------
+// Same contract as qr_panel_kernel below, for rows - j0 <= RP_THREADS * RPT.  Every thread keeps
+// its RPT rows of the NB panel columns in registers; each column costs ONE block-wide reduction:
+// the sums s = sum_{i>=jj} |x_i|^2 and d_c = sum_{i>=jj} conj(x_i) y_c[i] give the reflector AND
+// its products with the remaining panel columns, because v differs from x only in the pivot row:
+//   v^H y_c = y_c[jj] + conj(scal) (d_c - conj(alpha) y_c[jj]),   v = [1; x_{i>jj} scal].
+constexpr int RP_THREADS = 256;
+constexpr int RP_WARPS = RP_THREADS / 32;
+
+template <int N>
+__device__ __forceinline__ void block_sum(double (&v)[N], double *sm /*[N][RP_THREADS] + [N]*/) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int i = 0; i < N; i++) sm[i * RP_THREADS + threadIdx.x] = v[i];
+  __syncthreads();
+  for (int i = warp; i < N; i += RP_WARPS) {             // fixed summation order: deterministic
+    double t = 0.0;
+#pragma unroll
+    for (int k = 0; k < RP_THREADS / 32; k++) t += sm[i * RP_THREADS + k * 32 + lane];
+    t = warp_sum_d(t);
+    if (lane == 0) sm[N * RP_THREADS + i] = t;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < N; i++) v[i] = sm[N * RP_THREADS + i];
+  __syncthreads();
+}
+
+template <int RPT, int NB, int JJ>
+__device__ __forceinline__ void qr_panel_col(c128 (&x)[RPT][NB], c128 (*pivot)[NB], double *sm, c128 *tau_s, c128 *Rm,
+                                             int cols, int j0, int len, int tid) {
+  constexpr int jj = JJ;
+  constexpr int NRED = 1 + 2 * (NB - 1);
+
+      double red[NRED];
+#pragma unroll
+      for (int q = 0; q < NRED; q++) red[q] = 0.0;
+#pragma unroll
+      for (int r = 0; r < RPT; r++) {
+        const int i = tid + r * RP_THREADS;
+        if (i >= jj && i < len) {
+          const c128 u = x[r][jj];
+          red[0] += u.x * u.x + u.y * u.y;
+          if (i == jj) pivot[jj & 1][jj] = u;
+#pragma unroll
+          for (int c = jj + 1; c < NB; c++) {
+            const c128 yv = x[r][c];
+            red[1 + 2 * (c - 1)] += u.x * yv.x + u.y * yv.y;
+            red[2 + 2 * (c - 1)] += u.x * yv.y - u.y * yv.x;
+            if (i == jj) pivot[jj & 1][c] = yv;
+          }
+        }
+      }
+      block_sum<NRED>(red, sm);
+      const c128 alpha = pivot[jj & 1][jj];
+      double xn2 = red[0] - (alpha.x * alpha.x + alpha.y * alpha.y);
+      if (xn2 < 0.0) xn2 = 0.0;
+      c128 tau, scal;
+      double beta;
+      if (xn2 == 0.0 && alpha.y == 0.0) {
+        tau = make_double2(0.0, 0.0); scal = make_double2(0.0, 0.0); beta = alpha.x;
+      } else {
+        const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xn2);
+        beta = alpha.x >= 0.0 ? -nrm : nrm;
+        tau = make_double2((beta - alpha.x) / beta, -alpha.y / beta);
+        const double dr = alpha.x - beta, di = alpha.y, dn = dr * dr + di * di;
+        scal = make_double2(dr / dn, -di / dn);
+      }
+      if (tid == 0) { tau_s[jj] = tau; Rm[(long long)(j0 + jj) * cols + j0 + jj] = make_double2(beta, 0.0); }
+      c128 g[NB];                                        // conj(tau) * (v^H y_c)
+#pragma unroll
+      for (int c = jj + 1; c < NB; c++) {
+        const c128 dc = make_double2(red[1 + 2 * (c - 1)], red[2 + 2 * (c - 1)]);
+        const c128 yj = pivot[jj & 1][c];
+        const c128 t1 = cmul(cconj(alpha), yj);
+        const c128 t2 = cmul(cconj(scal), make_double2(dc.x - t1.x, dc.y - t1.y));
+        g[c] = cmul(cconj(tau), make_double2(yj.x + t2.x, yj.y + t2.y));
+      }
+#pragma unroll
+      for (int r = 0; r < RPT; r++) {
+        const int i = tid + r * RP_THREADS;
+        if (i < len) {
+          if (i < jj) {                                  // above the diagonal: an R entry, zero in V
+            Rm[(long long)(j0 + i) * cols + j0 + jj] = x[r][jj];
+            x[r][jj] = make_double2(0.0, 0.0);
+          } else {
+            const c128 v = (i == jj) ? make_double2(1.0, 0.0) : cmul(x[r][jj], scal);
+            x[r][jj] = v;
+#pragma unroll
+            for (int c = jj + 1; c < NB; c++) {
+              const c128 t = cmul(g[c], v);
+              x[r][c].x -= t.x; x[r][c].y -= t.y;
+            }
+          }
+        }
+      }
+}
+
+template <int RPT, int NB>
+__global__ void __launch_bounds__(RP_THREADS, 1) qr_panel_reg_kernel(c128 *X, int rows, int cols, int j0, int w,
+                                                                   c128 *Rm, c128 *Tm /*[NB_MAX][NB_MAX]*/) {
+  constexpr int NRED = 1 + 2 * (NB - 1);                 // s and d_c for the other columns
+  __shared__ c128 pivot[2][NB];                          // pivot row (alpha, y_c[jj]), double-buffered over jj
+  constexpr int NSM = NRED;
+  __shared__ double sm[(RP_THREADS + 1) * (NSM > 0 ? NSM : 1)];
+  __shared__ c128 tau_s[NB];
+  __shared__ c128 Ts[NB_MAX * NB_MAX];
+  __shared__ c128 Gs[NB_MAX * NB_MAX];
+  const int len = rows - j0, tid = threadIdx.x;
+  c128 x[RPT][NB];
+#pragma unroll
+  for (int r = 0; r < RPT; r++) {
+    const int i = tid + r * RP_THREADS;
+#pragma unroll
+    for (int c = 0; c < NB; c++)
+      x[r][c] = (i < len && c < w) ? X[(long long)(j0 + c) * rows + j0 + i] : make_double2(0.0, 0.0);
+  }
+  for (int e = tid; e < w * j0; e += RP_THREADS) {        // R entries above the panel rows are final
+    int c = e / j0, i = e % j0;
+    Rm[(long long)i * cols + j0 + c] = X[(long long)(j0 + c) * rows + i];
+  }
+  for (int e = tid; e < w * cols; e += RP_THREADS) {      // zeros below the diagonal of R
+    int c = e / cols, i = e % cols;
+    if (i > j0 + c) Rm[(long long)i * cols + j0 + c] = make_double2(0.0, 0.0);
+  }
+  // columns one by one (compile-time column index keeps the panel in registers)
+#define TDVP_QR_COL(J) if (J < NB && J < w) qr_panel_col<RPT, NB, (J < NB ? J : 0)>(x, pivot, sm, tau_s, Rm, cols, j0, len, tid);
+  TDVP_QR_COL(0) TDVP_QR_COL(1) TDVP_QR_COL(2) TDVP_QR_COL(3) TDVP_QR_COL(4) TDVP_QR_COL(5) TDVP_QR_COL(6) TDVP_QR_COL(7)
+#undef TDVP_QR_COL
+  // compact WY factor from the strictly upper Gram entries v_a^H v_b
+  if (NB > 1) {
+#pragma unroll
+    for (int a = 0; a < NB - 1; a++) {                   // row a of the strictly upper Gram matrix v_a^H v_b
+      double gr[2 * (NB - 1)];
+#pragma unroll
+      for (int q = 0; q < 2 * (NB - 1); q++) gr[q] = 0.0;
+#pragma unroll
+      for (int r = 0; r < RPT; r++) {
+        const c128 u = x[r][a];
+#pragma unroll
+        for (int b = a + 1; b < NB; b++) {
+          const c128 v = x[r][b];
+          gr[2 * (b - 1)] += u.x * v.x + u.y * v.y;
+          gr[2 * (b - 1) + 1] += u.x * v.y - u.y * v.x;
+        }
+      }
+      block_sum<2 * (NB - 1)>(gr, sm);
+      if (tid == 0) {
+#pragma unroll
+        for (int b = a + 1; b < NB; b++) Gs[a * NB_MAX + b] = make_double2(gr[2 * (b - 1)], gr[2 * (b - 1) + 1]);
+      }
+    }
+    if (tid == 0) {
+      auto gram = [&](int a, int b) -> c128 { return Gs[a * NB_MAX + b]; };
+      for (int a = 0; a < NB_MAX * NB_MAX; a++) Ts[a] = make_double2(0.0, 0.0);
+      for (int c = 0; c < w; c++) {
+        Ts[c * NB_MAX + c] = tau_s[c];
+        for (int a = 0; a < c; a++) {
+          c128 acc = make_double2(0.0, 0.0);
+          for (int qq = a; qq < c; qq++) { c128 t = cmul(Ts[a * NB_MAX + qq], gram(qq, c)); acc.x += t.x; acc.y += t.y; }
+          c128 t = cmul(tau_s[c], acc);
+          Ts[a * NB_MAX + c] = make_double2(-t.x, -t.y);
+        }
+      }
+      for (int a = 0; a < NB_MAX * NB_MAX; a++) Tm[a] = Ts[a];
+    }
+  } else if (tid == 0) {
+    for (int a = 0; a < NB_MAX * NB_MAX; a++) Tm[a] = make_double2(0.0, 0.0);
+    Tm[0] = tau_s[0];
+  }
+#pragma unroll
+  for (int r = 0; r < RPT; r++) {
+    const int i = tid + r * RP_THREADS;
+#pragma unroll
+    for (int c = 0; c < NB; c++)
+      if (i < len && c < w) X[(long long)(j0 + c) * rows + j0 + i] = x[r][c];
+  }
+}
+
 // Factor the panel of columns [j0, j0+w) on rows [j0, rows).  Writes reflectors back into X (unit
 // diagonal explicit, zeros above it inside the panel rows), R entries of these columns into Rm
 // (row-major cols x cols, zeros below the diagonal), tau and the w x w upper-triangular T.
@@ -312,6 +491,80 @@ __global__ void __launch_bounds__(TRAIL_THREADS) qr_apply_kernel(const c128 *X, 
   }
 }
 
+// One trailing column per CTA, rows distributed over the threads, the reflector block V and the
+// column kept in registers between the product V^H y and the update y -= V (Top V^H y): V is read
+// once, and the launch fills up to cols CTAs instead of cols / CB.
+template <int AT, int RA>
+__global__ void __launch_bounds__(AT) qr_apply1_kernel(const c128 *X, c128 *Y, int rows, int j0, int w,
+                                                        const c128 *Tm, int adjoint, int c_begin) {
+  __shared__ double sm[(AT + 1) * 2 * NB_MAX];
+  const int len = rows - j0, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int c = c_begin + blockIdx.x;
+  c128 y[RA], v[RA][NB_MAX];
+#pragma unroll
+  for (int r = 0; r < RA; r++) {
+    const int i = tid + r * AT;
+    y[r] = i < len ? Y[(long long)c * rows + j0 + i] : make_double2(0.0, 0.0);
+#pragma unroll
+    for (int q = 0; q < NB_MAX; q++)
+      v[r][q] = (i < len && q < w) ? X[(long long)(j0 + q) * rows + j0 + i] : make_double2(0.0, 0.0);
+  }
+  double acc[2 * NB_MAX];
+#pragma unroll
+  for (int q = 0; q < 2 * NB_MAX; q++) acc[q] = 0.0;
+#pragma unroll
+  for (int r = 0; r < RA; r++)
+#pragma unroll
+    for (int q = 0; q < NB_MAX; q++) {
+      acc[2 * q] += v[r][q].x * y[r].x + v[r][q].y * y[r].y;
+      acc[2 * q + 1] += v[r][q].x * y[r].y - v[r][q].y * y[r].x;
+    }
+#pragma unroll
+  for (int q = 0; q < 2 * NB_MAX; q++) sm[q * AT + tid] = acc[q];
+  __syncthreads();
+  for (int q = warp; q < 2 * NB_MAX; q += AT / 32) {
+    double t = 0.0;
+#pragma unroll
+    for (int k = 0; k < AT / 32; k++) t += sm[q * AT + k * 32 + lane];
+    t = warp_sum_d(t);
+    if (lane == 0) sm[2 * NB_MAX * AT + q] = t;
+  }
+  __syncthreads();
+  c128 dv[NB_MAX], sv[NB_MAX];
+#pragma unroll
+  for (int q = 0; q < NB_MAX; q++) dv[q] = make_double2(sm[2 * NB_MAX * AT + 2 * q], sm[2 * NB_MAX * AT + 2 * q + 1]);
+#pragma unroll
+  for (int q = 0; q < NB_MAX; q++) {
+    c128 a = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int r = 0; r < NB_MAX; r++) {
+      const c128 t = adjoint ? cconj(__ldg(Tm + r * NB_MAX + q)) : __ldg(Tm + q * NB_MAX + r);
+      const c128 pr = cmul(t, dv[r]);
+      a.x += pr.x; a.y += pr.y;
+    }
+    sv[q] = a;
+  }
+#pragma unroll
+  for (int r = 0; r < RA; r++) {
+    const int i = tid + r * AT;
+    if (i < len) {
+      c128 o = y[r];
+#pragma unroll
+      for (int q = 0; q < NB_MAX; q++) { const c128 t = cmul(v[r][q], sv[q]); o.x -= t.x; o.y -= t.y; }
+      Y[(long long)c * rows + j0 + i] = o;
+    }
+  }
+}
+
+void launch_apply(cudaStream_t st, const c128 *X, c128 *Y, int rows, int j0, int w, const c128 *Tp, int adjoint,
+                  int c_begin, int c_end) {
+  if (c_begin >= c_end) return;
+  const int len = rows - j0, n = c_end - c_begin;
+  if (len <= 10 * 128) TDVP_LAUNCH((qr_apply1_kernel<128, 10>), n, 128, 0, st, X, Y, rows, j0, w, Tp, adjoint, c_begin);
+  else if (len <= 10 * 256) TDVP_LAUNCH((qr_apply1_kernel<256, 10>), n, 256, 0, st, X, Y, rows, j0, w, Tp, adjoint, c_begin);
+  else TDVP_LAUNCH(qr_apply_kernel, (n + CB - 1) / CB, TRAIL_THREADS, 0, st, X, Y, rows, j0, w, Tp, adjoint, c_begin, c_end);
+}
+
 int panel_width(int rows) {
   long long budget = 200 * 1024;
   int nb = (int)(budget / ((long long)rows * 16));
@@ -325,9 +578,19 @@ void qr_configure() {
   cudaFuncSetAttribute(qr_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024 + 1024);
 }
 
+// Panel variant by height: register-resident panels up to 5120 rows, the shared-memory panel beyond.
+int panel_mode(int rows, int *nb) {
+  if (rows <= 5 * RP_THREADS) { *nb = 8; return 1; }
+  if (rows <= 10 * RP_THREADS) { *nb = 4; return 2; }
+  if (rows <= 20 * RP_THREADS) { *nb = 2; return 3; }
+  *nb = panel_width(rows);
+  return 0;
+}
+
 size_t qr_ws_bytes(int rows, int cols) {
   size_t mat = up256((size_t)rows * cols * 16);
-  int nb = panel_width(rows);
+  int nb = 1;
+  panel_mode(rows, &nb);
   if (nb < 1) nb = 1;
   size_t npanels = (cols + nb - 1) / nb;
   return 2 * mat + up256((size_t)cols * cols * 16) + up256(npanels * NB_MAX * NB_MAX * 16) + 512;
@@ -336,7 +599,8 @@ size_t qr_ws_bytes(int rows, int cols) {
 void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c128 *Q, c128 *D, void *ws) {
   const int rows = side == 0 ? Ml * d : d * Mr;
   const int cols = side == 0 ? Mr : Ml;
-  const int nb = panel_width(rows);
+  int nb = 1;
+  const int mode = panel_mode(rows, &nb);
   ProfScope ps(st, PH_QR);
   char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
   size_t mat = up256((size_t)rows * cols * 16);
@@ -353,17 +617,18 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
   for (int pz = 0; pz < npanels; pz++) {
     int j0 = pz * nb, w = cols - j0 < nb ? cols - j0 : nb;
     size_t smem = (size_t)w * (rows - j0) * 16;
-    TDVP_LAUNCH(qr_panel_kernel, 1, PANEL_THREADS, smem, st, X, rows, cols, j0, w, Rm, Tm + (size_t)pz * NB_MAX * NB_MAX);
+    c128 *Tp = Tm + (size_t)pz * NB_MAX * NB_MAX;
+    if (mode == 1) TDVP_LAUNCH((qr_panel_reg_kernel<5, 8>), 1, RP_THREADS, 0, st, X, rows, cols, j0, w, Rm, Tp);
+    else if (mode == 2) TDVP_LAUNCH((qr_panel_reg_kernel<10, 4>), 1, RP_THREADS, 0, st, X, rows, cols, j0, w, Rm, Tp);
+    else if (mode == 3) TDVP_LAUNCH((qr_panel_reg_kernel<20, 2>), 1, RP_THREADS, 0, st, X, rows, cols, j0, w, Rm, Tp);
+    else TDVP_LAUNCH(qr_panel_kernel, 1, PANEL_THREADS, smem, st, X, rows, cols, j0, w, Rm, Tp);
     int c_begin = j0 + w;
-    if (c_begin < cols)
-      TDVP_LAUNCH(qr_apply_kernel, (cols - c_begin + CB - 1) / CB, TRAIL_THREADS, 0, st, X, X, rows, j0, w,
-                  Tm + (size_t)pz * NB_MAX * NB_MAX, 1, c_begin, cols);
+    launch_apply(st, X, X, rows, j0, w, Tp, 1, c_begin, cols);
   }
   TDVP_LAUNCH(identity_kernel, gcopy, 256, 0, st, Y, rows, cols);
   for (int pz = npanels - 1; pz >= 0; pz--) {
     int j0 = pz * nb, w = cols - j0 < nb ? cols - j0 : nb;
-    TDVP_LAUNCH(qr_apply_kernel, (cols - j0 + CB - 1) / CB, TRAIL_THREADS, 0, st, X, Y, rows, j0, w,
-                Tm + (size_t)pz * NB_MAX * NB_MAX, 0, j0, cols);
+    launch_apply(st, X, Y, rows, j0, w, Tm + (size_t)pz * NB_MAX * NB_MAX, 0, j0, cols);
   }
   if (side == 0) TDVP_LAUNCH(transpose_out_kernel, tg, tb, 0, st, Y, Q, rows, cols);
   else TDVP_LAUNCH(copy_kernel, gcopy, 256, 0, st, Q, Y, n);

@@ -9,14 +9,17 @@
 //      even when C is rank deficient (columns of X with norm ~ 0)
 //   4. lam = |diag R'| sorted descending, U = U' sgn(R') permuted, Vh = (J permuted)^H Q  (DMMA GEMM)
 //
-// The Jacobi sweeps run in ONE CTA (32 warps, a column pair per warp and round, round-robin
-// ordering, __syncthreads between rounds; X and J live in L2): no host round trip, deterministic,
-// capturable in the step graph.
+// The Jacobi sweeps run in one thread-block cluster (8 CTAs, a column pair per warp and round,
+// round-robin ordering, cluster barrier between rounds; X and J live in L2): no host round trip,
+// deterministic, capturable in the step graph.
+#include <cooperative_groups.h>
+
 #include "common.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace {
 
-constexpr int JT = 1024;            // threads of the Jacobi CTA
 constexpr int MAX_SWEEPS = 40;
 inline size_t up256(size_t x) { return (x + 255) & ~size_t(255); }
 
@@ -36,59 +39,105 @@ __global__ void svd_init_kernel(const c128 *D, c128 *Xt, c128 *Jt, int n) {
 }
 
 // One-sided Jacobi: rotate column pairs of X (and J) until all columns are mutually orthogonal.
-__global__ void __launch_bounds__(JT) svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *sweeps_out) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = JT / 32;
+// The n/2 pairs of a round are independent; the scalar FP64 work per pair (three square roots, three
+// divisions) is what a single SM cannot issue fast enough, so the round is spread over a thread-block
+// CLUSTER of 8 CTAs (8 SMs, one pair per warp and round at n = 128) with a hardware cluster barrier
+// between rounds.  X and J live in L2: loads bypass L1 (ld.global.cg), the barrier's release /
+// acquire orders the stores of one round before the loads of the next.
+// NPL = rows per lane held in registers (n <= 32 * NPL); NPL = 0 is the generic looped variant.
+constexpr int JC = 8;               // CTAs per cluster
+constexpr int JW = 8;               // warps per CTA
+
+template <int NPL>
+__global__ void __cluster_dims__(JC, 1, 1) __launch_bounds__(JW * 32)
+svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/) {
+  cg::cluster_group cluster = cg::this_cluster();
+  const int lane = threadIdx.x & 31;
+  const int gwarp = blockIdx.x * JW + (threadIdx.x >> 5), nwarps = JC * JW;
   const int np = (n + 1) & ~1;             // players of the round-robin tournament (a bye if n is odd)
   const int npairs = np / 2;
-  __shared__ int rotated;
-  const double tol = 1e-15;
-  int sweep = 0;
-  for (; sweep < MAX_SWEEPS; sweep++) {
-    if (threadIdx.x == 0) rotated = 0;
-    __syncthreads();
+  const double tol = 2.220446049250313e-16 * sqrt((double)n);   // LAPACK zgesvj: sqrt(m) * eps
+  const double tol2 = tol * tol;
+  for (int sweep = 0; sweep < MAX_SWEEPS; sweep++) {
+    bool any = false;
     for (int round = 0; round < np - 1; round++) {
-      for (int k = warp; k < npairs; k += nwarps) {
+      for (int k = gwarp; k < npairs; k += nwarps) {
         int p, q;
         if (k == 0) { p = round; q = np - 1; }
         else { p = (round + k) % (np - 1); q = (round - k + (np - 1)) % (np - 1); }
         if (p > q) { int t = p; p = q; q = t; }
         if (q >= n) continue;                                    // the bye
         c128 *xp = Xt + (long long)p * n, *xq = Xt + (long long)q * n;
+        c128 *jp = Jt + (long long)p * n, *jq = Jt + (long long)q * n;
+        constexpr int NR = NPL > 0 ? NPL : 1;
+        c128 xu[NR], xv[NR], ju[NR], jv[NR];
         double a = 0.0, b = 0.0, cr = 0.0, ci = 0.0;
-        for (int i = lane; i < n; i += 32) {
-          c128 u = xp[i], v = xq[i];
-          a += u.x * u.x + u.y * u.y;
-          b += v.x * v.x + v.y * v.y;
-          cr += u.x * v.x + u.y * v.y;                           // conj(u) * v
-          ci += u.x * v.y - u.y * v.x;
+        if (NPL > 0) {
+#pragma unroll
+          for (int r = 0; r < NR; r++) {
+            const int i = lane + 32 * r;
+            const bool ok = i < n;
+            xu[r] = ok ? __ldcg(xp + i) : make_double2(0.0, 0.0);
+            xv[r] = ok ? __ldcg(xq + i) : make_double2(0.0, 0.0);
+            ju[r] = ok ? __ldcg(jp + i) : make_double2(0.0, 0.0);
+            jv[r] = ok ? __ldcg(jq + i) : make_double2(0.0, 0.0);
+          }
+#pragma unroll
+          for (int r = 0; r < NR; r++) {
+            const c128 u = xu[r], v = xv[r];
+            a += u.x * u.x + u.y * u.y;
+            b += v.x * v.x + v.y * v.y;
+            cr += u.x * v.x + u.y * v.y;                         // conj(u) * v
+            ci += u.x * v.y - u.y * v.x;
+          }
+        } else {
+          for (int i = lane; i < n; i += 32) {
+            c128 u = __ldcg(xp + i), v = __ldcg(xq + i);
+            a += u.x * u.x + u.y * u.y;
+            b += v.x * v.x + v.y * v.y;
+            cr += u.x * v.x + u.y * v.y;
+            ci += u.x * v.y - u.y * v.x;
+          }
         }
         a = wsum(a); b = wsum(b); cr = wsum(cr); ci = wsum(ci);
-        const double cabs = sqrt(cr * cr + ci * ci);
-        if (!(cabs > tol * sqrt(a) * sqrt(b)) || cabs == 0.0) continue;
-        if (lane == 0) rotated = 1;
+        const double c2 = cr * cr + ci * ci;
+        if (!(c2 > tol2 * a * b) || c2 == 0.0) continue;
+        any = true;
         // y_q = e^{-i phi} x_q makes <x_p, y_q> = |c| real; then a real rotation (cs, sn)
-        const double er = cr / cabs, ei = -ci / cabs;            // e^{-i phi}
-        const double zeta = (b - a) / (2.0 * cabs);
+        const double cabs = sqrt(c2), icabs = 1.0 / cabs;
+        const double er = cr * icabs, ei = -ci * icabs;          // e^{-i phi}
+        const double zeta = 0.5 * (b - a) * icabs;
         const double t = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
         const double cs = 1.0 / sqrt(1.0 + t * t), sn = cs * t;
-        c128 *jp = Jt + (long long)p * n, *jq = Jt + (long long)q * n;
-        for (int i = lane; i < n; i += 32) {
-          c128 u = xp[i], v = xq[i];
-          c128 y = make_double2(er * v.x - ei * v.y, er * v.y + ei * v.x);
-          xp[i] = make_double2(cs * u.x - sn * y.x, cs * u.y - sn * y.y);
-          xq[i] = make_double2(sn * u.x + cs * y.x, sn * u.y + cs * y.y);
-          u = jp[i]; v = jq[i];
-          y = make_double2(er * v.x - ei * v.y, er * v.y + ei * v.x);
-          jp[i] = make_double2(cs * u.x - sn * y.x, cs * u.y - sn * y.y);
-          jq[i] = make_double2(sn * u.x + cs * y.x, sn * u.y + cs * y.y);
+        auto rot = [&](c128 u, c128 v, c128 &o1, c128 &o2) {
+          const c128 y = make_double2(er * v.x - ei * v.y, er * v.y + ei * v.x);
+          o1 = make_double2(cs * u.x - sn * y.x, cs * u.y - sn * y.y);
+          o2 = make_double2(sn * u.x + cs * y.x, sn * u.y + cs * y.y);
+        };
+        if (NPL > 0) {
+#pragma unroll
+          for (int r = 0; r < NR; r++) {
+            const int i = lane + 32 * r;
+            if (i < n) {
+              c128 o1, o2;
+              rot(xu[r], xv[r], o1, o2); xp[i] = o1; xq[i] = o2;
+              rot(ju[r], jv[r], o1, o2); jp[i] = o1; jq[i] = o2;
+            }
+          }
+        } else {
+          for (int i = lane; i < n; i += 32) {
+            c128 o1, o2;
+            rot(__ldcg(xp + i), __ldcg(xq + i), o1, o2); xp[i] = o1; xq[i] = o2;
+            rot(__ldcg(jp + i), __ldcg(jq + i), o1, o2); jp[i] = o1; jq[i] = o2;
+          }
         }
       }
-      __syncthreads();
+      if (round == np - 2 && any && lane == 0) flags[sweep] = 1;   // benign race: every writer stores 1
+      cluster.sync();
     }
-    if (!rotated) break;
-    __syncthreads();
+    if (np < 2) break;
+    if (__ldcg(flags + sweep) == 0) break;                          // nobody rotated in this sweep
   }
-  if (threadIdx.x == 0 && sweeps_out) *sweeps_out = sweep;
 }
 
 // lam (descending), U and the permuted J from X = U' R' (Qp = U'^T, Dp = R'^T as qr_gauge side 1 returns them).
@@ -127,7 +176,7 @@ __global__ void svd_finish_kernel(const c128 *Qp, const c128 *Dp, const c128 *Jt
 size_t svd_ws_bytes(int Ml, int d, int Mr) {
   const size_t n = Ml, nn = up256(n * n * 16);
   size_t q1 = qr_ws_bytes(d * Mr, Ml), q2 = qr_ws_bytes(Ml, Ml);
-  return up256((size_t)Ml * d * Mr * 16) + 6 * nn + up256(q1 > q2 ? q1 : q2) + 1024;
+  return up256((size_t)Ml * d * Mr * 16) + 6 * nn + 256 + up256(q1 > q2 ? q1 : q2) + 1024;
 }
 
 // C [Ml, d, Mr] -> U [Ml, Ml], lam [Ml], Vh [Ml, d, Mr]
@@ -143,11 +192,16 @@ void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, do
   c128 *Qp = reinterpret_cast<c128 *>(p); p += nn;
   c128 *Dp = reinterpret_cast<c128 *>(p); p += nn;
   c128 *JtP = reinterpret_cast<c128 *>(p); p += nn;
+  int *flags = reinterpret_cast<int *>(p); p += 256;
   void *qws = p;
   qr_gauge(st, 1, Ml, d, Mr, C, Q, D, qws);                               // C = D Q
   const int g = (n * n + 255) / 256 > 296 ? 296 : (n * n + 255) / 256;
   TDVP_LAUNCH(svd_init_kernel, g, 256, 0, st, D, Xt, Jt, n);
-  TDVP_LAUNCH(svd_jacobi_kernel, 1, JT, 0, st, Xt, Jt, n, (int *)nullptr);
+  cudaMemsetAsync(flags, 0, MAX_SWEEPS * sizeof(int), st);
+  if (n <= 32) TDVP_LAUNCH(svd_jacobi_kernel<1>, JC, JW * 32, 0, st, Xt, Jt, n, flags);
+  else if (n <= 64) TDVP_LAUNCH(svd_jacobi_kernel<2>, JC, JW * 32, 0, st, Xt, Jt, n, flags);
+  else if (n <= 128) TDVP_LAUNCH(svd_jacobi_kernel<4>, JC, JW * 32, 0, st, Xt, Jt, n, flags);
+  else TDVP_LAUNCH(svd_jacobi_kernel<0>, JC, JW * 32, 0, st, Xt, Jt, n, flags);
   // X = U' R'  <=>  Xt = R'^T U'^T: "side 1" factorisation of the n x n matrix Xt (d = 1)
   qr_gauge(st, 1, n, 1, n, Xt, Qp, Dp, qws);
   TDVP_LAUNCH(svd_finish_kernel, n < 148 ? n : 148, 128, n * sizeof(double), st, Qp, Dp, Jt, n, U, lam, JtP);
