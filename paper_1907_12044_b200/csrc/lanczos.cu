@@ -8,8 +8,13 @@
 // memory: reductions finish in the last CTA to arrive (fixed summation order: deterministic), the
 // breakdown decision is a device flag that turns the remaining iterations into no-ops (q = 0), and
 // the k x k tridiagonal eigenproblem runs in one warp.  Nothing is read back by the host.
+#include <cooperative_groups.h>
+#include <cstdlib>
+
 #include "common.cuh"
 #include "tridiag.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace {
 
@@ -171,6 +176,105 @@ __global__ void __launch_bounds__(VT) lz_update_kernel(long long n, int nd, int 
   }
 }
 
+// ---- fused orthogonalisation step (cooperative launch) ---------------------------------------
+// One kernel per Lanczos iteration instead of five: every CTA keeps its chunk of w = H q_j and of
+// q_0..q_j in shared memory (one pass over HBM/L2), and the three global reductions (the two
+// Gram-Schmidt passes and the norm) are grid-wide barriers of a cooperative launch.  Partial sums are
+// added in a fixed order by every CTA, so all CTAs hold bit-identical scalars: deterministic.
+constexpr int FT = 256;
+constexpr size_t FUSED_SMEM_MAX = 200 * 1024;
+
+__device__ __forceinline__ void fused_dots(const c128 *sw, const c128 *sq, int chunk, int len, int nd, c128 *partial,
+                                           int lane, int warp) {
+  for (int i = warp; i < nd; i += FT / 32) {
+    const c128 *q = sq + (size_t)i * chunk;
+    double sx = 0.0, sy = 0.0;
+    for (int e = lane; e < len; e += 32) {
+      c128 a = q[e], x = sw[e];
+      sx += a.x * x.x + a.y * x.y;
+      sy += a.x * x.y - a.y * x.x;
+    }
+    sx = warp_sum(sx); sy = warp_sum(sy);
+    if (lane == 0) partial[(size_t)blockIdx.x * nd + i] = make_double2(sx, sy);
+  }
+}
+// every CTA: cs[i] = sum_g partial[g][i] in a fixed order
+__device__ __forceinline__ void fused_gather(const c128 *partial, int nd, c128 *cs, int lane, int warp) {
+  for (int i = warp; i < nd; i += FT / 32) {
+    double sx = 0.0, sy = 0.0;
+    for (int g = lane; g < (int)gridDim.x; g += 32) { c128 pz = __ldcg(partial + (size_t)g * nd + i); sx += pz.x; sy += pz.y; }
+    sx = warp_sum(sx); sy = warp_sum(sy);
+    if (lane == 0) cs[i] = make_double2(sx, sy);
+  }
+  __syncthreads();
+}
+
+__global__ void __launch_bounds__(FT) lz_fused_orth_kernel(long long n, int chunk, int j, int k, LzBuffers b) {
+  cg::grid_group grid = cg::this_grid();
+  extern __shared__ __align__(16) unsigned char fsm[];
+  c128 *sw = reinterpret_cast<c128 *>(fsm);                       // [chunk]
+  c128 *sq = sw + chunk;                                          // [j + 1][chunk]
+  __shared__ c128 cs[TDVP_MAX_KRYLOV + 1];
+  __shared__ double red[FT / 32];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nd = j + 1;
+  const long long e0 = (long long)blockIdx.x * chunk;
+  const int len = (int)((e0 + chunk <= n) ? chunk : (n > e0 ? n - e0 : 0));
+  const int was_done = b.state->done;                             // read before anybody can change it
+  c128 *wg = b.Q + (long long)(j + 1) * n + e0;
+  for (int e = tid; e < len; e += FT) sw[e] = wg[e];
+  for (int i = 0; i < nd; i++) {
+    const c128 *qg = b.Q + (long long)i * n + e0;
+    for (int e = tid; e < len; e += FT) sq[(size_t)i * chunk + e] = qg[e];
+  }
+  __syncthreads();
+  for (int pass = 0; pass < 2; pass++) {
+    c128 *partial = b.partial + (size_t)pass * MAXG * (TDVP_MAX_KRYLOV + 1);
+    fused_dots(sw, sq, chunk, len, nd, partial, lane, warp);
+    grid.sync();
+    fused_gather(partial, nd, cs, lane, warp);
+    if (pass == 0 && blockIdx.x == 0 && tid == 0 && !was_done) b.alpha[j] = cs[j].x;
+    for (int e = tid; e < len; e += FT) {
+      c128 x = sw[e];
+      for (int i = 0; i < nd; i++) {
+        c128 q = sq[(size_t)i * chunk + e], c = cs[i];
+        x.x -= c.x * q.x - c.y * q.y;
+        x.y -= c.x * q.y + c.y * q.x;
+      }
+      sw[e] = x;
+    }
+    __syncthreads();
+  }
+  double s = 0.0;
+  for (int e = tid; e < len; e += FT) { c128 x = sw[e]; s += x.x * x.x + x.y * x.y; }
+  s = warp_sum(s);
+  if (lane == 0) red[warp] = s;
+  __syncthreads();
+  if (tid == 0) { double t = 0; for (int i = 0; i < FT / 32; i++) t += red[i]; b.npartial[blockIdx.x] = t; }
+  grid.sync();
+  double t = 0.0;
+  for (int g = lane; g < (int)gridDim.x; g += 32) t += __ldcg(b.npartial + g);
+  t = warp_sum(t);
+  const double beta = sqrt(t);
+  double inv_beta = 0.0;
+  bool now_done = was_done;
+  if (!was_done) {
+    const double aj = fabs(__ldcg(b.alpha + j));
+    if (j == k - 1 || beta < BREAKDOWN_TOL * (aj > 1.0 ? aj : 1.0)) now_done = true;
+    else inv_beta = 1.0 / beta;
+  }
+  if (blockIdx.x == 0 && tid == 0) {
+    LzState *st = b.state;
+    if (!was_done) {
+      if (now_done) { st->done = 1; st->m = j + 1; st->inv_beta = 0.0; }
+      else { b.beta[j] = beta; st->inv_beta = inv_beta; }
+    } else {
+      st->inv_beta = 0.0;
+    }
+  }
+  if (j < k - 1)
+    for (int e = tid; e < len; e += FT) { c128 x = sw[e]; wg[e] = make_double2(x.x * inv_beta, x.y * inv_beta); }
+}
+
 // One warp: coef = beta0 * V exp(z Lambda) V^T e_1 for the m x m tridiagonal (alpha, beta).
 __global__ void lz_coef_kernel(int k, double zr, double zi, LzBuffers b, int *m_out) {
   __shared__ double V[TDVP_MAX_KRYLOV * TDVP_MAX_KRYLOV];
@@ -222,10 +326,18 @@ size_t apply_ws_bytes(const LanczosOp &op) {
 
 }  // namespace
 
+bool g_lanczos_unfused = false;   // test hook (TDVP_LANCZOS_UNFUSED=1): force the five-kernel path
+
+void lanczos_configure() {
+  cudaFuncSetAttribute(lz_fused_orth_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSED_SMEM_MAX);
+  const char *e = getenv("TDVP_LANCZOS_UNFUSED");
+  g_lanczos_unfused = e && e[0] == '1';
+}
+
 size_t lanczos_ws_bytes(const LanczosOp &op, int k) {
   size_t n = (size_t)op.Ml * (op.kind == 0 ? op.d : 1) * op.Mr;
   return up256((k + 1) * n * 16) + up256((k + 1) * 16) + up256(k * 16) + 2 * up256(k * 8) +
-         up256(sizeof(LzState)) + 256 + up256((size_t)MAXG * (k + 1) * 16) + up256(MAXG * 8) +
+         up256(sizeof(LzState)) + 256 + up256((size_t)2 * MAXG * (TDVP_MAX_KRYLOV + 1) * 16) + up256(MAXG * 8) +
          apply_ws_bytes(op) + 512;
 }
 
@@ -241,13 +353,21 @@ void lanczos_expm(cudaStream_t st, const LanczosOp &op, int k, double z_re, doub
   b.beta = reinterpret_cast<double *>(p); p += up256(k * 8);
   b.state = reinterpret_cast<LzState *>(p); p += up256(sizeof(LzState));
   b.counter = reinterpret_cast<unsigned *>(p); p += 256;
-  b.partial = reinterpret_cast<c128 *>(p); p += up256((size_t)MAXG * (k + 1) * 16);
+  b.partial = reinterpret_cast<c128 *>(p); p += up256((size_t)2 * MAXG * (TDVP_MAX_KRYLOV + 1) * 16);
   b.npartial = reinterpret_cast<double *>(p); p += up256(MAXG * 8);
   b.apply_ws = p;
 
   int G = (int)((n + VT - 1) / VT);
   if (G > MAXG) G = MAXG;
   if (G < 1) G = 1;
+  // fused cooperative path: one CTA per SM at most, the chunk of all k + 1 vectors in shared memory
+  static int num_sms = 0;
+  if (!num_sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev); }
+  int FG = (int)((n + FT - 1) / FT);
+  if (FG > num_sms) FG = num_sms;
+  if (FG < 1) FG = 1;
+  const int chunk = (int)((n + FG - 1) / FG);
+  const bool fused = !g_lanczos_unfused && (size_t)(k + 1) * chunk * 16 <= FUSED_SMEM_MAX;
   {
     ProfScope ps(st, PH_VEC);
     cudaMemsetAsync(b.counter, 0, sizeof(unsigned), st);
@@ -261,11 +381,18 @@ void lanczos_expm(cudaStream_t st, const LanczosOp &op, int k, double z_re, doub
     else
       bond_apply(st, op.Ml, op.Mr, op.Dl, op.L, qj, op.R, w, b.apply_ws);
     ProfScope ps(st, PH_VEC);
-    TDVP_LAUNCH(lz_dots_kernel, G, VT, 0, st, n, j + 1, j, 1, b);
-    TDVP_LAUNCH(lz_update_kernel, G, VT, 0, st, n, j + 1, j, k, 0, b);
-    TDVP_LAUNCH(lz_dots_kernel, G, VT, 0, st, n, j + 1, j, 0, b);
-    TDVP_LAUNCH(lz_update_kernel, G, VT, 0, st, n, j + 1, j, k, 1, b);
-    if (j < k - 1) TDVP_LAUNCH(lz_scale_kernel, G, VT, 0, st, w, w, n, b.state);
+    if (fused) {
+      long long nn = n; int ch = chunk, jj = j, kk = k;
+      void *args[] = {&nn, &ch, &jj, &kk, &b};
+      cudaLaunchCooperativeKernel((void *)lz_fused_orth_kernel, dim3(FG), dim3(FT), args, (size_t)(j + 2) * chunk * 16, st);
+      count_launch();
+    } else {
+      TDVP_LAUNCH(lz_dots_kernel, G, VT, 0, st, n, j + 1, j, 1, b);
+      TDVP_LAUNCH(lz_update_kernel, G, VT, 0, st, n, j + 1, j, k, 0, b);
+      TDVP_LAUNCH(lz_dots_kernel, G, VT, 0, st, n, j + 1, j, 0, b);
+      TDVP_LAUNCH(lz_update_kernel, G, VT, 0, st, n, j + 1, j, k, 1, b);
+      if (j < k - 1) TDVP_LAUNCH(lz_scale_kernel, G, VT, 0, st, w, w, n, b.state);
+    }
   }
   ProfScope ps(st, PH_VEC);
   TDVP_LAUNCH(lz_coef_kernel, 1, 32, 0, st, k, z_re, z_im, b, m_used_dev);
