@@ -68,7 +68,7 @@ tdvp_handle *default_handle() {
   static tdvp_handle *h = nullptr;
   static std::mutex mu;
   std::lock_guard<std::mutex> g(mu);
-  if (!h) { h = new tdvp_handle(); tdvp_default_options(&h->opt); h->stream = nullptr; }
+  if (!h) { h = new tdvp_handle(); tdvp_default_options(&h->opt); h->stream = nullptr; zgemm_prepare_stream(nullptr); }
   return h;
 }
 
@@ -101,6 +101,7 @@ int tdvp_create_context(tdvp_handle **out, const tdvp_options *opt, void *cuda_s
   if (rc) { delete h; return rc; }
   h->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
   configure_kernels_once();
+  zgemm_prepare_stream(h->stream);
   *out = h;
   return TDVP_OK;
 }

@@ -69,11 +69,17 @@ struct ZGemm {
   long long a_bsi = 0, b_bsi = 0, c_bsi = 0;   // inner batch strides
   long long a_bso = 0, b_bso = 0, c_bso = 0;   // outer batch strides
   int conjA = 0, conjB = 0;
-  int splitk = 0;                               // 0 = choose
+  int splitk = 0;                               // unused (the schedule is chosen by zgemm)
 };
-// ws: split-K workspace of at least zgemm_ws_elems(p) complex numbers (may be NULL if 0).
-size_t zgemm_ws_elems(const ZGemm &p);          // upper bound for any split the heuristic may pick
+// The kernel is a persistent stream-K schedule; its partial-tile slots and flags belong to the
+// stream (one context per stream, made by zgemm_prepare_stream outside any capture; a private
+// capture stream is aliased to the stream the graph will be replayed on).  ws is unused (kept for
+// the call sites); zgemm_ws_elems returns 0.
+size_t zgemm_ws_elems(const ZGemm &p);
 void zgemm(cudaStream_t st, const ZGemm &p, c128 *ws);
+void zgemm_prepare_stream(cudaStream_t st);
+void zgemm_alias_stream(cudaStream_t alias, cudaStream_t of);
+void zgemm_forget_stream(cudaStream_t alias);
 
 // ---------------------------------------------------------------------------------------------
 // wstage.cu : sparse MPO stage.

@@ -84,6 +84,7 @@ static int run_step(tdvp_handle *h, StepGraph &sg, double dt, F enqueue, const c
       // the legacy default stream cannot be captured: record on a private stream, replay on h->stream
       if (int rc = check_cuda(h, cudaStreamCreateWithFlags(&own, cudaStreamNonBlocking), "stream")) return rc;
       cap = own;
+      zgemm_alias_stream(own, h->stream);
     }
     cudaStream_t saved = h->stream;
     h->stream = cap;
@@ -99,7 +100,7 @@ static int run_step(tdvp_handle *h, StepGraph &sg, double dt, F enqueue, const c
     h->stream = saved;
     if (e == cudaSuccess) e = cudaGraphInstantiate(&sg.exec, graph, 0);
     if (graph) cudaGraphDestroy(graph);
-    if (own) cudaStreamDestroy(own);
+    if (own) { zgemm_forget_stream(own); cudaStreamDestroy(own); }
     if (e != cudaSuccess) { sg.exec = nullptr; cudaGetLastError(); return check_cuda(h, e, what); }
     sg.dt = dt; sg.launches = tally;
   }

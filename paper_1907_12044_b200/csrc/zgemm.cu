@@ -8,47 +8,58 @@
 //   * CTA tile 64x64 complex, 4 warps, each warp a 32x32 complex tile = 4x4 m8n8 blocks, real and
 //     imaginary accumulators (64 f64 per thread); the complex product is 4 real MMAs per block
 //     pair, with -Im(A) made by a sign-bit XOR on the ALU pipe (no FP64 pipe work);
-//   * operands stay in their global layout (complex interleaved) in shared memory, staged by a
-//     4-stage cp.async (LDGSTS, 16 B = one complex number per copy, zero-fill at ragged edges);
-//     row paddings make every fragment LDS.128 bank-conflict free;
-//   * two CTAs per SM; split-K (deterministic: partials to a workspace, then one reduce kernel)
-//     when the output has too few tiles to fill 148 SMs (stage 3 of H_eff, the bond operator).
+//   * operands stay in their global layout (complex interleaved) in shared memory, staged by TMA
+//     (cp.async.bulk.tensor, dense boxes, zero fill at ragged edges) into a 3-slot ring guarded by
+//     full/empty mbarriers; one thread issues the loads.  Measured: every non-DMMA instruction a
+//     warp issues costs the FP64 tensor pipe ~1.6 cycles (no overlap with a DMMA in flight), so
+//     the loop carries no address arithmetic, predicates or per-element copies at all;
+//     box shapes are chosen so that every fragment LDS.128 is bank-conflict free;
+//   * two CTAs per SM, persistent, with a stream-K schedule: every CTA gets the same number of
+//     (tile, k-tile) units, tiles cut across CTAs are summed inside the kernel in a fixed order
+//     (deterministic), so neither wave quantisation (stage 1: 800 tiles on 296 CTA slots) nor a
+//     separate split-K reduce pass (stage 3 of H_eff, the bond operator: 40 tiles) is paid.
+#include <cuda.h>
+
+#include <mutex>
+#include <unordered_map>
+
 #include "common.cuh"
 
 namespace {
 
-constexpr int BM = 64, BN = 64, BK = 8, STAGES = 4;
+constexpr int BM = 64, BN = 64, BK = 16, STAGES = 3;
+constexpr int LOOKAHEAD = STAGES - 2;                  // k-tiles in flight ahead of the consumer
 constexpr int WM = 32, WN = 32;
 constexpr int NTHREADS = (BM / WM) * (BN / WN) * 32;   // 128
-constexpr int LDK = BK + 4;    // K-major tile row stride (complex): 12 == 4 (mod 8)
-constexpr int LDM = BM + 2;    // MN-major tile row stride: 66 == 2 (mod 8)
-constexpr int A_TILE = (BM * LDK > BK * LDM) ? BM * LDK : BK * LDM;   // complex elements
-constexpr int B_TILE = A_TILE;
-constexpr int SMEM_BYTES = STAGES * (A_TILE + B_TILE) * 16;
+constexpr int KG = BK / 4;     // k-groups of 4 complex numbers (one DMMA k-step) per k-tile
+// Shared-memory operand tiles, written by TMA (dense boxes, no swizzle), read by LDS.128:
+//   K-major operand  : [KG][64 rows][4 complex]  -- a quarter-warp (2 rows x 4 k) reads 128
+//                      contiguous bytes: bank-conflict free;
+//   MN-major operand : [BK][LDM = 66 complex]    -- the box is 66 wide (2 columns over-fetched) so
+//                      that the 4 k-rows of a quarter-warp start 8 banks apart: conflict free.
+constexpr int LDM = BM + 2;
+constexpr int TILE_K_BYTES = KG * BM * 4 * 16;         // 16384
+constexpr int TILE_MN_BYTES = BK * LDM * 16;           // 16896
+constexpr int TILE_BYTES = TILE_MN_BYTES;              // slot size of either layout (128 B multiple)
+constexpr int SMEM_BYTES = STAGES * 2 * TILE_BYTES + 128;
 
 struct KParams {
-  const c128 *A; const c128 *B; c128 *C;
+  c128 *C;
   int M, N, K;
-  long long a_ms, a_ks, b_ks, b_ns, ldc;
+  long long ldc;
   int batch_inner;
-  long long a_bsi, b_bsi, c_bsi, a_bso, b_bso, c_bso;
+  long long c_bsi, c_bso;
+  int a_batched_i, a_batched_o, b_batched_i, b_batched_o;   // 0: operand shared by the batch (coordinate 0)
   unsigned a_sign;      // 0x80000000 if conjA
   unsigned b_sign;      // 0x80000000 if conjB
-  int splitk, ktiles_per_split;
-  int tiles_m, tiles_n;
-  c128 *partial;        // split-K workspace [split][batch][M][N]
-  long long partial_split_stride;
+  int tiles_m, tiles_n, ktiles;
+  int G;                // CTAs of this launch (cooperative: all resident)
+  int upc_base, upc_rem;// units (tile, k-tile) per CTA: base, +1 for the first upc_rem CTAs
+  c128 *slots;          // [2 G][BM*BN] partial tiles of segments that do not cover their tile's whole K
+  int *cnt;             // [G] partial segments published for the cut tile whose LAST unit CTA j holds
+  int *done;            // [G] contributors that have finished reducing it (the last one zeroes both)
 };
 
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem, bool pred) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  int sz = pred ? 16 : 0;
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(sz));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N> __device__ __forceinline__ void cp_async_wait() {
-  asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
-}
 __device__ __forceinline__ double flip(double x, unsigned mask) {
   return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
 }
@@ -56,55 +67,131 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
       : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
+__device__ __forceinline__ int ld_acquire(const int *p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void red_release_add(int *p, int v) {
+  asm volatile("red.release.gpu.global.add.s32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
+}
+// ---- mbarrier / TMA (cp.async.bulk.tensor) ----
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  unsigned ok;
+  do {
+    asm volatile(
+        "{\n.reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap *tm, unsigned bar, int c0, int c1, int c2, int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];\n"
+      ::"r"(dst), "l"(reinterpret_cast<unsigned long long>(tm)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+      : "memory");
+}
 
-template <bool A_KMAJOR, bool B_KMAJOR>
-__global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(KParams p) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  c128 *sA = reinterpret_cast<c128 *>(smem_raw);
-  c128 *sB = sA + STAGES * A_TILE;
+// Work decomposition ("stream-K"): the (tile, k-tile) units of the whole batched GEMM, tile-major,
+// are cut into G equal contiguous ranges, one per CTA, G <= resident CTAs (cooperative launch), so
+// every SM carries the same number of DMMAs whatever the tile count.  A range is at most: the tail
+// of a tile begun by lower CTAs, whole tiles, and the head of a tile continued by higher CTAs.
+// Whole tiles go straight to C.  A partial segment is written to a slot (2 per CTA: [0] the CTA's
+// first segment, [1] its last) and counted on the tile's counter; when a CTA has finished its
+// units it waits for the counters of its (at most two) cut tiles and reduces ITS SLICE of each:
+// the C contributors of a tile each sum 1/C of its elements over all C slots in CTA order (fixed
+// order: deterministic, whoever does it) and write them to C.  The fix-up is therefore one
+// round trip deep whatever the split, and there is no separate reduce kernel.
+__device__ __forceinline__ int cta_of_unit(int u, int base, int rem) {
+  const int cut = rem * (base + 1);
+  return u < cut ? u / (base + 1) : rem + (u - cut) / base;
+}
+
+template <bool A_KMAJOR, bool B_KMAJOR, bool CONJ>
+__global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constant__ CUtensorMap tmA,
+                                                            const __grid_constant__ CUtensorMap tmB, KParams p) {
+  extern __shared__ __align__(128) unsigned char smem_dyn[];
+  __shared__ int s_fix_tile[2];
+  __shared__ __align__(8) unsigned long long s_full[STAGES], s_empty[STAGES];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm0 = (warp / (BN / WN)) * WM, wn0 = (warp % (BN / WN)) * WN;
-  const int tile = blockIdx.x;
-  const int tn = tile % p.tiles_n, tm = tile / p.tiles_n;
-  const int m0 = tm * BM, n0 = tn * BN;
-  const int split = blockIdx.y;
-  const int bz = blockIdx.z, bin = bz % p.batch_inner, bo = bz / p.batch_inner;
+  // the dynamic segment is only guaranteed 16 B alignment: round up to 128 B for TMA destinations
+  const unsigned smem_base = ((unsigned)__cvta_generic_to_shared(smem_dyn) + 127u) & ~127u;
+  unsigned char *smem_gen = smem_dyn + (smem_base - (unsigned)__cvta_generic_to_shared(smem_dyn));
+  const unsigned full0 = (unsigned)__cvta_generic_to_shared(s_full);
+  const unsigned empty0 = (unsigned)__cvta_generic_to_shared(s_empty);
+  if (tid == 0) {
+    s_fix_tile[0] = s_fix_tile[1] = -1;
+    for (int s = 0; s < STAGES; s++) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, NTHREADS / 32); }
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  const int cta = blockIdx.x;
+  const int ktiles = p.ktiles;
+  const int u0 = cta * p.upc_base + (cta < p.upc_rem ? cta : p.upc_rem);
+  const int nkt = p.upc_base + (cta < p.upc_rem ? 1 : 0);
+  const int t0 = u0 / ktiles, k_first = u0 - t0 * ktiles;
+  const int tiles_mn = p.tiles_m * p.tiles_n;
+  // order of work: the partial first segment (tail of tile t0), the partial last segment (head of
+  // tile tL), then the whole tiles -- so the partials are published long before anybody needs them
+  const int first_len = (ktiles - k_first) < nkt ? (ktiles - k_first) : nkt;
+  const int lenF = (k_first > 0 || first_len < ktiles) ? first_len : 0;
+  const int tL = (u0 + nkt - 1) / ktiles;
+  const int last_len = u0 + nkt - tL * ktiles;
+  const int lenL = (last_len < ktiles && tL != t0) ? last_len : 0;
+  const int lenFL = lenF + lenL;
+  const int tM0 = (u0 + lenF) / ktiles;                  // first whole tile
 
-  const c128 *Ab = p.A + bin * p.a_bsi + bo * p.a_bso;
-  const c128 *Bb = p.B + bin * p.b_bsi + bo * p.b_bso;
-
-  const int ktiles_total = (p.K + BK - 1) / BK;
-  const int kt_begin = split * p.ktiles_per_split;
-  int kt_end = kt_begin + p.ktiles_per_split;
-  if (kt_end > ktiles_total) kt_end = ktiles_total;
-  const int nkt = kt_end - kt_begin;   // may be <= 0 for a trailing split: writes zeros
-
-  auto load_tile = [&](int stage, int kt) {
-    const int k0 = kt * BK;
-    c128 *a = sA + stage * A_TILE;
-    c128 *b = sB + stage * B_TILE;
-#pragma unroll
-    for (int i = 0; i < (BM * BK) / NTHREADS; i++) {
-      int e = tid + i * NTHREADS;
-      int r, k, so;
-      if (A_KMAJOR) { r = e / BK; k = e % BK; so = r * LDK + k; }
-      else          { k = e / BM; r = e % BM; so = k * LDM + r; }
-      bool ok = (m0 + r < p.M) && (k0 + k < p.K);
-      const c128 *src = ok ? Ab + (long long)(m0 + r) * p.a_ms + (long long)(k0 + k) * p.a_ks : Ab;
-      cp_async16(a + so, src, ok);
-    }
-#pragma unroll
-    for (int i = 0; i < (BN * BK) / NTHREADS; i++) {
-      int e = tid + i * NTHREADS;
-      int r, k, so;
-      if (B_KMAJOR) { r = e / BK; k = e % BK; so = r * LDK + k; }
-      else          { k = e / BN; r = e % BN; so = k * LDM + r; }
-      bool ok = (n0 + r < p.N) && (k0 + k < p.K);
-      const c128 *src = ok ? Bb + (long long)(n0 + r) * p.b_ns + (long long)(k0 + k) * p.b_ks : Bb;
-      cp_async16(b + so, src, ok);
-    }
+  // ---- producer: thread 0 issues the TMA loads of position `pos` into slot pos % STAGES ----
+  // (its tile coordinates are decoded only when the tile changes; slot and parity are counters)
+  int l_tile = lenF ? t0 : (lenL ? tL : tM0), l_kt = lenF ? k_first : 0;
+  int l_m0 = 0, l_n0 = 0, l_abi = 0, l_abo = 0, l_bbi = 0, l_bbo = 0, p_slot = 0;
+  unsigned p_par = 0;                                    // parity of the "empty" phase to wait for
+  auto decode = [&]() {
+    const int bz = l_tile / tiles_mn, tr = l_tile - bz * tiles_mn;
+    l_m0 = (tr / p.tiles_n) * BM; l_n0 = (tr % p.tiles_n) * BN;
+    const int bin = bz % p.batch_inner, bo = bz / p.batch_inner;
+    l_abi = p.a_batched_i ? bin : 0; l_abo = p.a_batched_o ? bo : 0;
+    l_bbi = p.b_batched_i ? bin : 0; l_bbo = p.b_batched_o ? bo : 0;
   };
+  auto issue = [&](int pos) {
+    if (pos >= STAGES) mbar_wait(empty0 + 8 * p_slot, p_par);   // consumers of pos - STAGES are done
+    const int k0 = l_kt * BK;
+    const unsigned bar = full0 + 8 * p_slot;
+    const unsigned dA = smem_base + p_slot * (2 * TILE_BYTES), dB = dA + TILE_BYTES;
+    mbar_expect_tx(bar, (A_KMAJOR ? TILE_K_BYTES : TILE_MN_BYTES) + (B_KMAJOR ? TILE_K_BYTES : TILE_MN_BYTES));
+    if (A_KMAJOR) {
+#pragma unroll
+      for (int g = 0; g < KG; g++) tma_load_4d(dA + g * (BM * 64), &tmA, bar, 2 * (k0 + 4 * g), l_m0, l_abi, l_abo);
+    } else {
+      tma_load_4d(dA, &tmA, bar, 2 * l_m0, k0, l_abi, l_abo);
+    }
+    if (B_KMAJOR) {
+#pragma unroll
+      for (int g = 0; g < KG; g++) tma_load_4d(dB + g * (BN * 64), &tmB, bar, 2 * (k0 + 4 * g), l_n0, l_bbi, l_bbo);
+    } else {
+      tma_load_4d(dB, &tmB, bar, 2 * l_n0, k0, l_bbi, l_bbo);
+    }
+    if (++p_slot == STAGES) { p_slot = 0; if (pos >= STAGES) p_par ^= 1u; }
+    const int np = pos + 1;
+    if (np == lenF && lenL) { l_tile = tL; l_kt = 0; decode(); }
+    else if (np == lenFL) { l_tile = tM0; l_kt = 0; decode(); }
+    else if (++l_kt == ktiles) { l_kt = 0; ++l_tile; decode(); }
+  };
+  if (tid == 0) {
+    decode();
+    for (int s = 0; s < LOOKAHEAD && s < nkt; s++) issue(s);
+  }
 
   double cr[4][4][2], ci[4][4][2];
 #pragma unroll
@@ -112,40 +199,40 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(KParams p) {
 #pragma unroll
     for (int j = 0; j < 4; j++) { cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0; }
 
-#pragma unroll
-  for (int s = 0; s < STAGES - 1; s++) {
-    if (s < nkt) load_tile(s, kt_begin + s);
-    cp_async_commit();
-  }
-
   const int lr = lane >> 2, lk = lane & 3;
+  const unsigned na_sign = p.a_sign ^ 0x80000000u;
+  int c_tile = lenF ? t0 : (lenL ? tL : tM0), c_kt = lenF ? k_first : 0;
+  int slot = -1;
+  unsigned c_par = 1;
   for (int it = 0; it < nkt; it++) {
-    cp_async_wait<STAGES - 2>();
-    __syncthreads();
-    {
-      int nx = it + STAGES - 1;
-      if (nx < nkt) load_tile(nx % STAGES, kt_begin + nx);
-      cp_async_commit();
-    }
-    const c128 *a = sA + (it % STAGES) * A_TILE;
-    const c128 *b = sB + (it % STAGES) * B_TILE;
+    if (tid == 0 && it + LOOKAHEAD < nkt) issue(it + LOOKAHEAD);
+    __syncwarp();
+    if (++slot == STAGES) slot = 0;
+    if (slot == 0) c_par ^= 1u;
+    mbar_wait(full0 + 8 * slot, c_par);
+    const c128 *a = reinterpret_cast<const c128 *>(smem_gen + slot * (2 * TILE_BYTES));
+    const c128 *b = reinterpret_cast<const c128 *>(smem_gen + slot * (2 * TILE_BYTES) + TILE_BYTES);
 #pragma unroll
-    for (int ks = 0; ks < BK / 4; ks++) {
+    for (int ks = 0; ks < KG; ks++) {
       double ar[4], ai[4], nai[4], br[4], bi[4];
 #pragma unroll
       for (int i = 0; i < 4; i++) {
-        c128 v = A_KMAJOR ? a[(wm0 + i * 8 + lr) * LDK + ks * 4 + lk]
+        c128 v = A_KMAJOR ? a[(ks * BM + wm0 + i * 8 + lr) * 4 + lk]
                           : a[(ks * 4 + lk) * LDM + wm0 + i * 8 + lr];
         ar[i] = v.x;
-        ai[i] = flip(v.y, p.a_sign);
-        nai[i] = flip(ai[i], 0x80000000u);
+        ai[i] = CONJ ? flip(v.y, p.a_sign) : v.y;
+        nai[i] = flip(v.y, CONJ ? na_sign : 0x80000000u);
       }
 #pragma unroll
       for (int j = 0; j < 4; j++) {
-        c128 v = B_KMAJOR ? b[(wn0 + j * 8 + lr) * LDK + ks * 4 + lk]
+        c128 v = B_KMAJOR ? b[(ks * BN + wn0 + j * 8 + lr) * 4 + lk]
                           : b[(ks * 4 + lk) * LDM + wn0 + j * 8 + lr];
         br[j] = v.x;
-        bi[j] = flip(v.y, p.b_sign);
+        bi[j] = CONJ ? flip(v.y, p.b_sign) : v.y;
+      }
+      if (ks == KG - 1) {            // all operands of this slot are in registers: hand it back
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty0 + 8 * slot);
       }
 #pragma unroll
       for (int i = 0; i < 4; i++)
@@ -162,129 +249,268 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(KParams p) {
           dmma(ci[i][j][0], ci[i][j][1], ai[i], br[j]);
         }
     }
+    // ---- end of a segment? ----
+    const bool whole = it >= lenFL;
+    if (!(c_kt == ktiles - 1 || it == lenF - 1 || it == lenFL - 1)) { ++c_kt; continue; }
+    if (whole) {
+      const int bz = c_tile / tiles_mn, tr = c_tile - bz * tiles_mn;
+      const int m0 = (tr / p.tiles_n) * BM, n0 = (tr % p.tiles_n) * BN;
+      const int bin = bz % p.batch_inner, bo = bz / p.batch_inner;
+      c128 *Cb = p.C + bin * p.c_bsi + bo * p.c_bso;
+      // thread holds C(row = lane/4, cols = 2*(lane%4) + {0,1}) of every 8x8 block
+#pragma unroll
+      for (int i = 0; i < 4; i++) {
+        int m = m0 + wm0 + i * 8 + lr;
+        if (m >= p.M) continue;
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+          int n = n0 + wn0 + j * 8 + 2 * lk;
+          c128 *dst = Cb + (long long)m * p.ldc + n;
+          if (n < p.N) dst[0] = make_double2(cr[i][j][0], ci[i][j][0]);
+          if (n + 1 < p.N) dst[1] = make_double2(cr[i][j][1], ci[i][j][1]);
+        }
+      }
+    } else {
+      // partial tile: thread-native layout (element e = q * 128 + tid, q = (i*4 + j)*2 + h), coalesced
+      const int which = it < lenF ? 0 : 1;
+      c128 *sl = p.slots + (size_t)(2 * cta + which) * (BM * BN);
+#pragma unroll
+      for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+          __stcg(sl + ((i * 4 + j) * 2 + 0) * NTHREADS + tid, make_double2(cr[i][j][0], ci[i][j][0]));
+          __stcg(sl + ((i * 4 + j) * 2 + 1) * NTHREADS + tid, make_double2(cr[i][j][1], ci[i][j][1]));
+        }
+      __syncthreads();               // all stores of the CTA are ordered before thread 0's release
+      if (tid == 0) {
+        s_fix_tile[which] = c_tile;
+        const int j1 = cta_of_unit(c_tile * ktiles + ktiles - 1, p.upc_base, p.upc_rem);
+        red_release_add(p.cnt + j1, 1);
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; i++)
+#pragma unroll
+      for (int j = 0; j < 4; j++) { cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0; }
+    c_kt = 0;
+    if (it + 1 == lenF && lenL) c_tile = tL;
+    else if (it + 1 == lenFL) c_tile = tM0;
+    else ++c_tile;
   }
-  cp_async_wait<0>();
 
-  // epilogue: thread holds C(row = lane/4, cols = 2*(lane%4) + {0,1}) of every 8x8 block
-  c128 *Cb;
-  long long ldc;
-  if (p.splitk > 1) {
-    Cb = p.partial + (long long)split * p.partial_split_stride + (long long)bz * p.M * p.N;
-    ldc = p.N;
-  } else {
-    Cb = p.C + bin * p.c_bsi + bo * p.c_bso;
-    ldc = p.ldc;
-  }
-#pragma unroll
-  for (int i = 0; i < 4; i++) {
-    int m = m0 + wm0 + i * 8 + lr;
-    if (m >= p.M) continue;
-#pragma unroll
-    for (int j = 0; j < 4; j++) {
-      int n = n0 + wn0 + j * 8 + 2 * lk;
-      c128 *dst = Cb + (long long)m * ldc + n;
-      if (n < p.N) dst[0] = make_double2(cr[i][j][0], ci[i][j][0]);
-      if (n + 1 < p.N) dst[1] = make_double2(cr[i][j][1], ci[i][j][1]);
+  // ---- fix-up: reduce this CTA's slice of each tile it holds a partial segment of ----
+  __syncthreads();
+  for (int which = 0; which < 2; which++) {
+    const int t = s_fix_tile[which];
+    if (t < 0) continue;
+    const int tu0 = t * ktiles;
+    const int j0 = cta_of_unit(tu0, p.upc_base, p.upc_rem), j1 = cta_of_unit(tu0 + ktiles - 1, p.upc_base, p.upc_rem);
+    const int nc = j1 - j0 + 1, me = cta - j0;
+    if (tid == 0) while (ld_acquire(p.cnt + j1) < nc) {}
+    __syncthreads();
+    const int chunk = (BM * BN + nc - 1) / nc;
+    const int e_end = (me + 1) * chunk < BM * BN ? (me + 1) * chunk : BM * BN;
+    const int bz = t / tiles_mn, tr = t - bz * tiles_mn;
+    const int m0 = (tr / p.tiles_n) * BM, n0 = (tr % p.tiles_n) * BN;
+    c128 *Cb = p.C + (bz % p.batch_inner) * p.c_bsi + (bz / p.batch_inner) * p.c_bso;
+    // slot of contributor j: [0] if the tile holds j's first unit, else [1] (j began in an earlier
+    // tile): only j0 can have begun earlier
+    const int j0u0 = j0 * p.upc_base + (j0 < p.upc_rem ? j0 : p.upc_rem);
+    const c128 *s0 = p.slots + (size_t)(2 * j0 + (j0u0 == tu0 ? 0 : 1)) * (BM * BN);
+    const c128 *s1 = p.slots + (size_t)(2 * (j0 + 1)) * (BM * BN);
+    for (int e = me * chunk + tid; e < e_end; e += NTHREADS) {
+      const c128 v0 = __ldcg(s0 + e);
+      double sx = v0.x, sy = v0.y;
+#pragma unroll 8
+      for (int j = 0; j < nc - 1; j++) {
+        const c128 v = __ldcg(s1 + (size_t)j * (2 * BM * BN) + e);
+        sx += v.x; sy += v.y;
+      }
+      const int q = e >> 7, tx = e & 127;
+      const int i = q >> 3, jb = (q >> 1) & 3, h = q & 1;
+      const int wr = tx >> 5, ln = tx & 31;
+      const int m = m0 + (wr / (BN / WN)) * WM + i * 8 + (ln >> 2);
+      const int n = n0 + (wr % (BN / WN)) * WN + jb * 8 + 2 * (ln & 3) + h;
+      if (m < p.M && n < p.N) Cb[(long long)m * p.ldc + n] = make_double2(sx, sy);
+    }
+    __syncthreads();
+    if (tid == 0) {
+      if (atomicAdd(p.done + j1, 1) == nc - 1) { atomicExch(p.cnt + j1, 0); atomicExch(p.done + j1, 0); }
     }
   }
 }
 
-// C[b](m,n) = sum_s partial[s][b][m][n]   (fixed order: deterministic)
-__global__ void splitk_reduce_kernel(const c128 *partial, long long split_stride, int splitk,
-                                     c128 *C, int M, int N, long long ldc, int batch_inner,
-                                     long long c_bsi, long long c_bso, long long total) {
-  long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (idx >= total) return;
-  int n = idx % N;
-  long long t = idx / N;
-  int m = t % M;
-  int bz = t / M;
-  double sx = 0.0, sy = 0.0;
-  for (int s = 0; s < splitk; s++) {
-    c128 v = partial[s * split_stride + idx];
-    sx += v.x; sy += v.y;
-  }
-  int bin = bz % batch_inner, bo = bz / batch_inner;
-  C[bin * c_bsi + bo * c_bso + (long long)m * ldc + n] = make_double2(sx, sy);
+template <bool AK, bool BK_, bool CJ>
+void launch1(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, const KParams &kp) {
+  // cooperative: the CTAs of a cut tile wait for one another in the fix-up, so all must be resident
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(kp.G); cfg.blockDim = dim3(NTHREADS); cfg.dynamicSmemBytes = SMEM_BYTES; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeCooperative; attr[0].val.cooperative = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, zgemm_kernel<AK, BK_, CJ>, ta, tb, kp);
+  count_launch();
 }
-
-constexpr int SLOTS = 148 * 2;   // resident CTAs: 2 per SM on 148 SMs
-
-int choose_splitk(long long tiles, int ktiles) {
-  // cost model in k-tile units: waves * ktiles-per-split, plus the reduce pass for s > 1
-  int best_s = 1;
-  double best = 1e300;
-  int smax = ktiles < 32 ? ktiles : 32;
-  for (int s = 1; s <= smax; s++) {
-    int kps = (ktiles + s - 1) / s;
-    if (s > 1 && (ktiles + kps - 1) / kps != s) continue;     // skip splits that leave empty slices
-    long long waves = (tiles * s + SLOTS - 1) / SLOTS;
-    double cost = (double)waves * (kps + 2.0) + (s > 1 ? 3.0 + 0.5 * s : 0.0);
-    if (cost < best - 1e-9) { best = cost; best_s = s; }
-  }
-  return best_s;
-}
-
 template <bool AK, bool BK_>
-void launch(cudaStream_t st, const KParams &kp, dim3 grid) {
-  TDVP_LAUNCH((zgemm_kernel<AK, BK_>), grid, NTHREADS, SMEM_BYTES, st, kp);
+void launch(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, const KParams &kp) {
+  if (kp.a_sign || kp.b_sign) launch1<AK, BK_, true>(st, ta, tb, kp);
+  else launch1<AK, BK_, false>(st, ta, tb, kp);
+}
+template <bool AK, bool BK_>
+void set_smem_attr() {
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+}
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda).
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn g_encode = nullptr;
+
+// Tensor map of one operand seen as doubles.  K-major (unit stride along k): dims (2K, rows, bi, bo),
+// box (8 doubles = 4 complex, 64 rows); MN-major (unit stride along m/n): dims (2*rows, K, bi, bo),
+// box (2*LDM doubles, BK).  Out-of-range box elements read as zero: ragged edges need no predicates.
+bool encode_operand(CUtensorMap *tm, const c128 *base, bool kmajor, long long rows, long long K, long long ld /*complex*/,
+                    int nbi, long long bsi, int nbo, long long bso) {
+  cuuint64_t dims[4], strides[3];
+  cuuint32_t box[4], estr[4] = {1, 1, 1, 1};
+  dims[0] = (cuuint64_t)(kmajor ? 2 * K : 2 * rows);
+  dims[1] = (cuuint64_t)(kmajor ? rows : K);
+  if (dims[1] == 1) ld = (long long)(dims[0] / 2);   // a single row: any valid stride
+  strides[0] = (cuuint64_t)ld * 16;
+  const bool bi = nbi > 1 && bsi != 0, bo = nbo > 1 && bso != 0;
+  dims[2] = bi ? nbi : 1; dims[3] = bo ? nbo : 1;
+  const cuuint64_t dummy = strides[0] * dims[1];
+  strides[1] = bi ? (cuuint64_t)bsi * 16 : dummy;
+  strides[2] = bo ? (cuuint64_t)bso * 16 : dummy;
+  box[0] = kmajor ? 8 : 2 * LDM; box[1] = kmajor ? BM : BK; box[2] = 1; box[3] = 1;
+  CUresult r = g_encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<c128 *>(base), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    fprintf(stderr, "libtdvp: cuTensorMapEncodeTiled failed (%d): dims %llu %llu %llu %llu strides %llu %llu %llu box %u %u\n",
+            (int)r, (unsigned long long)dims[0], (unsigned long long)dims[1], (unsigned long long)dims[2],
+            (unsigned long long)dims[3], (unsigned long long)strides[0], (unsigned long long)strides[1],
+            (unsigned long long)strides[2], box[0], box[1]);
+    return false;
+  }
+  return true;
+}
+
+// Per-stream scheduling state: partial-tile slots and the two counter arrays.  Kernels of one
+// stream run one after the other, so one context per stream is enough; it is created outside any
+// stream capture (zgemm_prepare_stream) because cudaMalloc is not allowed while capturing.
+struct StreamCtx { c128 *slots = nullptr; int *cnt = nullptr; int *done = nullptr; };
+std::mutex g_ctx_mu;
+std::unordered_map<cudaStream_t, StreamCtx> g_ctx;
+int g_slots = 0;      // resident CTAs of zgemm_kernel on this device (2 per SM)
+int g_sms = 0;
+
+StreamCtx *get_ctx(cudaStream_t st, bool create) {
+  std::lock_guard<std::mutex> lk(g_ctx_mu);
+  auto it = g_ctx.find(st);
+  if (it != g_ctx.end()) return &it->second;
+  if (!create) return nullptr;
+  StreamCtx c;
+  if (cudaMalloc(&c.slots, (size_t)2 * g_slots * BM * BN * sizeof(c128)) != cudaSuccess) return nullptr;
+  if (cudaMalloc(&c.cnt, (size_t)2 * g_slots * sizeof(int)) != cudaSuccess) { cudaFree(c.slots); return nullptr; }
+  cudaMemset(c.cnt, 0, (size_t)2 * g_slots * sizeof(int));
+  c.done = c.cnt + g_slots;
+  return &(g_ctx[st] = c);
+}
+
+// CTAs for `units` (tile, k-tile) units: the count that minimises the modelled time, in units of
+// one k-tile on an SM of its own.  Two CTAs sharing an SM take twice as long per unit (one CTA
+// alone reaches ~90 % of the pipe); cutting tiles costs the publish + slice reduction, measured at
+// about 8 us = four units whatever the depth of the cut.
+int choose_grid(long long units, int ktiles) {
+  int best_g = 1;
+  double best = 1e300;
+  const int gmax = units < g_slots ? (int)units : g_slots;
+  for (int g = 1; g <= gmax; g++) {
+    const long long upc = (units + g - 1) / g;
+    const bool split = (units % g != 0) || (upc % ktiles != 0);
+    const double cost = (double)upc * (g > g_sms ? 2.0 : 1.1) + (split ? 4.0 : 0.0) - 1e-6 * g;
+    if (cost < best) { best = cost; best_g = g; }
+  }
+  return best_g;
 }
 
 }  // namespace
 
 void zgemm_configure() {
-  cudaFuncSetAttribute(zgemm_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-  cudaFuncSetAttribute(zgemm_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-  cudaFuncSetAttribute(zgemm_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-  cudaFuncSetAttribute(zgemm_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  set_smem_attr<true, true>(); set_smem_attr<true, false>(); set_smem_attr<false, true>(); set_smem_attr<false, false>();
+  int dev = 0, per_sm = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, zgemm_kernel<true, true, true>, NTHREADS, SMEM_BYTES);
+  if (per_sm < 1) per_sm = 1;
+  if (per_sm > 2) per_sm = 2;
+  if (g_sms < 1) g_sms = 1;
+  g_slots = g_sms * per_sm;
+  void *fn = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess &&
+      q == cudaDriverEntryPointSuccess)
+    g_encode = reinterpret_cast<EncodeTiledFn>(fn);
 }
 
-size_t zgemm_ws_elems(const ZGemm &p) {
-  long long batch = (long long)p.batch_inner * p.batch_outer;
-  long long tiles = ceil_div_ll(p.M, BM) * ceil_div_ll(p.N, BN) * batch;
-  int ktiles = (p.K + BK - 1) / BK;
-  int s = p.splitk > 0 ? p.splitk : choose_splitk(tiles, ktiles);
-  if (s <= 1) return 0;
-  return (size_t)s * batch * p.M * p.N;
+void zgemm_prepare_stream(cudaStream_t st) { configure_kernels_once(); get_ctx(st, true); }
+
+void zgemm_alias_stream(cudaStream_t alias, cudaStream_t of) {
+  configure_kernels_once();
+  StreamCtx *c = get_ctx(of, true);
+  if (!c) return;
+  std::lock_guard<std::mutex> lk(g_ctx_mu);
+  g_ctx[alias] = *c;
 }
 
-void zgemm(cudaStream_t st, const ZGemm &p, c128 *ws) {
+void zgemm_forget_stream(cudaStream_t alias) {
+  std::lock_guard<std::mutex> lk(g_ctx_mu);
+  g_ctx.erase(alias);
+}
+
+size_t zgemm_ws_elems(const ZGemm &) { return 0; }   // the scheduling workspace belongs to the stream
+
+void zgemm(cudaStream_t st, const ZGemm &p, c128 *) {
   if (p.M <= 0 || p.N <= 0) return;
+  StreamCtx *ctx = get_ctx(st, true);
+  if (!ctx || !g_encode) {
+    fprintf(stderr, "libtdvp: zgemm has no scheduling context for this stream (allocation failed, first use inside a "
+                    "capture) or no cuTensorMapEncodeTiled entry point\n");
+    abort();
+  }
+  const bool ak = (p.a_ks == 1), bk = (p.b_ks == 1);
+  CUtensorMap ta, tb;
+  if (!encode_operand(&ta, p.A, ak, p.M, p.K, ak ? p.a_ms : p.a_ks, p.batch_inner, p.a_bsi, p.batch_outer, p.a_bso) ||
+      !encode_operand(&tb, p.B, bk, p.N, p.K, bk ? p.b_ns : p.b_ks, p.batch_inner, p.b_bsi, p.batch_outer, p.b_bso))
+    abort();
   KParams kp;
-  kp.A = p.A; kp.B = p.B; kp.C = p.C;
+  kp.C = p.C;
   kp.M = p.M; kp.N = p.N; kp.K = p.K;
-  kp.a_ms = p.a_ms; kp.a_ks = p.a_ks; kp.b_ks = p.b_ks; kp.b_ns = p.b_ns; kp.ldc = p.ldc;
+  kp.ldc = p.ldc;
   kp.batch_inner = p.batch_inner;
-  kp.a_bsi = p.a_bsi; kp.b_bsi = p.b_bsi; kp.c_bsi = p.c_bsi;
-  kp.a_bso = p.a_bso; kp.b_bso = p.b_bso; kp.c_bso = p.c_bso;
+  kp.c_bsi = p.c_bsi; kp.c_bso = p.c_bso;
+  kp.a_batched_i = p.batch_inner > 1 && p.a_bsi != 0; kp.a_batched_o = p.batch_outer > 1 && p.a_bso != 0;
+  kp.b_batched_i = p.batch_inner > 1 && p.b_bsi != 0; kp.b_batched_o = p.batch_outer > 1 && p.b_bso != 0;
   kp.a_sign = p.conjA ? 0x80000000u : 0u;
   kp.b_sign = p.conjB ? 0x80000000u : 0u;
   kp.tiles_m = (p.M + BM - 1) / BM;
   kp.tiles_n = (p.N + BN - 1) / BN;
-  long long batch = (long long)p.batch_inner * p.batch_outer;
-  long long tiles = (long long)kp.tiles_m * kp.tiles_n * batch;
+  const long long batch = (long long)p.batch_inner * p.batch_outer;
+  const long long tiles = (long long)kp.tiles_m * kp.tiles_n * batch;
   int ktiles = (p.K + BK - 1) / BK;
   if (ktiles < 1) ktiles = 1;
-  int s = p.splitk > 0 ? p.splitk : choose_splitk(tiles, ktiles);
-  if (s > ktiles) s = ktiles;
-  if (ws == nullptr) s = 1;
-  kp.splitk = s;
-  kp.ktiles_per_split = (ktiles + s - 1) / s;
-  kp.partial = ws;
-  kp.partial_split_stride = batch * p.M * p.N;
-  dim3 grid((unsigned)(kp.tiles_m * kp.tiles_n), (unsigned)s, (unsigned)batch);
-  const bool ak = (p.a_ks == 1), bk = (p.b_ks == 1);
-  {
-    ProfScope ps(st, PH_ZGEMM);
-    if (ak && bk) launch<true, true>(st, kp, grid);
-    else if (ak && !bk) launch<true, false>(st, kp, grid);
-    else if (!ak && bk) launch<false, true>(st, kp, grid);
-    else launch<false, false>(st, kp, grid);
-  }
-  if (s > 1) {
-    ProfScope ps(st, PH_SPLITK);
-    long long total = batch * p.M * p.N;
-    TDVP_LAUNCH(splitk_reduce_kernel, (unsigned)ceil_div_ll(total, 256), 256, 0, st, ws,
-                kp.partial_split_stride, s, p.C, p.M, p.N, p.ldc, p.batch_inner, p.c_bsi, p.c_bso, total);
-  }
+  kp.ktiles = ktiles;
+  const long long units = tiles * ktiles;
+  kp.G = choose_grid(units, ktiles);
+  kp.upc_base = (int)(units / kp.G);
+  kp.upc_rem = (int)(units % kp.G);
+  kp.slots = ctx->slots; kp.cnt = ctx->cnt; kp.done = ctx->done;
+  ProfScope ps(st, PH_ZGEMM);
+  if (ak && bk) launch<true, true>(st, ta, tb, kp);
+  else if (ak && !bk) launch<true, false>(st, ta, tb, kp);
+  else if (!ak && bk) launch<false, true>(st, ta, tb, kp);
+  else launch<false, false>(st, ta, tb, kp);
 }

@@ -37,7 +37,7 @@ def test_sass_contains_fp64_tensor_instructions():
     cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
     out = subprocess.run([cuobjdump, "-sass", os.path.join(build.OBJ_DIR, "zgemm.o")], capture_output=True, text=True).stdout
     assert "DMMA" in out
-    assert "LDGSTS" in out or "UBLKCP" in out
+    assert "UTMALDG" in out          # TMA tensor loads feed the DMMA loop
 
 
 def test_default_options_roundtrip():
