@@ -86,12 +86,13 @@ void zgemm_forget_stream(cudaStream_t alias);
 // Device CSR of a dense W[Dl,d,d,Dr], rows r = s*Dr + v (heff order) and columns c = w*d + t.
 struct WSparse {
   int Dl, d, Dr;
-  int *rowptr;      // DEVICE [d*Dr + 1]
+  // row-padded sparse form: row r holds cnt[r] entries, sorted by column, at [r*ncols, r*ncols + cnt[r])
+  int *cnt;         // DEVICE [d*Dr]
   int *col;         // DEVICE [capacity]
   c128 *val;        // DEVICE [capacity]
-  // transposed-role CSR used by the right-to-left order: rows r = w*d + s, columns c = t*Dr + v
-  int *rowptr_r; int *col_r; c128 *val_r;
-  int capacity;
+  // transposed-role form used by the right-to-left order: rows r = w*d + s, columns c = t*Dr + v
+  int *cnt_r; int *col_r; c128 *val_r;
+  int capacity;     // Dl*d*d*Dr
 };
 size_t wsparse_bytes(int Dl, int d, int Dr);
 // carve a WSparse out of `mem` (DEVICE, wsparse_bytes) and build both CSRs from dense W (DEVICE)
