@@ -81,110 +81,140 @@ __global__ void store_d_kernel(const c128 *Rm, c128 *D, int cols, int transpose_
 }
 
 // ---- register-resident panel factorisation ---------------------------------------------------
-// Same contract as qr_panel_kernel below, for rows - j0 <= RP_THREADS * RPT.  Every thread keeps
+// Same contract as qr_panel_kernel below, for rows - j0 <= RP_THREADS * RPT (256 x 5, 512 x 5, 512 x 10).  Every thread keeps
 // its RPT rows of the NB panel columns in registers; each column costs ONE block-wide reduction:
 // the sums s = sum_{i>=jj} |x_i|^2 and d_c = sum_{i>=jj} conj(x_i) y_c[i] give the reflector AND
 // its products with the remaining panel columns, because v differs from x only in the pivot row:
 //   v^H y_c = y_c[jj] + conj(scal) (d_c - conj(alpha) y_c[jj]),   v = [1; x_{i>jj} scal].
-constexpr int RP_THREADS = 256;
-constexpr int RP_WARPS = RP_THREADS / 32;
 
-template <int N>
-__device__ __forceinline__ void block_sum(double (&v)[N], double *sm /*[N][RP_THREADS] + [N]*/) {
+// Sum N doubles over the CTA: warp shuffles, then one shared-memory round over the warps in a fixed
+// order (deterministic).  sm: [RP_WARPS][N] + [N].
+template <int N, int RP_THREADS>
+__device__ __forceinline__ void block_sum(double (&v)[N], double *sm) {
+  constexpr int RP_WARPS = RP_THREADS / 32;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
-  for (int i = 0; i < N; i++) sm[i * RP_THREADS + threadIdx.x] = v[i];
+  for (int i = 0; i < N; i++) {
+    const double t = warp_sum_d(v[i]);
+    if (lane == 0) sm[warp * N + i] = t;
+  }
   __syncthreads();
-  for (int i = warp; i < N; i += RP_WARPS) {             // fixed summation order: deterministic
+  if (threadIdx.x < N) {
     double t = 0.0;
 #pragma unroll
-    for (int k = 0; k < RP_THREADS / 32; k++) t += sm[i * RP_THREADS + k * 32 + lane];
-    t = warp_sum_d(t);
-    if (lane == 0) sm[N * RP_THREADS + i] = t;
+    for (int k = 0; k < RP_WARPS; k++) t += sm[k * N + threadIdx.x];
+    sm[RP_WARPS * N + threadIdx.x] = t;
   }
   __syncthreads();
 #pragma unroll
-  for (int i = 0; i < N; i++) v[i] = sm[N * RP_THREADS + i];
+  for (int i = 0; i < N; i++) v[i] = sm[RP_WARPS * N + i];
   __syncthreads();
 }
 
-template <int RPT, int NB, int JJ>
-__device__ __forceinline__ void qr_panel_col(c128 (&x)[RPT][NB], c128 (*pivot)[NB], double *sm, c128 *tau_s, c128 *Rm,
-                                             int cols, int j0, int len, int tid) {
-  constexpr int jj = JJ;
-  constexpr int NRED = 1 + 2 * (NB - 1);
-
-      double red[NRED];
-#pragma unroll
-      for (int q = 0; q < NRED; q++) red[q] = 0.0;
-#pragma unroll
-      for (int r = 0; r < RPT; r++) {
-        const int i = tid + r * RP_THREADS;
-        if (i >= jj && i < len) {
-          const c128 u = x[r][jj];
-          red[0] += u.x * u.x + u.y * u.y;
-          if (i == jj) pivot[jj & 1][jj] = u;
-#pragma unroll
-          for (int c = jj + 1; c < NB; c++) {
-            const c128 yv = x[r][c];
-            red[1 + 2 * (c - 1)] += u.x * yv.x + u.y * yv.y;
-            red[2 + 2 * (c - 1)] += u.x * yv.y - u.y * yv.x;
-            if (i == jj) pivot[jj & 1][c] = yv;
-          }
-        }
-      }
-      block_sum<NRED>(red, sm);
-      const c128 alpha = pivot[jj & 1][jj];
-      double xn2 = red[0] - (alpha.x * alpha.x + alpha.y * alpha.y);
-      if (xn2 < 0.0) xn2 = 0.0;
-      c128 tau, scal;
-      double beta;
-      if (xn2 == 0.0 && alpha.y == 0.0) {
-        tau = make_double2(0.0, 0.0); scal = make_double2(0.0, 0.0); beta = alpha.x;
-      } else {
-        const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xn2);
-        beta = alpha.x >= 0.0 ? -nrm : nrm;
-        tau = make_double2((beta - alpha.x) / beta, -alpha.y / beta);
-        const double dr = alpha.x - beta, di = alpha.y, dn = dr * dr + di * di;
-        scal = make_double2(dr / dn, -di / dn);
-      }
-      if (tid == 0) { tau_s[jj] = tau; Rm[(long long)(j0 + jj) * cols + j0 + jj] = make_double2(beta, 0.0); }
-      c128 g[NB];                                        // conj(tau) * (v^H y_c)
-#pragma unroll
-      for (int c = jj + 1; c < NB; c++) {
-        const c128 dc = make_double2(red[1 + 2 * (c - 1)], red[2 + 2 * (c - 1)]);
-        const c128 yj = pivot[jj & 1][c];
-        const c128 t1 = cmul(cconj(alpha), yj);
-        const c128 t2 = cmul(cconj(scal), make_double2(dc.x - t1.x, dc.y - t1.y));
-        g[c] = cmul(cconj(tau), make_double2(yj.x + t2.x, yj.y + t2.y));
-      }
-#pragma unroll
-      for (int r = 0; r < RPT; r++) {
-        const int i = tid + r * RP_THREADS;
-        if (i < len) {
-          if (i < jj) {                                  // above the diagonal: an R entry, zero in V
-            Rm[(long long)(j0 + i) * cols + j0 + jj] = x[r][jj];
-            x[r][jj] = make_double2(0.0, 0.0);
-          } else {
-            const c128 v = (i == jj) ? make_double2(1.0, 0.0) : cmul(x[r][jj], scal);
-            x[r][jj] = v;
-#pragma unroll
-            for (int c = jj + 1; c < NB; c++) {
-              const c128 t = cmul(g[c], v);
-              x[r][c].x -= t.x; x[r][c].y -= t.y;
-            }
-          }
-        }
-      }
+// Compact-WY factor T (w x w upper triangular, H_1...H_w = I - V T V^H) from the strictly upper Gram
+// entries G[a][b] = v_a^H v_b and the tau's; one warp, lane a owns row a of the new column.
+__device__ __noinline__ void build_T(const c128 *Gs, const c128 *tau_s, c128 *Ts, c128 *Tm, int w) {
+  const int lane = threadIdx.x & 31;
+  for (int a = lane; a < NB_MAX * NB_MAX; a += 32) Ts[a] = make_double2(0.0, 0.0);
+  __syncwarp();
+  for (int c = 0; c < w; c++) {
+    if (lane == c) Ts[c * NB_MAX + c] = tau_s[c];
+    if (lane < c) {                                      // T[0:c, c] = -tau_c T[0:c, 0:c] (V^H v_c)
+      c128 acc = make_double2(0.0, 0.0);
+      for (int qq = lane; qq < c; qq++) { c128 t = cmul(Ts[lane * NB_MAX + qq], Gs[qq * NB_MAX + c]); acc.x += t.x; acc.y += t.y; }
+      const c128 t = cmul(tau_s[c], acc);
+      Ts[lane * NB_MAX + c] = make_double2(-t.x, -t.y);
+    }
+    __syncwarp();
+  }
+  for (int a = lane; a < NB_MAX * NB_MAX; a += 32) Tm[a] = Ts[a];
 }
 
-template <int RPT, int NB>
-__global__ void __launch_bounds__(RP_THREADS, 1) qr_panel_reg_kernel(c128 *X, int rows, int cols, int j0, int w,
+// One column step with a RUN-TIME column index jj: the column being eliminated is always x[.][0]
+// and the panel is shifted left by one column afterwards, so the same (small) code runs for every
+// column (unrolling the step per column made the kernel 9000 instructions long and instruction-
+// fetch bound).  The finished reflector goes straight to X; R entries to Rm.
+template <int RP_THREADS, int RPT, int NB>
+__device__ __forceinline__ void qr_panel_col(c128 (&x)[RPT][NB], c128 (*pivot)[NB], double *sm, c128 *tau_s, c128 *Rm,
+                                             c128 *X, int rows, int cols, int j0, int len, int tid, int jj) {
+  constexpr int NRED = 1 + 2 * (NB - 1);
+  double red[NRED];
+#pragma unroll
+  for (int q = 0; q < NRED; q++) red[q] = 0.0;
+#pragma unroll
+  for (int r = 0; r < RPT; r++) {
+    const int i = tid + r * RP_THREADS;
+    if (i >= jj && i < len) {
+      const c128 u = x[r][0];
+      red[0] += u.x * u.x + u.y * u.y;
+      if (i == jj) pivot[jj & 1][0] = u;
+#pragma unroll
+      for (int c = 1; c < NB; c++) {
+        const c128 yv = x[r][c];
+        red[1 + 2 * (c - 1)] += u.x * yv.x + u.y * yv.y;
+        red[2 + 2 * (c - 1)] += u.x * yv.y - u.y * yv.x;
+        if (i == jj) pivot[jj & 1][c] = yv;
+      }
+    }
+  }
+  block_sum<NRED, RP_THREADS>(red, sm);
+  const c128 alpha = pivot[jj & 1][0];
+  double xn2 = red[0] - (alpha.x * alpha.x + alpha.y * alpha.y);
+  if (xn2 < 0.0) xn2 = 0.0;
+  c128 tau, scal;
+  double beta;
+  if (xn2 == 0.0 && alpha.y == 0.0) {
+    tau = make_double2(0.0, 0.0); scal = make_double2(0.0, 0.0); beta = alpha.x;
+  } else {
+    const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xn2);
+    beta = alpha.x >= 0.0 ? -nrm : nrm;
+    tau = make_double2((beta - alpha.x) / beta, -alpha.y / beta);
+    const double dr = alpha.x - beta, di = alpha.y, dn = dr * dr + di * di;
+    scal = make_double2(dr / dn, -di / dn);
+  }
+  if (tid == 0) { tau_s[jj] = tau; Rm[(long long)(j0 + jj) * cols + j0 + jj] = make_double2(beta, 0.0); }
+  c128 g[NB];                                            // conj(tau) * (v^H y_c)
+#pragma unroll
+  for (int c = 1; c < NB; c++) {
+    const c128 dc = make_double2(red[1 + 2 * (c - 1)], red[2 + 2 * (c - 1)]);
+    const c128 yj = pivot[jj & 1][c];
+    const c128 t1 = cmul(cconj(alpha), yj);
+    const c128 t2 = cmul(cconj(scal), make_double2(dc.x - t1.x, dc.y - t1.y));
+    g[c] = cmul(cconj(tau), make_double2(yj.x + t2.x, yj.y + t2.y));
+  }
+  c128 *Xc = X + (long long)(j0 + jj) * rows + j0;
+#pragma unroll
+  for (int r = 0; r < RPT; r++) {
+    const int i = tid + r * RP_THREADS;
+    if (i < len) {
+      if (i < jj) {                                      // above the diagonal: an R entry, zero in V
+        Rm[(long long)(j0 + i) * cols + j0 + jj] = x[r][0];
+        Xc[i] = make_double2(0.0, 0.0);
+      } else {
+        const c128 v = (i == jj) ? make_double2(1.0, 0.0) : cmul(x[r][0], scal);
+        Xc[i] = v;
+#pragma unroll
+        for (int c = 1; c < NB; c++) {
+          const c128 t = cmul(g[c], v);
+          x[r][c].x -= t.x; x[r][c].y -= t.y;
+        }
+      }
+    }
+#pragma unroll
+    for (int c = 0; c < NB - 1; c++) x[r][c] = x[r][c + 1];
+    x[r][NB - 1] = make_double2(0.0, 0.0);
+  }
+}
+
+template <int RP_THREADS, int RPT, int NB>
+__global__ void __maxnreg__(RP_THREADS == 256 ? 255 : 128) qr_panel_reg_kernel(c128 *X, int rows, int cols, int j0, int w,
                                                                    c128 *Rm, c128 *Tm /*[NB_MAX][NB_MAX]*/) {
   constexpr int NRED = 1 + 2 * (NB - 1);                 // s and d_c for the other columns
+  constexpr int NGRAM = NB * (NB - 1);                   // re/im of the strictly upper Gram entries
+  constexpr int NSM = NRED > NGRAM ? NRED : NGRAM;
+  constexpr int RP_WARPS = RP_THREADS / 32;
   __shared__ c128 pivot[2][NB];                          // pivot row (alpha, y_c[jj]), double-buffered over jj
-  constexpr int NSM = NRED;
-  __shared__ double sm[(RP_THREADS + 1) * (NSM > 0 ? NSM : 1)];
+  __shared__ double sm[(RP_WARPS + 1) * (NSM > 0 ? NSM : 1)];
   __shared__ c128 tau_s[NB];
   __shared__ c128 Ts[NB_MAX * NB_MAX];
   __shared__ c128 Gs[NB_MAX * NB_MAX];
@@ -205,58 +235,48 @@ __global__ void __launch_bounds__(RP_THREADS, 1) qr_panel_reg_kernel(c128 *X, in
     int c = e / cols, i = e % cols;
     if (i > j0 + c) Rm[(long long)i * cols + j0 + c] = make_double2(0.0, 0.0);
   }
-  // columns one by one (compile-time column index keeps the panel in registers)
-#define TDVP_QR_COL(J) if (J < NB && J < w) qr_panel_col<RPT, NB, (J < NB ? J : 0)>(x, pivot, sm, tau_s, Rm, cols, j0, len, tid);
-  TDVP_QR_COL(0) TDVP_QR_COL(1) TDVP_QR_COL(2) TDVP_QR_COL(3) TDVP_QR_COL(4) TDVP_QR_COL(5) TDVP_QR_COL(6) TDVP_QR_COL(7)
-#undef TDVP_QR_COL
-  // compact WY factor from the strictly upper Gram entries v_a^H v_b
-  if (NB > 1) {
-#pragma unroll
-    for (int a = 0; a < NB - 1; a++) {                   // row a of the strictly upper Gram matrix v_a^H v_b
-      double gr[2 * (NB - 1)];
-#pragma unroll
-      for (int q = 0; q < 2 * (NB - 1); q++) gr[q] = 0.0;
-#pragma unroll
-      for (int r = 0; r < RPT; r++) {
-        const c128 u = x[r][a];
-#pragma unroll
-        for (int b = a + 1; b < NB; b++) {
-          const c128 v = x[r][b];
-          gr[2 * (b - 1)] += u.x * v.x + u.y * v.y;
-          gr[2 * (b - 1) + 1] += u.x * v.y - u.y * v.x;
-        }
-      }
-      block_sum<2 * (NB - 1)>(gr, sm);
-      if (tid == 0) {
-#pragma unroll
-        for (int b = a + 1; b < NB; b++) Gs[a * NB_MAX + b] = make_double2(gr[2 * (b - 1)], gr[2 * (b - 1) + 1]);
-      }
-    }
-    if (tid == 0) {
-      auto gram = [&](int a, int b) -> c128 { return Gs[a * NB_MAX + b]; };
-      for (int a = 0; a < NB_MAX * NB_MAX; a++) Ts[a] = make_double2(0.0, 0.0);
-      for (int c = 0; c < w; c++) {
-        Ts[c * NB_MAX + c] = tau_s[c];
-        for (int a = 0; a < c; a++) {
-          c128 acc = make_double2(0.0, 0.0);
-          for (int qq = a; qq < c; qq++) { c128 t = cmul(Ts[a * NB_MAX + qq], gram(qq, c)); acc.x += t.x; acc.y += t.y; }
-          c128 t = cmul(tau_s[c], acc);
-          Ts[a * NB_MAX + c] = make_double2(-t.x, -t.y);
-        }
-      }
-      for (int a = 0; a < NB_MAX * NB_MAX; a++) Tm[a] = Ts[a];
-    }
-  } else if (tid == 0) {
-    for (int a = 0; a < NB_MAX * NB_MAX; a++) Tm[a] = make_double2(0.0, 0.0);
-    Tm[0] = tau_s[0];
-  }
+  // columns one by one; every finished reflector is written to X by the step itself
+  for (int jj = 0; jj < w; jj++) qr_panel_col<RP_THREADS, RPT, NB>(x, pivot, sm, tau_s, Rm, X, rows, cols, j0, len, tid, jj);
+  // read the reflector block back (own writes: same thread, same addresses) for the Gram matrix
 #pragma unroll
   for (int r = 0; r < RPT; r++) {
     const int i = tid + r * RP_THREADS;
 #pragma unroll
     for (int c = 0; c < NB; c++)
-      if (i < len && c < w) X[(long long)(j0 + c) * rows + j0 + i] = x[r][c];
+      x[r][c] = (i < len && c < w) ? X[(long long)(j0 + c) * rows + j0 + i] : make_double2(0.0, 0.0);
   }
+  // compact WY factor from the strictly upper Gram entries v_a^H v_b
+  if (NB > 1) {
+    // all strictly upper Gram entries v_a^H v_b in ONE block reduction
+    double gr[NGRAM > 0 ? NGRAM : 1];
+#pragma unroll
+    for (int q = 0; q < NGRAM; q++) gr[q] = 0.0;
+#pragma unroll
+    for (int r = 0; r < RPT; r++) {
+      int q = 0;
+#pragma unroll
+      for (int a = 0; a < NB - 1; a++) {
+        const c128 u = x[r][a];
+#pragma unroll
+        for (int b = a + 1; b < NB; b++) {
+          const c128 v = x[r][b];
+          gr[q] += u.x * v.x + u.y * v.y;
+          gr[q + 1] += u.x * v.y - u.y * v.x;
+          q += 2;
+        }
+      }
+    }
+    block_sum<NGRAM, RP_THREADS>(gr, sm);
+    if (tid == 0) {
+      int q = 0;
+#pragma unroll
+      for (int a = 0; a < NB - 1; a++)
+#pragma unroll
+        for (int b = a + 1; b < NB; b++) { Gs[a * NB_MAX + b] = make_double2(gr[q], gr[q + 1]); q += 2; }
+    }
+  }
+  __syncthreads();
+  if (tid < 32) build_T(Gs, tau_s, Ts, Tm, w);
 }
 
 // Factor the panel of columns [j0, j0+w) on rows [j0, rows).  Writes reflectors back into X (unit
@@ -491,77 +511,104 @@ __global__ void __launch_bounds__(TRAIL_THREADS) qr_apply_kernel(const c128 *X, 
   }
 }
 
-// One trailing column per CTA, rows distributed over the threads, the reflector block V and the
-// column kept in registers between the product V^H y and the update y -= V (Top V^H y): V is read
-// once, and the launch fills up to cols CTAs instead of cols / CB.
-template <int AT, int RA>
-__global__ void __launch_bounds__(AT) qr_apply1_kernel(const c128 *X, c128 *Y, int rows, int j0, int w,
-                                                        const c128 *Tm, int adjoint, int c_begin) {
-  __shared__ double sm[(AT + 1) * 2 * NB_MAX];
-  const int len = rows - j0, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+// One column per CTA, rows distributed over the threads, the reflector block V and the column kept
+// in registers between the product V^H y and the update y -= V (Top V^H y): V is read once.
+// NBW = widest panel of this mode (RA * NBW <= 40 keeps V in registers without spills).
+//   FORMQ = false: trailing update of column c_begin + blockIdx.x by panel (j0, w), Top = T^H.
+//   FORMQ = true : column c = blockIdx.x of Q = H_1 ... H_n [I; 0]: starts from e_c and applies the
+//                  panels p = c / nb .. 0 with Top = T (panels above leave e_c untouched), ONE launch
+//                  for the whole Q instead of one per panel.
+template <int AT, int RA, int NBW, bool FORMQ>
+__global__ void __launch_bounds__(AT) qr_apply1_kernel(const c128 *__restrict__ X, c128 *Y, int rows, int j0_in, int w_in,
+                                                        const c128 *__restrict__ Tm, int nb, int cols, int c_begin) {
+  __shared__ double sm[(AT / 32 + 1) * 2 * NBW];
+  __shared__ c128 Tsm[NB_MAX * NB_MAX];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int c = c_begin + blockIdx.x;
-  c128 y[RA], v[RA][NB_MAX];
+  c128 y[RA];
+  int p_hi = 0, p_lo = 0;
+  if (FORMQ) {
+    p_hi = c / nb;
+#pragma unroll
+    for (int r = 0; r < RA; r++) y[r] = make_double2((tid + r * AT) == c ? 1.0 : 0.0, 0.0);
+  } else {
+#pragma unroll
+    for (int r = 0; r < RA; r++) {
+      const int i = j0_in + tid + r * AT;
+      y[r] = i < rows ? Y[(long long)c * rows + i] : make_double2(0.0, 0.0);
+    }
+  }
+  for (int pz = p_hi; pz >= p_lo; pz--) {
+    const int j0 = FORMQ ? pz * nb : j0_in;
+    const int w = FORMQ ? (cols - j0 < nb ? cols - j0 : nb) : w_in;
+    const c128 *Tp = FORMQ ? Tm + (size_t)pz * NB_MAX * NB_MAX : Tm;
+    // rows of this thread: FORMQ indexes rows from 0 (i >= j0 take part), else from j0
+    c128 v[RA][NBW];
+#pragma unroll
+    for (int r = 0; r < RA; r++) {
+      const int i = FORMQ ? tid + r * AT : j0 + tid + r * AT;
+      const bool in = i < rows && i >= j0;
+#pragma unroll
+      for (int q = 0; q < NBW; q++)
+        v[r][q] = (in && q < w) ? X[(long long)(j0 + q) * rows + i] : make_double2(0.0, 0.0);
+    }
+    if (tid < NB_MAX * NB_MAX) Tsm[tid] = Tp[tid];
+    double acc[2 * NBW];
+#pragma unroll
+    for (int q = 0; q < 2 * NBW; q++) acc[q] = 0.0;
+#pragma unroll
+    for (int r = 0; r < RA; r++)
+#pragma unroll
+      for (int q = 0; q < NBW; q++) {
+        acc[2 * q] += v[r][q].x * y[r].x + v[r][q].y * y[r].y;
+        acc[2 * q + 1] += v[r][q].x * y[r].y - v[r][q].y * y[r].x;
+      }
+#pragma unroll
+    for (int q = 0; q < 2 * NBW; q++) {
+      const double t = warp_sum_d(acc[q]);
+      if (lane == 0) sm[warp * 2 * NBW + q] = t;
+    }
+    __syncthreads();
+    if (tid < 2 * NBW) {
+      double t = 0.0;
+#pragma unroll
+      for (int k = 0; k < AT / 32; k++) t += sm[k * 2 * NBW + tid];   // fixed order: deterministic
+      sm[(AT / 32) * 2 * NBW + tid] = t;
+    }
+    __syncthreads();
+    c128 sv[NBW];
+#pragma unroll
+    for (int q = 0; q < NBW; q++) {
+      c128 a = make_double2(0.0, 0.0);
+#pragma unroll
+      for (int r = 0; r < NBW; r++) {
+        const c128 dv = make_double2(sm[(AT / 32) * 2 * NBW + 2 * r], sm[(AT / 32) * 2 * NBW + 2 * r + 1]);
+        const c128 t = FORMQ ? Tsm[q * NB_MAX + r] : cconj(Tsm[r * NB_MAX + q]);
+        const c128 pr = cmul(t, dv);
+        a.x += pr.x; a.y += pr.y;
+      }
+      sv[q] = a;
+    }
+#pragma unroll
+    for (int r = 0; r < RA; r++)
+#pragma unroll
+      for (int q = 0; q < NBW; q++) { const c128 t = cmul(v[r][q], sv[q]); y[r].x -= t.x; y[r].y -= t.y; }
+    __syncthreads();                                     // sm / Tsm are reused by the next panel
+  }
 #pragma unroll
   for (int r = 0; r < RA; r++) {
-    const int i = tid + r * AT;
-    y[r] = i < len ? Y[(long long)c * rows + j0 + i] : make_double2(0.0, 0.0);
-#pragma unroll
-    for (int q = 0; q < NB_MAX; q++)
-      v[r][q] = (i < len && q < w) ? X[(long long)(j0 + q) * rows + j0 + i] : make_double2(0.0, 0.0);
-  }
-  double acc[2 * NB_MAX];
-#pragma unroll
-  for (int q = 0; q < 2 * NB_MAX; q++) acc[q] = 0.0;
-#pragma unroll
-  for (int r = 0; r < RA; r++)
-#pragma unroll
-    for (int q = 0; q < NB_MAX; q++) {
-      acc[2 * q] += v[r][q].x * y[r].x + v[r][q].y * y[r].y;
-      acc[2 * q + 1] += v[r][q].x * y[r].y - v[r][q].y * y[r].x;
-    }
-#pragma unroll
-  for (int q = 0; q < 2 * NB_MAX; q++) sm[q * AT + tid] = acc[q];
-  __syncthreads();
-  for (int q = warp; q < 2 * NB_MAX; q += AT / 32) {
-    double t = 0.0;
-#pragma unroll
-    for (int k = 0; k < AT / 32; k++) t += sm[q * AT + k * 32 + lane];
-    t = warp_sum_d(t);
-    if (lane == 0) sm[2 * NB_MAX * AT + q] = t;
-  }
-  __syncthreads();
-  c128 dv[NB_MAX], sv[NB_MAX];
-#pragma unroll
-  for (int q = 0; q < NB_MAX; q++) dv[q] = make_double2(sm[2 * NB_MAX * AT + 2 * q], sm[2 * NB_MAX * AT + 2 * q + 1]);
-#pragma unroll
-  for (int q = 0; q < NB_MAX; q++) {
-    c128 a = make_double2(0.0, 0.0);
-#pragma unroll
-    for (int r = 0; r < NB_MAX; r++) {
-      const c128 t = adjoint ? cconj(__ldg(Tm + r * NB_MAX + q)) : __ldg(Tm + q * NB_MAX + r);
-      const c128 pr = cmul(t, dv[r]);
-      a.x += pr.x; a.y += pr.y;
-    }
-    sv[q] = a;
-  }
-#pragma unroll
-  for (int r = 0; r < RA; r++) {
-    const int i = tid + r * AT;
-    if (i < len) {
-      c128 o = y[r];
-#pragma unroll
-      for (int q = 0; q < NB_MAX; q++) { const c128 t = cmul(v[r][q], sv[q]); o.x -= t.x; o.y -= t.y; }
-      Y[(long long)c * rows + j0 + i] = o;
-    }
+    const int i = FORMQ ? tid + r * AT : j0_in + tid + r * AT;
+    if (i < rows) Y[(long long)c * rows + i] = y[r];
   }
 }
 
-void launch_apply(cudaStream_t st, const c128 *X, c128 *Y, int rows, int j0, int w, const c128 *Tp, int adjoint,
+void launch_apply(cudaStream_t st, int mode, const c128 *X, c128 *Y, int rows, int j0, int w, const c128 *Tp, int adjoint,
                   int c_begin, int c_end) {
   if (c_begin >= c_end) return;
-  const int len = rows - j0, n = c_end - c_begin;
-  if (len <= 10 * 128) TDVP_LAUNCH((qr_apply1_kernel<128, 10>), n, 128, 0, st, X, Y, rows, j0, w, Tp, adjoint, c_begin);
-  else if (len <= 10 * 256) TDVP_LAUNCH((qr_apply1_kernel<256, 10>), n, 256, 0, st, X, Y, rows, j0, w, Tp, adjoint, c_begin);
+  const int n = c_end - c_begin;
+  if (mode == 1 && adjoint) TDVP_LAUNCH((qr_apply1_kernel<256, 5, 8, false>), n, 256, 0, st, X, Y, rows, j0, w, Tp, 0, 0, c_begin);
+  else if (mode == 2 && adjoint) TDVP_LAUNCH((qr_apply1_kernel<256, 10, 4, false>), n, 256, 0, st, X, Y, rows, j0, w, Tp, 0, 0, c_begin);
+  else if (mode == 3 && adjoint) TDVP_LAUNCH((qr_apply1_kernel<256, 20, 2, false>), n, 256, 0, st, X, Y, rows, j0, w, Tp, 0, 0, c_begin);
   else TDVP_LAUNCH(qr_apply_kernel, (n + CB - 1) / CB, TRAIL_THREADS, 0, st, X, Y, rows, j0, w, Tp, adjoint, c_begin, c_end);
 }
 
@@ -578,11 +625,12 @@ void qr_configure() {
   cudaFuncSetAttribute(qr_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024 + 1024);
 }
 
-// Panel variant by height: register-resident panels up to 5120 rows, the shared-memory panel beyond.
+// Panel variant by height: register-resident panels up to 5120 rows (512 threads, 3/5/10 rows per
+// thread, 8/4/2 columns per panel: at most 48 doubles of panel per thread), the shared-memory panel beyond.
 int panel_mode(int rows, int *nb) {
-  if (rows <= 5 * RP_THREADS) { *nb = 8; return 1; }
-  if (rows <= 10 * RP_THREADS) { *nb = 4; return 2; }
-  if (rows <= 20 * RP_THREADS) { *nb = 2; return 3; }
+  if (rows <= 5 * 256) { *nb = 8; return 1; }
+  if (rows <= 10 * 256) { *nb = 4; return 2; }
+  if (rows <= 20 * 256) { *nb = 2; return 3; }
   *nb = panel_width(rows);
   return 0;
 }
@@ -618,17 +666,22 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
     int j0 = pz * nb, w = cols - j0 < nb ? cols - j0 : nb;
     size_t smem = (size_t)w * (rows - j0) * 16;
     c128 *Tp = Tm + (size_t)pz * NB_MAX * NB_MAX;
-    if (mode == 1) TDVP_LAUNCH((qr_panel_reg_kernel<5, 8>), 1, RP_THREADS, 0, st, X, rows, cols, j0, w, Rm, Tp);
-    else if (mode == 2) TDVP_LAUNCH((qr_panel_reg_kernel<10, 4>), 1, RP_THREADS, 0, st, X, rows, cols, j0, w, Rm, Tp);
-    else if (mode == 3) TDVP_LAUNCH((qr_panel_reg_kernel<20, 2>), 1, RP_THREADS, 0, st, X, rows, cols, j0, w, Rm, Tp);
+    if (mode == 1) TDVP_LAUNCH((qr_panel_reg_kernel<256, 5, 8>), 1, 256, 0, st, X, rows, cols, j0, w, Rm, Tp);
+    else if (mode == 2) TDVP_LAUNCH((qr_panel_reg_kernel<512, 5, 4>), 1, 512, 0, st, X, rows, cols, j0, w, Rm, Tp);
+    else if (mode == 3) TDVP_LAUNCH((qr_panel_reg_kernel<512, 10, 2>), 1, 512, 0, st, X, rows, cols, j0, w, Rm, Tp);
     else TDVP_LAUNCH(qr_panel_kernel, 1, PANEL_THREADS, smem, st, X, rows, cols, j0, w, Rm, Tp);
     int c_begin = j0 + w;
-    launch_apply(st, X, X, rows, j0, w, Tp, 1, c_begin, cols);
+    launch_apply(st, mode, X, X, rows, j0, w, Tp, 1, c_begin, cols);
   }
-  TDVP_LAUNCH(identity_kernel, gcopy, 256, 0, st, Y, rows, cols);
-  for (int pz = npanels - 1; pz >= 0; pz--) {
-    int j0 = pz * nb, w = cols - j0 < nb ? cols - j0 : nb;
-    launch_apply(st, X, Y, rows, j0, w, Tm + (size_t)pz * NB_MAX * NB_MAX, 0, j0, cols);
+  if (mode == 1) TDVP_LAUNCH((qr_apply1_kernel<256, 5, 8, true>), cols, 256, 0, st, X, Y, rows, 0, 0, Tm, nb, cols, 0);
+  else if (mode == 2) TDVP_LAUNCH((qr_apply1_kernel<256, 10, 4, true>), cols, 256, 0, st, X, Y, rows, 0, 0, Tm, nb, cols, 0);
+  else if (mode == 3) TDVP_LAUNCH((qr_apply1_kernel<256, 20, 2, true>), cols, 256, 0, st, X, Y, rows, 0, 0, Tm, nb, cols, 0);
+  else {
+    TDVP_LAUNCH(identity_kernel, gcopy, 256, 0, st, Y, rows, cols);
+    for (int pz = npanels - 1; pz >= 0; pz--) {
+      int j0 = pz * nb, w = cols - j0 < nb ? cols - j0 : nb;
+      launch_apply(st, mode, X, Y, rows, j0, w, Tm + (size_t)pz * NB_MAX * NB_MAX, 0, j0, cols);
+    }
   }
   if (side == 0) TDVP_LAUNCH(transpose_out_kernel, tg, tb, 0, st, Y, Q, rows, cols);
   else TDVP_LAUNCH(copy_kernel, gcopy, 256, 0, st, Q, Y, n);
