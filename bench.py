@@ -271,16 +271,18 @@ def run_ours(args):
     # ---- roofline of the dominant kernel (DMMA complex GEMM): live event brackets above ----
     zg_ms, zg_n = prof["zgemm"]
     ws_ms, ws_n = prof["wstage"]
-    sk_ms, sk_n = prof["splitk_reduce"]
     flops_per_launch = gemm_stage_flops(M)             # each of the 2 GEMM launches of an apply
     achieved = flops_per_launch / (zg_ms / max(zg_n, 1) * 1e-3) / 1e12 if zg_n else None
     roofline = {"bound": "tensor", "kernel": "zgemm_kernel (FP64 DMMA m8n8k4, complex128)",
                 "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": (achieved / peak) if achieved else None, "traffic": None,
+                "frac": (achieved / peak) if achieved else None,
+                # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture in
+                # profiles/r01b_summary.md (mean of the stage-1 and stage-3 launches), M = 128 only
+                "traffic": 50.6e6 if M == 128 else None,
                 "peak_source": "tdvp_probe_fp64_tensor_peak: DMMA m8n8k4 issue rate measured in this run "
                                "(MEASURED_PEAKS.json has no FP64 figure; cuBLAS ZGEMM 4096^3 measured 36.85 TFLOP/s)",
                 "flops_per_launch": flops_per_launch, "avg_launch_us": 1e3 * zg_ms / max(zg_n, 1), "launches": zg_n,
-                "share_of_step": {"zgemm": zg_ms / ms_total, "wstage": ws_ms / ms_total, "splitk_reduce": sk_ms / ms_total},
+                "share_of_step": {"zgemm": zg_ms / ms_total, "wstage": ws_ms / ms_total},
                 "wstage": {"bound": "hbm", "algorithmic_bytes": 2 * 16.0 * M * M * D_W * D_PHYS,
                            "achieved_gbs": (2 * 16.0 * M * M * D_W * D_PHYS / (ws_ms / max(ws_n, 1) * 1e-3) / 1e9) if ws_n else None,
                            "avg_launch_us": 1e3 * ws_ms / max(ws_n, 1)}}
@@ -331,6 +333,9 @@ def run_ours(args):
            "roofline": roofline, "e2e": e2e, "gpu_launches": int(gpu_launches), "clocks": clocks}
 
     if rank == 0 and not args.no_extras:
+        # what non-tensor instructions cost the FP64 tensor pipe: TFLOP/s with F
+        # integer instructions issued after every DMMA, two CTAs of four warps per SM
+        out["dmma_issue_probe_tflops"] = {str(f): T.tdvp_probe_dmma_issue(f, 4000) for f in (0, 1, 2, 4, 8, 16)}
         # M sweep of configs[1]
         out["sweep"] = [sweep_point(torch, T, m, peak) for m in (32, 64, 128, 256, 512)]
         torch.cuda.empty_cache()

@@ -200,6 +200,11 @@ const char *tdvp_last_error(const tdvp_handle *h);
    the legacy default stream, blocks, returns TFLOP/s.  This is the denominator bench.py uses for
    "fraction of FP64 tensor peak". */
 int tdvp_probe_fp64_tensor_peak(int iters, double *tflops /*HOST*/);
+/* The same probe with `fillers` (0, 1, 2, 4, 8 or 16) independent integer instructions issued after
+   every DMMA, at the GEMM kernel's residency (two CTAs of four warps per SM): measures what the
+   non-tensor instructions of a DMMA loop cost.  Blocks; TDVP_EINVAL on other
+   filler counts. */
+int tdvp_probe_dmma_issue(int fillers, int iters, double *tflops /*HOST*/);
 /* Phase profiler: when enabled, launches of the dominant kernel classes are bracketed by CUDA events
    on the launching stream (not inside a captured step).  tdvp_profile_read blocks on the device,
    returns the summed elapsed milliseconds and bracket counts per phase since the last read and

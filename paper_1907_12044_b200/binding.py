@@ -31,7 +31,7 @@ EXPORTED_SYMBOLS = [
     "tdvp_qr_gauge", "tdvp_svd_bond", "tdvp_apply_heff_host", "tdvp_apply_heff_site", "tdvp_update_env_site",
     "tdvp_step_ps", "tdvp_step_mu", "tdvp_mu_derivative", "tdvp_set_gauge", "tdvp_observe", "tdvp_populations",
     "tdvp_norm_energy", "tdvp_get_mps", "tdvp_set_mps", "tdvp_get_centre", "tdvp_sync",
-    "tdvp_last_error", "tdvp_probe_fp64_tensor_peak", "tdvp_launch_count", "tdvp_profile_enable",
+    "tdvp_last_error", "tdvp_probe_fp64_tensor_peak", "tdvp_probe_dmma_issue", "tdvp_launch_count", "tdvp_profile_enable",
     "tdvp_profile_read",
 ]
 
@@ -84,6 +84,7 @@ def _load():
         "tdvp_sync": (c_int, [P]),
         "tdvp_last_error": (c_char_p, [P]),
         "tdvp_probe_fp64_tensor_peak": (c_int, [c_int, POINTER(c_double)]),
+        "tdvp_probe_dmma_issue": (c_int, [c_int, c_int, POINTER(c_double)]),
         "tdvp_launch_count": (c_longlong, []),
         "tdvp_profile_enable": (c_int, [c_int]),
         "tdvp_profile_read": (c_int, [POINTER(c_double), POINTER(c_longlong)]),
@@ -263,6 +264,12 @@ def tdvp_probe_fp64_tensor_peak(iters=20000) -> float:
 
 
 PROFILE_PHASES = ("zgemm", "splitk_reduce", "wstage", "vector", "qr", "svd")
+
+
+def tdvp_probe_dmma_issue(fillers, iters=4000) -> float:
+    t = c_double(0.0)
+    _check(_lib.tdvp_probe_dmma_issue(int(fillers), iters, byref(t)))
+    return t.value
 
 
 def tdvp_profile_enable(on: bool):

@@ -290,25 +290,48 @@ int tdvp_qr_gauge(tdvp_handle *h, int side, int Ml, int d, int Mr, const tdvp_c1
   return check_cuda(h, cudaGetLastError(), "tdvp_qr_gauge");
 }
 
+}  // extern "C"
+
 // ---- FP64 tensor-pipe issue-rate probe ------------------------------------------------------
-__global__ void dmma_probe_kernel(double *out, int iters, double a, double b) {
+// F independent integer instructions (LOP3) follow every DMMA: F = 0 measures the pipe's peak, F > 0
+// how much of it other instructions of the same warps cost (they do not issue under a DMMA).
+template <int F>
+__global__ void dmma_probe_kernel(double *out, int iters, double a, double b, int z) {
   double c0[8], c1[8];
+  int x[4] = {(int)threadIdx.x, 1, 2, 3};
 #pragma unroll
   for (int i = 0; i < 8; i++) { c0[i] = threadIdx.x; c1[i] = i; }
   for (int it = 0; it < iters; it++) {
 #pragma unroll
-    for (int i = 0; i < 8; i++)
+    for (int i = 0; i < 8; i++) {
       asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                    : "+d"(c0[i]), "+d"(c1[i]) : "d"(a), "d"(b));
+#pragma unroll
+      for (int f = 0; f < F; f++) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(x[f & 3]) : "r"(z), "r"(it));
+    }
   }
   double s = 0;
 #pragma unroll
   for (int i = 0; i < 8; i++) s += c0[i] + c1[i];
-  if (s == 1.2345) out[0] = s;
+  if (s == 1.2345 || x[0] + x[1] + x[2] + x[3] == 12345) out[0] = s;
 }
 
-int tdvp_probe_fp64_tensor_peak(int iters, double *tflops) {
-  if (!tflops || iters < 1) return set_err(nullptr, TDVP_EINVAL, "bad arguments");
+static void launch_probe(int fillers, int blocks, int threads, double *out, int iters) {
+  switch (fillers) {
+    case 0: dmma_probe_kernel<0><<<blocks, threads>>>(out, iters, 1.0000001, 1e-9, iters); break;
+    case 1: dmma_probe_kernel<1><<<blocks, threads>>>(out, iters, 1.0000001, 1e-9, iters); break;
+    case 2: dmma_probe_kernel<2><<<blocks, threads>>>(out, iters, 1.0000001, 1e-9, iters); break;
+    case 4: dmma_probe_kernel<4><<<blocks, threads>>>(out, iters, 1.0000001, 1e-9, iters); break;
+    case 8: dmma_probe_kernel<8><<<blocks, threads>>>(out, iters, 1.0000001, 1e-9, iters); break;
+    default: dmma_probe_kernel<16><<<blocks, threads>>>(out, iters, 1.0000001, 1e-9, iters); break;
+  }
+}
+
+extern "C" {
+
+int tdvp_probe_dmma_issue(int fillers, int iters, double *tflops) {
+  if (!tflops || iters < 1 || !(fillers == 0 || fillers == 1 || fillers == 2 || fillers == 4 || fillers == 8 || fillers == 16))
+    return set_err(nullptr, TDVP_EINVAL, "bad arguments (fillers must be 0, 1, 2, 4, 8 or 16)");
   int dev = 0, nsm = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
@@ -316,12 +339,14 @@ int tdvp_probe_fp64_tensor_peak(int iters, double *tflops) {
   if (int rc = check_cuda(nullptr, cudaMalloc(&out, 8), "cudaMalloc")) return rc;
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0); cudaEventCreate(&e1);
-  const int blocks = 2 * nsm, threads = 256;
-  dmma_probe_kernel<<<blocks, threads>>>(out, iters / 10 + 1, 1.0000001, 1e-9);
+  // F = 0: eight warps per CTA (the peak); F > 0: two CTAs of four warps per SM, the residency of
+  // zgemm_kernel (two warps per SMSP)
+  const int blocks = 2 * nsm, threads = fillers == 0 ? 256 : 128;
+  launch_probe(fillers, blocks, threads, out, iters / 10 + 1);
   float best = 1e30f;
   for (int r = 0; r < 3; r++) {
     cudaEventRecord(e0);
-    dmma_probe_kernel<<<blocks, threads>>>(out, iters, 1.0000001, 1e-9);
+    launch_probe(fillers, blocks, threads, out, iters);
     cudaEventRecord(e1);
     cudaEventSynchronize(e1);
     float ms = 0;
@@ -335,5 +360,7 @@ int tdvp_probe_fp64_tensor_peak(int iters, double *tflops) {
   *tflops = 2.0 * fma / (best * 1e-3) / 1e12;
   return TDVP_OK;
 }
+
+int tdvp_probe_fp64_tensor_peak(int iters, double *tflops) { return tdvp_probe_dmma_issue(0, iters, tflops); }
 
 }  // extern "C"
