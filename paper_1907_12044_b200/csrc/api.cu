@@ -177,13 +177,33 @@ int tdvp_apply_heff_host(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr, 
   void *wmem = hh->arena.take(wb);
   void *ws = hh->arena.take(hb);
   cudaStream_t st = hh->stream;
-  if (int rc = check_cuda(h, cudaMemcpyAsync(dL, L, nL, cudaMemcpyHostToDevice, st), "h2d L")) return rc;
-  if (int rc = check_cuda(h, cudaMemcpyAsync(dW, W, nW, cudaMemcpyHostToDevice, st), "h2d W")) return rc;
-  if (int rc = check_cuda(h, cudaMemcpyAsync(dA, A, nA, cudaMemcpyHostToDevice, st), "h2d A")) return rc;
-  if (int rc = check_cuda(h, cudaMemcpyAsync(dR, R, nR, cudaMemcpyHostToDevice, st), "h2d R")) return rc;
-  WSparse wsp;
-  wsparse_build(st, wsp, wmem, Dl, d, Dr, dW, hh->opt.w_zero_tol);
-  heff_apply(st, Ml, Mr, d, Dl, Dr, dL, wsp, dA, dR, dO, ws);
+  if (!hh->copy_stream) {
+    if (int rc = check_cuda(h, cudaStreamCreateWithFlags(&hh->copy_stream, cudaStreamNonBlocking), "copy stream")) return rc;
+    cudaEventCreateWithFlags(&hh->ev_first, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&hh->ev_w, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&hh->ev_r, cudaEventDisableTiming);
+    for (int i = 0; i < 4; i++) cudaEventCreateWithFlags(&hh->ev_l[i], cudaEventDisableTiming);
+  }
+  // all H2D copies go to the copy queue in the order the stages need them -- A, L in slices of the
+  // bond index, W, R -- and the compute stream waits for each piece by event, so stage 1 starts
+  // after A and the first slice of L and the W stage / stage 3 never wait if the link keeps up
+  cudaStream_t cq = hh->copy_stream;
+  const int nsl = Ml >= 64 ? 4 : 1;
+  cudaEventRecord(hh->ev_first, st);                     // the arena's previous users are done
+  cudaStreamWaitEvent(cq, hh->ev_first, 0);
+  if (int rc = check_cuda(h, cudaMemcpyAsync(dA, A, nA, cudaMemcpyHostToDevice, cq), "h2d A")) return rc;
+  for (int s = 0; s < nsl; s++) {
+    const size_t a0 = (size_t)Ml * s / nsl, a1 = (size_t)Ml * (s + 1) / nsl, row = (size_t)Dl * Ml;
+    if (a1 > a0)
+      if (int rc = check_cuda(h, cudaMemcpyAsync(dL + a0 * row, reinterpret_cast<const c128 *>(L) + a0 * row, (a1 - a0) * row * 16,
+                                                 cudaMemcpyHostToDevice, cq), "h2d L")) return rc;
+    cudaEventRecord(hh->ev_l[s], cq);
+  }
+  if (int rc = check_cuda(h, cudaMemcpyAsync(dW, W, nW, cudaMemcpyHostToDevice, cq), "h2d W")) return rc;
+  cudaEventRecord(hh->ev_w, cq);
+  if (int rc = check_cuda(h, cudaMemcpyAsync(dR, R, nR, cudaMemcpyHostToDevice, cq), "h2d R")) return rc;
+  cudaEventRecord(hh->ev_r, cq);
+  heff_apply_staged(st, Ml, Mr, d, Dl, Dr, dL, dW, wmem, hh->opt.w_zero_tol, dA, dR, dO, ws, nsl, hh->ev_l, hh->ev_w, hh->ev_r);
   if (int rc = check_cuda(h, cudaGetLastError(), "tdvp_apply_heff_host")) return rc;
   if (int rc = check_cuda(h, cudaMemcpyAsync(out, dO, nA, cudaMemcpyDeviceToHost, st), "d2h out")) return rc;
   return check_cuda(h, cudaStreamSynchronize(st), "tdvp_apply_heff_host sync");

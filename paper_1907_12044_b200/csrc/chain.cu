@@ -120,6 +120,11 @@ int tdvp_destroy(tdvp_handle *h) {
   if (!h) return TDVP_OK;
   cudaStreamSynchronize(h->stream);
   free_chain(h);
+  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+  if (h->ev_first) cudaEventDestroy(h->ev_first);
+  if (h->ev_w) cudaEventDestroy(h->ev_w);
+  if (h->ev_r) cudaEventDestroy(h->ev_r);
+  for (int i = 0; i < 4; i++) if (h->ev_l[i]) cudaEventDestroy(h->ev_l[i]);
   delete h;
   return TDVP_OK;
 }

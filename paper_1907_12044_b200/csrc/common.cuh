@@ -122,6 +122,12 @@ struct Arena {
 size_t heff_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr);
 void heff_apply(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c128 *L,
                 const WSparse &W, const c128 *A, const c128 *R, c128 *out, void *ws);
+// The same for the host-entry path, whose inputs are still arriving on a copy queue: stage 1 runs in
+// nsl slices of the bond index a, slice s after ev_l[s] (A and rows [s*Ml/nsl, (s+1)*Ml/nsl) of L
+// have landed); the sparse form of W is built after ev_w, stage 3 waits for ev_r (R).
+void heff_apply_staged(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c128 *L, const c128 *W_dense,
+                       void *wmem, double zero_tol, const c128 *A, const c128 *R, c128 *out, void *ws,
+                       int nsl, const cudaEvent_t *ev_l, cudaEvent_t ev_w, cudaEvent_t ev_r);
 size_t env_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr);
 void env_update(cudaStream_t st, int side, int Ml, int Mr, int d, int Dl, int Dr,
                 const c128 *env_in, const WSparse &W, const c128 *A, c128 *env_out, void *ws);

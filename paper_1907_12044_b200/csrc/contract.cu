@@ -96,6 +96,30 @@ void heff_apply(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c1
   zgemm(st, g_stage3_heff(Ml, Mr, d, Dr, T2, R, out), sk);
 }
 
+void heff_apply_staged(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c128 *L, const c128 *W_dense,
+                       void *wmem, double zero_tol, const c128 *A, const c128 *R, c128 *out, void *ws,
+                       int nsl, const cudaEvent_t *ev_l, cudaEvent_t ev_w, cudaEvent_t ev_r) {
+  size_t t1 = (size_t)Ml * Dl * d * Mr, t2 = (size_t)Ml * d * Dr * Mr;
+  char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
+  c128 *T1 = reinterpret_cast<c128 *>(p); p += up256(t1 * 16);
+  c128 *T2 = reinterpret_cast<c128 *>(p); p += up256(t2 * 16);
+  c128 *sk = reinterpret_cast<c128 *>(p);
+  for (int s = 0; s < nsl; s++) {
+    const int a0 = (int)((long long)Ml * s / nsl), a1 = (int)((long long)Ml * (s + 1) / nsl);
+    cudaStreamWaitEvent(st, ev_l[s], 0);
+    if (a1 == a0) continue;
+    ZGemm g = g_stage1_left(Ml, Mr, d, Dl, L + (size_t)a0 * Dl * Ml, A, T1 + (size_t)a0 * Dl * d * Mr);
+    g.M = (a1 - a0) * Dl;
+    zgemm(st, g, sk);
+  }
+  cudaStreamWaitEvent(st, ev_w, 0);
+  WSparse W;
+  wsparse_build(st, W, wmem, Dl, d, Dr, W_dense, zero_tol);
+  wstage_left(st, W, Ml, Mr, T1, T2);
+  cudaStreamWaitEvent(st, ev_r, 0);
+  zgemm(st, g_stage3_heff(Ml, Mr, d, Dr, T2, R, out), sk);
+}
+
 size_t env_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr) {
   size_t t1 = (size_t)Ml * Dl * d * Mr, t2 = (size_t)Ml * d * Dr * Mr;
   size_t big = t1 > t2 ? t1 : t2;

@@ -15,6 +15,8 @@ struct tdvp_handle {
   tdvp_options opt;
   std::string err;
   Arena arena;                     // scratch for the current call (reset per call)
+  cudaStream_t copy_stream = nullptr;   // host-entry calls: second H2D queue (created on first use)
+  cudaEvent_t ev_first = nullptr, ev_w = nullptr, ev_r = nullptr, ev_l[4] = {nullptr, nullptr, nullptr, nullptr};
 
   // ---- resident chain state (n == 0 for a context-only handle) ----
   int n = 0;
