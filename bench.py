@@ -211,6 +211,23 @@ def build_chain(name, M=None):
     return cfg, mpo, mps
 
 
+def rank_max(x, world, device):
+    """Replicas only: the ranks share nothing but the clock -- the step time of the job
+    is the MAX over ranks (all-reduce on `device`: "cuda" under NCCL, "cpu" under gloo in the tests)."""
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(units_per_rank, world, ms_max):
+    """Whole-job throughput: the units ALL ranks processed divided by the slowest rank's time."""
+    return world * units_per_rank / (ms_max * 1e-3)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -231,11 +248,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return rank_max(x, world, "cuda")
 
     peak = T.tdvp_probe_fp64_tensor_peak(20000)        # DMMA issue-rate ceiling, measured live
     M = M_HEADLINE
@@ -266,7 +279,7 @@ def run_ours(args):
     T.tdvp_profile_enable(False)
     clocks = sampler.stop()
     n_applies = args.steps * APPLIES_PER_STEP
-    value = world * n_applies / (ms_total * 1e-3)
+    value = job_value(n_applies, world, ms_total)
 
     # ---- roofline of the dominant kernel (DMMA complex GEMM): live event brackets above ----
     zg_ms, zg_n = prof["zgemm"]

@@ -347,7 +347,9 @@ void launch1(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, cons
   cfg.gridDim = dim3(kp.G); cfg.blockDim = dim3(NTHREADS); cfg.dynamicSmemBytes = SMEM_BYTES; cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeCooperative; attr[0].val.cooperative = 1;
-  cfg.attrs = attr; cfg.numAttrs = 1;
+  // no tile is cut when the ranges are whole tiles: nobody waits for anybody, a plain launch will do
+  const bool cut = kp.upc_rem != 0 || (kp.upc_base % kp.ktiles) != 0;
+  cfg.attrs = attr; cfg.numAttrs = cut ? 1 : 0;
   cudaLaunchKernelEx(&cfg, zgemm_kernel<AK, BK_, CJ>, ta, tb, kp);
   count_launch();
 }

@@ -99,7 +99,27 @@ def test_update_env_microbench_config(T, M):
     assert rel(host(T.tdvp_update_env(1, dev(R), dev(W), dev(A))), oc.envR(R, W, A)) <= REL_TOL
 
 
-@pytest.mark.parametrize("dims", [(1, 1, 1), (5, 3, 4), (40, 72, 9), (128, 128, 20)])
+@pytest.mark.parametrize("M", [256, 512])
+def test_apply_heff_microbench_config_sampled(T, M):
+    """The sweep's largest sizes in the launch configuration bench.py times (stream-K cuts in both GEMM
+    stages, several W-stage items per SM): sampled output slabs out[a, :, :], each computed by the
+    oracle from the definition restricted to that a (Eq. 29: L[a] is the only place a enters)."""
+    L, W, A, R = si.microbench_tensors(M)
+    got = host(T.tdvp_apply_heff(dev(L), dev(W), dev(A), dev(R)))
+    rng = np.random.default_rng(M)
+    for a in sorted(set([0, M - 1] + list(rng.integers(0, M, 4)))):
+        want = oc.heff(L[a:a + 1], W, A, R)[0]
+        assert rel(got[a], want) <= REL_TOL
+    # env update at the same size: sampled slabs L'[b, :, :] need conj(A[:, :, b]) only
+    gotE = host(T.tdvp_update_env(0, dev(L), dev(W), dev(A)))
+    t2 = np.tensordot(np.tensordot(L, A, axes=([2], [0])), W, axes=([1, 2], [0, 2]))   # [a, y, s, v]
+    for b in (0, M // 2 + 1, M - 1):
+        want = np.tensordot(np.conj(A[:, :, b]), t2, axes=([0, 1], [0, 2]))             # [y, v]
+        assert rel(gotE[b], want.T) <= REL_TOL
+
+
+@pytest.mark.parametrize("dims", [(1, 1, 1), (5, 3, 4), (40, 72, 9), (128, 128, 20), (64, 64, 1), (100, 36, 3),
+                                  (257, 129, 2), (8, 300, 1)])
 def test_apply_bond(T, dims):
     Ml, Mr, Dw = dims
     rng = np.random.default_rng(300 + Ml)
