@@ -390,6 +390,26 @@ def run_ours(args):
         out["ps_step"]["phase_ms"] = {k: round(v[0], 3) for k, v in ph.items()}
         out["ps_step"]["phase_brackets"] = {k: v[1] for k, v in ph.items()}
         ch.close()
+        # configs[4]: the large chain (147 sites, layout B, M = 256): one warm-up and two timed PS steps,
+        # gated on invariants (oracle steps at this size take minutes)
+        if args.large:
+            cfg, mpo, mps = build_chain("fmo256")
+            ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=cfg.krylov_dim))
+            n0, en0 = ch.tdvp_norm_energy()
+            ch.tdvp_step_ps(cfg.dt_fs)
+            ch.tdvp_sync()
+            e0.record()
+            for _ in range(2):
+                ch.tdvp_step_ps(cfg.dt_fs)
+            e1.record()
+            ch.tdvp_sync()
+            torch.cuda.synchronize()
+            nrm, en = ch.tdvp_norm_energy()
+            out["ps_step_large"] = {"workload": "configs[4]: FMO-like chain, 7 x 20 modes, layout B, 147 sites, M=256, D_W<=15, "
+                                                "k=10, dt=20 fs, CUDA graph",
+                                    "ms_per_step": e0.elapsed_time(e1) / 2, "steps_timed": 2, "norm_sq": nrm,
+                                    "energy_drift_rel": (en - en0) / abs(en0), "population_sum": float(sum(ch.tdvp_populations(0)))}
+            ch.close()
         # the oracle as it stands on the host cores, bounded sample
         v, n, el = time_oracle_heff(M, min_seconds=10.0)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": oracle_cores(), "kind": "oracle",
@@ -409,6 +429,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the M sweep, the PS step and the CPU baseline")
+    ap.add_argument("--large", action="store_true", help="also time the M=256, 147-site chain (about a minute more)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":

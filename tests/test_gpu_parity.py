@@ -131,7 +131,9 @@ def test_apply_bond(T, dims):
 
 
 # ---- QR gauge move (Eq. 9) ------------------------------------------------------------------
-@pytest.mark.parametrize("shape", [(1, 3, 3), (3, 4, 12), (16, 4, 16), (37, 5, 29), (64, 10, 64), (130, 3, 70)])
+# the last four shapes reach the panel variants for tall sides of 1280 / 2560 / 5120 rows and beyond
+@pytest.mark.parametrize("shape", [(1, 3, 3), (3, 4, 12), (16, 4, 16), (37, 5, 29), (64, 10, 64), (130, 3, 70),
+                                   (128, 10, 128), (200, 10, 200), (260, 16, 64), (90, 64, 40)])
 @pytest.mark.parametrize("side", [0, 1])
 def test_qr_gauge(T, shape, side):
     Ml, d, Mr = shape
@@ -261,6 +263,26 @@ def test_fmo_like_chain_delta_seeded(T):
         E = np.einsum("ax,asb,xsy->by", E, A.conj(), B)
     assert abs(abs(E[0, 0]) - 1.0) <= 1e-9
     ch.close()
+
+
+def test_large_chain_invariants(T):
+    """BASELINE.json configs[4] at full size (147 sites, layout B, M = 256): the oracle needs minutes per
+    step there, so the full-size run is gated on what holds at any size -- norm, energy and the
+    population sum are conserved by TDVP-PS (pin p4 for the oracle)."""
+    cfg = si.CONFIGS["fmo256"]
+    params = si.draw_vibronic_params(cfg)
+    mpo = model.build_mpo(params)
+    mps = si.padded_product_mps(si.site_dims(params), si.initial_occupations(params), cfg.M, cfg.pad_seed, cfg.delta, cfg.delta_seed)
+    assert len(mps) == 147 and max(a.shape[2] for a in mps) == 256
+    ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=cfg.krylov_dim))
+    n0, e0 = ch.tdvp_norm_energy()
+    ch.tdvp_step_ps(cfg.dt_fs)
+    n1, e1 = ch.tdvp_norm_energy()
+    pops = ch.tdvp_populations(0)
+    ch.close()
+    assert abs(n1 - 1.0) < 1e-11 and abs(n0 - 1.0) < 1e-12
+    assert abs(e1 - e0) < 1e-9 * abs(e0)
+    assert abs(float(np.sum(pops)) - 1.0) < 1e-11 and np.all(pops > -1e-12)
 
 
 def test_teacher_forced_step(T):
