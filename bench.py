@@ -390,6 +390,33 @@ def run_ours(args):
         out["ps_step"]["phase_ms"] = {k: round(v[0], 3) for k, v in ph.items()}
         out["ps_step"]["phase_brackets"] = {k: v[1] for k, v in ph.items()}
         ch.close()
+        # TDVP-MU on the same chain (configs[3]): five PS steps of warm-up (the MU right-hand side needs
+        # full-rank bonds, DESIGN.md c18), then Dormand-Prince steps of h = 0.004 fs: with eps = 1e-10 the
+        # right-hand side is stiff (1 / sqrt(eps) = 1e5 on the weakly occupied bonds of this chain), the
+        # explicit 5(4) pair is stable up to h ~ 0.02 fs and overflows at 0.1 fs (DESIGN.md c12)
+        ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=cfg.krylov_dim))
+        for _ in range(5):
+            ch.tdvp_step_ps(cfg.dt_fs)
+        H_MU = 0.004
+        ch.tdvp_step_mu(H_MU)
+        ch.tdvp_sync()
+        T.tdvp_profile_enable(True)
+        T.tdvp_profile_read()
+        e0.record()
+        n_mu = 2
+        for _ in range(n_mu):
+            err = ch.tdvp_step_mu(H_MU, want_err=True)
+        e1.record()
+        ch.tdvp_sync()
+        torch.cuda.synchronize()
+        ph = T.tdvp_profile_read()
+        T.tdvp_profile_enable(False)
+        nrm, en = ch.tdvp_norm_energy()
+        out["mu_step"] = {"workload": "configs[3] chain, 71 sites, M=128: one Dormand-Prince 5(4) step of h = 0.004 fs "
+                                      "(7 right-hand sides: SVD + environments + H_eff per site) after 5 PS steps",
+                          "ms_per_step": e0.elapsed_time(e1) / n_mu, "steps_timed": n_mu, "err_est": err, "norm_sq": nrm,
+                          "energy": en, "phase_ms_per_step": {k: round(v[0] / n_mu, 3) for k, v in ph.items()}}
+        ch.close()
         # configs[4]: the large chain (147 sites, layout B, M = 256): one warm-up and two timed PS steps,
         # gated on invariants (oracle steps at this size take minutes)
         if args.large:

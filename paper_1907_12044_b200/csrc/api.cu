@@ -60,7 +60,7 @@ void Arena::release() { if (base) cudaFree(base); base = nullptr; cap = 0; off =
 
 void configure_kernels_once() {
   static std::once_flag once;
-  std::call_once(once, [] { zgemm_configure(); wstage_configure(); qr_configure(); lanczos_configure(); });
+  std::call_once(once, [] { zgemm_configure(); wstage_configure(); qr_configure(); lanczos_configure(); svd_configure(); });
 }
 
 tdvp_handle *default_handle() {

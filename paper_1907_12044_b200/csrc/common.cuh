@@ -49,6 +49,7 @@ __host__ __device__ static inline c128 cconj(c128 a) { return make_double2(a.x, 
 void zgemm_configure();
 void wstage_configure();
 void qr_configure();
+void svd_configure();
 void lanczos_configure();
 void configure_kernels_once();
 

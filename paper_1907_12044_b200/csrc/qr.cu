@@ -117,13 +117,24 @@ __device__ __noinline__ void build_T(const c128 *Gs, const c128 *tau_s, c128 *Ts
   const int lane = threadIdx.x & 31;
   for (int a = lane; a < NB_MAX * NB_MAX; a += 32) Ts[a] = make_double2(0.0, 0.0);
   __syncwarp();
+  // column c: T[a][c] = -tau_c sum_{qq<c} T[a][qq] G[qq][c]; lane = 4 a' + part handles two rows a (a', a' + 4... )
+  // spread as: lane = a * 4 + s, s = quarter of the qq range; partial sums are combined by two shuffles
   for (int c = 0; c < w; c++) {
-    if (lane == c) Ts[c * NB_MAX + c] = tau_s[c];
-    if (lane < c) {                                      // T[0:c, c] = -tau_c T[0:c, 0:c] (V^H v_c)
-      c128 acc = make_double2(0.0, 0.0);
-      for (int qq = lane; qq < c; qq++) { c128 t = cmul(Ts[lane * NB_MAX + qq], Gs[qq * NB_MAX + c]); acc.x += t.x; acc.y += t.y; }
+    if (lane == 0) Ts[c * NB_MAX + c] = tau_s[c];
+    const int a = lane >> 2, sgm = lane & 3;             // 8 rows x 4 segments of two qq each
+    c128 acc = make_double2(0.0, 0.0);
+    if (a < c) {
+#pragma unroll
+      for (int u = 0; u < 2; u++) {
+        const int qq = 2 * sgm + u;
+        if (qq >= a && qq < c) { const c128 t = cmul(Ts[a * NB_MAX + qq], Gs[qq * NB_MAX + c]); acc.x += t.x; acc.y += t.y; }
+      }
+    }
+    acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 1); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 1);
+    acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 2); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 2);
+    if (a < c && sgm == 0) {
       const c128 t = cmul(tau_s[c], acc);
-      Ts[lane * NB_MAX + c] = make_double2(-t.x, -t.y);
+      Ts[a * NB_MAX + c] = make_double2(-t.x, -t.y);
     }
     __syncwarp();
   }
@@ -168,9 +179,10 @@ __device__ __forceinline__ void qr_panel_col(c128 (&x)[RPT][NB], c128 (*pivot)[N
   } else {
     const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xn2);
     beta = alpha.x >= 0.0 ? -nrm : nrm;
-    tau = make_double2((beta - alpha.x) / beta, -alpha.y / beta);
-    const double dr = alpha.x - beta, di = alpha.y, dn = dr * dr + di * di;
-    scal = make_double2(dr / dn, -di / dn);
+    const double ib = 1.0 / beta;
+    tau = make_double2((beta - alpha.x) * ib, -alpha.y * ib);
+    const double dr = alpha.x - beta, di = alpha.y, idn = 1.0 / (dr * dr + di * di);
+    scal = make_double2(dr * idn, -di * idn);
   }
   if (tid == 0) { tau_s[jj] = tau; Rm[(long long)(j0 + jj) * cols + j0 + jj] = make_double2(beta, 0.0); }
   c128 g[NB];                                            // conj(tau) * (v^H y_c)
@@ -207,7 +219,7 @@ __device__ __forceinline__ void qr_panel_col(c128 (&x)[RPT][NB], c128 (*pivot)[N
 }
 
 template <int RP_THREADS, int RPT, int NB>
-__global__ void __maxnreg__(RP_THREADS == 256 ? 255 : 128) qr_panel_reg_kernel(c128 *X, int rows, int cols, int j0, int w,
+__global__ void __maxnreg__(RP_THREADS <= 256 ? 255 : 128) qr_panel_reg_kernel(c128 *X, int rows, int cols, int j0, int w,
                                                                    c128 *Rm, c128 *Tm /*[NB_MAX][NB_MAX]*/) {
   constexpr int NRED = 1 + 2 * (NB - 1);                 // s and d_c for the other columns
   constexpr int NGRAM = NB * (NB - 1);                   // re/im of the strictly upper Gram entries
@@ -227,14 +239,11 @@ __global__ void __maxnreg__(RP_THREADS == 256 ? 255 : 128) qr_panel_reg_kernel(c
     for (int c = 0; c < NB; c++)
       x[r][c] = (i < len && c < w) ? X[(long long)(j0 + c) * rows + j0 + i] : make_double2(0.0, 0.0);
   }
-  for (int e = tid; e < w * j0; e += RP_THREADS) {        // R entries above the panel rows are final
-    int c = e / j0, i = e % j0;
-    Rm[(long long)i * cols + j0 + c] = X[(long long)(j0 + c) * rows + i];
-  }
-  for (int e = tid; e < w * cols; e += RP_THREADS) {      // zeros below the diagonal of R
-    int c = e / cols, i = e % cols;
-    if (i > j0 + c) Rm[(long long)i * cols + j0 + c] = make_double2(0.0, 0.0);
-  }
+  for (int i = tid; i < j0; i += RP_THREADS)              // R entries above the panel rows are final
+    for (int c = 0; c < w; c++) Rm[(long long)i * cols + j0 + c] = X[(long long)(j0 + c) * rows + i];
+  for (int i = j0 + 1 + tid; i < cols; i += RP_THREADS)   // zeros below the diagonal of R
+    for (int c = 0; c < w; c++)
+      if (i > j0 + c) Rm[(long long)i * cols + j0 + c] = make_double2(0.0, 0.0);
   // columns one by one; every finished reflector is written to X by the step itself
   for (int jj = 0; jj < w; jj++) qr_panel_col<RP_THREADS, RPT, NB>(x, pivot, sm, tau_s, Rm, X, rows, cols, j0, len, tid, jj);
   // read the reflector block back (own writes: same thread, same addresses) for the Gram matrix
@@ -666,7 +675,11 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
     int j0 = pz * nb, w = cols - j0 < nb ? cols - j0 : nb;
     size_t smem = (size_t)w * (rows - j0) * 16;
     c128 *Tp = Tm + (size_t)pz * NB_MAX * NB_MAX;
-    if (mode == 1) TDVP_LAUNCH((qr_panel_reg_kernel<256, 5, 8>), 1, 256, 0, st, X, rows, cols, j0, w, Rm, Tp);
+    const int plen = rows - j0;                            // the panel only lives on rows >= j0
+    if (mode == 1 && plen <= 128) TDVP_LAUNCH((qr_panel_reg_kernel<128, 1, 8>), 1, 128, 0, st, X, rows, cols, j0, w, Rm, Tp);
+    else if (mode == 1 && plen <= 256) TDVP_LAUNCH((qr_panel_reg_kernel<256, 1, 8>), 1, 256, 0, st, X, rows, cols, j0, w, Rm, Tp);
+    else if (mode == 1 && plen <= 512) TDVP_LAUNCH((qr_panel_reg_kernel<256, 2, 8>), 1, 256, 0, st, X, rows, cols, j0, w, Rm, Tp);
+    else if (mode == 1) TDVP_LAUNCH((qr_panel_reg_kernel<256, 5, 8>), 1, 256, 0, st, X, rows, cols, j0, w, Rm, Tp);
     else if (mode == 2) TDVP_LAUNCH((qr_panel_reg_kernel<512, 5, 4>), 1, 512, 0, st, X, rows, cols, j0, w, Rm, Tp);
     else if (mode == 3) TDVP_LAUNCH((qr_panel_reg_kernel<512, 10, 2>), 1, 512, 0, st, X, rows, cols, j0, w, Rm, Tp);
     else TDVP_LAUNCH(qr_panel_kernel, 1, PANEL_THREADS, smem, st, X, rows, cols, j0, w, Rm, Tp);

@@ -140,6 +140,137 @@ svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/)
   }
 }
 
+// Block variant for n <= 128: the same rotations, but the cluster barrier is paid once per BLOCK pair
+// instead of once per column pair.  Columns are grouped into 16 blocks of bw = ceil(n / 16); a sweep
+// is (i) all pairs inside a block (CTA c takes blocks 2c, 2c + 1) and (ii) a round-robin tournament
+// of the 16 blocks, 15 outer rounds of 8 block pairs, one per CTA: the CTA copies its two blocks of X
+// and J into shared memory, orthogonalises every column of one against every column of the other in
+// bw inner rounds (one pair per warp, __syncthreads between), and writes them back.  127 cluster
+// barriers per sweep become 16.  Same pair set per sweep, fixed order: deterministic.
+constexpr int JB = 16;              // column blocks
+
+template <int NPL>
+__device__ __forceinline__ bool jacobi_pair_smem(c128 *xp, c128 *xq, c128 *jp, c128 *jq, int n, int lane, double tol2) {
+  c128 xu[NPL], xv[NPL], ju[NPL], jv[NPL];
+  double a = 0.0, b = 0.0, cr = 0.0, ci = 0.0;
+#pragma unroll
+  for (int r = 0; r < NPL; r++) {
+    const int i = lane + 32 * r;
+    const bool ok = i < n;
+    xu[r] = ok ? xp[i] : make_double2(0.0, 0.0);
+    xv[r] = ok ? xq[i] : make_double2(0.0, 0.0);
+    ju[r] = ok ? jp[i] : make_double2(0.0, 0.0);
+    jv[r] = ok ? jq[i] : make_double2(0.0, 0.0);
+    const c128 u = xu[r], v = xv[r];
+    a += u.x * u.x + u.y * u.y;
+    b += v.x * v.x + v.y * v.y;
+    cr += u.x * v.x + u.y * v.y;                                 // conj(u) * v
+    ci += u.x * v.y - u.y * v.x;
+  }
+  a = wsum(a); b = wsum(b); cr = wsum(cr); ci = wsum(ci);
+  const double c2 = cr * cr + ci * ci;
+  if (!(c2 > tol2 * a * b) || c2 == 0.0) return false;
+  // the scalar chain is the critical path of a round: reciprocal square roots instead of sqrt + divide
+  const double icabs = rsqrt(c2);
+  const double er = cr * icabs, ei = -ci * icabs;                // e^{-i phi}
+  const double zeta = 0.5 * (b - a) * icabs;
+  const double t = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+  const double cs = rsqrt(1.0 + t * t), sn = cs * t;
+  auto rot = [&](c128 u, c128 v, c128 &o1, c128 &o2) {
+    const c128 y = make_double2(er * v.x - ei * v.y, er * v.y + ei * v.x);
+    o1 = make_double2(cs * u.x - sn * y.x, cs * u.y - sn * y.y);
+    o2 = make_double2(sn * u.x + cs * y.x, sn * u.y + cs * y.y);
+  };
+#pragma unroll
+  for (int r = 0; r < NPL; r++) {
+    const int i = lane + 32 * r;
+    if (i < n) {
+      c128 o1, o2;
+      rot(xu[r], xv[r], o1, o2); xp[i] = o1; xq[i] = o2;
+      rot(ju[r], jv[r], o1, o2); jp[i] = o1; jq[i] = o2;
+    }
+  }
+  return true;
+}
+
+template <int NPL>
+__global__ void __cluster_dims__(JC, 1, 1) __launch_bounds__(JW * 32)
+svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/) {
+  cg::cluster_group cluster = cg::this_cluster();
+  extern __shared__ __align__(16) unsigned char jsm[];
+  const int bw = (n + JB - 1) / JB;                       // columns per block (<= 8 for n <= 128)
+  c128 *Xs = reinterpret_cast<c128 *>(jsm);               // [2 bw][n]
+  c128 *Js = Xs + (size_t)2 * bw * n;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int cta = blockIdx.x;                             // one cluster: rank == blockIdx.x
+  const double tol = 2.220446049250313e-16 * sqrt((double)n);
+  const double tol2 = tol * tol;
+  auto load_blocks = [&](int bp, int bq) {
+    for (int e = tid; e < 2 * bw * n; e += JW * 32) {
+      const int lc = e / n, i = e - lc * n;
+      const int g = (lc < bw ? bp * bw + lc : bq * bw + (lc - bw));
+      if (g < n) { Xs[e] = __ldcg(Xt + (size_t)g * n + i); Js[e] = __ldcg(Jt + (size_t)g * n + i); }
+    }
+    __syncthreads();
+  };
+  auto store_blocks = [&](int bp, int bq) {
+    __syncthreads();
+    for (int e = tid; e < 2 * bw * n; e += JW * 32) {
+      const int lc = e / n, i = e - lc * n;
+      const int g = (lc < bw ? bp * bw + lc : bq * bw + (lc - bw));
+      if (g < n) { Xt[(size_t)g * n + i] = Xs[e]; Jt[(size_t)g * n + i] = Js[e]; }
+    }
+  };
+  const int bwp = (bw + 1) & ~1;                          // players of the in-block tournament
+  for (int sweep = 0; sweep < MAX_SWEEPS; sweep++) {
+    bool any = false;
+    // (i) pairs inside blocks 2 cta and 2 cta + 1: warps 0-3 take the first block, 4-7 the second
+    {
+      const int b0 = 2 * cta, b1 = 2 * cta + 1;
+      load_blocks(b0, b1);
+      for (int round = 0; round < bwp - 1; round++) {
+        const int half = warp >> 2, k = warp & 3;
+        if (k < bwp / 2) {
+          int p, q;
+          if (k == 0) { p = round; q = bwp - 1; }
+          else { p = (round + k) % (bwp - 1); q = (round - k + (bwp - 1)) % (bwp - 1); }
+          if (p > q) { const int t = p; p = q; q = t; }
+          const int base = half ? b1 * bw : b0 * bw;
+          if (q < bw && base + q < n) {
+            const int lp = half * bw + p, lq = half * bw + q;
+            any |= jacobi_pair_smem<NPL>(Xs + (size_t)lp * n, Xs + (size_t)lq * n, Js + (size_t)lp * n, Js + (size_t)lq * n, n, lane, tol2);
+          }
+        }
+        __syncthreads();
+      }
+      store_blocks(b0, b1);
+      cluster.sync();
+    }
+    // (ii) tournament of the blocks: CTA k plays block pair k of the round
+    for (int round = 0; round < JB - 1; round++) {
+      int bp, bq;
+      if (cta == 0) { bp = round; bq = JB - 1; }
+      else { bp = (round + cta) % (JB - 1); bq = (round - cta + (JB - 1)) % (JB - 1); }
+      if (bp > bq) { const int t = bp; bp = bq; bq = t; }
+      if (bq * bw < n) {                                   // both blocks hold real columns
+        load_blocks(bp, bq);
+        for (int r = 0; r < bw; r++) {
+          if (warp < bw) {
+            const int lp = warp, lq = bw + (warp + r) % bw;
+            if (bp * bw + lp < n && bq * bw + (lq - bw) < n)
+              any |= jacobi_pair_smem<NPL>(Xs + (size_t)lp * n, Xs + (size_t)lq * n, Js + (size_t)lp * n, Js + (size_t)lq * n, n, lane, tol2);
+          }
+          __syncthreads();
+        }
+        store_blocks(bp, bq);
+      }
+      if (round == JB - 2 && any && lane == 0) flags[sweep] = 1;   // benign race: every writer stores 1
+      cluster.sync();
+    }
+    if (__ldcg(flags + sweep) == 0) break;                          // nobody rotated in this sweep
+  }
+}
+
 // lam (descending), U and the permuted J from X = U' R' (Qp = U'^T, Dp = R'^T as qr_gauge side 1 returns them).
 // U[i][k] = Qp[r][i] * sgn(Dp[r][r]),  JtP[k][j] = Jt[r][j]   with k = rank of r.
 __global__ void svd_finish_kernel(const c128 *Qp, const c128 *Dp, const c128 *Jt, int n, c128 *U, double *lam,
@@ -173,6 +304,13 @@ __global__ void svd_finish_kernel(const c128 *Qp, const c128 *Dp, const c128 *Jt
 
 }  // namespace
 
+void svd_configure() {
+  const int bytes = 4 * 8 * 128 * (int)sizeof(c128);     // X and J of two blocks at n = 128
+  cudaFuncSetAttribute(svd_jacobi_block_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  cudaFuncSetAttribute(svd_jacobi_block_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  cudaFuncSetAttribute(svd_jacobi_block_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
 size_t svd_ws_bytes(int Ml, int d, int Mr) {
   const size_t n = Ml, nn = up256(n * n * 16);
   size_t q1 = qr_ws_bytes(d * Mr, Ml), q2 = qr_ws_bytes(Ml, Ml);
@@ -198,9 +336,11 @@ void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, do
   const int g = (n * n + 255) / 256 > 296 ? 296 : (n * n + 255) / 256;
   TDVP_LAUNCH(svd_init_kernel, g, 256, 0, st, D, Xt, Jt, n);
   cudaMemsetAsync(flags, 0, MAX_SWEEPS * sizeof(int), st);
-  if (n <= 32) TDVP_LAUNCH(svd_jacobi_kernel<1>, JC, JW * 32, 0, st, Xt, Jt, n, flags);
-  else if (n <= 64) TDVP_LAUNCH(svd_jacobi_kernel<2>, JC, JW * 32, 0, st, Xt, Jt, n, flags);
-  else if (n <= 128) TDVP_LAUNCH(svd_jacobi_kernel<4>, JC, JW * 32, 0, st, Xt, Jt, n, flags);
+  const size_t bsm = (size_t)4 * ((n + JB - 1) / JB) * n * sizeof(c128);      // X and J of two blocks
+  if (n <= 16) TDVP_LAUNCH(svd_jacobi_kernel<1>, JC, JW * 32, 0, st, Xt, Jt, n, flags);
+  else if (n <= 32) TDVP_LAUNCH(svd_jacobi_block_kernel<1>, JC, JW * 32, bsm, st, Xt, Jt, n, flags);
+  else if (n <= 64) TDVP_LAUNCH(svd_jacobi_block_kernel<2>, JC, JW * 32, bsm, st, Xt, Jt, n, flags);
+  else if (n <= 128) TDVP_LAUNCH(svd_jacobi_block_kernel<4>, JC, JW * 32, bsm, st, Xt, Jt, n, flags);
   else TDVP_LAUNCH(svd_jacobi_kernel<0>, JC, JW * 32, 0, st, Xt, Jt, n, flags);
   // X = U' R'  <=>  Xt = R'^T U'^T: "side 1" factorisation of the n x n matrix Xt (d = 1)
   qr_gauge(st, 1, n, 1, n, Xt, Qp, Dp, qws);
