@@ -40,6 +40,7 @@ struct tdvp_handle {
   std::vector<c128 *> mu_k[7];     // Dormand-Prince stage derivatives
   std::vector<c128 *> mu_y;        // stage states
   double *mu_err_dev = nullptr;
+  bool mu_fsal = false;            // mu_k[6] holds the right-hand side at the CURRENT state (first-same-as-last)
   void *mu_scratch = nullptr;      // U, Lambda, V^dagger, centre forms ... of one derivative evaluation
   StepGraph ps_graph, mu_graph;
 };

@@ -171,6 +171,7 @@ int tdvp_get_mps(tdvp_handle *h, int site, tdvp_c128 *out_host, int *Ml, int *Mr
 }
 
 int tdvp_set_mps(tdvp_handle *h, const tdvp_c128 *const *mps_host, int centre) {
+  if (h) h->mu_fsal = false;
   if (!h || h->n < 1) return set_err(h, TDVP_EINVAL, "handle has no chain");
   if (!mps_host) return set_err(h, TDVP_EINVAL, "null pointer");
   if (centre != 0 && centre != h->n - 1) return set_err(h, TDVP_EINVAL, "centre must be 0 or N-1");

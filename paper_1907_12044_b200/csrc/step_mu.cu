@@ -12,6 +12,9 @@
 #include <algorithm>
 #include <cmath>
 
+#include <cstdlib>
+#include <utility>
+
 #include "handle.cuh"
 
 int move_gauge(tdvp_handle *h, int centre);
@@ -169,7 +172,12 @@ const double DP_B4[7] = {5179.0 / 57600, 0.0, 7571.0 / 16695, 393.0 / 640, -9209
 int enqueue_mu_step(tdvp_handle *h, double dt) {
   cudaStream_t st = h->stream;
   const int n = h->n;
-  for (int sidx = 0; sidx < 7; sidx++) {
+  // first-same-as-last: stage 7 of the previous step was evaluated at what is now the state, so its
+  // right-hand side is stage 1 of this step (any call that changes the tensors clears the flag)
+  const bool fsal = h->mu_fsal && !getenv("TDVP_NO_FSAL");
+  if (fsal) std::swap(h->mu_k[0], h->mu_k[6]);
+  h->mu_fsal = false;
+  for (int sidx = fsal ? 1 : 0; sidx < 7; sidx++) {
     const std::vector<c128 *> *Y = &h->A;
     if (sidx > 0) {
       for (int i = 0; i < n; i++) {
@@ -196,7 +204,9 @@ int enqueue_mu_step(tdvp_handle *h, double dt) {
     TDVP_LAUNCH(lincomb_kernel, grid_for(site_elems(h, i)), VT, 0, st, h->A[i], (const c128 *)h->A[i], cb, site_elems(h, i));
   }
   TDVP_LAUNCH(err_final_kernel, 1, 1, 0, st, h->mu_err_dev + 1, n, h->mu_err_dev);
-  return check_cuda(h, cudaGetLastError(), "tdvp_step_mu");
+  if (int rc = check_cuda(h, cudaGetLastError(), "tdvp_step_mu")) return rc;
+  h->mu_fsal = true;
+  return TDVP_OK;
 }
 
 int prepare_mu(tdvp_handle *h) {

@@ -115,6 +115,7 @@ extern "C" {
 
 int tdvp_step_ps(tdvp_handle *h, double dt) {
   if (!h || h->n < 1) return set_err(h, TDVP_EINVAL, "handle has no chain");
+  h->mu_fsal = false;
   if (h->centre != 0) {
     if (int rc = move_gauge(h, 0)) return rc;
   }
@@ -160,6 +161,7 @@ int tdvp_get_centre(tdvp_handle *h) {
 
 // QR / RQ sweep without time evolution (Eq. 9); rebuilds the environments the sweep passes.
 int move_gauge(tdvp_handle *h, int centre) {
+  h->mu_fsal = false;
   cudaStream_t st = h->stream;
   while (h->centre < centre) {
     const int i = h->centre;

@@ -393,6 +393,27 @@ def test_mu_step_matches_oracle_and_ps(T):
     ch.close()
 
 
+def test_mu_first_same_as_last_is_exact(T):
+    """Dormand-Prince's stage 7 is evaluated at the new state, so the library reuses it as stage 1 of
+    the next step; TDVP_NO_FSAL=1 (read at every step) recomputes it: both must give the same bits."""
+    cfg, mpo, mpsL = _warm_left_canonical()
+    from oracle import tdvp_mu
+    res = []
+    for no_fsal in (False, True):
+        ch = T.tdvp_create(mpo, tdvp_mu.to_right_canonical(mpsL))
+        ch.tdvp_set_mps(mpsL, centre=ch.n - 1)
+        if no_fsal:
+            os.environ["TDVP_NO_FSAL"] = "1"
+        try:
+            errs = [ch.tdvp_step_mu(0.1, want_err=True) for _ in range(3)]
+        finally:
+            os.environ.pop("TDVP_NO_FSAL", None)
+        res.append((errs, ch.tdvp_populations(0)))
+        ch.close()
+    assert res[0][0] == res[1][0]
+    assert np.array_equal(res[0][1], res[1][1])
+
+
 def test_mu_step_from_ps_gauge(T):
     """tdvp_step_mu on a handle in the PS gauge first moves the centre (no time evolution)."""
     cfg, mpo, st = _tiny_state(3)
