@@ -173,7 +173,8 @@ int enqueue_mu_step(tdvp_handle *h, double dt) {
   cudaStream_t st = h->stream;
   const int n = h->n;
   // first-same-as-last: stage 7 of the previous step was evaluated at what is now the state, so its
-  // right-hand side is stage 1 of this step (any call that changes the tensors clears the flag)
+  // right-hand side is stage 1 of this step (any call that changes the tensors clears the flag;
+  // TDVP_NO_FSAL=1, read at every step, recomputes it -- the exactness test toggles it)
   const bool fsal = h->mu_fsal && !getenv("TDVP_NO_FSAL");
   if (fsal) std::swap(h->mu_k[0], h->mu_k[6]);
   h->mu_fsal = false;

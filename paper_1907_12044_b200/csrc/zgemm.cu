@@ -433,7 +433,7 @@ int choose_grid(long long units, int ktiles) {
   for (int g = 1; g <= gmax; g++) {
     const long long upc = (units + g - 1) / g;
     const bool split = (units % g != 0) || (upc % ktiles != 0);
-    const double cost = (double)upc * (g > g_sms ? 2.0 : 1.1) + (split ? 4.0 : 0.0) - 1e-6 * g;
+    const double cost = (double)upc * (g > g_sms ? 2.0 : 1.1) + (split ? 5.0 : 0.0) - 1e-6 * g;
     if (cost < best) { best = cost; best_g = g; }
   }
   return best_g;
