@@ -449,6 +449,26 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_ps_only(args):
+    """One direct-enqueue (no graph) TDVP-PS step of the configs[3] chain between cudaProfilerStart/Stop,
+    after one warm-up step: the target of `ncu --profile-from-start off` for the per-kernel launch list
+    of a step (profiles/).  Prints the step's wall time; not a bench value."""
+    import torch
+    import paper_1907_12044_b200 as T
+    cfg, mpo, mps = build_chain("fmo128")
+    ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=cfg.krylov_dim, flags=T.TDVP_FLAG_NO_GRAPH))
+    ch.tdvp_step_ps(cfg.dt_fs)
+    ch.tdvp_sync()
+    torch.cuda.cudart().cudaProfilerStart()
+    t0 = time.perf_counter()
+    ch.tdvp_step_ps(cfg.dt_fs)
+    ch.tdvp_sync()
+    el = time.perf_counter() - t0
+    torch.cuda.cudart().cudaProfilerStop()
+    print(json.dumps({"ps_step_only_ms": 1e3 * el, "launches": None, "note": "direct enqueue, one step, for profiling"}))
+    ch.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -457,9 +477,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the M sweep, the PS step and the CPU baseline")
     ap.add_argument("--large", action="store_true", help="also time the M=256, 147-site chain (about a minute more)")
+    ap.add_argument("--ps-step-only", action="store_true", help="one un-graphed TDVP-PS step between cudaProfilerStart/Stop (for ncu)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
-    if args.impl == "reference":
+    if args.ps_step_only:
+        run_ps_only(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
