@@ -130,6 +130,25 @@ def test_apply_bond(T, dims):
     assert rel(got, oc.bond(L, D, R)) <= REL_TOL
 
 
+def test_contractions_random_shapes(T):
+    """Seeded random shapes: many different stream-K schedules of the GEMM kernel (uncut, cut once,
+    cut many times, batched right-environment stage, ragged k-tiles) and W-stage panel shapes."""
+    rng = np.random.default_rng(20240611)
+    for _ in range(24):
+        Ml, Mr, Dw = int(rng.integers(1, 200)), int(rng.integers(1, 200)), int(rng.integers(1, 7))
+        L = si.complex_normal(rng, (Ml, Dw, Ml))
+        R = si.complex_normal(rng, (Mr, Dw, Mr))
+        D = si.complex_normal(rng, (Ml, Mr))
+        assert rel(host(T.tdvp_apply_bond(dev(L), dev(D), dev(R))), oc.bond(L, D, R)) <= REL_TOL, (Ml, Mr, Dw)
+    for k in range(10):
+        Ml, Mr = int(rng.integers(1, 90)), int(rng.integers(1, 90))
+        d, Dl, Dr = int(rng.integers(1, 6)), int(rng.integers(1, 8)), int(rng.integers(1, 8))
+        L, W, A, R = si.random_site_problem(Ml, Mr, d, Dl, Dr, 0.3, seed=900 + k)
+        assert rel(host(T.tdvp_apply_heff(dev(L), dev(W), dev(A), dev(R))), oc.heff(L, W, A, R)) <= REL_TOL, (Ml, Mr, d, Dl, Dr)
+        assert rel(host(T.tdvp_update_env(0, dev(L), dev(W), dev(A))), oc.envL(L, W, A)) <= REL_TOL, (Ml, Mr, d, Dl, Dr)
+        assert rel(host(T.tdvp_update_env(1, dev(R), dev(W), dev(A))), oc.envR(R, W, A)) <= REL_TOL, (Ml, Mr, d, Dl, Dr)
+
+
 # ---- QR gauge move (Eq. 9) ------------------------------------------------------------------
 # the last four shapes reach the panel variants for tall sides of 1280 / 2560 / 5120 rows and beyond
 @pytest.mark.parametrize("shape", [(1, 3, 3), (3, 4, 12), (16, 4, 16), (37, 5, 29), (64, 10, 64), (130, 3, 70),
