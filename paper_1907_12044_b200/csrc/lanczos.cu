@@ -12,7 +12,6 @@
 #include <cstdlib>
 
 #include "common.cuh"
-#include "tridiag.cuh"
 
 namespace cg = cooperative_groups;
 
@@ -275,18 +274,74 @@ __global__ void __launch_bounds__(FT) lz_fused_orth_kernel(long long n, int chun
     for (int e = tid; e < len; e += FT) { c128 x = sw[e]; wg[e] = make_double2(x.x * inv_beta, x.y * inv_beta); }
 }
 
-// One warp: coef = beta0 * V exp(z Lambda) V^T e_1 for the m x m tridiagonal (alpha, beta).
-__global__ void lz_coef_kernel(int k, double zr, double zi, LzBuffers b, int *m_out) {
+// One warp: coef = beta0 * V exp(z Lambda) V^T e_1 for the m x m tridiagonal (alpha, beta)
+// ("diagonalize the tridiagonal matrix in the subspace").  Implicit symmetric QR
+// iteration with Wilkinson shift and deflation (Golub & Van Loan, "Matrix Computations", sec. 8.3).
+// The scalar recurrence of a sweep is a dependent FP64 chain: lane 0 alone runs it on shared-memory
+// copies of the diagonals and records the sweep's rotations; then every lane applies them to the
+// eigenvector rows it owns.  (All 32 lanes used to repeat the chain on local-memory arrays: 66 us.)
+__global__ void __launch_bounds__(32) lz_coef_kernel(int k, double zr, double zi, LzBuffers b, int *m_out) {
   __shared__ double V[TDVP_MAX_KRYLOV * TDVP_MAX_KRYLOV];
-  double a[TDVP_MAX_KRYLOV], off[TDVP_MAX_KRYLOV];
+  __shared__ double a[TDVP_MAX_KRYLOV], off[TDVP_MAX_KRYLOV], rc[TDVP_MAX_KRYLOV], rs[TDVP_MAX_KRYLOV];
+  __shared__ int s_lo, s_hi;
   const int lane = threadIdx.x;
   const int m = b.state->m;
   if (lane == 0 && m_out) *m_out = m;
-  for (int i = 0; i < m; i++) { a[i] = b.alpha[i]; off[i] = (i < m - 1) ? b.beta[i] : 0.0; }
+  for (int i = lane; i < m; i += 32) { a[i] = b.alpha[i]; off[i] = (i < m - 1) ? b.beta[i] : 0.0; }
   for (int r = lane; r < m; r += 32)
     for (int c = 0; c < m; c++) V[r * m + c] = (r == c) ? 1.0 : 0.0;
-  tridiag_qr_eig(m, a, off, V, m, lane, 32);
   __syncwarp();
+  const double eps = 2.220446049250313e-16;
+  int hi = m - 1, guard = 0;
+  while (true) {
+    if (lane == 0) {
+      int lo = -1;
+      while (hi > 0 && guard < 64 * m) {
+        guard++;
+        for (int i = 0; i < hi; i++)
+          if (fabs(off[i]) <= eps * (fabs(a[i]) + fabs(a[i + 1]))) off[i] = 0.0;
+        if (off[hi - 1] == 0.0) { hi--; continue; }
+        lo = hi - 1;
+        while (lo > 0 && off[lo - 1] != 0.0) lo--;
+        break;
+      }
+      if (hi > 0 && guard < 64 * m && lo >= 0) {
+        // Wilkinson shift from the trailing 2x2 of the unreduced block [lo, hi]
+        const double dd = 0.5 * (a[hi - 1] - a[hi]), bb = off[hi - 1];
+        const double den = dd + (dd >= 0.0 ? 1.0 : -1.0) * sqrt(dd * dd + bb * bb);
+        const double mu = a[hi] - bb * bb / den;
+        double x = a[lo] - mu, z = off[lo];
+        for (int q = lo; q < hi; q++) {
+          // the chain sqrt -> two divisions is the latency of the sweep: one reciprocal square root instead
+          const double r2 = x * x + z * z;
+          double c = 1.0, sn = 0.0, r = 0.0;
+          if (r2 > 0.0) { const double ri = rsqrt(r2); c = x * ri; sn = z * ri; r = r2 * ri; }
+          if (q > lo) off[q - 1] = r;
+          const double ak = a[q], ak1 = a[q + 1], bk = off[q];
+          a[q] = c * c * ak + 2.0 * c * sn * bk + sn * sn * ak1;
+          a[q + 1] = sn * sn * ak - 2.0 * c * sn * bk + c * c * ak1;
+          off[q] = c * sn * (ak1 - ak) + (c * c - sn * sn) * bk;
+          x = off[q];
+          if (q < hi - 1) { z = sn * off[q + 1]; off[q + 1] = c * off[q + 1]; }
+          rc[q] = c; rs[q] = sn;
+        }
+        s_lo = lo; s_hi = hi;
+      } else {
+        s_lo = 0; s_hi = 0;                              // converged (or the guard tripped)
+      }
+    }
+    __syncwarp();
+    const int lo = s_lo, h2 = s_hi;
+    if (h2 == 0) break;
+    for (int row = lane; row < m; row += 32)
+      for (int q = lo; q < h2; q++) {
+        const double c = rc[q], sn = rs[q];
+        const double vk = V[row * m + q], vk1 = V[row * m + q + 1];
+        V[row * m + q] = c * vk + sn * vk1;
+        V[row * m + q + 1] = -sn * vk + c * vk1;
+      }
+    __syncwarp();
+  }
   const double beta0 = b.state->beta0;
   for (int r = lane; r < k; r += 32) {
     double cx = 0.0, cy = 0.0;
