@@ -220,11 +220,19 @@ __global__ void __launch_bounds__(FT) lz_fused_orth_kernel(long long n, int chun
   const int len = (int)((e0 + chunk <= n) ? chunk : (n > e0 ? n - e0 : 0));
   const int was_done = b.state->done;                             // read before anybody can change it
   c128 *wg = b.Q + (long long)(j + 1) * n + e0;
-  for (int e = tid; e < len; e += FT) sw[e] = wg[e];
+  // all loads of the chunk in flight at once (16 B asynchronous copies), one wait
+  for (int e = tid; e < len; e += FT) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(sw + e);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(wg + e));
+  }
   for (int i = 0; i < nd; i++) {
     const c128 *qg = b.Q + (long long)i * n + e0;
-    for (int e = tid; e < len; e += FT) sq[(size_t)i * chunk + e] = qg[e];
+    for (int e = tid; e < len; e += FT) {
+      const unsigned sa = (unsigned)__cvta_generic_to_shared(sq + (size_t)i * chunk + e);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(qg + e));
+    }
   }
+  asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
   __syncthreads();
   for (int pass = 0; pass < 2; pass++) {
     c128 *partial = b.partial + (size_t)pass * MAXG * (TDVP_MAX_KRYLOV + 1);
