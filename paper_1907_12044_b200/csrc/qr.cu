@@ -157,13 +157,13 @@ __device__ __forceinline__ void qr_panel_col(c128 (&x)[RPT][NB], c128 (*pivot)[N
     const int i = tid + r * RP_THREADS;
     if (i >= jj && i < len) {
       const c128 u = x[r][0];
-      red[0] += u.x * u.x + u.y * u.y;
+      red[0] = fma(u.x, u.x, fma(u.y, u.y, red[0]));     // explicit FMA chains: the step is FP64-issue bound
       if (i == jj) pivot[jj & 1][0] = u;
 #pragma unroll
       for (int c = 1; c < NB; c++) {
         const c128 yv = x[r][c];
-        red[1 + 2 * (c - 1)] += u.x * yv.x + u.y * yv.y;
-        red[2 + 2 * (c - 1)] += u.x * yv.y - u.y * yv.x;
+        red[1 + 2 * (c - 1)] = fma(u.x, yv.x, fma(u.y, yv.y, red[1 + 2 * (c - 1)]));
+        red[2 + 2 * (c - 1)] = fma(u.x, yv.y, fma(-u.y, yv.x, red[2 + 2 * (c - 1)]));
         if (i == jj) pivot[jj & 1][c] = yv;
       }
     }
@@ -207,8 +207,8 @@ __device__ __forceinline__ void qr_panel_col(c128 (&x)[RPT][NB], c128 (*pivot)[N
         Xc[i] = v;
 #pragma unroll
         for (int c = 1; c < NB; c++) {
-          const c128 t = cmul(g[c], v);
-          x[r][c].x -= t.x; x[r][c].y -= t.y;
+          x[r][c].x = fma(g[c].y, v.y, fma(-g[c].x, v.x, x[r][c].x));
+          x[r][c].y = fma(-g[c].y, v.x, fma(-g[c].x, v.y, x[r][c].y));
         }
       }
     }
@@ -269,8 +269,8 @@ __global__ void __maxnreg__(RP_THREADS <= 256 ? 255 : 128) qr_panel_reg_kernel(c
 #pragma unroll
         for (int b = a + 1; b < NB; b++) {
           const c128 v = x[r][b];
-          gr[q] += u.x * v.x + u.y * v.y;
-          gr[q + 1] += u.x * v.y - u.y * v.x;
+          gr[q] = fma(u.x, v.x, fma(u.y, v.y, gr[q]));
+          gr[q + 1] = fma(u.x, v.y, fma(-u.y, v.x, gr[q + 1]));
           q += 2;
         }
       }
@@ -569,8 +569,8 @@ __global__ void __launch_bounds__(AT) qr_apply1_kernel(const c128 *__restrict__ 
     for (int r = 0; r < RA; r++)
 #pragma unroll
       for (int q = 0; q < NBW; q++) {
-        acc[2 * q] += v[r][q].x * y[r].x + v[r][q].y * y[r].y;
-        acc[2 * q + 1] += v[r][q].x * y[r].y - v[r][q].y * y[r].x;
+        acc[2 * q] = fma(v[r][q].x, y[r].x, fma(v[r][q].y, y[r].y, acc[2 * q]));
+        acc[2 * q + 1] = fma(v[r][q].x, y[r].y, fma(-v[r][q].y, y[r].x, acc[2 * q + 1]));
       }
 #pragma unroll
     for (int q = 0; q < 2 * NBW; q++) {
@@ -601,7 +601,10 @@ __global__ void __launch_bounds__(AT) qr_apply1_kernel(const c128 *__restrict__ 
 #pragma unroll
     for (int r = 0; r < RA; r++)
 #pragma unroll
-      for (int q = 0; q < NBW; q++) { const c128 t = cmul(v[r][q], sv[q]); y[r].x -= t.x; y[r].y -= t.y; }
+      for (int q = 0; q < NBW; q++) {
+        y[r].x = fma(v[r][q].y, sv[q].y, fma(-v[r][q].x, sv[q].x, y[r].x));
+        y[r].y = fma(-v[r][q].y, sv[q].x, fma(-v[r][q].x, sv[q].y, y[r].y));
+      }
     __syncthreads();                                     // sm / Tsm are reused by the next panel
   }
 #pragma unroll
