@@ -205,6 +205,17 @@ int tdvp_probe_fp64_tensor_peak(int iters, double *tflops /*HOST*/);
    non-tensor instructions of a DMMA loop cost.  Blocks; TDVP_EINVAL on other
    filler counts. */
 int tdvp_probe_dmma_issue(int fillers, int iters, double *tflops /*HOST*/);
+/* How the complex128 GEMM stages (the M_S^3 M_O d terms of Table I,
+   PAPER.md:375-388) split the complex product into real FP64 tensor-core products (north_star:
+   "complex product split into real MMAs"; reading c15):
+     products = 3 (default): X1 = Ar Br, X2 = Ai Bi, X3 = (Ar + Ai)(Br + Bi); C = (X1 - X2) + i (X3 - X1 - X2)
+                 -- 25 % fewer DMMAs; error bounded normwise (relative to |A||B|), not per component;
+     products = 4: Cr = Ar Br - Ai Bi, Ci = Ar Bi + Ai Br.
+   Process-wide (every handle and stream), takes effect at the next launch; not to be changed while
+   a captured step graph exists (the graph keeps the kernels it was captured with).  The
+   environment variable TDVP_ZGEMM_4M=1 selects 4 at load time.  Returns 0, or TDVP_EINVAL. */
+int tdvp_set_gemm_products(int products);
+int tdvp_get_gemm_products(void);
 /* Phase profiler: when enabled, launches of the dominant kernel classes are bracketed by CUDA events
    on the launching stream (not inside a captured step).  tdvp_profile_read blocks on the device,
    returns the summed elapsed milliseconds and bracket counts per phase since the last read and

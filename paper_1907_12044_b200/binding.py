@@ -31,7 +31,7 @@ EXPORTED_SYMBOLS = [
     "tdvp_qr_gauge", "tdvp_svd_bond", "tdvp_apply_heff_host", "tdvp_apply_heff_site", "tdvp_update_env_site",
     "tdvp_step_ps", "tdvp_step_mu", "tdvp_mu_derivative", "tdvp_set_gauge", "tdvp_observe", "tdvp_populations",
     "tdvp_norm_energy", "tdvp_get_mps", "tdvp_set_mps", "tdvp_get_centre", "tdvp_sync",
-    "tdvp_last_error", "tdvp_probe_fp64_tensor_peak", "tdvp_probe_dmma_issue", "tdvp_launch_count", "tdvp_profile_enable",
+    "tdvp_last_error", "tdvp_probe_fp64_tensor_peak", "tdvp_probe_dmma_issue", "tdvp_set_gemm_products", "tdvp_get_gemm_products", "tdvp_launch_count", "tdvp_profile_enable",
     "tdvp_profile_read",
 ]
 
@@ -86,6 +86,8 @@ def _load():
         "tdvp_probe_fp64_tensor_peak": (c_int, [c_int, POINTER(c_double)]),
         "tdvp_probe_dmma_issue": (c_int, [c_int, c_int, POINTER(c_double)]),
         "tdvp_launch_count": (c_longlong, []),
+        "tdvp_set_gemm_products": (c_int, [c_int]),
+        "tdvp_get_gemm_products": (c_int, []),
         "tdvp_profile_enable": (c_int, [c_int]),
         "tdvp_profile_read": (c_int, [POINTER(c_double), POINTER(c_longlong)]),
     }
@@ -282,6 +284,15 @@ def tdvp_profile_read():
     cnt = (c_longlong * len(PROFILE_PHASES))()
     _check(_lib.tdvp_profile_read(ms, cnt))
     return {name: (ms[i], int(cnt[i])) for i, name in enumerate(PROFILE_PHASES)}
+
+
+def tdvp_set_gemm_products(products: int) -> None:
+    """3 (default) or 4 real DMMA products per complex product in the GEMM stages (include/tdvp.h)."""
+    _check(_lib.tdvp_set_gemm_products(int(products)))
+
+
+def tdvp_get_gemm_products() -> int:
+    return int(_lib.tdvp_get_gemm_products())
 
 
 def tdvp_launch_count() -> int:

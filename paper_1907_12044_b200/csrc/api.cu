@@ -381,6 +381,13 @@ int tdvp_probe_dmma_issue(int fillers, int iters, double *tflops) {
   return TDVP_OK;
 }
 
+int tdvp_set_gemm_products(int products) {
+  if (products != 3 && products != 4) return TDVP_EINVAL;
+  zgemm_set_mode(products);
+  return 0;
+}
+int tdvp_get_gemm_products(void) { return zgemm_get_mode(); }
+
 int tdvp_probe_fp64_tensor_peak(int iters, double *tflops) { return tdvp_probe_dmma_issue(0, iters, tflops); }
 
 }  // extern "C"

@@ -79,6 +79,8 @@ struct ZGemm {
 size_t zgemm_ws_elems(const ZGemm &p);
 void zgemm(cudaStream_t st, const ZGemm &p, c128 *ws);
 void zgemm_prepare_stream(cudaStream_t st);
+void zgemm_set_mode(int products);   // 3 or 4 real DMMA products per complex product
+int zgemm_get_mode();
 void zgemm_alias_stream(cudaStream_t alias, cudaStream_t of);
 void zgemm_forget_stream(cudaStream_t alias);
 

@@ -116,7 +116,7 @@ __device__ __forceinline__ int cta_of_unit(int u, int base, int rem) {
   return u < cut ? u / (base + 1) : rem + (u - cut) / base;
 }
 
-template <bool A_KMAJOR, bool B_KMAJOR, bool CONJ>
+template <bool A_KMAJOR, bool B_KMAJOR, bool CONJ, bool M3>
 __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constant__ CUtensorMap tmA,
                                                             const __grid_constant__ CUtensorMap tmB, KParams p) {
   extern __shared__ __align__(128) unsigned char smem_dyn[];
@@ -193,11 +193,24 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
     for (int s = 0; s < LOOKAHEAD && s < nkt; s++) issue(s);
   }
 
-  double cr[4][4][2], ci[4][4][2];
+  // 4M: cr = sum ar br - ai bi, ci = sum ar bi + ai br.
+  // 3M: cr = sum ar br, ci = sum ai bi, cs = sum (ar + ai)(br + bi); the tile is cr - ci and
+  //     cs - cr - ci, formed once per segment (fin()).
+  double cr[4][4][2], ci[4][4][2], cs[M3 ? 4 : 1][M3 ? 4 : 1][2];
 #pragma unroll
   for (int i = 0; i < 4; i++)
 #pragma unroll
-    for (int j = 0; j < 4; j++) { cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0; }
+    for (int j = 0; j < 4; j++) {
+      cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+      if (M3) cs[M3 ? i : 0][M3 ? j : 0][0] = cs[M3 ? i : 0][M3 ? j : 0][1] = 0.0;
+    }
+  auto fin = [&](int i, int j, int h) -> c128 {
+    if (M3) {
+      const double x1 = cr[i][j][h], x2 = ci[i][j][h];
+      return make_double2(x1 - x2, cs[M3 ? i : 0][M3 ? j : 0][h] - x1 - x2);
+    }
+    return make_double2(cr[i][j][h], ci[i][j][h]);
+  };
 
   const int lr = lane >> 2, lk = lane & 3;
   const unsigned na_sign = p.a_sign ^ 0x80000000u;
@@ -214,6 +227,37 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
     const c128 *b = reinterpret_cast<const c128 *>(smem_gen + slot * (2 * TILE_BYTES) + TILE_BYTES);
 #pragma unroll
     for (int ks = 0; ks < KG; ks++) {
+      if (M3) {
+        double ar[4], ai[4], as[4], br[4], bi[4], bs[4];
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+          c128 v = B_KMAJOR ? b[(ks * BN + wn0 + j * 8 + lr) * 4 + lk]
+                            : b[(ks * 4 + lk) * LDM + wn0 + j * 8 + lr];
+          br[j] = v.x;
+          bi[j] = CONJ ? flip(v.y, p.b_sign) : v.y;
+          bs[j] = br[j] + bi[j];
+        }
+#pragma unroll
+        for (int i = 0; i < 4; i++) {
+          c128 v = A_KMAJOR ? a[(ks * BM + wm0 + i * 8 + lr) * 4 + lk]
+                            : a[(ks * 4 + lk) * LDM + wm0 + i * 8 + lr];
+          ar[i] = v.x;
+          ai[i] = CONJ ? flip(v.y, p.a_sign) : v.y;
+          as[i] = ar[i] + ai[i];
+        }
+        if (ks == KG - 1) {            // all operands of this slot are in registers: hand it back
+          __syncwarp();
+          if (lane == 0) mbar_arrive(empty0 + 8 * slot);
+        }
+#pragma unroll
+        for (int i = 0; i < 4; i++)
+#pragma unroll
+          for (int j = 0; j < 4; j++) {
+            dmma(cr[i][j][0], cr[i][j][1], ar[i], br[j]);
+            dmma(ci[i][j][0], ci[i][j][1], ai[i], bi[j]);
+            dmma(cs[M3 ? i : 0][M3 ? j : 0][0], cs[M3 ? i : 0][M3 ? j : 0][1], as[i], bs[j]);
+          }
+      } else {
       double ar[4], ai[4], nai[4], br[4], bi[4];
 #pragma unroll
       for (int i = 0; i < 4; i++) {
@@ -248,6 +292,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
           dmma(cr[i][j][0], cr[i][j][1], nai[i], bi[j]);
           dmma(ci[i][j][0], ci[i][j][1], ai[i], br[j]);
         }
+      }
     }
     // ---- end of a segment? ----
     const bool whole = it >= lenFL;
@@ -266,8 +311,8 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
         for (int j = 0; j < 4; j++) {
           int n = n0 + wn0 + j * 8 + 2 * lk;
           c128 *dst = Cb + (long long)m * p.ldc + n;
-          if (n < p.N) dst[0] = make_double2(cr[i][j][0], ci[i][j][0]);
-          if (n + 1 < p.N) dst[1] = make_double2(cr[i][j][1], ci[i][j][1]);
+          if (n < p.N) dst[0] = fin(i, j, 0);
+          if (n + 1 < p.N) dst[1] = fin(i, j, 1);
         }
       }
     } else {
@@ -278,8 +323,8 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
       for (int i = 0; i < 4; i++)
 #pragma unroll
         for (int j = 0; j < 4; j++) {
-          __stcg(sl + ((i * 4 + j) * 2 + 0) * NTHREADS + tid, make_double2(cr[i][j][0], ci[i][j][0]));
-          __stcg(sl + ((i * 4 + j) * 2 + 1) * NTHREADS + tid, make_double2(cr[i][j][1], ci[i][j][1]));
+          __stcg(sl + ((i * 4 + j) * 2 + 0) * NTHREADS + tid, fin(i, j, 0));
+          __stcg(sl + ((i * 4 + j) * 2 + 1) * NTHREADS + tid, fin(i, j, 1));
         }
       __syncthreads();               // all stores of the CTA are ordered before thread 0's release
       if (tid == 0) {
@@ -291,7 +336,10 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
 #pragma unroll
     for (int i = 0; i < 4; i++)
 #pragma unroll
-      for (int j = 0; j < 4; j++) { cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0; }
+      for (int j = 0; j < 4; j++) {
+        cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+        if (M3) cs[M3 ? i : 0][M3 ? j : 0][0] = cs[M3 ? i : 0][M3 ? j : 0][1] = 0.0;
+      }
     c_kt = 0;
     if (it + 1 == lenF && lenL) c_tile = tL;
     else if (it + 1 == lenFL) c_tile = tM0;
@@ -340,8 +388,12 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
   }
 }
 
-template <bool AK, bool BK_, bool CJ>
-void launch1(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, const KParams &kp) {
+// Complex product as three real DMMA products per k-step (default) or four (TDVP_ZGEMM_4M=1 in the
+// environment, or zgemm_set_mode(4)): see DESIGN.md 5, reading c15.
+int g_mode3m = 1;
+
+template <bool AK, bool BK_, bool CJ, bool M3>
+void launch2(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, const KParams &kp) {
   // cooperative: the CTAs of a cut tile wait for one another in the fix-up, so all must be resident
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(kp.G); cfg.blockDim = dim3(NTHREADS); cfg.dynamicSmemBytes = SMEM_BYTES; cfg.stream = st;
@@ -350,8 +402,13 @@ void launch1(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, cons
   // no tile is cut when the ranges are whole tiles: nobody waits for anybody, a plain launch will do
   const bool cut = kp.upc_rem != 0 || (kp.upc_base % kp.ktiles) != 0;
   cfg.attrs = attr; cfg.numAttrs = cut ? 1 : 0;
-  cudaLaunchKernelEx(&cfg, zgemm_kernel<AK, BK_, CJ>, ta, tb, kp);
+  cudaLaunchKernelEx(&cfg, zgemm_kernel<AK, BK_, CJ, M3>, ta, tb, kp);
   count_launch();
+}
+template <bool AK, bool BK_, bool CJ>
+void launch1(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, const KParams &kp) {
+  if (g_mode3m) launch2<AK, BK_, CJ, true>(st, ta, tb, kp);
+  else launch2<AK, BK_, CJ, false>(st, ta, tb, kp);
 }
 template <bool AK, bool BK_>
 void launch(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, const KParams &kp) {
@@ -360,8 +417,10 @@ void launch(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, const
 }
 template <bool AK, bool BK_>
 void set_smem_attr() {
-  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda).
@@ -446,7 +505,12 @@ void zgemm_configure() {
   int dev = 0, per_sm = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, zgemm_kernel<true, true, true>, NTHREADS, SMEM_BYTES);
+  int per_sm4 = 0;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, zgemm_kernel<true, true, true, true>, NTHREADS, SMEM_BYTES);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm4, zgemm_kernel<true, true, true, false>, NTHREADS, SMEM_BYTES);
+  if (per_sm4 < per_sm) per_sm = per_sm4;
+  const char *e4 = getenv("TDVP_ZGEMM_4M");
+  if (e4 && e4[0] == '1') g_mode3m = 0;
   if (per_sm < 1) per_sm = 1;
   if (per_sm > 2) per_sm = 2;
   if (g_sms < 1) g_sms = 1;
@@ -457,6 +521,9 @@ void zgemm_configure() {
       q == cudaDriverEntryPointSuccess)
     g_encode = reinterpret_cast<EncodeTiledFn>(fn);
 }
+
+void zgemm_set_mode(int products) { configure_kernels_once(); g_mode3m = products == 4 ? 0 : 1; }
+int zgemm_get_mode() { configure_kernels_once(); return g_mode3m ? 3 : 4; }
 
 void zgemm_prepare_stream(cudaStream_t st) { configure_kernels_once(); get_ctx(st, true); }
 
