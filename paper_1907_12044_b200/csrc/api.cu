@@ -141,6 +141,30 @@ static int bad_dims(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr) {
   return 0;
 }
 
+namespace {
+// second queue + events of a handle (host-entry copies; sparse build of W beside stage 1)
+int ensure_side_queue(tdvp_handle *h, tdvp_handle *hh) {
+  if (hh->copy_stream) return 0;
+  if (int rc = check_cuda(h, cudaStreamCreateWithFlags(&hh->copy_stream, cudaStreamNonBlocking), "copy stream")) return rc;
+  cudaEventCreateWithFlags(&hh->ev_first, cudaEventDisableTiming);
+  cudaEventCreateWithFlags(&hh->ev_w, cudaEventDisableTiming);
+  cudaEventCreateWithFlags(&hh->ev_r, cudaEventDisableTiming);
+  for (int i = 0; i < 4; i++) cudaEventCreateWithFlags(&hh->ev_l[i], cudaEventDisableTiming);
+  return 0;
+}
+// The stateless calls get a dense W and must build its sparse form first; that build does not depend
+// on stage 1, so it runs on the side queue (fork after the arena's previous users, join before the
+// W stage) and its ~8 us latency disappears behind the first GEMM.
+int build_w_beside(tdvp_handle *h, tdvp_handle *hh, WSparse &wsp, void *wmem, int Dl, int d, int Dr, const c128 *W) {
+  if (int rc = ensure_side_queue(h, hh)) return rc;
+  cudaEventRecord(hh->ev_first, hh->stream);
+  cudaStreamWaitEvent(hh->copy_stream, hh->ev_first, 0);
+  wsparse_build(hh->copy_stream, wsp, wmem, Dl, d, Dr, W, hh->opt.w_zero_tol);
+  cudaEventRecord(hh->ev_w, hh->copy_stream);
+  return 0;
+}
+}  // namespace
+
 int tdvp_apply_heff(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr, const tdvp_c128 *L,
                     const tdvp_c128 *W, const tdvp_c128 *A, const tdvp_c128 *R, tdvp_c128 *out) {
   tdvp_handle *hh = h ? h : default_handle();
@@ -152,10 +176,10 @@ int tdvp_apply_heff(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr, const
   void *wmem = hh->arena.take(wb);
   void *ws = hh->arena.take(hb);
   WSparse wsp;
-  wsparse_build(hh->stream, wsp, wmem, Dl, d, Dr, reinterpret_cast<const c128 *>(W), hh->opt.w_zero_tol);
+  if (int rc = build_w_beside(h, hh, wsp, wmem, Dl, d, Dr, reinterpret_cast<const c128 *>(W))) return rc;
   heff_apply(hh->stream, Ml, Mr, d, Dl, Dr, reinterpret_cast<const c128 *>(L), wsp,
              reinterpret_cast<const c128 *>(A), reinterpret_cast<const c128 *>(R),
-             reinterpret_cast<c128 *>(out), ws);
+             reinterpret_cast<c128 *>(out), ws, hh->ev_w);
   return check_cuda(h, cudaGetLastError(), "tdvp_apply_heff");
 }
 
@@ -177,13 +201,7 @@ int tdvp_apply_heff_host(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr, 
   void *wmem = hh->arena.take(wb);
   void *ws = hh->arena.take(hb);
   cudaStream_t st = hh->stream;
-  if (!hh->copy_stream) {
-    if (int rc = check_cuda(h, cudaStreamCreateWithFlags(&hh->copy_stream, cudaStreamNonBlocking), "copy stream")) return rc;
-    cudaEventCreateWithFlags(&hh->ev_first, cudaEventDisableTiming);
-    cudaEventCreateWithFlags(&hh->ev_w, cudaEventDisableTiming);
-    cudaEventCreateWithFlags(&hh->ev_r, cudaEventDisableTiming);
-    for (int i = 0; i < 4; i++) cudaEventCreateWithFlags(&hh->ev_l[i], cudaEventDisableTiming);
-  }
+  if (int rc = ensure_side_queue(h, hh)) return rc;
   // all H2D copies go to the copy queue in the order the stages need them -- A, L in slices of the
   // bond index, W, R -- and the compute stream waits for each piece by event, so stage 1 starts
   // after A and the first slice of L and the W stage / stage 3 never wait if the link keeps up
@@ -222,9 +240,9 @@ int tdvp_update_env(tdvp_handle *h, int side, int Ml, int Mr, int d, int Dl, int
   void *wmem = hh->arena.take(wb);
   void *ws = hh->arena.take(eb);
   WSparse wsp;
-  wsparse_build(hh->stream, wsp, wmem, Dl, d, Dr, reinterpret_cast<const c128 *>(W), hh->opt.w_zero_tol);
+  if (int rc = build_w_beside(h, hh, wsp, wmem, Dl, d, Dr, reinterpret_cast<const c128 *>(W))) return rc;
   env_update(hh->stream, side, Ml, Mr, d, Dl, Dr, reinterpret_cast<const c128 *>(env_in), wsp,
-             reinterpret_cast<const c128 *>(A), reinterpret_cast<c128 *>(env_out), ws);
+             reinterpret_cast<const c128 *>(A), reinterpret_cast<c128 *>(env_out), ws, hh->ev_w);
   return check_cuda(h, cudaGetLastError(), "tdvp_update_env");
 }
 

@@ -124,7 +124,8 @@ struct Arena {
 // contract.cu : the local contractions on explicit device pointers.
 size_t heff_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr);
 void heff_apply(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c128 *L,
-                const WSparse &W, const c128 *A, const c128 *R, c128 *out, void *ws);
+                const WSparse &W, const c128 *A, const c128 *R, c128 *out, void *ws,
+                cudaEvent_t w_ready = nullptr);   // if set: the W stage waits for it (W built on a side queue)
 // The same for the host-entry path, whose inputs are still arriving on a copy queue: stage 1 runs in
 // nsl slices of the bond index a, slice s after ev_l[s] (A and rows [s*Ml/nsl, (s+1)*Ml/nsl) of L
 // have landed); the sparse form of W is built after ev_w, stage 3 waits for ev_r (R).
@@ -133,7 +134,7 @@ void heff_apply_staged(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, c
                        int nsl, const cudaEvent_t *ev_l, cudaEvent_t ev_w, cudaEvent_t ev_r);
 size_t env_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr);
 void env_update(cudaStream_t st, int side, int Ml, int Mr, int d, int Dl, int Dr,
-                const c128 *env_in, const WSparse &W, const c128 *A, c128 *env_out, void *ws);
+                const c128 *env_in, const WSparse &W, const c128 *A, c128 *env_out, void *ws, cudaEvent_t w_ready = nullptr);
 size_t bond_ws_bytes(int Ml, int Mr, int Dw);
 void bond_apply(cudaStream_t st, int Ml, int Mr, int Dw, const c128 *L, const c128 *D,
                 const c128 *R, c128 *out, void *ws);

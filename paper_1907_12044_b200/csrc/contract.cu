@@ -85,13 +85,14 @@ size_t heff_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr) {
 }
 
 void heff_apply(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c128 *L,
-                const WSparse &W, const c128 *A, const c128 *R, c128 *out, void *ws) {
+                const WSparse &W, const c128 *A, const c128 *R, c128 *out, void *ws, cudaEvent_t w_ready) {
   size_t t1 = (size_t)Ml * Dl * d * Mr, t2 = (size_t)Ml * d * Dr * Mr;
   char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
   c128 *T1 = reinterpret_cast<c128 *>(p); p += up256(t1 * 16);
   c128 *T2 = reinterpret_cast<c128 *>(p); p += up256(t2 * 16);
   c128 *sk = reinterpret_cast<c128 *>(p);
   zgemm(st, g_stage1_left(Ml, Mr, d, Dl, L, A, T1), sk);
+  if (w_ready) cudaStreamWaitEvent(st, w_ready, 0);
   wstage_left(st, W, Ml, Mr, T1, T2);
   zgemm(st, g_stage3_heff(Ml, Mr, d, Dr, T2, R, out), sk);
 }
@@ -132,7 +133,7 @@ size_t env_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr) {
 }
 
 void env_update(cudaStream_t st, int side, int Ml, int Mr, int d, int Dl, int Dr,
-                const c128 *env_in, const WSparse &W, const c128 *A, c128 *env_out, void *ws) {
+                const c128 *env_in, const WSparse &W, const c128 *A, c128 *env_out, void *ws, cudaEvent_t w_ready) {
   size_t t1 = (size_t)Ml * Dl * d * Mr, t2 = (size_t)Ml * d * Dr * Mr;
   size_t big = t1 > t2 ? t1 : t2;
   char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
@@ -141,10 +142,12 @@ void env_update(cudaStream_t st, int side, int Ml, int Mr, int d, int Dl, int Dr
   c128 *sk = reinterpret_cast<c128 *>(p);
   if (side == 0) {
     zgemm(st, g_stage1_left(Ml, Mr, d, Dl, env_in, A, T1), sk);
+    if (w_ready) cudaStreamWaitEvent(st, w_ready, 0);
     wstage_left(st, W, Ml, Mr, T1, T2);
     zgemm(st, g_stage3_envL(Ml, Mr, d, Dr, A, T2, env_out), sk);
   } else {
     zgemm(st, g_stage1_right(Ml, Mr, d, Dr, A, env_in, T1), sk);
+    if (w_ready) cudaStreamWaitEvent(st, w_ready, 0);
     wstage_right(st, W, Ml, Mr, T1, T2);
     zgemm(st, g_stage3_envR(Ml, Mr, d, Dl, A, T2, env_out), sk);
   }

@@ -59,7 +59,7 @@ __device__ __forceinline__ void cfma(double &sx, double &sy, c128 w, c128 t) {
   sy = fma(w.x, t.y, sy); sy = fma(w.y, t.x, sy);
 }
 
-// Persistent kernel: one CTA of 32 warps per SM walks over work items (a, tile of 64 y, row split).
+// Persistent kernel: one CTA of 32 warps per SM walks over its contiguous range of (panel, row) units.
 // The panel T1[a, :, y0:y0+64] is staged in shared memory by 16 B cp.async copies; each warp then
 // produces output rows, every lane owning TWO y (l and l + 32), so that the warp-uniform loads of an
 // entry's value and column are amortised over two panel loads (the kernel is bound by shared-memory
@@ -69,14 +69,20 @@ __device__ __forceinline__ void cfma(double &sx, double &sy, c128 w, c128 t) {
 // L1/L2 with the next four prefetched into registers.  Entry batches are padded with zero weights,
 // so the inner loop has no tail.
 constexpr int WP_THREADS = 1024;
-constexpr int WP_SMEM = 227 * 1024;
+constexpr int WP_SMEM = 227 * 1024 - 64;   // dynamic part; the row counter is static
 
 template <bool CSR_SMEM>
 __device__ __forceinline__ void wp_rows(const WStageParams &p, const c128 *tile, const c128 *__restrict__ vals,
                                         const int *__restrict__ cols, const int *rbeg, const int *rend, c128 *out,
-                                        int y0, int lane, int warp, int split, int nsplit) {
+                                        int y0, int lane, int r1, int *next_row) {
   const c128 zero = make_double2(0.0, 0.0);
-  for (int r = split + nsplit * warp; r < p.nrows; r += nsplit * (WP_THREADS / 32)) {
+  for (;;) {
+    // rows are handed out one at a time (they differ in length): the warps of the CTA stay busy
+    // until the segment is used up
+    int r = 0;
+    if (lane == 0) r = atomicAdd(next_row, 1);
+    r = __shfl_sync(0xffffffffu, r, 0);
+    if (r >= r1) break;
     const int e0 = rbeg[r], e1 = rend[r];
     double ax = 0.0, ay = 0.0, bx = 0.0, by = 0.0;     // y0 + lane ; y0 + 32 + lane
     int c[4]; c128 w[4];
@@ -108,8 +114,9 @@ __device__ __forceinline__ void wp_rows(const WStageParams &p, const c128 *tile,
   }
 }
 
-__global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStageParams p, int ntile, int nitems, int nsplit) {
+__global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStageParams p, int ntile, int npanels) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ int s_next_row;
   c128 *tile = reinterpret_cast<c128 *>(smem_raw);                        // [ncols][YT]
   const int tile_elems = p.ncols * YT;
   int *rbeg = reinterpret_cast<int *>(smem_raw + (size_t)tile_elems * 16);   // [nrows]
@@ -150,11 +157,19 @@ __global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStage
       rbeg[r] = r * p.ncols; rend[r] = r * p.ncols + n;
     }
   }
-  for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-    const int split = item % nsplit, panel = item / nsplit;
+  // Work = (panel, row) units in panel-major order, cut into gridDim.x equal contiguous ranges: a CTA
+  // stages at most (its share of panels + 2) panels, each once, whatever the row count.
+  const long long units = (long long)npanels * p.nrows;
+  long long u = units * blockIdx.x / gridDim.x;
+  const long long u_end = units * (blockIdx.x + 1) / gridDim.x;
+  while (u < u_end) {
+    const int panel = (int)(u / p.nrows), r0 = (int)(u - (long long)panel * p.nrows);
+    const int r1 = (u_end - u) < (long long)(p.nrows - r0) ? r0 + (int)(u_end - u) : p.nrows;
+    u += r1 - r0;
     const int a = panel / ntile, y0 = (panel % ntile) * YT;
     const c128 *in = p.in + a * p.in_bs;
-    __syncthreads();                                   // previous item's readers are done with the panel
+    __syncthreads();                                   // previous segment's readers are done with the panel
+    if (threadIdx.x == 0) s_next_row = r0;
     for (int e = threadIdx.x; e < tile_elems; e += WP_THREADS) {
       const int c = e / YT, yy = e % YT;
       const bool ok = (y0 + yy) < p.Mr;
@@ -167,9 +182,9 @@ __global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStage
     __syncthreads();
     c128 *out = p.out + a * p.o_bs;
     if (csr_smem) {
-      wp_rows<true>(p, tile, sval, scol, rbeg, rend, out, y0, lane, warp, split, nsplit);
+      wp_rows<true>(p, tile, sval, scol, rbeg, rend, out, y0, lane, r1, &s_next_row);
     } else {
-      wp_rows<false>(p, tile, p.val, p.col, rbeg, rend, out, y0, lane, warp, split, nsplit);
+      wp_rows<false>(p, tile, p.val, p.col, rbeg, rend, out, y0, lane, r1, &s_next_row);
     }
   }
 }
@@ -198,17 +213,13 @@ void launch_wstage(cudaStream_t st, const WStageParams &p, int nbatch) {
   ProfScope ps(st, PH_WSTAGE);
   if (panel <= (size_t)WP_SMEM) {
     if (!g_num_sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev); }
-    // split the rows of a panel over several work items when the panels alone balance badly
-    int nsplit = 1;
-    while (nsplit < 8 && p.nrows >= 64 * nsplit) {
-      const long long it = (long long)nbatch * ntile * nsplit;
-      const long long rounds = (it + g_num_sms - 1) / g_num_sms;
-      if (it >= g_num_sms && (double)it / (double)(rounds * g_num_sms) > 0.93) break;
-      nsplit *= 2;
-    }
-    const int nitems = nbatch * ntile * nsplit;
-    const int grid = nitems < g_num_sms ? nitems : g_num_sms;
-    TDVP_LAUNCH(wstage_persistent_kernel, grid, WP_THREADS, WP_SMEM, st, p, ntile, nitems, nsplit);
+    // one CTA per SM when there is enough work; never more CTAs than 32-row chunks or panels
+    const long long npanels = (long long)nbatch * ntile, units = npanels * p.nrows;
+    long long want = (units + 31) / 32;
+    if (want < npanels) want = npanels;
+    if (want > units) want = units;
+    const int grid = want < g_num_sms ? (int)(want < 1 ? 1 : want) : g_num_sms;
+    TDVP_LAUNCH(wstage_persistent_kernel, grid, WP_THREADS, WP_SMEM, st, p, ntile, (int)npanels);
     return;
   }
   dim3 grid((p.Mr + 31) / 32, nbatch, (p.nrows + 7) / 8 < 8 ? (p.nrows + 7) / 8 : 8);
