@@ -74,14 +74,19 @@ constexpr int WP_SMEM = 227 * 1024 - 64;   // dynamic part; the row counter is s
 template <bool CSR_SMEM>
 __device__ __forceinline__ void wp_rows(const WStageParams &p, const c128 *tile, const c128 *__restrict__ vals,
                                         const int *__restrict__ cols, const int *rbeg, const int *rend, c128 *out,
-                                        int y0, int lane, int r1, int *next_row) {
+                                        int y0, int lane, int r0, int r1, int *next_row) {
   const c128 zero = make_double2(0.0, 0.0);
+  int rs = r0 + (threadIdx.x >> 5) - WP_THREADS / 32;
   for (;;) {
-    // rows are handed out one at a time (they differ in length): the warps of the CTA stay busy
-    // until the segment is used up
+    // long rows (they differ in length) are handed out one at a time, so that the warps of the CTA
+    // stay busy until the segment is used up; short rows (real MPOs: ~2 entries) go round-robin
     int r = 0;
-    if (lane == 0) r = atomicAdd(next_row, 1);
-    r = __shfl_sync(0xffffffffu, r, 0);
+    if (next_row) {
+      if (lane == 0) r = atomicAdd(next_row, 1);
+      r = __shfl_sync(0xffffffffu, r, 0);
+    } else {
+      r = (rs += WP_THREADS / 32);
+    }
     if (r >= r1) break;
     const int e0 = rbeg[r], e1 = rend[r];
     double ax = 0.0, ay = 0.0, bx = 0.0, by = 0.0;     // y0 + lane ; y0 + 32 + lane
@@ -142,6 +147,7 @@ __global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStage
   const int nnz = rend[p.nrows - 1];
   const bool csr_smem = csr_off + (size_t)nnz * 20 + 16 <= (size_t)WP_SMEM;
   int *scol = reinterpret_cast<int *>(sval + nnz);
+  const bool dyn = nnz >= 8 * p.nrows;
   __syncthreads();
   if (csr_smem) {
     for (int r = warp; r < p.nrows; r += WP_THREADS / 32) {
@@ -161,7 +167,11 @@ __global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStage
   // stages at most (its share of panels + 2) panels, each once, whatever the row count.
   const long long units = (long long)npanels * p.nrows;
   long long u = units * blockIdx.x / gridDim.x;
-  const long long u_end = units * (blockIdx.x + 1) / gridDim.x;
+  long long u_end = units * (blockIdx.x + 1) / gridDim.x;
+  if (!dyn) {   // short rows: staging a panel costs as much as its rows, so ranges are whole panels
+    u = ((long long)npanels * blockIdx.x / gridDim.x) * p.nrows;
+    u_end = ((long long)npanels * (blockIdx.x + 1) / gridDim.x) * p.nrows;
+  }
   while (u < u_end) {
     const int panel = (int)(u / p.nrows), r0 = (int)(u - (long long)panel * p.nrows);
     const int r1 = (u_end - u) < (long long)(p.nrows - r0) ? r0 + (int)(u_end - u) : p.nrows;
@@ -182,9 +192,9 @@ __global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStage
     __syncthreads();
     c128 *out = p.out + a * p.o_bs;
     if (csr_smem) {
-      wp_rows<true>(p, tile, sval, scol, rbeg, rend, out, y0, lane, r1, &s_next_row);
+      wp_rows<true>(p, tile, sval, scol, rbeg, rend, out, y0, lane, r0, r1, dyn ? &s_next_row : nullptr);
     } else {
-      wp_rows<false>(p, tile, p.val, p.col, rbeg, rend, out, y0, lane, r1, &s_next_row);
+      wp_rows<false>(p, tile, p.val, p.col, rbeg, rend, out, y0, lane, r0, r1, dyn ? &s_next_row : nullptr);
     }
   }
 }

@@ -504,6 +504,7 @@ StreamCtx *get_ctx(cudaStream_t st, bool create) {
 // one k-tile on an SM of its own.  Two CTAs sharing an SM take twice as long per unit (one CTA
 // alone reaches ~90 % of the pipe); cutting tiles costs the publish + slice reduction, measured at
 // about 8 us = four units whatever the depth of the cut.
+double g_split_cost = 5.0;
 int choose_grid(long long units, int ktiles) {
   int best_g = 1;
   double best = 1e300;
@@ -511,7 +512,7 @@ int choose_grid(long long units, int ktiles) {
   for (int g = 1; g <= gmax; g++) {
     const long long upc = (units + g - 1) / g;
     const bool split = (units % g != 0) || (upc % ktiles != 0);
-    const double cost = (double)upc * (g > g_sms ? 2.0 : 1.1) + (split ? 5.0 : 0.0) - 1e-6 * g;
+    const double cost = (double)upc * (g > g_sms ? 2.0 : 1.1) + (split ? g_split_cost : 0.0) - 1e-6 * g;
     if (cost < best) { best = cost; best_g = g; }
   }
   return best_g;
@@ -528,6 +529,7 @@ void zgemm_configure() {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, zgemm_kernel<true, true, true, true>, NTHREADS, SMEM_BYTES);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm4, zgemm_kernel<true, true, true, false>, NTHREADS, SMEM_BYTES);
   if (per_sm4 < per_sm) per_sm = per_sm4;
+  if (const char *es = getenv("TDVP_ZGEMM_SPLIT_COST")) g_split_cost = atof(es);
   const char *e4 = getenv("TDVP_ZGEMM_4M");
   if (e4 && e4[0] == '1') g_mode3m = 0;
   if (per_sm < 1) per_sm = 1;
