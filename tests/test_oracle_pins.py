@@ -254,3 +254,45 @@ def test_p6_mu_agrees_with_ps(warmed_up):
         y, err = tdvp_mu.step_mu(mpo, y, 0.25)
     assert np.abs(obs.populations(y) - obs.populations(st.mps)).max() < 1e-8
     assert err < 1e-3
+
+
+# ---------------------------------------------------------------- p12, p13: TDVP-MU with CMF integration
+def test_p12_cmf_local_rhs_is_the_mu_derivative(warmed_up):
+    """With the mean fields taken at the state itself, the constant-mean-field right-hand side of
+    every site is the (pinned: p6, p7, T4) TDVP-MU derivative of Eq. 37 -- and it obeys Eq. 34."""
+    from oracle import tdvp_cmf
+    mpo, warm = warmed_up
+    lc = tdvp_mu.to_left_canonical(warm)
+    deriv = tdvp_mu.mu_derivative(mpo, lc)
+    Lenv, Renv, U, lam = tdvp_cmf.mean_fields(mpo, lc)
+    big = 0
+    for i in range(len(lc) - 1):
+        r = tdvp_cmf.local_rhs(lc[i], Lenv[i], mpo[i], Renv[i], U[i], lam[i])
+        assert np.abs(r - deriv[i]).max() <= 1e-13 * max(1.0, np.abs(deriv[i]).max())
+        assert np.abs(np.einsum("asb,asc->bc", lc[i].conj(), r)).max() < 1e-12
+        big += np.abs(r).max() > 1e-3
+    assert big >= 3
+
+
+def test_p13_cmf_is_second_order_and_agrees_with_ps(warmed_up):
+    """PAPER.md:224 "second order CMF with a midpoint scheme"; Fig. 7 / PAPER.md:359: fitted slope
+    2.03 of the CMF error against the step size; the TDVP schemes agree once
+    the step is converged.  Reference: TDVP-PS with a converged step and Krylov dimension."""
+    from oracle import tdvp_cmf
+    mpo, warm = warmed_up
+    T = 2.0
+    ref = tdvp_ps.PSState(mpo, warm)
+    for _ in range(16):
+        tdvp_ps.step_ps(ref, T / 16, 30)
+    p_ref = obs.populations(ref.mps)
+    lc = tdvp_mu.to_left_canonical(warm)
+    errs = []
+    for tau in (0.5, 0.25, 0.125):
+        y = [a.copy() for a in lc]
+        for _ in range(int(round(T / tau))):
+            y = tdvp_cmf.step_cmf(mpo, y, tau, max(2, int(tau / 0.0625)), 20)
+        assert abs(obs.norm_sq(y) - 1.0) < 1e-10
+        errs.append(np.abs(obs.populations(y) - p_ref).max())
+    slopes = [np.log2(errs[i] / errs[i + 1]) for i in range(2)]
+    assert all(1.7 < s < 2.5 for s in slopes), (errs, slopes)
+    assert errs[-1] < 1e-5
