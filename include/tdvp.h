@@ -167,6 +167,17 @@ int tdvp_step_ps(tdvp_handle *h, double dt);
    embedded (5th - 4th order) difference. */
 int tdvp_step_mu(tdvp_handle *h, double dt, double *err_est);
 
+/* One step of length dt of TDVP-MU with constant-mean-field (CMF) integration, second-order
+   midpoint scheme (cost PAPER.md:253, Table I): the mean
+   fields -- environments h[1:i-1], h[i+1:N] and the unfolded bond U, Lambda of Eq. 36 -- are built
+   at t, every local matrix is propagated to t + dt/2 with them held constant, the mean fields
+   are rebuilt there, and every local matrix is propagated from t to t + dt with those.  Local
+   propagation (readings, DESIGN.md c19): L_i by n_sub classical Runge-Kutta (RK4) sub-steps of
+   Eq. 37/33/38 (ceil(n_sub/2) over the half step), C_N by the Lanczos exponential of Eq. 27 with
+   the handle's krylov_dim.  SVDs and environment updates therefore run twice per step whatever
+   n_sub is.  Same gauge handling as tdvp_step_mu; enqueue only.  TDVP_EINVAL if n_sub < 1. */
+int tdvp_step_mu_cmf(tdvp_handle *h, double dt, int n_sub);
+
 /* One evaluation of the TDVP-MU right-hand side (Eq. 27 and Eq. 37-38) on the resident MPS, which
    must be in the MU gauge (centre N-1; else TDVP_ESTATE).  out_host[N]: HOST pointers to HOST
    buffers [Ml_i, d_i, Mr_i] receiving dL_i/dt (i < N-1) and dC_N/dt.  Blocks on the stream. */

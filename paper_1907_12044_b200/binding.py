@@ -29,7 +29,7 @@ EXPORTED_SYMBOLS = [
     "tdvp_default_options", "tdvp_create_context", "tdvp_create", "tdvp_destroy",
     "tdvp_apply_heff", "tdvp_update_env", "tdvp_apply_bond", "tdvp_expm_heff", "tdvp_expm_bond",
     "tdvp_qr_gauge", "tdvp_svd_bond", "tdvp_apply_heff_host", "tdvp_apply_heff_site", "tdvp_update_env_site",
-    "tdvp_step_ps", "tdvp_step_mu", "tdvp_mu_derivative", "tdvp_set_gauge", "tdvp_observe", "tdvp_populations",
+    "tdvp_step_ps", "tdvp_step_mu", "tdvp_step_mu_cmf", "tdvp_mu_derivative", "tdvp_set_gauge", "tdvp_observe", "tdvp_populations",
     "tdvp_norm_energy", "tdvp_get_mps", "tdvp_set_mps", "tdvp_get_centre", "tdvp_sync",
     "tdvp_last_error", "tdvp_probe_fp64_tensor_peak", "tdvp_probe_dmma_issue", "tdvp_set_gemm_products", "tdvp_get_gemm_products", "tdvp_launch_count", "tdvp_profile_enable",
     "tdvp_profile_read",
@@ -73,6 +73,7 @@ def _load():
         "tdvp_update_env_site": (c_int, [P, c_int, c_int]),
         "tdvp_step_ps": (c_int, [P, c_double]),
         "tdvp_step_mu": (c_int, [P, c_double, POINTER(c_double)]),
+        "tdvp_step_mu_cmf": (c_int, [P, c_double, c_int]),
         "tdvp_mu_derivative": (c_int, [P, POINTER(P)]),
         "tdvp_set_gauge": (c_int, [P, c_int]),
         "tdvp_observe": (c_int, [P, c_int, P, P]),
@@ -345,6 +346,9 @@ class Chain:
         e = c_double(0.0)
         _check(_lib.tdvp_step_mu(self._h, float(dt), byref(e) if want_err else None), self._h)
         return e.value if want_err else None
+
+    def tdvp_step_mu_cmf(self, dt, n_sub):
+        _check(_lib.tdvp_step_mu_cmf(self._h, float(dt), int(n_sub)), self._h)
 
     def tdvp_mu_derivative(self):
         """Time derivatives of the resident (left-canonical) MPS, as HOST numpy arrays."""

@@ -42,6 +42,7 @@ struct tdvp_handle {
   double *mu_err_dev = nullptr;
   bool mu_fsal = false;            // mu_k[6] holds the right-hand side at the CURRENT state (first-same-as-last)
   void *mu_scratch = nullptr;      // U, Lambda, V^dagger, centre forms ... of one derivative evaluation
+  std::vector<void *> cmf_mem;     // CMF mean fields per bond b: [3b] U, [3b+1] U Lambda, [3b+2] Lambda (first use)
   StepGraph ps_graph, mu_graph;
 };
 

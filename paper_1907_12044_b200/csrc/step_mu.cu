@@ -210,6 +210,145 @@ int enqueue_mu_step(tdvp_handle *h, double dt) {
   return TDVP_OK;
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// TDVP-MU with constant-mean-field (CMF) integration, second-order midpoint scheme
+// (cost PAPER.md:253 and Table I; readings: DESIGN.md c19).
+// The mean field of site j < N-1 is (h[1:j-1], h[j+1:N] rebuilt from the R of Eq. 36, U, Lambda of
+// the bond to its right); it is held constant while L_j is integrated by classical RK4 sub-steps of
+//     i dL_j/dt = (1 - L_j L_j^dagger) H[j](L_j U Lambda) Lambda~^{-1} U^dagger       (Eq. 37, 33, 38)
+// and C_N by the Lanczos exponential of Eq. 27.  One step: mean field at t = 0 -> every local
+// matrix to tau/2 -> mean field there -> every local matrix from 0 to tau with that mean field.
+// SVDs and environment updates run twice per step, whatever the number of local sub-steps.
+struct CmfFields {                 // per bond b = 1..n-1 (between sites b-1 and b): U, U*Lambda, Lambda
+  std::vector<c128 *> U, UL;
+  std::vector<double *> lam;
+};
+
+int cmf_alloc(tdvp_handle *h) {
+  if (!h->cmf_mem.empty()) return TDVP_OK;
+  const int n = h->n;
+  h->cmf_mem.assign(3 * n, nullptr);
+  for (int b = 1; b < n; b++) {
+    const size_t m = (size_t)h->M[b];
+    if (int rc = check_cuda(h, cudaMalloc(&h->cmf_mem[3 * b], m * m * 16), "cudaMalloc CMF U")) return rc;
+    if (int rc = check_cuda(h, cudaMalloc(&h->cmf_mem[3 * b + 1], m * m * 16), "cudaMalloc CMF U Lambda")) return rc;
+    if (int rc = check_cuda(h, cudaMalloc(&h->cmf_mem[3 * b + 2], m * 8), "cudaMalloc CMF Lambda")) return rc;
+  }
+  return TDVP_OK;
+}
+
+// Mean fields of the left-canonical state Y: Lenv[i] for every site, Renv[j] / U / Lambda for j < n-1.
+int cmf_mean_fields(tdvp_handle *h, const std::vector<c128 *> &Y) {
+  cudaStream_t st = h->stream;
+  const int n = h->n;
+  MuScratch s = mu_scratch(h);
+  if (!s.U) return set_err(h, TDVP_ENOMEM, "TDVP-MU scratch allocation failed");
+  void *ws = h->step_ws;
+  for (int i = 0; i < n - 1; i++)                                                        // "Get Env"
+    env_update(st, 0, h->M[i], h->M[i + 1], h->d[i], h->Dw[i], h->Dw[i + 1], h->Lenv[i], h->Wsp[i], Y[i],
+               h->Lenv[i + 1], ws);
+  const c128 *C = Y[n - 1];
+  c128 *Cnext = s.C0;
+  for (int i = n - 1; i >= 1; i--) {
+    const int Ml = h->M[i], Mr = h->M[i + 1], d = h->d[i];
+    c128 *U = reinterpret_cast<c128 *>(h->cmf_mem[3 * i]), *UL = reinterpret_cast<c128 *>(h->cmf_mem[3 * i + 1]);
+    double *lam = reinterpret_cast<double *>(h->cmf_mem[3 * i + 2]);
+    svd_bond(st, Ml, d, Mr, C, U, lam, s.Vh, ws);                                        // Eq. 36
+    env_update(st, 1, Ml, Mr, d, h->Dw[i], h->Dw[i + 1], h->Renv[i], h->Wsp[i], s.Vh, h->Renv[i - 1], ws);
+    vec_copy(st, UL, U, (long long)Ml * Ml);
+    TDVP_LAUNCH(scale_cols_kernel, grid_for((long long)Ml * Ml), VT, 0, st, UL, (long long)Ml, Ml, lam, 0, 0.0);
+    if (i > 1) {                                           // centre form of site i-1, unfolded next
+      const int j = i - 1;
+      ZGemm g{};
+      g.A = Y[j]; g.B = UL; g.C = Cnext;
+      g.M = h->M[j] * h->d[j]; g.K = Ml; g.N = Ml; g.a_ms = Ml; g.a_ks = 1; g.b_ks = Ml; g.b_ns = 1; g.ldc = Ml;
+      gemm1(st, g);
+      C = Cnext;
+      Cnext = (Cnext == s.C0) ? s.C1 : s.C0;
+    }
+  }
+  return check_cuda(h, cudaGetLastError(), "CMF mean fields");
+}
+
+// K = dL_j/dt of Eq. 37 at the local matrix Yj, mean fields of site j held in the handle.
+void cmf_local_rhs(tdvp_handle *h, int j, const c128 *Yj, c128 *K, const MuScratch &s) {
+  cudaStream_t st = h->stream;
+  void *ws = h->step_ws;
+  const double sq = std::sqrt(h->opt.mu_eps);
+  const int Jl = h->M[j], Jr = h->M[j + 1], dj = h->d[j];
+  const long long ne = site_elems(h, j), rows = (long long)Jl * dj;
+  const c128 *U = reinterpret_cast<const c128 *>(h->cmf_mem[3 * (j + 1)]);
+  const c128 *UL = reinterpret_cast<const c128 *>(h->cmf_mem[3 * (j + 1) + 1]);
+  const double *lam = reinterpret_cast<const double *>(h->cmf_mem[3 * (j + 1) + 2]);
+  ZGemm g{};
+  g.A = Yj; g.B = UL; g.C = s.C0;                          // C[(a,s)][r] = sum_l L[(a,s)][l] (U Lambda)[l][r]
+  g.M = (int)rows; g.K = Jr; g.N = Jr; g.a_ms = Jr; g.a_ks = 1; g.b_ks = Jr; g.b_ns = 1; g.ldc = Jr;
+  gemm1(st, g);
+  heff_apply(st, Jl, Jr, dj, h->Dw[j], h->Dw[j + 1], h->Lenv[j], h->Wsp[j], s.C0, h->Renv[j], s.HC, ws);
+  TDVP_LAUNCH(scale_cols_kernel, grid_for(ne), VT, 0, st, s.HC, rows, Jr, lam, 1, sq);   // Lambda~^{-1}, Eq. 38
+  ZGemm g2{};
+  g2.A = s.HC; g2.B = U; g2.C = s.G;                       // G = HC U^dagger
+  g2.M = (int)rows; g2.K = Jr; g2.N = Jr; g2.a_ms = Jr; g2.a_ks = 1; g2.b_ns = Jr; g2.b_ks = 1; g2.conjB = 1; g2.ldc = Jr;
+  gemm1(st, g2);
+  ZGemm g3{};
+  g3.A = Yj; g3.B = s.G; g3.C = s.P;                       // P = L^dagger G
+  g3.M = Jr; g3.N = Jr; g3.K = (int)rows; g3.a_ms = 1; g3.a_ks = Jr; g3.conjA = 1; g3.b_ks = Jr; g3.b_ns = 1; g3.ldc = Jr;
+  gemm1(st, g3);
+  ZGemm g4{};
+  g4.A = Yj; g4.B = s.P; g4.C = s.T;                       // T = L P
+  g4.M = (int)rows; g4.K = Jr; g4.N = Jr; g4.a_ms = Jr; g4.a_ks = 1; g4.b_ks = Jr; g4.b_ns = 1; g4.ldc = Jr;
+  gemm1(st, g4);
+  TDVP_LAUNCH(minus_i_diff_kernel, grid_for(ne), VT, 0, st, K, s.G, s.T, ne);             // -i (1 - p) G
+}
+
+// Z[i] = every local matrix of X propagated over time t with the handle's mean fields.
+int cmf_propagate(tdvp_handle *h, const std::vector<c128 *> &X, const std::vector<c128 *> &Z, double t, int n_sub) {
+  cudaStream_t st = h->stream;
+  const int n = h->n;
+  MuScratch s = mu_scratch(h);
+  const double hs = t / n_sub;
+  for (int j = 0; j < n - 1; j++) {
+    const long long ne = site_elems(h, j);
+    c128 *y = Z[j], *ys = h->mu_y[j];
+    c128 *k1 = h->mu_k[0][j], *k2 = h->mu_k[1][j], *k3 = h->mu_k[2][j], *k4 = h->mu_k[3][j];
+    vec_copy(st, y, X[j], ne);
+    for (int q = 0; q < n_sub; q++) {                      // classical RK4
+      cmf_local_rhs(h, j, y, k1, s);
+      { Comb c{}; c.n = 1; c.k[0] = k1; c.c[0] = 0.5 * hs;
+        TDVP_LAUNCH(lincomb_kernel, grid_for(ne), VT, 0, st, ys, (const c128 *)y, c, ne); }
+      cmf_local_rhs(h, j, ys, k2, s);
+      { Comb c{}; c.n = 1; c.k[0] = k2; c.c[0] = 0.5 * hs;
+        TDVP_LAUNCH(lincomb_kernel, grid_for(ne), VT, 0, st, ys, (const c128 *)y, c, ne); }
+      cmf_local_rhs(h, j, ys, k3, s);
+      { Comb c{}; c.n = 1; c.k[0] = k3; c.c[0] = hs;
+        TDVP_LAUNCH(lincomb_kernel, grid_for(ne), VT, 0, st, ys, (const c128 *)y, c, ne); }
+      cmf_local_rhs(h, j, ys, k4, s);
+      { Comb c{}; c.n = 4; c.k[0] = k1; c.k[1] = k2; c.k[2] = k3; c.k[3] = k4;
+        c.c[0] = hs / 6.0; c.c[1] = hs / 3.0; c.c[2] = hs / 3.0; c.c[3] = hs / 6.0;
+        TDVP_LAUNCH(lincomb_kernel, grid_for(ne), VT, 0, st, y, (const c128 *)y, c, ne); }
+    }
+  }
+  {                                                        // Eq. 27 by the Krylov exponential
+    const int i = n - 1;
+    LanczosOp op{};
+    op.kind = 0; op.Ml = h->M[i]; op.Mr = h->M[i + 1]; op.d = h->d[i]; op.Dl = h->Dw[i]; op.Dr = h->Dw[i + 1];
+    op.L = h->Lenv[i]; op.R = h->Renv[i]; op.W = &h->Wsp[i];
+    lanczos_expm(st, op, h->opt.krylov_dim, 0.0, -t, X[i], Z[i], h->step_ws, nullptr);
+  }
+  return check_cuda(h, cudaGetLastError(), "CMF local propagation");
+}
+
+int enqueue_cmf_step(tdvp_handle *h, double dt, int n_sub) {
+  h->mu_fsal = false;
+  if (int rc = cmf_mean_fields(h, h->A)) return rc;
+  if (int rc = cmf_propagate(h, h->A, h->mu_k[4], 0.5 * dt, (n_sub + 1) / 2)) return rc;
+  if (int rc = cmf_mean_fields(h, h->mu_k[4])) return rc;
+  if (int rc = cmf_propagate(h, h->A, h->mu_k[5], dt, n_sub)) return rc;
+  for (int i = 0; i < h->n; i++) vec_copy(h->stream, h->A[i], h->mu_k[5][i], site_elems(h, i));
+  return check_cuda(h, cudaGetLastError(), "tdvp_step_mu_cmf");
+}
+
 int prepare_mu(tdvp_handle *h) {
   if (!h || h->n < 1) return set_err(h, TDVP_EINVAL, "handle has no chain");
   if (h->n < 2) return set_err(h, TDVP_EINVAL, "TDVP-MU needs at least two sites");
@@ -232,6 +371,16 @@ int tdvp_step_mu(tdvp_handle *h, double dt, double *err_est) {
     return check_cuda(h, cudaStreamSynchronize(h->stream), "tdvp_step_mu sync");
   }
   return TDVP_OK;
+}
+
+int tdvp_step_mu_cmf(tdvp_handle *h, double dt, int n_sub) {
+  if (int rc = prepare_mu(h)) return rc;
+  if (n_sub < 1) return set_err(h, TDVP_EINVAL, "n_sub must be >= 1");
+  if (int rc = cmf_alloc(h)) return rc;
+  if (h->centre != h->n - 1) {
+    if (int rc = move_gauge(h, h->n - 1)) return rc;
+  }
+  return enqueue_cmf_step(h, dt, n_sub);
 }
 
 int tdvp_mu_derivative(tdvp_handle *h, tdvp_c128 *const *out_host) {
