@@ -286,12 +286,18 @@ def run_ours(args):
     ws_ms, ws_n = prof["wstage"]
     flops_per_launch = gemm_stage_flops(M)             # each of the 2 GEMM launches of an apply
     achieved = flops_per_launch / (zg_ms / max(zg_n, 1) * 1e-3) / 1e12 if zg_n else None
+    products = T.tdvp_get_gemm_products()
     roofline = {"bound": "tensor", "kernel": "zgemm_kernel (FP64 DMMA m8n8k4, complex128)",
                 "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": (achieved / peak) if achieved else None,
+                # "achieved" counts ALGORITHMIC flops (8 per complex multiply-add); the kernel forms
+                # the complex product from `gemm_products` real DMMA products (3 by default: 6 executed flops per
+                # complex multiply-add), so the share of the DMMA pipe it keeps busy is frac * products / 4
+                "gemm_products": products,
+                "dmma_pipe_frac": (achieved / peak * products / 4.0) if achieved else None,
                 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture in
-                # profiles/r01b_summary.md (mean of the stage-1 and stage-3 launches), M = 128 only
-                "traffic": 50.6e6 if M == 128 else None,
+                # profiles/r01d_summary.md (mean of the stage-1 and stage-3 launches), M = 128 only
+                "traffic": 49.5e6 if M == 128 else None,
                 "peak_source": "tdvp_probe_fp64_tensor_peak: DMMA m8n8k4 issue rate measured in this run "
                                "(MEASURED_PEAKS.json has no FP64 figure; cuBLAS ZGEMM 4096^3 measured 36.85 TFLOP/s)",
                 "flops_per_launch": flops_per_launch, "avg_launch_us": 1e3 * zg_ms / max(zg_n, 1), "launches": zg_n,
@@ -416,6 +422,31 @@ def run_ours(args):
                                       "(7 right-hand sides: SVD + environments + H_eff per site) after 5 PS steps",
                           "ms_per_step": e0.elapsed_time(e1) / n_mu, "steps_timed": n_mu, "err_est": err, "norm_sq": nrm,
                           "energy": en, "phase_ms_per_step": {k: round(v[0] / n_mu, 3) for k, v in ph.items()}}
+        # TDVP-MU with constant-mean-field integration from the
+        # same state: CMF steps of tau = 0.1 fs, 10 RK4 sub-steps per site (local step 0.01 fs, inside the
+        # stability limit the stiff right-hand side sets, see above); SVDs and environments twice per step
+        TAU_CMF, NSUB_CMF = 0.1, 10
+        ch.tdvp_step_mu_cmf(TAU_CMF, NSUB_CMF)
+        ch.tdvp_sync()
+        T.tdvp_profile_enable(True)
+        T.tdvp_profile_read()
+        l0 = T.tdvp_launch_count()
+        e0.record()
+        n_cmf = 2
+        for _ in range(n_cmf):
+            ch.tdvp_step_mu_cmf(TAU_CMF, NSUB_CMF)
+        e1.record()
+        ch.tdvp_sync()
+        torch.cuda.synchronize()
+        ph = T.tdvp_profile_read()
+        T.tdvp_profile_enable(False)
+        nrm, en = ch.tdvp_norm_energy()
+        out["mu_cmf_step"] = {"workload": "configs[3] chain, 71 sites, M=128: one second-order CMF step of tau = %g fs (%d RK4 sub-steps per "
+                                          "site, Krylov dimension %d at the last site; mean fields built twice per step)" % (TAU_CMF, NSUB_CMF, cfg.krylov_dim),
+                              "ms_per_step": e0.elapsed_time(e1) / n_cmf, "steps_timed": n_cmf, "ms_per_fs": e0.elapsed_time(e1) / n_cmf / TAU_CMF,
+                              "launches_per_step": (T.tdvp_launch_count() - l0) // n_cmf, "norm_sq": nrm, "energy": en,
+                              "phase_ms_per_step": {k: round(v[0] / n_cmf, 3) for k, v in ph.items()}}
+        out["mu_step"]["ms_per_fs"] = out["mu_step"]["ms_per_step"] / H_MU
         ch.close()
         # configs[4]: the large chain (147 sites, layout B, M = 256): one warm-up and two timed PS steps,
         # gated on invariants (oracle steps at this size take minutes)
