@@ -49,6 +49,9 @@ SITE_CASES = [
     (37, 29, 5, 7, 3, 0.2),      # ragged, several tiles with tails
     (64, 64, 10, 9, 9, 0.04),    # real-MPO-like density
     (70, 130, 3, 6, 11, 0.15),   # more than one 64-tile in both bonds, ragged
+    (37, 70, 7, 9, 13, 0.3),     # long rows (row-block W kernel): 91 x 63 / 63 x 91, neither a multiple of 8 / 4
+    (20, 33, 10, 20, 20, 0.5),   # long rows, half dense, 200 x 200
+    (9, 64, 6, 12, 5, 1.0),      # dense W, rows 30 x cols 72 and the mirror
 ]
 
 
@@ -59,6 +62,30 @@ def test_apply_heff_ragged(T, case):
     want = oc.heff_definition(L, W, A, R) if Ml * Mr <= 600 else oc.heff(L, W, A, R)
     got = host(T.tdvp_apply_heff(dev(L), dev(W), dev(A), dev(R)))
     assert rel(got, want) <= REL_TOL
+
+
+def test_gemm_products_three_and_four(T):
+    """The GEMM stages with the complex product from 3 (default) or 4 real DMMA products
+    (include/tdvp.h, DESIGN.md c15): both inside the 1e-11 gate, each reproducible bit for bit."""
+    L, W, A, R = si.microbench_tensors(64)
+    want = oc.heff(L, W, A, R)
+    args = [dev(x) for x in (L, W, A, R)]
+    assert T.tdvp_get_gemm_products() == 3
+    try:
+        res = {}
+        for products in (3, 4, 3):
+            T.tdvp_set_gemm_products(products)
+            assert T.tdvp_get_gemm_products() == products
+            got = host(T.tdvp_apply_heff(*args))
+            assert rel(got, want) <= REL_TOL
+            if products in res:
+                assert np.array_equal(res[products], got)
+            res[products] = got
+        assert not np.array_equal(res[3], res[4])           # they are different arithmetic
+        with pytest.raises(T.TdvpError):
+            T.tdvp_set_gemm_products(5)
+    finally:
+        T.tdvp_set_gemm_products(3)
 
 
 @pytest.mark.parametrize("M", [32, 64, 128])
