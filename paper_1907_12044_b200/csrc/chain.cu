@@ -165,6 +165,7 @@ int tdvp_create(tdvp_handle **out, int n_sites, const int *phys_dim, const int *
     if (int rc = check_cuda(h, cudaMemcpyAsync(h->W[i], mpo[i], wn * 16, kind, h->stream), "copy W")) return fail(rc);
     if (int rc = check_cuda(h, cudaMemcpyAsync(h->A[i], mps[i], site_elems(h, i) * 16, kind, h->stream), "copy A")) return fail(rc);
     wsparse_build(h->stream, h->Wsp[i], h->Wsp_mem[i], h->Dw[i], h->d[i], h->Dw[i + 1], h->W[i], h->opt.w_zero_tol);
+    wsparse_classify(h->Wsp[i], h->stream);             // long or short rows: known on the host from here on
     max_site = std::max(max_site, site_elems(h, i));
     max_bond = std::max(max_bond, (long long)h->M[i + 1] * h->M[i + 1]);
   }

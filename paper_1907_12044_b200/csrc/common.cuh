@@ -96,7 +96,15 @@ struct WSparse {
   // transposed-role form used by the right-to-left order: rows r = w*d + s, columns c = t*Dr + v
   int *cnt_r; int *col_r; c128 *val_r;
   int capacity;     // Dl*d*d*Dr
+  // rows sorted by entry count, longest first (both forms): the long-row kernel works on groups of
+  // four consecutive rows of this order, so that the rows of a group are about equally long
+  int *order, *order_r;
+  // are the rows long (entries >= 8 per row on average)?  -1 = only known on the device (stateless
+  // calls: both W-stage kernels are launched and the one whose turn it is not returns at once),
+  // 0 / 1 = known on the host (resident chains: read back once at create)
+  int long_rows = -1, long_rows_r = -1;
 };
+void wsparse_classify(WSparse &ws, cudaStream_t st);   // fills long_rows / long_rows_r (blocks on st)
 size_t wsparse_bytes(int Dl, int d, int Dr);
 // carve a WSparse out of `mem` (DEVICE, wsparse_bytes) and build both CSRs from dense W (DEVICE)
 void wsparse_build(cudaStream_t st, WSparse &ws, void *mem, int Dl, int d, int Dr,

@@ -5,6 +5,8 @@
 // For every bond-index pair the stage is a sparse (rows x cols) matrix applied to a dense
 // cols x Mr panel whose rows are contiguous in y.  HBM/L2 traffic is exactly one read of T1 and one
 // write of T2; see wstage_persistent_kernel for the work split and what bounds it.
+#include <vector>
+
 #include "common.cuh"
 
 namespace {
@@ -52,6 +54,8 @@ struct WStageParams {
   int rdiv; long long o_s1, o_s2;  // output offset of row r: (r / rdiv) * o_s1 + (r % rdiv) * o_s2
   long long o_bs;                  // output batch stride
   const int *cnt; const int *col; const c128 *val;   // row-padded sparse W (see csr_build_kernel)
+  const int *order;                // rows by entry count, longest first
+  int long_rows;                   // -1 unknown on the host, 0, 1
 };
 
 __device__ __forceinline__ void cfma(double &sx, double &sy, c128 w, c128 t) {
@@ -119,7 +123,7 @@ __device__ __forceinline__ void wp_rows(const WStageParams &p, const c128 *tile,
   }
 }
 
-__global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStageParams p, int ntile, int npanels) {
+__global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStageParams p, int ntile, int npanels, int quad_follows) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ int s_next_row;
   c128 *tile = reinterpret_cast<c128 *>(smem_raw);                        // [ncols][YT]
@@ -148,6 +152,7 @@ __global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStage
   const bool csr_smem = csr_off + (size_t)nnz * 20 + 16 <= (size_t)WP_SMEM;
   int *scol = reinterpret_cast<int *>(sval + nnz);
   const bool dyn = nnz >= 8 * p.nrows;
+  if (dyn && quad_follows) return;                     // long rows: wstage_quad_kernel does the stage
   __syncthreads();
   if (csr_smem) {
     for (int r = warp; r < p.nrows; r += WP_THREADS / 32) {
@@ -199,6 +204,123 @@ __global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStage
   }
 }
 
+
+// rank of every row by entry count (longest first, ties by row index): order[rank] = row
+__global__ void row_order_kernel(const int *cnt0, int n0, int *ord0, const int *cnt1, int n1, int *ord1) {
+  const int *cnt = blockIdx.x ? cnt1 : cnt0;
+  const int n = blockIdx.x ? n1 : n0;
+  int *ord = blockIdx.x ? ord1 : ord0;
+  for (int r = threadIdx.x; r < n; r += blockDim.x) {
+    const int c = cnt[r];
+    int rank = 0;
+    for (int q = 0; q < n; q++) { const int cq = cnt[q]; rank += (cq > c) || (cq == c && q < r); }
+    ord[rank] = r;
+  }
+}
+
+// ---- long rows (configs[1]: ~30 entries per row, the sparse W does not fit beside the panel) ----
+// In the row-at-a-time kernel a warp-uniform load of an entry (value + column) costs the LSU pipe
+// about 5.4 wavefronts, 40 % of the kernel's total, because it serves one row only.  Here a warp
+// works on FOUR rows at once: lane = (row slot g = lane / 8, j = lane % 8) owns y = j + 8 m,
+// m = 0..7, of its row, so one load instruction fetches the next entry of four rows, while the
+// panel loads stay what they were (a quarter-warp reads 128 contiguous bytes of its row's column:
+// 4 conflict-free wavefronts per LDS.128, 16 B per entry and y).  Rows are taken in groups of four
+// from the order sorted by length, so the four rows of a group finish together.
+constexpr int WQ_THREADS = 512;
+constexpr int WQ_SMEM = 227 * 1024 - 64;
+
+__global__ void __launch_bounds__(WQ_THREADS, 1) wstage_quad_kernel(WStageParams p, int ntile, int npanels, int forced) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ int s_next, s_nnz;
+  c128 *tile = reinterpret_cast<c128 *>(smem_raw);                        // [ncols][YT]
+  const int tile_elems = p.ncols * YT;
+  int *scnt = reinterpret_cast<int *>(smem_raw + (size_t)tile_elems * 16);    // [nrows], in sorted order
+  int *srow = scnt + p.nrows;                                              // [nrows] the row itself
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int g = lane >> 3, j = lane & 7;
+  if (warp == 0) {
+    int t = 0;
+    for (int r = lane; r < p.nrows; r += 32) t += __ldg(p.cnt + r);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if (lane == 0) s_nnz = t;
+  }
+  for (int i = threadIdx.x; i < p.nrows; i += WQ_THREADS) { const int r = __ldg(p.order + i); srow[i] = r; scnt[i] = __ldg(p.cnt + r); }
+  __syncthreads();
+  if (!forced && s_nnz < 8 * p.nrows) return;          // short rows: the row-at-a-time kernel does the stage
+  const int ngroups = (p.nrows + 3) / 4;
+  const long long units = (long long)npanels * ngroups;
+  long long u = units * blockIdx.x / gridDim.x;
+  const long long u_end = units * (blockIdx.x + 1) / gridDim.x;
+  const c128 zero = make_double2(0.0, 0.0);
+  while (u < u_end) {
+    const int panel = (int)(u / ngroups), g0 = (int)(u - (long long)panel * ngroups);
+    const int g1 = (u_end - u) < (long long)(ngroups - g0) ? g0 + (int)(u_end - u) : ngroups;
+    u += g1 - g0;
+    const int a = panel / ntile, y0 = (panel % ntile) * YT;
+    const c128 *in = p.in + a * p.in_bs;
+    __syncthreads();
+    if (threadIdx.x == 0) s_next = g0;
+    for (int e = threadIdx.x; e < tile_elems; e += WQ_THREADS) {
+      const int c = e / YT, yy = e % YT;
+      const bool ok = (y0 + yy) < p.Mr;
+      const c128 *src = ok ? in + (long long)c * p.Mr + y0 + yy : in;
+      unsigned sa = (unsigned)__cvta_generic_to_shared(tile + e);
+      int sz = ok ? 16 : 0;
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(src), "r"(sz));
+    }
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::);
+    __syncthreads();
+    c128 *out = p.out + a * p.o_bs;
+    for (;;) {
+      int grp = 0;
+      if (lane == 0) grp = atomicAdd(&s_next, 1);
+      grp = __shfl_sync(0xffffffffu, grp, 0);
+      if (grp >= g1) break;
+      const int slot = 4 * grp + g;
+      const bool have = slot < p.nrows;
+      const int r = have ? srow[slot] : 0;
+      const int len = have ? scnt[slot] : 0;
+      int steps = len;                                  // the longest of the four rows
+      steps = max(steps, __shfl_xor_sync(0xffffffffu, steps, 8));
+      steps = max(steps, __shfl_xor_sync(0xffffffffu, steps, 16));
+      const c128 *__restrict__ vp = p.val + (size_t)r * p.ncols;
+      const int *__restrict__ cp = p.col + (size_t)r * p.ncols;
+      double ax[8], ay[8];
+#pragma unroll
+      for (int m = 0; m < 8; m++) ax[m] = ay[m] = 0.0;
+      c128 w0 = 0 < len ? __ldg(vp) : zero, w1 = 1 < len ? __ldg(vp + 1) : zero;
+      int c0 = 0 < len ? __ldg(cp) : 0, c1 = 1 < len ? __ldg(cp + 1) : 0;
+      const c128 *tl = tile + j;
+      for (int sI = 0; sI < steps; sI += 2) {
+        const c128 wn0 = sI + 2 < len ? __ldg(vp + sI + 2) : zero, wn1 = sI + 3 < len ? __ldg(vp + sI + 3) : zero;
+        const int cn0 = sI + 2 < len ? __ldg(cp + sI + 2) : 0, cn1 = sI + 3 < len ? __ldg(cp + sI + 3) : 0;
+        {
+          c128 t[8];
+#pragma unroll
+          for (int m = 0; m < 8; m++) t[m] = tl[c0 * YT + 8 * m];
+#pragma unroll
+          for (int m = 0; m < 8; m++) cfma(ax[m], ay[m], w0, t[m]);
+        }
+        {
+          c128 t[8];
+#pragma unroll
+          for (int m = 0; m < 8; m++) t[m] = tl[c1 * YT + 8 * m];
+#pragma unroll
+          for (int m = 0; m < 8; m++) cfma(ax[m], ay[m], w1, t[m]);
+        }
+        w0 = wn0; w1 = wn1; c0 = cn0; c1 = cn1;
+      }
+      if (have) {
+        c128 *o = out + (r / p.rdiv) * p.o_s1 + (r % p.rdiv) * p.o_s2 + y0 + j;
+#pragma unroll
+        for (int m = 0; m < 8; m++)
+          if (y0 + j + 8 * m < p.Mr) o[8 * m] = make_double2(ax[m], ay[m]);
+      }
+    }
+  }
+}
+
 // Fallback for panels that do not fit in shared memory (ncols * 1 KB > ~220 KB): one warp per
 // (a, 32 y, row), panel and entries read through L1/L2.
 __global__ void __launch_bounds__(256) wstage_direct_kernel(WStageParams p) {
@@ -229,7 +351,21 @@ void launch_wstage(cudaStream_t st, const WStageParams &p, int nbatch) {
     if (want < npanels) want = npanels;
     if (want > units) want = units;
     const int grid = want < g_num_sms ? (int)(want < 1 ? 1 : want) : g_num_sms;
-    TDVP_LAUNCH(wstage_persistent_kernel, grid, WP_THREADS, WP_SMEM, st, p, ntile, (int)npanels);
+    // long rows that do not fit beside the panel go to the four-rows-per-warp kernel.  Whether the rows
+    // are long is known on the host for resident chains; for the stateless calls both kernels are
+    // launched and the one whose turn it is not returns at once.
+    const bool quad_fits = (size_t)p.ncols * YT * 16 + (size_t)p.nrows * 8 + 64 <= (size_t)WQ_SMEM &&
+                           (long long)p.nrows * p.ncols >= 4096;
+    const int lr = quad_fits ? p.long_rows : 0;
+    if (lr != 1) TDVP_LAUNCH(wstage_persistent_kernel, grid, WP_THREADS, WP_SMEM, st, p, ntile, (int)npanels, lr == -1 ? 1 : 0);
+    if (lr != 0) {
+      const long long qunits = npanels * ((p.nrows + 3) / 4);
+      long long qw = (qunits + (WQ_THREADS / 32) - 1) / (WQ_THREADS / 32);
+      if (qw < npanels) qw = npanels;
+      if (qw > qunits) qw = qunits;
+      const int qgrid = qw < g_num_sms ? (int)(qw < 1 ? 1 : qw) : g_num_sms;
+      TDVP_LAUNCH(wstage_quad_kernel, qgrid, WQ_THREADS, WQ_SMEM, st, p, ntile, (int)npanels, lr == 1 ? 1 : 0);
+    }
     return;
   }
   dim3 grid((p.Mr + 31) / 32, nbatch, (p.nrows + 7) / 8 < 8 ? (p.nrows + 7) / 8 : 8);
@@ -240,13 +376,14 @@ void launch_wstage(cudaStream_t st, const WStageParams &p, int nbatch) {
 
 void wstage_configure() {
   cudaFuncSetAttribute(wstage_persistent_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, WP_SMEM);
+  cudaFuncSetAttribute(wstage_quad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, WQ_SMEM);
 }
 
 size_t wsparse_bytes(int Dl, int d, int Dr) {
   size_t cap = (size_t)Dl * d * d * Dr;
   size_t rows0 = (size_t)d * Dr + 1, rows1 = (size_t)Dl * d + 1;
   auto up = [](size_t x) { return (x + 255) & ~size_t(255); };
-  return up(rows0 * 4) + up(rows1 * 4) + 2 * up(cap * 4) + 2 * up(cap * 16) + 256;
+  return 2 * up(rows0 * 4) + 2 * up(rows1 * 4) + 2 * up(cap * 4) + 2 * up(cap * 16) + 256;
 }
 
 void wsparse_build(cudaStream_t st, WSparse &ws, void *mem, int Dl, int d, int Dr, const c128 *W,
@@ -261,11 +398,28 @@ void wsparse_build(cudaStream_t st, WSparse &ws, void *mem, int Dl, int d, int D
   ws.col = reinterpret_cast<int *>(p); p += up(cap * 4);
   ws.col_r = reinterpret_cast<int *>(p); p += up(cap * 4);
   ws.cnt = reinterpret_cast<int *>(p); p += up(((size_t)d * Dr + 1) * 4);
-  ws.cnt_r = reinterpret_cast<int *>(p);
+  ws.cnt_r = reinterpret_cast<int *>(p); p += up(((size_t)Dl * d + 1) * 4);
+  ws.order = reinterpret_cast<int *>(p); p += up(((size_t)d * Dr + 1) * 4);
+  ws.order_r = reinterpret_cast<int *>(p);
+  ws.long_rows = ws.long_rows_r = -1;
   int maxrows = (d * Dr > Dl * d ? d * Dr : Dl * d);
   dim3 grid((maxrows + CSR_WARPS - 1) / CSR_WARPS, 2);
   TDVP_LAUNCH(csr_build_kernel, grid, CSR_WARPS * 32, 0, st, W, Dl, d, Dr, zero_tol,
               ws.cnt, ws.col, ws.val, ws.cnt_r, ws.col_r, ws.val_r);
+  TDVP_LAUNCH(row_order_kernel, 2, 256, 0, st, ws.cnt, d * Dr, ws.order, ws.cnt_r, Dl * d, ws.order_r);
+}
+
+void wsparse_classify(WSparse &ws, cudaStream_t st) {
+  const int n0 = ws.d * ws.Dr, n1 = ws.Dl * ws.d;
+  std::vector<int> c0(n0), c1(n1);
+  cudaMemcpyAsync(c0.data(), ws.cnt, n0 * sizeof(int), cudaMemcpyDeviceToHost, st);
+  cudaMemcpyAsync(c1.data(), ws.cnt_r, n1 * sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess) return;
+  long long t0 = 0, t1 = 0;
+  for (int x : c0) t0 += x;
+  for (int x : c1) t1 += x;
+  ws.long_rows = t0 >= 8LL * n0 ? 1 : 0;
+  ws.long_rows_r = t1 >= 8LL * n1 ? 1 : 0;
 }
 
 void wstage_left(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2) {
@@ -275,7 +429,7 @@ void wstage_left(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 
   p.in_bs = (long long)ws.Dl * ws.d * Mr;
   p.rdiv = p.nrows > 0 ? p.nrows : 1; p.o_s1 = 0; p.o_s2 = Mr;
   p.o_bs = (long long)ws.d * ws.Dr * Mr;
-  p.cnt = ws.cnt; p.col = ws.col; p.val = ws.val;
+  p.cnt = ws.cnt; p.col = ws.col; p.val = ws.val; p.order = ws.order; p.long_rows = ws.long_rows;
   launch_wstage(st, p, Ml);
 }
 
@@ -286,6 +440,6 @@ void wstage_right(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128
   p.in_bs = (long long)ws.d * ws.Dr * Mr;
   p.rdiv = ws.d; p.o_s1 = (long long)Ml * ws.d * Mr; p.o_s2 = Mr;
   p.o_bs = (long long)ws.d * Mr;
-  p.cnt = ws.cnt_r; p.col = ws.col_r; p.val = ws.val_r;
+  p.cnt = ws.cnt_r; p.col = ws.col_r; p.val = ws.val_r; p.order = ws.order_r; p.long_rows = ws.long_rows_r;
   launch_wstage(st, p, Ml);
 }
