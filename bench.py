@@ -302,7 +302,9 @@ def run_ours(args):
                                "(MEASURED_PEAKS.json has no FP64 figure; cuBLAS ZGEMM 4096^3 measured 36.85 TFLOP/s)",
                 "flops_per_launch": flops_per_launch, "avg_launch_us": 1e3 * zg_ms / max(zg_n, 1), "launches": zg_n,
                 "share_of_step": {"zgemm": zg_ms / ms_total, "wstage": ws_ms / ms_total},
-                "wstage": {"bound": "hbm", "algorithmic_bytes": 2 * 16.0 * M * M * D_W * D_PHYS,
+                "wstage": {"bound": "hbm", "note": "algorithmic bytes = one read of T1 + one write of T2; ncu shows the kernel bound by "
+                                                  "shared-memory (LSU) wavefronts, not by HBM (profiles/r01e_summary.md)",
+                           "algorithmic_bytes": 2 * 16.0 * M * M * D_W * D_PHYS,
                            "achieved_gbs": (2 * 16.0 * M * M * D_W * D_PHYS / (ws_ms / max(ws_n, 1) * 1e-3) / 1e9) if ws_n else None,
                            "avg_launch_us": 1e3 * ws_ms / max(ws_n, 1)}}
     try:
