@@ -109,6 +109,11 @@ static void free_chain(tdvp_handle *h) {
   for (int s = 0; s < 7; s++) for (auto p : h->mu_k[s]) fr(p);
   for (auto p : h->mu_y) fr(p);
   for (auto p : h->cmf_mem) fr(p);
+  for (auto p : h->cmf_ws) fr(p);
+  for (auto p : h->cmf_scratch) fr(p);
+  for (auto q : h->cmf_streams) { cudaStreamSynchronize(q); zgemm_release_stream(q); cudaStreamDestroy(q); }
+  for (auto e : h->cmf_join) cudaEventDestroy(e);
+  if (h->cmf_fork) cudaEventDestroy(h->cmf_fork);
   fr(h->tmpA); fr(h->tmpB); fr(h->bondD); fr(h->bondD2); fr(h->step_ws); fr(h->mu_err_dev); fr(h->mu_scratch);
   if (h->ps_graph.exec) cudaGraphExecDestroy(h->ps_graph.exec);
   if (h->mu_graph.exec) cudaGraphExecDestroy(h->mu_graph.exec);

@@ -83,6 +83,7 @@ void zgemm_set_mode(int products);   // 3 or 4 real DMMA products per complex pr
 int zgemm_get_mode();
 void zgemm_alias_stream(cudaStream_t alias, cudaStream_t of);
 void zgemm_forget_stream(cudaStream_t alias);
+void zgemm_release_stream(cudaStream_t st);
 
 // ---------------------------------------------------------------------------------------------
 // wstage.cu : sparse MPO stage.

@@ -43,6 +43,10 @@ struct tdvp_handle {
   bool mu_fsal = false;            // mu_k[6] holds the right-hand side at the CURRENT state (first-same-as-last)
   void *mu_scratch = nullptr;      // U, Lambda, V^dagger, centre forms ... of one derivative evaluation
   std::vector<void *> cmf_mem;     // CMF mean fields per bond b: [3b] U, [3b+1] U Lambda, [3b+2] Lambda (first use)
+  std::vector<cudaStream_t> cmf_streams;   // side queues of the CMF local propagation, each with scratch
+  std::vector<cudaEvent_t> cmf_join;
+  std::vector<void *> cmf_ws, cmf_scratch;
+  cudaEvent_t cmf_fork = nullptr;
   StepGraph ps_graph, mu_graph;
 };
 

@@ -65,15 +65,20 @@ struct MuScratch {
   double *lam;
 };
 
-MuScratch mu_scratch(tdvp_handle *h) {
+size_t mu_scratch_bytes(const tdvp_handle *h, size_t *sb_out, size_t *bb_out) {
   long long ms = 0; int mm = 1;
   for (int i = 0; i < h->n; i++) { ms = std::max(ms, site_elems(h, i)); mm = std::max(mm, h->M[i + 1]); }
   const size_t sb = up256(ms * 16), bb = up256((size_t)mm * mm * 16);
-  if (!h->mu_scratch) {
-    if (cudaMalloc(&h->mu_scratch, 6 * sb + 3 * bb + up256(mm * 8) + 1024) != cudaSuccess) { h->mu_scratch = nullptr; }
-  }
+  if (sb_out) *sb_out = sb;
+  if (bb_out) *bb_out = bb;
+  return 6 * sb + 3 * bb + up256(mm * 8) + 1024;
+}
+
+MuScratch mu_carve(const tdvp_handle *h, void *mem) {
+  size_t sb = 0, bb = 0;
+  mu_scratch_bytes(h, &sb, &bb);
   MuScratch s{};
-  char *p = reinterpret_cast<char *>(h->mu_scratch);
+  char *p = reinterpret_cast<char *>(mem);
   if (!p) return s;
   s.Vh = reinterpret_cast<c128 *>(p); p += sb;
   s.C0 = reinterpret_cast<c128 *>(p); p += sb;
@@ -86,6 +91,13 @@ MuScratch mu_scratch(tdvp_handle *h) {
   s.P = reinterpret_cast<c128 *>(p); p += bb;
   s.lam = reinterpret_cast<double *>(p);
   return s;
+}
+
+MuScratch mu_scratch(tdvp_handle *h) {
+  if (!h->mu_scratch) {
+    if (cudaMalloc(&h->mu_scratch, mu_scratch_bytes(h, nullptr, nullptr)) != cudaSuccess) { h->mu_scratch = nullptr; }
+  }
+  return mu_carve(h, h->mu_scratch);
 }
 
 void gemm1(cudaStream_t st, ZGemm g) { g.splitk = 1; zgemm(st, g, nullptr); }
@@ -272,9 +284,7 @@ int cmf_mean_fields(tdvp_handle *h, const std::vector<c128 *> &Y) {
 }
 
 // K = dL_j/dt of Eq. 37 at the local matrix Yj, mean fields of site j held in the handle.
-void cmf_local_rhs(tdvp_handle *h, int j, const c128 *Yj, c128 *K, const MuScratch &s) {
-  cudaStream_t st = h->stream;
-  void *ws = h->step_ws;
+void cmf_local_rhs(tdvp_handle *h, int j, const c128 *Yj, c128 *K, const MuScratch &s, cudaStream_t st, void *ws) {
   const double sq = std::sqrt(h->opt.mu_eps);
   const int Jl = h->M[j], Jr = h->M[j + 1], dj = h->d[j];
   const long long ne = site_elems(h, j), rows = (long long)Jl * dj;
@@ -302,32 +312,62 @@ void cmf_local_rhs(tdvp_handle *h, int j, const c128 *Yj, c128 *K, const MuScrat
   TDVP_LAUNCH(minus_i_diff_kernel, grid_for(ne), VT, 0, st, K, s.G, s.T, ne);             // -i (1 - p) G
 }
 
+// Side queues for the local propagation: once the mean fields are fixed the local problems of
+// different sites are independent, and each is a chain of small GEMMs that leaves
+// most of the GPU idle, so sites are dealt round-robin to a few queues, each with its own scratch.
+int cmf_queues(tdvp_handle *h) {
+  if (!h->cmf_streams.empty()) return TDVP_OK;
+  int nq = 4;
+  if (const char *e = getenv("TDVP_CMF_QUEUES")) nq = atoi(e);
+  if (nq < 1) nq = 1;
+  if (nq > 8) nq = 8;
+  if (int rc = check_cuda(h, cudaEventCreateWithFlags(&h->cmf_fork, cudaEventDisableTiming), "event")) return rc;
+  for (int q = 0; q < nq; q++) {
+    cudaStream_t st = nullptr; cudaEvent_t ev = nullptr; void *ws = nullptr, *sc = nullptr;
+    if (int rc = check_cuda(h, cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking), "CMF queue")) return rc;
+    if (int rc = check_cuda(h, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming), "event")) return rc;
+    if (int rc = check_cuda(h, cudaMalloc(&ws, h->step_ws_bytes), "cudaMalloc CMF workspace")) return rc;
+    if (int rc = check_cuda(h, cudaMalloc(&sc, mu_scratch_bytes(h, nullptr, nullptr)), "cudaMalloc CMF scratch")) return rc;
+    zgemm_prepare_stream(st);
+    h->cmf_streams.push_back(st); h->cmf_join.push_back(ev); h->cmf_ws.push_back(ws); h->cmf_scratch.push_back(sc);
+  }
+  return TDVP_OK;
+}
+
+// RK4 sub-steps of site j on queue st
+void cmf_site(tdvp_handle *h, int j, const c128 *Xj, c128 *y, double t, int n_sub, const MuScratch &s, cudaStream_t st, void *ws) {
+  const double hs = t / n_sub;
+  const long long ne = site_elems(h, j);
+  c128 *ys = h->mu_y[j];
+  c128 *k1 = h->mu_k[0][j], *k2 = h->mu_k[1][j], *k3 = h->mu_k[2][j], *k4 = h->mu_k[3][j];
+  vec_copy(st, y, Xj, ne);
+  for (int q = 0; q < n_sub; q++) {                        // classical RK4
+    cmf_local_rhs(h, j, y, k1, s, st, ws);
+    { Comb c{}; c.n = 1; c.k[0] = k1; c.c[0] = 0.5 * hs;
+      TDVP_LAUNCH(lincomb_kernel, grid_for(ne), VT, 0, st, ys, (const c128 *)y, c, ne); }
+    cmf_local_rhs(h, j, ys, k2, s, st, ws);
+    { Comb c{}; c.n = 1; c.k[0] = k2; c.c[0] = 0.5 * hs;
+      TDVP_LAUNCH(lincomb_kernel, grid_for(ne), VT, 0, st, ys, (const c128 *)y, c, ne); }
+    cmf_local_rhs(h, j, ys, k3, s, st, ws);
+    { Comb c{}; c.n = 1; c.k[0] = k3; c.c[0] = hs;
+      TDVP_LAUNCH(lincomb_kernel, grid_for(ne), VT, 0, st, ys, (const c128 *)y, c, ne); }
+    cmf_local_rhs(h, j, ys, k4, s, st, ws);
+    { Comb c{}; c.n = 4; c.k[0] = k1; c.k[1] = k2; c.k[2] = k3; c.k[3] = k4;
+      c.c[0] = hs / 6.0; c.c[1] = hs / 3.0; c.c[2] = hs / 3.0; c.c[3] = hs / 6.0;
+      TDVP_LAUNCH(lincomb_kernel, grid_for(ne), VT, 0, st, y, (const c128 *)y, c, ne); }
+  }
+}
+
 // Z[i] = every local matrix of X propagated over time t with the handle's mean fields.
 int cmf_propagate(tdvp_handle *h, const std::vector<c128 *> &X, const std::vector<c128 *> &Z, double t, int n_sub) {
   cudaStream_t st = h->stream;
   const int n = h->n;
-  MuScratch s = mu_scratch(h);
-  const double hs = t / n_sub;
+  const int nq = (int)h->cmf_streams.size();
+  cudaEventRecord(h->cmf_fork, st);                          // the mean fields are ready
+  for (int q = 0; q < nq; q++) cudaStreamWaitEvent(h->cmf_streams[q], h->cmf_fork, 0);
   for (int j = 0; j < n - 1; j++) {
-    const long long ne = site_elems(h, j);
-    c128 *y = Z[j], *ys = h->mu_y[j];
-    c128 *k1 = h->mu_k[0][j], *k2 = h->mu_k[1][j], *k3 = h->mu_k[2][j], *k4 = h->mu_k[3][j];
-    vec_copy(st, y, X[j], ne);
-    for (int q = 0; q < n_sub; q++) {                      // classical RK4
-      cmf_local_rhs(h, j, y, k1, s);
-      { Comb c{}; c.n = 1; c.k[0] = k1; c.c[0] = 0.5 * hs;
-        TDVP_LAUNCH(lincomb_kernel, grid_for(ne), VT, 0, st, ys, (const c128 *)y, c, ne); }
-      cmf_local_rhs(h, j, ys, k2, s);
-      { Comb c{}; c.n = 1; c.k[0] = k2; c.c[0] = 0.5 * hs;
-        TDVP_LAUNCH(lincomb_kernel, grid_for(ne), VT, 0, st, ys, (const c128 *)y, c, ne); }
-      cmf_local_rhs(h, j, ys, k3, s);
-      { Comb c{}; c.n = 1; c.k[0] = k3; c.c[0] = hs;
-        TDVP_LAUNCH(lincomb_kernel, grid_for(ne), VT, 0, st, ys, (const c128 *)y, c, ne); }
-      cmf_local_rhs(h, j, ys, k4, s);
-      { Comb c{}; c.n = 4; c.k[0] = k1; c.k[1] = k2; c.k[2] = k3; c.k[3] = k4;
-        c.c[0] = hs / 6.0; c.c[1] = hs / 3.0; c.c[2] = hs / 3.0; c.c[3] = hs / 6.0;
-        TDVP_LAUNCH(lincomb_kernel, grid_for(ne), VT, 0, st, y, (const c128 *)y, c, ne); }
-    }
+    const int q = j % nq;
+    cmf_site(h, j, X[j], Z[j], t, n_sub, mu_carve(h, h->cmf_scratch[q]), h->cmf_streams[q], h->cmf_ws[q]);
   }
   {                                                        // Eq. 27 by the Krylov exponential
     const int i = n - 1;
@@ -335,6 +375,10 @@ int cmf_propagate(tdvp_handle *h, const std::vector<c128 *> &X, const std::vecto
     op.kind = 0; op.Ml = h->M[i]; op.Mr = h->M[i + 1]; op.d = h->d[i]; op.Dl = h->Dw[i]; op.Dr = h->Dw[i + 1];
     op.L = h->Lenv[i]; op.R = h->Renv[i]; op.W = &h->Wsp[i];
     lanczos_expm(st, op, h->opt.krylov_dim, 0.0, -t, X[i], Z[i], h->step_ws, nullptr);
+  }
+  for (int q = 0; q < nq; q++) {
+    cudaEventRecord(h->cmf_join[q], h->cmf_streams[q]);
+    cudaStreamWaitEvent(st, h->cmf_join[q], 0);
   }
   return check_cuda(h, cudaGetLastError(), "CMF local propagation");
 }
@@ -377,6 +421,7 @@ int tdvp_step_mu_cmf(tdvp_handle *h, double dt, int n_sub) {
   if (int rc = prepare_mu(h)) return rc;
   if (n_sub < 1) return set_err(h, TDVP_EINVAL, "n_sub must be >= 1");
   if (int rc = cmf_alloc(h)) return rc;
+  if (int rc = cmf_queues(h)) return rc;
   if (h->centre != h->n - 1) {
     if (int rc = move_gauge(h, h->n - 1)) return rc;
   }

@@ -561,6 +561,15 @@ void zgemm_forget_stream(cudaStream_t alias) {
   g_ctx.erase(alias);
 }
 
+void zgemm_release_stream(cudaStream_t st) {           // a queue the caller owned: free its context
+  std::lock_guard<std::mutex> lk(g_ctx_mu);
+  auto it = g_ctx.find(st);
+  if (it == g_ctx.end()) return;
+  cudaFree(it->second.slots);
+  cudaFree(it->second.cnt);
+  g_ctx.erase(it);
+}
+
 size_t zgemm_ws_elems(const ZGemm &) { return 0; }   // the scheduling workspace belongs to the stream
 
 void zgemm(cudaStream_t st, const ZGemm &p, c128 *) {
