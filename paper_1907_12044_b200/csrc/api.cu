@@ -155,11 +155,13 @@ int ensure_side_queue(tdvp_handle *h, tdvp_handle *hh) {
 // The stateless calls get a dense W and must build its sparse form first; that build does not depend
 // on stage 1, so it runs on the side queue (fork after the arena's previous users, join before the
 // W stage) and its ~8 us latency disappears behind the first GEMM.
-int build_w_beside(tdvp_handle *h, tdvp_handle *hh, WSparse &wsp, void *wmem, int Dl, int d, int Dr, const c128 *W) {
+int build_w_beside(tdvp_handle *h, tdvp_handle *hh, WSparse &wsp, void *wmem, int Dl, int d, int Dr, const c128 *W,
+                   int Ml, int Mr) {
   if (int rc = ensure_side_queue(h, hh)) return rc;
   cudaEventRecord(hh->ev_first, hh->stream);
   cudaStreamWaitEvent(hh->copy_stream, hh->ev_first, 0);
-  wsparse_build(hh->copy_stream, wsp, wmem, Dl, d, Dr, W, hh->opt.w_zero_tol);
+  const bool many_panels = (long long)Ml * ((Mr + 63) / 64) >= W_QUAD_MIN_PANELS;
+  wsparse_build(hh->copy_stream, wsp, wmem, Dl, d, Dr, W, hh->opt.w_zero_tol, many_panels);
   cudaEventRecord(hh->ev_w, hh->copy_stream);
   return 0;
 }
@@ -176,7 +178,7 @@ int tdvp_apply_heff(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr, const
   void *wmem = hh->arena.take(wb);
   void *ws = hh->arena.take(hb);
   WSparse wsp;
-  if (int rc = build_w_beside(h, hh, wsp, wmem, Dl, d, Dr, reinterpret_cast<const c128 *>(W))) return rc;
+  if (int rc = build_w_beside(h, hh, wsp, wmem, Dl, d, Dr, reinterpret_cast<const c128 *>(W), Ml, Mr)) return rc;
   heff_apply(hh->stream, Ml, Mr, d, Dl, Dr, reinterpret_cast<const c128 *>(L), wsp,
              reinterpret_cast<const c128 *>(A), reinterpret_cast<const c128 *>(R),
              reinterpret_cast<c128 *>(out), ws, hh->ev_w);
@@ -240,7 +242,7 @@ int tdvp_update_env(tdvp_handle *h, int side, int Ml, int Mr, int d, int Dl, int
   void *wmem = hh->arena.take(wb);
   void *ws = hh->arena.take(eb);
   WSparse wsp;
-  if (int rc = build_w_beside(h, hh, wsp, wmem, Dl, d, Dr, reinterpret_cast<const c128 *>(W))) return rc;
+  if (int rc = build_w_beside(h, hh, wsp, wmem, Dl, d, Dr, reinterpret_cast<const c128 *>(W), Ml, Mr)) return rc;
   env_update(hh->stream, side, Ml, Mr, d, Dl, Dr, reinterpret_cast<const c128 *>(env_in), wsp,
              reinterpret_cast<const c128 *>(A), reinterpret_cast<c128 *>(env_out), ws, hh->ev_w);
   return check_cuda(h, cudaGetLastError(), "tdvp_update_env");

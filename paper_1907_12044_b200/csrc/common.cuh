@@ -109,7 +109,8 @@ void wsparse_classify(WSparse &ws, cudaStream_t st);   // fills long_rows / long
 size_t wsparse_bytes(int Dl, int d, int Dr);
 // carve a WSparse out of `mem` (DEVICE, wsparse_bytes) and build both CSRs from dense W (DEVICE)
 void wsparse_build(cudaStream_t st, WSparse &ws, void *mem, int Dl, int d, int Dr,
-                   const c128 *W, double zero_tol);
+                   const c128 *W, double zero_tol, bool want_order = true);
+constexpr int W_QUAD_MIN_PANELS = 48;   // fewer (a, 64-y) panels than this: the long-row kernel is not considered
 // T2[a,s,v,y] = sum_{w,t} W[w,s,t,v] T1[a,w,t,y];  T1 [Ml,Dl,d,Mr] -> T2 [Ml,d,Dr,Mr]
 void wstage_left(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2);
 // T2[w,x,s,b] = sum_{t,v} W[w,s,t,v] T1[x,t,v,b];  T1 [Ml,d,Dr,Mr] -> T2 [Dl,Ml,d,Mr]

@@ -227,6 +227,7 @@ __global__ void row_order_kernel(const int *cnt0, int n0, int *ord0, const int *
 // 4 conflict-free wavefronts per LDS.128, 16 B per entry and y).  Rows are taken in groups of four
 // from the order sorted by length, so the four rows of a group finish together.
 constexpr int WQ_THREADS = 512;
+constexpr int WQ_MIN_PANELS = W_QUAD_MIN_PANELS;       // below this the stage is launch-bound: one kernel, no row order
 constexpr int WQ_SMEM = 227 * 1024 - 64;
 
 __global__ void __launch_bounds__(WQ_THREADS, 1) wstage_quad_kernel(WStageParams p, int ntile, int npanels, int forced) {
@@ -355,7 +356,7 @@ void launch_wstage(cudaStream_t st, const WStageParams &p, int nbatch) {
     // are long is known on the host for resident chains; for the stateless calls both kernels are
     // launched and the one whose turn it is not returns at once.
     const bool quad_fits = (size_t)p.ncols * YT * 16 + (size_t)p.nrows * 8 + 64 <= (size_t)WQ_SMEM &&
-                           (long long)p.nrows * p.ncols >= 4096;
+                           (long long)p.nrows * p.ncols >= 4096 && npanels >= WQ_MIN_PANELS;
     const int lr = quad_fits ? p.long_rows : 0;
     if (lr != 1) TDVP_LAUNCH(wstage_persistent_kernel, grid, WP_THREADS, WP_SMEM, st, p, ntile, (int)npanels, lr == -1 ? 1 : 0);
     if (lr != 0) {
@@ -387,7 +388,7 @@ size_t wsparse_bytes(int Dl, int d, int Dr) {
 }
 
 void wsparse_build(cudaStream_t st, WSparse &ws, void *mem, int Dl, int d, int Dr, const c128 *W,
-                   double zero_tol) {
+                   double zero_tol, bool want_order) {
   size_t cap = (size_t)Dl * d * d * Dr;
   auto up = [](size_t x) { return (x + 255) & ~size_t(255); };
   char *p = reinterpret_cast<char *>(mem);
@@ -406,7 +407,10 @@ void wsparse_build(cudaStream_t st, WSparse &ws, void *mem, int Dl, int d, int D
   dim3 grid((maxrows + CSR_WARPS - 1) / CSR_WARPS, 2);
   TDVP_LAUNCH(csr_build_kernel, grid, CSR_WARPS * 32, 0, st, W, Dl, d, Dr, zero_tol,
               ws.cnt, ws.col, ws.val, ws.cnt_r, ws.col_r, ws.val_r);
-  TDVP_LAUNCH(row_order_kernel, 2, 256, 0, st, ws.cnt, d * Dr, ws.order, ws.cnt_r, Dl * d, ws.order_r);
+  // the sorted row order serves the long-row kernel only; callers that know it will not run (few
+  // panels: the stage is launch-bound there) skip it and pin the choice
+  if (want_order) TDVP_LAUNCH(row_order_kernel, 2, 256, 0, st, ws.cnt, d * Dr, ws.order, ws.cnt_r, Dl * d, ws.order_r);
+  else ws.long_rows = ws.long_rows_r = 0;
 }
 
 void wsparse_classify(WSparse &ws, cudaStream_t st) {
