@@ -497,6 +497,32 @@ def test_mu_cmf_odd_substeps_and_ps_gauge(T):
     ch.close()
 
 
+def test_mu_cmf_fmo_like_chain(T):
+    """CMF steps on a short FMO-like chain (layout A, d = 6 phonon sites, D_W up to 6, M = 12) after a
+    shared PS warm-up from the delta-seeded start: populations, a phonon-site observable, overlap."""
+    from oracle import tdvp_mu, tdvp_cmf
+    cfg = dataclasses.replace(si.CONFIGS["fmo64"], n_el=4, n_modes=2, n_ph=6, M=12, dt_fs=5.0)
+    params = si.draw_vibronic_params(cfg)
+    mpo = model.build_mpo(params)
+    dims = si.site_dims(params)
+    mps = si.padded_product_mps(dims, si.initial_occupations(params), cfg.M, cfg.pad_seed, cfg.delta, cfg.delta_seed)
+    st = tdvp_ps.PSState(mpo, mps)
+    for _ in range(4):
+        tdvp_ps.step_ps(st, cfg.dt_fs, cfg.krylov_dim)
+    cur = tdvp_mu.to_left_canonical(st.mps)
+    ch = T.tdvp_create(mpo, st.mps, T.make_options(krylov_dim=cfg.krylov_dim))
+    ch.tdvp_set_mps(cur, centre=ch.n - 1)
+    for s in range(2):
+        cur = tdvp_cmf.step_cmf(mpo, cur, 0.05, 10, cfg.krylov_dim)
+        ch.tdvp_step_mu_cmf(0.05, 10)
+        assert np.abs(ch.tdvp_populations(0) - obs.populations(cur, 0)).max() <= 1e-8
+    num = np.diag(np.arange(dims[3], dtype=np.float64)).astype(np.complex128)
+    assert abs(ch.tdvp_observe(3, num) - np.trace(num @ obs.one_site_rdm(cur, 3))) <= 1e-8
+    ov = np.vdot(obs.mps_to_vector(cur), obs.mps_to_vector(ch.tdvp_get_mps()))
+    assert abs(abs(ov) - 1.0) <= 1e-8
+    ch.close()
+
+
 def test_mu_step_from_ps_gauge(T):
     """tdvp_step_mu on a handle in the PS gauge first moves the centre (no time evolution)."""
     cfg, mpo, st = _tiny_state(3)
