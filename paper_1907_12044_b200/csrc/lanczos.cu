@@ -220,6 +220,32 @@ __global__ void __launch_bounds__(FT) lz_fused_orth_kernel(long long n, int chun
   const int len = (int)((e0 + chunk <= n) ? chunk : (n > e0 ? n - e0 : 0));
   const int was_done = b.state->done;                             // read before anybody can change it
   c128 *wg = b.Q + (long long)(j + 1) * n + e0;
+  if (j == k - 1) {
+    // last iteration: only alpha_j = Re<q_j, w> is needed (the recurrence stops before q_{k+1} is
+    // formed, PAPER.md:292-296 / oracle O3) -- one reduction, one grid barrier, no orthogonalisation
+    const c128 *qg = b.Q + (long long)j * n + e0;
+    double s = 0.0;
+    for (int e = tid; e < len; e += FT) {
+      const c128 q = __ldcg(qg + e), x = __ldcg(wg + e);
+      s = fma(q.x, x.x, fma(q.y, x.y, s));
+    }
+    s = warp_sum(s);
+    if (lane == 0) red[warp] = s;
+    __syncthreads();
+    if (tid == 0) { double t = 0; for (int i = 0; i < FT / 32; i++) t += red[i]; b.npartial[blockIdx.x] = t; }
+    grid.sync();
+    if (blockIdx.x == 0 && warp == 0) {
+      double t = 0.0;
+      for (int g = lane; g < (int)gridDim.x; g += 32) t += __ldcg(b.npartial + g);
+      t = warp_sum(t);
+      if (lane == 0) {
+        LzState *st = b.state;
+        if (!was_done) { b.alpha[j] = t; st->done = 1; st->m = j + 1; }
+        st->inv_beta = 0.0;
+      }
+    }
+    return;
+  }
   // all loads of the chunk in flight at once (16 B asynchronous copies), one wait
   for (int e = tid; e < len; e += FT) {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(sw + e);
