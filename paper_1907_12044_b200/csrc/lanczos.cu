@@ -208,8 +208,24 @@ __device__ __forceinline__ void fused_gather(const c128 *partial, int nd, c128 *
   __syncthreads();
 }
 
+// Grid barrier on a counter that only grows during one exponential (zeroed by the host before the
+// first iteration): arrival = one atomic add per CTA, release when the count reaches `target`.  The
+// launch is cooperative, so all CTAs are resident.  (cg::grid_group::sync does the same with more
+// bookkeeping; three barriers per call are most of this kernel's time.)
+__device__ __forceinline__ void lz_grid_bar(unsigned *ctr, unsigned target) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(ctr, 1u);
+    unsigned v;
+    do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(ctr) : "memory"); } while (v < target);
+  }
+  __syncthreads();
+}
+
 __global__ void __launch_bounds__(FT) lz_fused_orth_kernel(long long n, int chunk, int j, int k, LzBuffers b) {
-  cg::grid_group grid = cg::this_grid();
+  unsigned *bar = b.counter + 1;
+  const unsigned bar0 = 3u * (unsigned)j * gridDim.x;     // every earlier iteration passed three barriers
   extern __shared__ __align__(16) unsigned char fsm[];
   c128 *sw = reinterpret_cast<c128 *>(fsm);                       // [chunk]
   c128 *sq = sw + chunk;                                          // [j + 1][chunk]
@@ -233,7 +249,7 @@ __global__ void __launch_bounds__(FT) lz_fused_orth_kernel(long long n, int chun
     if (lane == 0) red[warp] = s;
     __syncthreads();
     if (tid == 0) { double t = 0; for (int i = 0; i < FT / 32; i++) t += red[i]; b.npartial[blockIdx.x] = t; }
-    grid.sync();
+    lz_grid_bar(bar, bar0 + gridDim.x);
     if (blockIdx.x == 0 && warp == 0) {
       double t = 0.0;
       for (int g = lane; g < (int)gridDim.x; g += 32) t += __ldcg(b.npartial + g);
@@ -263,7 +279,7 @@ __global__ void __launch_bounds__(FT) lz_fused_orth_kernel(long long n, int chun
   for (int pass = 0; pass < 2; pass++) {
     c128 *partial = b.partial + (size_t)pass * MAXG * (TDVP_MAX_KRYLOV + 1);
     fused_dots(sw, sq, chunk, len, nd, partial, lane, warp);
-    grid.sync();
+    lz_grid_bar(bar, bar0 + (unsigned)(pass + 1) * gridDim.x);
     fused_gather(partial, nd, cs, lane, warp);
     if (pass == 0 && blockIdx.x == 0 && tid == 0 && !was_done) b.alpha[j] = cs[j].x;
     for (int e = tid; e < len; e += FT) {
@@ -283,7 +299,7 @@ __global__ void __launch_bounds__(FT) lz_fused_orth_kernel(long long n, int chun
   if (lane == 0) red[warp] = s;
   __syncthreads();
   if (tid == 0) { double t = 0; for (int i = 0; i < FT / 32; i++) t += red[i]; b.npartial[blockIdx.x] = t; }
-  grid.sync();
+  lz_grid_bar(bar, bar0 + 3u * gridDim.x);
   double t = 0.0;
   for (int g = lane; g < (int)gridDim.x; g += 32) t += __ldcg(b.npartial + g);
   t = warp_sum(t);
@@ -459,7 +475,7 @@ void lanczos_expm(cudaStream_t st, const LanczosOp &op, int k, double z_re, doub
   const bool fused = !g_lanczos_unfused && (size_t)(k + 1) * chunk * 16 <= FUSED_SMEM_MAX;
   {
     ProfScope ps(st, PH_VEC);
-    cudaMemsetAsync(b.counter, 0, sizeof(unsigned), st);
+    cudaMemsetAsync(b.counter, 0, 2 * sizeof(unsigned), st);   // [0] last-block counter, [1] grid-barrier counter
     TDVP_LAUNCH(lz_init_kernel, G, VT, 0, st, v, n, b);
     TDVP_LAUNCH(lz_scale_kernel, G, VT, 0, st, b.Q, v, n, b.state);
   }
