@@ -351,6 +351,9 @@ def run_ours(args):
                       "multi_gpu": "replicas only (SURVEY.md 8(e))", "seed": "1000+M+7919*set"},
            "us_per_apply": 1e3 * ms_total / n_applies, "tflops": value / world * heff_flops(M) / 1e12,
            "frac_fp64_tensor_peak": value / world * heff_flops(M) / 1e12 / peak,
+           "flop_convention": "tflops / frac_fp64_tensor_peak count ALGORITHMIC flops: 8 per complex multiply-add (SURVEY.md 8(d)); "
+                              "with gemm_products = 3 the GEMM stages execute 6, so a fraction above 0.75 x (GEMM share) is not "
+                              "tensor-pipe utilisation -- that is roofline.dmma_pipe_frac",
            "roofline": roofline, "e2e": e2e, "gpu_launches": int(gpu_launches), "clocks": clocks}
 
     if rank == 0 and not args.no_extras:
