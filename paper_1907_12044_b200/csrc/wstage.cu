@@ -233,6 +233,7 @@ constexpr int WQ_SMEM = 227 * 1024 - 64;
 __global__ void __launch_bounds__(WQ_THREADS, 1) wstage_quad_kernel(WStageParams p, int ntile, int npanels, int forced) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ int s_next, s_nnz;
+  __shared__ __align__(8) unsigned long long s_bar;       // completion barrier of the bulk panel copies
   c128 *tile = reinterpret_cast<c128 *>(smem_raw);                        // [ncols][YT]
   const int tile_elems = p.ncols * YT;
   int *scnt = reinterpret_cast<int *>(smem_raw + (size_t)tile_elems * 16);    // [nrows], in sorted order
@@ -247,6 +248,12 @@ __global__ void __launch_bounds__(WQ_THREADS, 1) wstage_quad_kernel(WStageParams
     if (lane == 0) s_nnz = t;
   }
   for (int i = threadIdx.x; i < p.nrows; i += WQ_THREADS) { const int r = __ldg(p.order + i); srow[i] = r; scnt[i] = __ldg(p.cnt + r); }
+  const unsigned bar_sa = (unsigned)__cvta_generic_to_shared(&s_bar);
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(bar_sa));
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  unsigned bar_phase = 0;
   __syncthreads();
   if (!forced && s_nnz < 8 * p.nrows) return;          // short rows: the row-at-a-time kernel does the stage
   const int ngroups = (p.nrows + 3) / 4;
@@ -262,15 +269,33 @@ __global__ void __launch_bounds__(WQ_THREADS, 1) wstage_quad_kernel(WStageParams
     const c128 *in = p.in + a * p.in_bs;
     __syncthreads();
     if (threadIdx.x == 0) s_next = g0;
-    for (int e = threadIdx.x; e < tile_elems; e += WQ_THREADS) {
-      const int c = e / YT, yy = e % YT;
-      const bool ok = (y0 + yy) < p.Mr;
-      const c128 *src = ok ? in + (long long)c * p.Mr + y0 + yy : in;
-      unsigned sa = (unsigned)__cvta_generic_to_shared(tile + e);
-      int sz = ok ? 16 : 0;
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(src), "r"(sz));
+    if (y0 + YT <= p.Mr) {
+      // whole tile in range: one 1 KB bulk copy per panel row (TMA engine), completion on the mbarrier
+      asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // earlier reads of the panel before async writes
+      if (threadIdx.x == 0)
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar_sa), "r"((unsigned)(p.ncols * YT * 16)) : "memory");
+      for (int c = threadIdx.x; c < p.ncols; c += WQ_THREADS) {
+        const unsigned sa = (unsigned)__cvta_generic_to_shared(tile + (size_t)c * YT);
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+                     ::"r"(sa), "l"(in + (long long)c * p.Mr + y0), "r"((unsigned)(YT * 16)), "r"(bar_sa) : "memory");
+      }
+      unsigned ok;
+      do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+                     : "=r"(ok) : "r"(bar_sa), "r"(bar_phase) : "memory");
+      } while (!ok);
+      bar_phase ^= 1u;
+    } else {
+      for (int e = threadIdx.x; e < tile_elems; e += WQ_THREADS) {
+        const int c = e / YT, yy = e % YT;
+        const bool ok = (y0 + yy) < p.Mr;
+        const c128 *src = ok ? in + (long long)c * p.Mr + y0 + yy : in;
+        unsigned sa = (unsigned)__cvta_generic_to_shared(tile + e);
+        int sz = ok ? 16 : 0;
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sa), "l"(src), "r"(sz));
+      }
+      asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::);
     }
-    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::);
     __syncthreads();
     c128 *out = p.out + a * p.o_bs;
     for (;;) {
