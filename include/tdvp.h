@@ -239,6 +239,18 @@ int tdvp_profile_read(double *ms, long long *count);
    launches replayed from a captured CUDA graph are counted when the graph is launched). */
 long long tdvp_launch_count(void);
 
+/* Environment variables (diagnostic switches; none of them changes what is computed beyond rounding):
+     TDVP_ZGEMM_4M=1          complex GEMM from four real products instead of three (tdvp_set_gemm_products),
+                              read once when the library configures its kernels;
+     TDVP_ZGEMM_SPLIT_COST=x  cost, in k-tile units, that the stream-K grid model charges for cutting
+                              tiles (default 5), read once;
+     TDVP_LANCZOS_UNFUSED=1   separate dot / update kernels instead of the fused cooperative kernel of a
+                              Lanczos iteration, read once;
+     TDVP_NO_FSAL=1           tdvp_step_mu recomputes stage 1 instead of reusing stage 7 of the step
+                              before (bit-identical by construction; read at every step);
+     TDVP_CMF_QUEUES=n        side queues of the CMF local propagation (1..8, default 4; results are
+                              bit-identical for any n), read when a handle first runs tdvp_step_mu_cmf. */
+
 #ifdef __cplusplus
 }
 #endif
