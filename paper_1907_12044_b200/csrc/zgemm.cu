@@ -50,6 +50,7 @@ struct KParams {
   int batch_inner;
   long long c_bsi, c_bso;
   int a_batched_i, a_batched_o, b_batched_i, b_batched_o;   // 0: operand shared by the batch (coordinate 0)
+  int a5, b5;           // K-major operand has a 5-D map (k-group as its own dimension): one TMA per k-tile
   unsigned a_sign;      // 0x80000000 if conjA
   unsigned b_sign;      // 0x80000000 if conjB
   int tiles_m, tiles_n, ktiles;
@@ -98,6 +99,13 @@ __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap *tm,
   asm volatile(
       "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];\n"
       ::"r"(dst), "l"(reinterpret_cast<unsigned long long>(tm)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+      : "memory");
+}
+
+__device__ __forceinline__ void tma_load_5d(unsigned dst, const CUtensorMap *tm, unsigned bar, int c0, int c1, int c2, int c3, int c4) {
+  asm volatile(
+      "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];\n"
+      ::"r"(dst), "l"(reinterpret_cast<unsigned long long>(tm)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
       : "memory");
 }
 
@@ -173,14 +181,20 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
     const unsigned dA = smem_base + p_slot * (2 * TILE_BYTES), dB = dA + TILE_BYTES;
     mbar_expect_tx(bar, (A_KMAJOR ? TILE_K_BYTES : TILE_MN_BYTES) + (B_KMAJOR ? TILE_K_BYTES : TILE_MN_BYTES));
     if (A_KMAJOR) {
+      if (p.a5) tma_load_5d(dA, &tmA, bar, 0, l_m0, k0 >> 2, l_abi, l_abo);
+      else {
 #pragma unroll
-      for (int g = 0; g < KG; g++) tma_load_4d(dA + g * (BM * 64), &tmA, bar, 2 * (k0 + 4 * g), l_m0, l_abi, l_abo);
+        for (int g = 0; g < KG; g++) tma_load_4d(dA + g * (BM * 64), &tmA, bar, 2 * (k0 + 4 * g), l_m0, l_abi, l_abo);
+      }
     } else {
       tma_load_4d(dA, &tmA, bar, 2 * l_m0, k0, l_abi, l_abo);
     }
     if (B_KMAJOR) {
+      if (p.b5) tma_load_5d(dB, &tmB, bar, 0, l_n0, k0 >> 2, l_bbi, l_bbo);
+      else {
 #pragma unroll
-      for (int g = 0; g < KG; g++) tma_load_4d(dB + g * (BN * 64), &tmB, bar, 2 * (k0 + 4 * g), l_n0, l_bbi, l_bbo);
+        for (int g = 0; g < KG; g++) tma_load_4d(dB + g * (BN * 64), &tmB, bar, 2 * (k0 + 4 * g), l_n0, l_bbi, l_bbo);
+      }
     } else {
       tma_load_4d(dB, &tmB, bar, 2 * l_n0, k0, l_bbi, l_bbo);
     }
@@ -447,6 +461,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeTiledFn g_encode = nullptr;
+int g_no_5d = 0;       // set when the driver rejects a 5-D map once (or by TDVP_ZGEMM_NO_5D=1)
 
 // Tensor map of one operand seen as doubles.  K-major (unit stride along k): dims (2K, rows, bi, bo),
 // box (8 doubles = 4 complex, 64 rows); MN-major (unit stride along m/n): dims (2*rows, K, bi, bo),
@@ -475,6 +490,33 @@ bool encode_operand(CUtensorMap *tm, const c128 *base, bool kmajor, long long ro
             (unsigned long long)strides[2], box[0], box[1]);
     return false;
   }
+  return true;
+}
+
+// K-major operand with K a multiple of 4: dims (8 doubles of a k-group, rows, k-groups, bi, bo), box
+// (8, 64, KG, 1, 1) -- written to shared memory as [k-group][row][4 complex], the layout the four
+// separate boxes of the 4-D map produce, with one TMA instruction.  Returns false if the driver
+// rejects the map (the caller then keeps the 4-D one).
+bool encode_operand_5d(CUtensorMap *tm, const c128 *base, long long rows, long long K, long long ld /*complex*/,
+                       int nbi, long long bsi, int nbo, long long bso) {
+  if (K % 4 != 0 || g_no_5d) return false;
+  cuuint64_t dims[5], strides[4];
+  cuuint32_t box[5] = {8, (cuuint32_t)BM, (cuuint32_t)KG, 1, 1}, estr[5] = {1, 1, 1, 1, 1};
+  dims[0] = 8; dims[1] = (cuuint64_t)rows; dims[2] = (cuuint64_t)(K / 4);
+  if (rows == 1) ld = K;
+  strides[0] = (cuuint64_t)ld * 16;      // rows
+  strides[1] = 64;                       // k-groups
+  const bool bi = nbi > 1 && bsi != 0, bo = nbo > 1 && bso != 0;
+  dims[3] = bi ? nbi : 1; dims[4] = bo ? nbo : 1;
+  const cuuint64_t dummy = strides[0] * dims[1];
+  strides[2] = bi ? (cuuint64_t)bsi * 16 : dummy;
+  strides[3] = bo ? (cuuint64_t)bso * 16 : dummy;
+  CUtensorMap tmp;
+  CUresult r = g_encode(&tmp, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, const_cast<c128 *>(base), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { g_no_5d = 1; return false; }
+  *tm = tmp;
   return true;
 }
 
@@ -530,6 +572,7 @@ void zgemm_configure() {
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm4, zgemm_kernel<true, true, true, false>, NTHREADS, SMEM_BYTES);
   if (per_sm4 < per_sm) per_sm = per_sm4;
   if (const char *es = getenv("TDVP_ZGEMM_SPLIT_COST")) g_split_cost = atof(es);
+  if (const char *e5 = getenv("TDVP_ZGEMM_NO_5D")) g_no_5d = e5[0] == '1';
   const char *e4 = getenv("TDVP_ZGEMM_4M");
   if (e4 && e4[0] == '1') g_mode3m = 0;
   if (per_sm < 1) per_sm = 1;
@@ -586,6 +629,8 @@ void zgemm(cudaStream_t st, const ZGemm &p, c128 *) {
       !encode_operand(&tb, p.B, bk, p.N, p.K, bk ? p.b_ns : p.b_ks, p.batch_inner, p.b_bsi, p.batch_outer, p.b_bso))
     abort();
   KParams kp;
+  kp.a5 = ak && encode_operand_5d(&ta, p.A, p.M, p.K, p.a_ms, p.batch_inner, p.a_bsi, p.batch_outer, p.a_bso) ? 1 : 0;
+  kp.b5 = bk && encode_operand_5d(&tb, p.B, p.N, p.K, p.b_ns, p.batch_inner, p.b_bsi, p.batch_outer, p.b_bso) ? 1 : 0;
   kp.C = p.C;
   kp.M = p.M; kp.N = p.N; kp.K = p.K;
   kp.ldc = p.ldc;
