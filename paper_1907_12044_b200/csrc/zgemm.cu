@@ -372,7 +372,9 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
     const int nc = j1 - j0 + 1, me = cta - j0;
     if (tid == 0) while (ld_acquire(p.cnt + j1) < nc) {}
     __syncthreads();
-    const int chunk = (BM * BN + nc - 1) / nc;
+    // slices are whole groups of 128 elements, so that element e of a slice belongs to thread e % 128
+    // of the tile's thread-native layout whoever reduces it: the row / column decode is per thread
+    const int chunk = ((BM * BN / NTHREADS + nc - 1) / nc) * NTHREADS;
     const int e_end = (me + 1) * chunk < BM * BN ? (me + 1) * chunk : BM * BN;
     const int bz = t / tiles_mn, tr = t - bz * tiles_mn;
     const int m0 = (tr / p.tiles_n) * BM, n0 = (tr % p.tiles_n) * BN;
@@ -382,6 +384,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
     const int j0u0 = j0 * p.upc_base + (j0 < p.upc_rem ? j0 : p.upc_rem);
     const c128 *s0 = p.slots + (size_t)(2 * j0 + (j0u0 == tu0 ? 0 : 1)) * (BM * BN);
     const c128 *s1 = p.slots + (size_t)(2 * (j0 + 1)) * (BM * BN);
+    const int fm0 = m0 + (warp / (BN / WN)) * WM + (lane >> 2), fn0 = n0 + (warp % (BN / WN)) * WN + 2 * (lane & 3);
     // four elements per thread and pass, all their loads in flight together (the fix-up is a chain
     // of L2 round trips: one element at a time it cost ~0.4 us per element and thread)
     constexpr int FU = 4;
@@ -406,11 +409,9 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
       for (int u = 0; u < FU; u++) {
         const int e = eb + u * NTHREADS;
         if (e >= e_end) continue;
-        const int q = e >> 7, tx = e & 127;
+        const int q = e >> 7;                               // e & 127 == tid
         const int i = q >> 3, jb = (q >> 1) & 3, h = q & 1;
-        const int wr = tx >> 5, ln = tx & 31;
-        const int m = m0 + (wr / (BN / WN)) * WM + i * 8 + (ln >> 2);
-        const int n = n0 + (wr % (BN / WN)) * WN + jb * 8 + 2 * (ln & 3) + h;
+        const int m = fm0 + i * 8, n = fn0 + jb * 8 + h;
         if (m < p.M && n < p.N) Cb[(long long)m * p.ldc + n] = make_double2(sx[u], sy[u]);
       }
     }
