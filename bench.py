@@ -47,6 +47,123 @@ def gemm_stage_flops(M, d=D_PHYS, Dw=D_W):
     return 8.0 * M ** 3 * Dw * d
 
 
+def heff_executed_flops(M, products, d=D_PHYS, Dw=D_W, nnz=NNZ):
+    """Flops the kernels EXECUTE for one apply: the GEMM stages form a complex multiply-add from
+    `products` real DMMA products (2 flops each: 6 or 8 per complex multiply-add), the W stage from 4 DFMA."""
+    return 2.0 * products * 2.0 * M ** 3 * Dw * d + 8.0 * M ** 2 * nnz
+
+
+def site_apply_flops(Ml, Mr, d, Dl, Dr, nnz):
+    """(GEMM-stage, W-stage) algorithmic flops of one H_eff apply / environment update of a site
+    (8 flops per complex multiply-add)."""
+    return 8.0 * (Ml * Ml * Dl * d * Mr + Ml * d * Dr * Mr * Mr), 8.0 * Ml * Mr * nnz
+
+
+def qr_flops(rows, cols):
+    """Householder QR of a complex rows x cols matrix plus forming Q: 2 x (8 rows cols^2 - 8/3 cols^3)."""
+    return 2.0 * (8.0 * rows * cols * cols - 8.0 / 3.0 * cols ** 3)
+
+
+def ps_step_flops(mpo, mps, k):
+    """Algorithmic flops of one TDVP-PS step (Eq. 42) of THIS chain, from its actual M_i, D_W,i and
+    nnz(W_i), with the formula of SURVEY.md 8(a) a8: (2N-1) k H_eff applies, 2(N-1) environment updates,
+    2(N-1) k bond applies, 2(N-1) QR gauge moves + absorbs, and the Krylov vector work (two Gram-Schmidt
+    passes over j+1 vectors per iteration + the final combination).  Returns (gemm, wstage, other)."""
+    n = len(mps)
+    gemm = wst = other = 0.0
+    for i in range(n):
+        Ml, d, Mr = mps[i].shape
+        Dl, Dr = mpo[i].shape[0], mpo[i].shape[3]
+        g, w = site_apply_flops(Ml, Mr, d, Dl, Dr, int(np.count_nonzero(mpo[i])))
+        n_exp = 1 if i == n - 1 else 2
+        gemm += n_exp * k * g
+        wst += n_exp * k * w
+        nvec = Ml * d * Mr
+        other += n_exp * (8.0 * nvec * (k * (k + 1) + k))          # 2 passes x (dot + axpy) x sum_j (j+1), + combine
+        if i < n - 1:                                             # forward QR + left environment, Eq. 9, 30-32
+            gemm += g
+            wst += w
+            other += qr_flops(Ml * d, Mr)
+        if i > 0:                                                 # backward RQ + right environment
+            gemm += g
+            wst += w
+            other += qr_flops(d * Mr, Ml)
+            gemm += 2 * k * 8.0 * (Ml * Ml * Dl * Ml + Ml * Dl * Ml * Ml)   # bond applies of bond i, both sweeps (Eq. 44)
+            gemm += 2 * 8.0 * Ml * Ml * d * Mr                                # absorbs C = D B, C = A D
+            other += 2 * (8.0 * Ml * Ml * (k * (k + 1) + k))
+    return gemm, wst, other
+
+
+def cmf_step_flops(mpo, mps, k, n_sub):
+    """Algorithmic flops of one second-order CMF step: two mean-field builds (N-1 left
+    and N-1 right environments, N-1 centre-form GEMMs; SVDs counted as QR + 8 Ml^3 x 10 sweeps of Jacobi),
+    local RK4 propagation with ceil(n_sub/2) + n_sub sub-steps x 4 right-hand sides per site (one H_eff apply +
+    four (rows x Jr x Jr) GEMMs each), and two Krylov exponentials at the last site."""
+    n = len(mps)
+    gemm = wst = other = 0.0
+    nrhs = 4 * ((n_sub + 1) // 2 + n_sub)
+    for i in range(n):
+        Ml, d, Mr = mps[i].shape
+        Dl, Dr = mpo[i].shape[0], mpo[i].shape[3]
+        g, w = site_apply_flops(Ml, Mr, d, Dl, Dr, int(np.count_nonzero(mpo[i])))
+        if i < n - 1:
+            gemm += 2 * g + nrhs * (g + 4 * 8.0 * Ml * d * Mr * Mr)
+            wst += 2 * w + nrhs * w
+        else:
+            gemm += 2 * k * g
+            wst += 2 * k * w
+        if i > 0:
+            gemm += 2 * (g + 8.0 * Ml * Ml * d * Mr)
+            wst += 2 * w
+            other += 2 * (qr_flops(d * Mr, Ml) + 80.0 * Ml ** 3)
+    return gemm, wst, other
+
+
+def time_cublas_fp64(torch, seconds=4.0):
+    """cuBLAS FP64 ceilings of THIS box, measured in this run (SURVEY.md 8(d) "Peaks to divide by"): they are
+    DENOMINATORS only -- torch.matmul is never on the hot path.  ZGEMM 4096^3 (8 flops per complex multiply-add)
+    and DGEMM 8192^3, best of 10 (burst) and back to back for `seconds` (sustained)."""
+    out = {}
+    for name, n, dtype, flops in (("zgemm", 4096, torch.complex128, 8.0 * 4096 ** 3), ("dgemm", 8192, torch.float64, 2.0 * 8192 ** 3)):
+        a = torch.randn(n, n, dtype=dtype, device="cuda")
+        b = torch.randn(n, n, dtype=dtype, device="cuda")
+        c = torch.empty_like(a)
+        for _ in range(2):
+            torch.matmul(a, b, out=c)
+        best = 1e30
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(10):
+            e0.record(); torch.matmul(a, b, out=c); e1.record(); torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        reps = max(3, int(seconds * 1e3 / best))
+        e0.record()
+        for _ in range(reps):
+            torch.matmul(a, b, out=c)
+        e1.record(); torch.cuda.synchronize()
+        out[name] = {"n": n, "burst_tflops": flops / (best * 1e-3) / 1e12,
+                     "sustained_tflops": flops * reps / (e0.elapsed_time(e1) * 1e-3) / 1e12, "sustained_s": e0.elapsed_time(e1) * 1e-3}
+        del a, b, c
+    torch.cuda.empty_cache()
+    return out
+
+
+def committed_traffic(kernel, M):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` at bond dimension M from the
+    committed ncu --set full summary profiles/kernel_traffic.csv (columns: kernel, M, dram_bytes_per_launch,
+    capture); None if there is no such row.  bench.py never runs under ncu, so this is the only place the
+    number can come from; the csv names the capture it was read from."""
+    path = os.path.join(ROOT, "profiles", "kernel_traffic.csv")
+    try:
+        rows = [l.strip().split(",") for l in open(path) if l.strip() and not l.startswith("#")]
+    except OSError:
+        return None, None
+    best = (None, None)
+    for r in rows[1:]:
+        if len(r) >= 4 and r[0] == kernel and int(r[1]) == M:
+            best = (float(r[2]), r[3])                  # later rows (later rounds) win
+    return best
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -191,8 +308,12 @@ def sweep_point(torch, T, M, peak_tflops):
     ms_env = e0.elapsed_time(e1)
     ctx.close()
     aps = n / (ms * 1e-3)
-    return {"M": M, "applies_per_s": aps, "us_per_apply": 1e3 * ms / n, "tflops": aps * heff_flops(M) / 1e12,
-            "frac_fp64_tensor_peak": aps * heff_flops(M) / 1e12 / peak_tflops,
+    products = T.tdvp_get_gemm_products()
+    # effective_tflops counts ALGORITHMIC flops (8 per complex multiply-add) and may exceed the pipe's peak when
+    # the GEMM stages run the 3-product form; frac_fp64_tensor_peak counts the flops actually EXECUTED: <= 1
+    return {"M": M, "applies_per_s": aps, "us_per_apply": 1e3 * ms / n, "effective_tflops": aps * heff_flops(M) / 1e12,
+            "executed_tflops": aps * heff_executed_flops(M, products) / 1e12,
+            "frac_fp64_tensor_peak": aps * heff_executed_flops(M, products) / 1e12 / peak_tflops,
             "env_updates_per_s": n / (ms_env * 1e-3), "input_sets": n_sets}
 
 
@@ -287,6 +408,7 @@ def run_ours(args):
     flops_per_launch = gemm_stage_flops(M)             # each of the 2 GEMM launches of an apply
     achieved = flops_per_launch / (zg_ms / max(zg_n, 1) * 1e-3) / 1e12 if zg_n else None
     products = T.tdvp_get_gemm_products()
+    traffic, traffic_src = committed_traffic("zgemm_kernel", M)
     roofline = {"bound": "tensor", "kernel": "zgemm_kernel (FP64 DMMA m8n8k4, complex128)",
                 "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": (achieved / peak) if achieved else None,
@@ -295,11 +417,11 @@ def run_ours(args):
                 # complex multiply-add), so the share of the DMMA pipe it keeps busy is frac * products / 4
                 "gemm_products": products,
                 "dmma_pipe_frac": (achieved / peak * products / 4.0) if achieved else None,
-                # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture in
-                # profiles/r01d_summary.md (mean of the stage-1 and stage-3 launches), M = 128 only
-                "traffic": 49.5e6 if M == 128 else None,
-                "peak_source": "tdvp_probe_fp64_tensor_peak: DMMA m8n8k4 issue rate measured in this run "
-                               "(MEASURED_PEAKS.json has no FP64 figure; cuBLAS ZGEMM 4096^3 measured 36.85 TFLOP/s)",
+                # dram__bytes_read.sum + dram__bytes_write.sum per launch, read from the committed ncu --set full
+                # summary (profiles/kernel_traffic.csv names the capture); null if no capture of this kernel at this M
+                "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": "tdvp_probe_fp64_tensor_peak: DMMA m8n8k4 issue rate measured in this run (MEASURED_PEAKS.json has "
+                               "no FP64 figure); the cuBLAS ZGEMM / DGEMM rates of this box, measured in this run, are beside it",
                 "flops_per_launch": flops_per_launch, "avg_launch_us": 1e3 * zg_ms / max(zg_n, 1), "launches": zg_n,
                 "share_of_step": {"zgemm": zg_ms / ms_total, "wstage": ws_ms / ms_total},
                 "wstage": {"bound": "hbm", "note": "algorithmic bytes = one read of T1 + one write of T2; ncu shows the kernel bound by "
@@ -349,14 +471,35 @@ def run_ours(args):
            "config": {"workload": WORKLOAD, "applies_per_step": APPLIES_PER_STEP, "input_sets": N_SETS,
                       "l2": "inputs rotate over %d resident sets (188 MB > 126 MB L2); T1/T2 intermediates 52 MB each" % N_SETS,
                       "multi_gpu": "replicas only (SURVEY.md 8(e))", "seed": "1000+M+7919*set"},
-           "us_per_apply": 1e3 * ms_total / n_applies, "tflops": value / world * heff_flops(M) / 1e12,
-           "frac_fp64_tensor_peak": value / world * heff_flops(M) / 1e12 / peak,
-           "flop_convention": "tflops / frac_fp64_tensor_peak count ALGORITHMIC flops: 8 per complex multiply-add (SURVEY.md 8(d)); "
-                              "with gemm_products = 3 the GEMM stages execute 6, so a fraction above 0.75 x (GEMM share) is not "
-                              "tensor-pipe utilisation -- that is roofline.dmma_pipe_frac",
+           "us_per_apply": 1e3 * ms_total / n_applies,
+           "effective_tflops": value / world * heff_flops(M) / 1e12,
+           "executed_tflops": value / world * heff_executed_flops(M, products) / 1e12,
+           "frac_fp64_tensor_peak": value / world * heff_executed_flops(M, products) / 1e12 / peak,
+           "flop_convention": "frac_fp64_tensor_peak divides the flops the kernels EXECUTE (GEMM stages: 2 x gemm_products per complex "
+                              "multiply-add, 6 with the default 3-product form; W stage: 8) by the measured DMMA peak: pipe utilisation, "
+                              "never above 1.  effective_tflops counts ALGORITHMIC flops (8 per complex multiply-add, SURVEY.md 8(d)), as "
+                              "does roofline.achieved (the contract's definition); roofline.dmma_pipe_frac is its executed counterpart",
            "roofline": roofline, "e2e": e2e, "gpu_launches": int(gpu_launches), "clocks": clocks}
 
     if rank == 0 and not args.no_extras:
+        # cuBLAS FP64 ceilings of this box (denominators only)
+        cub = time_cublas_fp64(torch)
+        out["roofline"]["peak_cublas_zgemm"] = cub["zgemm"]
+        out["roofline"]["peak_cublas_dgemm"] = cub["dgemm"]
+        # the same resident-input loop with the complex product from FOUR real DMMA products (reading c15)
+        sets = make_sets(torch, M, N_SETS)
+        ctx = T.tdvp_create_context()
+        T.tdvp_set_gemm_products(4)
+        try:
+            time_applies(torch, T, ctx, sets, APPLIES_PER_STEP)
+            ms4 = time_applies(torch, T, ctx, sets, 4 * APPLIES_PER_STEP)
+        finally:
+            T.tdvp_set_gemm_products(3)
+        out["gemm_products_4"] = {"applies_per_s": 4 * APPLIES_PER_STEP / (ms4 * 1e-3), "us_per_apply": 1e3 * ms4 / (4 * APPLIES_PER_STEP),
+                                  "frac_fp64_tensor_peak": 4 * APPLIES_PER_STEP / (ms4 * 1e-3) * heff_executed_flops(M, 4) / 1e12 / peak}
+        ctx.close()
+        del sets
+        torch.cuda.empty_cache()
         # what non-tensor instructions cost the FP64 tensor pipe: TFLOP/s with F
         # integer instructions issued after every DMMA, two CTAs of four warps per SM
         out["dmma_issue_probe_tflops"] = {str(f): T.tdvp_probe_dmma_issue(f, 4000) for f in (0, 1, 2, 4, 8, 16)}
@@ -379,8 +522,15 @@ def run_ours(args):
         ch.tdvp_sync()
         torch.cuda.synchronize()
         nrm, en = ch.tdvp_norm_energy()
+        fg, fw, fo = ps_step_flops(mpo, mps, cfg.krylov_dim)
+        ps_ms = e0.elapsed_time(e1) / n_ps
         out["ps_step"] = {"workload": "configs[3]: FMO-like chain, 71 sites, M=128, D_W<=9 (real MPO), k=10, dt=5 fs, CUDA graph",
-                          "ms_per_step": e0.elapsed_time(e1) / n_ps, "steps_timed": n_ps,
+                          "ms_per_step": ps_ms, "steps_timed": n_ps,
+                          # algorithmic flops of one step of THIS chain (its M_i, D_W,i, nnz(W_i))
+                          "flops": {"gemm": fg, "wstage": fw, "qr_and_vectors": fo, "total": fg + fw + fo},
+                          "effective_tflops": (fg + fw + fo) / (ps_ms * 1e-3) / 1e12,
+                          "frac_fp64_tensor_peak": (products / 4.0 * fg + fw + fo) / (ps_ms * 1e-3) / 1e12 / peak,
+                          "ms_at_peak": (products / 4.0 * fg + fw + fo) / (peak * 1e12) * 1e3,
                           "launches_per_step": (T.tdvp_launch_count() - l0) // n_ps,
                           "norm_sq": nrm, "energy": en, "populations": ch.tdvp_populations(0).tolist()}
         ch.close()
@@ -446,9 +596,13 @@ def run_ours(args):
         ph = T.tdvp_profile_read()
         T.tdvp_profile_enable(False)
         nrm, en = ch.tdvp_norm_energy()
+        cg, cw, co = cmf_step_flops(mpo, mps, cfg.krylov_dim, NSUB_CMF)
+        cmf_ms = e0.elapsed_time(e1) / n_cmf
         out["mu_cmf_step"] = {"workload": "configs[3] chain, 71 sites, M=128: one second-order CMF step of tau = %g fs (%d RK4 sub-steps per "
                                           "site, Krylov dimension %d at the last site; mean fields built twice per step)" % (TAU_CMF, NSUB_CMF, cfg.krylov_dim),
-                              "ms_per_step": e0.elapsed_time(e1) / n_cmf, "steps_timed": n_cmf, "ms_per_fs": e0.elapsed_time(e1) / n_cmf / TAU_CMF,
+                              "ms_per_step": cmf_ms, "steps_timed": n_cmf, "ms_per_fs": cmf_ms / TAU_CMF,
+                              "flops": {"gemm": cg, "wstage": cw, "svd_qr": co, "total": cg + cw + co},
+                              "frac_fp64_tensor_peak": (products / 4.0 * cg + cw + co) / (cmf_ms * 1e-3) / 1e12 / peak,
                               "launches_per_step": (T.tdvp_launch_count() - l0) // n_cmf, "norm_sq": nrm, "energy": en,
                               "phase_ms_per_step": {k: round(v[0] / n_cmf, 3) for k, v in ph.items()}}
         out["mu_step"]["ms_per_fs"] = out["mu_step"]["ms_per_step"] / H_MU

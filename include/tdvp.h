@@ -20,7 +20,12 @@
  *
  * Errors: every int-returning call returns TDVP_OK (0) or a negative TDVP_E* code and stores a
  * message retrievable with tdvp_last_error(h) (h may be NULL: the last error of the calling
- * thread's handle-less calls).  No exceptions or signals cross the boundary.
+ * thread's handle-less calls).  No exceptions or signals cross the boundary.  DEVICE pointers to
+ * complex data must be 16-byte aligned (TDVP_EINVAL from the call that enqueues the first GEMM on
+ * them).  Conditions only a kernel can detect (a bond SVD that ran out of Jacobi sweeps) are
+ * recorded on the device and returned as TDVP_ESTATE by the NEXT blocking call on that handle
+ * (tdvp_sync, tdvp_populations, tdvp_observe, tdvp_norm_energy, tdvp_get_mps, tdvp_mu_derivative,
+ * tdvp_step_mu with err_est), which also clears them.
  */
 #ifndef TDVP_H
 #define TDVP_H
@@ -131,7 +136,8 @@ int tdvp_expm_bond(tdvp_handle *h, int Ml, int Mr, int Dw,
 /* QR gauge move (Eq. 9), Householder, on the device.
    side = 0: C[Ml,d,Mr] viewed as (Ml*d) x Mr = Q D,  Q[Ml,d,Mr] left-canonical (Eq. 7), D[Mr,Mr]
    side = 1: C viewed as Ml x (d*Mr) = D Q,  Q[Ml,d,Mr] right-canonical (Eq. 8), D[Ml,Ml]
-   Requires Ml*d >= Mr (side 0) or d*Mr >= Ml (side 1).  Q and D are unique only up to a unitary
+   Requires Ml*d >= Mr (side 0) or d*Mr >= Ml (side 1), and that tall side <= 12800 (TDVP_EINVAL
+   otherwise; the same limit M_i * d_i <= 12800 holds in tdvp_create).  Q and D are unique only up to a unitary
    on the bond (the paper does not distinguish QR from RQ); the product is exact. */
 int tdvp_qr_gauge(tdvp_handle *h, int side, int Ml, int d, int Mr,
                   const tdvp_c128 *C /*DEVICE*/, tdvp_c128 *Q /*DEVICE*/, tdvp_c128 *D /*DEVICE*/);
@@ -222,17 +228,18 @@ int tdvp_probe_dmma_issue(int fillers, int iters, double *tflops /*HOST*/);
      products = 3 (default): X1 = Ar Br, X2 = Ai Bi, X3 = (Ar + Ai)(Br + Bi); C = (X1 - X2) + i (X3 - X1 - X2)
                  -- 25 % fewer DMMAs; error bounded normwise (relative to |A||B|), not per component;
      products = 4: Cr = Ar Br - Ai Bi, Ci = Ar Bi + Ai Br.
-   Process-wide (every handle and stream), takes effect at the next launch; not to be changed while
-   a captured step graph exists (the graph keeps the kernels it was captured with).  The
+   Process-wide (every handle and stream; an atomic switch, safe to flip from any host thread), takes
+   effect at the next launch; a captured step graph keeps the kernels it was captured with.  The
    environment variable TDVP_ZGEMM_4M=1 selects 4 at load time.  Returns 0, or TDVP_EINVAL. */
 int tdvp_set_gemm_products(int products);
 int tdvp_get_gemm_products(void);
 /* Phase profiler: when enabled, launches of the dominant kernel classes are bracketed by CUDA events
    on the launching stream (not inside a captured step).  tdvp_profile_read blocks on the device,
    returns the summed elapsed milliseconds and bracket counts per phase since the last read and
-   resets them.  Phases: 0 complex GEMM (DMMA), 1 split-K reduce, 2 MPO (W) stage, 3 Lanczos /
-   vector kernels, 4 QR, 5 SVD.  ms, count: HOST arrays of TDVP_PROFILE_PHASES entries. */
-#define TDVP_PROFILE_PHASES 6
+   resets them.  Phases: 0 complex GEMM (DMMA), 1 MPO (W) stage, 2 Lanczos / vector kernels, 3 QR,
+   4 SVD.  ms, count: HOST arrays of TDVP_PROFILE_PHASES entries.  The profiler state is process-wide
+   (one record list for all handles, guarded by a mutex; safe to use from several host threads). */
+#define TDVP_PROFILE_PHASES 5
 int tdvp_profile_enable(int on);
 int tdvp_profile_read(double *ms, long long *count);
 /* Number of kernel launches this library has enqueued since load (for bench.py's gpu_launches;
@@ -249,7 +256,10 @@ long long tdvp_launch_count(void);
      TDVP_NO_FSAL=1           tdvp_step_mu recomputes stage 1 instead of reusing stage 7 of the step
                               before (bit-identical by construction; read at every step);
      TDVP_CMF_QUEUES=n        side queues of the CMF local propagation (1..8, default 4; results are
-                              bit-identical for any n), read when a handle first runs tdvp_step_mu_cmf. */
+                              bit-identical for any n), read when a handle first runs tdvp_step_mu_cmf;
+     TDVP_SVD_MAX_SWEEPS=n    Jacobi sweeps a bond SVD may use (1..40, default 40; lowering it forces the
+                              TDVP_ESTATE "did not converge" report: used by the error-path test), read at
+                              every SVD. */
 
 #ifdef __cplusplus
 }

@@ -144,6 +144,9 @@ class Context:
         self._h = c_void_p()
         _check(_lib.tdvp_create_context(byref(self._h), byref(options) if options else None, _stream_ptr(stream)))
 
+    def tdvp_sync(self):
+        _check(_lib.tdvp_sync(self._h), self._h)
+
     def close(self):
         if self._h:
             _lib.tdvp_destroy(self._h)
@@ -266,7 +269,7 @@ def tdvp_probe_fp64_tensor_peak(iters=20000) -> float:
     return t.value
 
 
-PROFILE_PHASES = ("zgemm", "splitk_reduce", "wstage", "vector", "qr", "svd")
+PROFILE_PHASES = ("zgemm", "wstage", "vector", "qr", "svd")
 
 
 def tdvp_probe_dmma_issue(fillers, iters=4000) -> float:

@@ -10,37 +10,80 @@ thread_local long long *g_capture_tally = nullptr;
 static thread_local std::string g_null_err;
 
 // ---- phase profiler ---------------------------------------------------------------------------
-bool g_prof_on = false;
-int g_prof_depth = 0;
+// Process-wide measurement state (include/tdvp.h says so): the record list is guarded by a mutex,
+// the on/off switch is atomic, the nesting depth belongs to the enqueueing host thread.
+std::atomic<bool> g_prof_on{false};
+thread_local int g_prof_depth = 0;
 namespace {
-struct ProfRec { cudaEvent_t e0, e1; int phase; };
+struct ProfRec { cudaEvent_t e0, e1; int phase; bool closed; };
+std::mutex g_prof_mu;
 std::vector<ProfRec> g_prof_recs;
 size_t g_prof_used = 0;
 constexpr size_t PROF_MAX = 1 << 16;
 }
-void prof_begin(cudaStream_t st, int phase) {
-  if (g_prof_used >= PROF_MAX) return;
+int prof_begin(cudaStream_t st, int phase) {
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  if (g_prof_used >= PROF_MAX) return -1;
   if (g_prof_used == g_prof_recs.size()) {
-    ProfRec r; cudaEventCreate(&r.e0); cudaEventCreate(&r.e1); r.phase = phase;
+    ProfRec r; r.phase = phase; r.closed = false;
+    if (cudaEventCreate(&r.e0) != cudaSuccess || cudaEventCreate(&r.e1) != cudaSuccess) { cudaGetLastError(); return -1; }
     g_prof_recs.push_back(r);
   }
-  g_prof_recs[g_prof_used].phase = phase;
-  cudaEventRecord(g_prof_recs[g_prof_used].e0, st);
+  const int rec = (int)g_prof_used++;
+  g_prof_recs[rec].phase = phase; g_prof_recs[rec].closed = false;
+  cudaEventRecord(g_prof_recs[rec].e0, st);
+  return rec;
 }
-void prof_end(cudaStream_t st) {
-  if (g_prof_used >= PROF_MAX) return;
-  cudaEventRecord(g_prof_recs[g_prof_used].e1, st);
-  g_prof_used++;
+void prof_end(cudaStream_t st, int rec) {
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  if (rec < 0 || (size_t)rec >= g_prof_used) return;       // the list was read and reset in between
+  cudaEventRecord(g_prof_recs[rec].e1, st);
+  g_prof_recs[rec].closed = true;
+}
+
+// ---- errors -----------------------------------------------------------------------------------
+namespace {
+thread_local int g_sticky_code = 0;
+thread_local std::string g_sticky_msg;
+}
+void sticky_error(int code, const std::string &msg) {
+  if (g_sticky_code == 0 && code != 0) { g_sticky_code = code; g_sticky_msg = msg; }
+}
+int sticky_take(std::string *msg) {
+  const int c = g_sticky_code;
+  if (c && msg) *msg = g_sticky_msg;
+  g_sticky_code = 0; g_sticky_msg.clear();
+  return c;
 }
 
 int set_err(tdvp_handle *h, int code, const std::string &msg) {
   if (h) h->err = msg; else g_null_err = msg;
   return code;
 }
+// End of (a stage of) a public call: a pending internal error (see sticky_error) wins over the CUDA
+// status, because whatever was enqueued after it ran on missing data.
 int check_cuda(tdvp_handle *h, cudaError_t e, const char *what) {
+  std::string smsg;
+  if (const int sc = sticky_take(&smsg)) {
+    if (e != cudaSuccess) cudaGetLastError();
+    return set_err(h, sc, std::string(what) + ": " + smsg);
+  }
   if (e == cudaSuccess) return TDVP_OK;
   return set_err(h, e == cudaErrorMemoryAllocation ? TDVP_ENOMEM : TDVP_ECUDA,
                  std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+int finish_blocking(tdvp_handle *h, const char *what) {
+  if (int rc = check_cuda(h, cudaStreamSynchronize(h->stream), what)) return rc;
+  if (!h->status_dev) return TDVP_OK;
+  int bits = 0;
+  if (int rc = check_cuda(h, cudaMemcpy(&bits, h->status_dev, sizeof(int), cudaMemcpyDeviceToHost), what)) return rc;
+  if (!bits) return TDVP_OK;
+  cudaMemset(h->status_dev, 0, sizeof(int));
+  if (bits & TDVP_STATUS_SVD_UNCONVERGED)
+    return set_err(h, TDVP_ESTATE, std::string(what) + ": a bond SVD (Eq. 36) used up its Jacobi sweeps without converging; "
+                                                       "results since the last blocking call are not to tolerance");
+  return set_err(h, TDVP_ESTATE, std::string(what) + ": unknown device status");
 }
 
 cudaError_t Arena::reserve(size_t bytes, cudaStream_t st) {
@@ -68,8 +111,12 @@ tdvp_handle *default_handle() {
   static tdvp_handle *h = nullptr;
   static std::mutex mu;
   std::lock_guard<std::mutex> g(mu);
-  if (!h) { h = new tdvp_handle(); tdvp_default_options(&h->opt); h->stream = nullptr; zgemm_prepare_stream(nullptr); }
-  return h;
+  if (!h) {
+    h = new tdvp_handle(); tdvp_default_options(&h->opt); h->stream = nullptr; zgemm_prepare_stream(nullptr);
+    if (cudaMalloc(&h->status_dev, sizeof(int)) == cudaSuccess) cudaMemset(h->status_dev, 0, sizeof(int));
+    else { h->status_dev = nullptr; cudaGetLastError(); }
+  }
+  return h;   // if the context could not be made, the sticky error surfaces at the caller's first GEMM
 }
 
 static int check_opts(tdvp_handle *h, const tdvp_options &o) {
@@ -101,7 +148,19 @@ int tdvp_create_context(tdvp_handle **out, const tdvp_options *opt, void *cuda_s
   if (rc) { delete h; return rc; }
   h->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
   configure_kernels_once();
-  zgemm_prepare_stream(h->stream);
+  if (zgemm_prepare_stream(h->stream) != TDVP_OK) {
+    const int rc2 = check_cuda(nullptr, cudaSuccess, "tdvp_create_context");
+    delete h;
+    return rc2 ? rc2 : TDVP_ECUDA;
+  }
+  h->owns_zgemm_ctx = true;
+  cudaError_t e = cudaMalloc(&h->status_dev, sizeof(int));
+  if (e == cudaSuccess) e = cudaMemset(h->status_dev, 0, sizeof(int));
+  if (e != cudaSuccess) {
+    const int rc2 = check_cuda(nullptr, e, "tdvp_create_context");
+    tdvp_destroy(h);
+    return rc2;
+  }
   *out = h;
   return TDVP_OK;
 }
@@ -110,15 +169,16 @@ const char *tdvp_last_error(const tdvp_handle *h) { return h ? h->err.c_str() : 
 
 long long tdvp_launch_count(void) { return g_launch_count.load(); }
 
-int tdvp_profile_enable(int on) { g_prof_on = on != 0; return TDVP_OK; }
+int tdvp_profile_enable(int on) { g_prof_on.store(on != 0); return TDVP_OK; }
 
 int tdvp_profile_read(double *ms, long long *count) {
   if (!ms || !count) return set_err(nullptr, TDVP_EINVAL, "null pointer");
   for (int i = 0; i < TDVP_PROFILE_PHASES; i++) { ms[i] = 0.0; count[i] = 0; }
   if (int rc = check_cuda(nullptr, cudaDeviceSynchronize(), "tdvp_profile_read")) return rc;
+  std::lock_guard<std::mutex> lk(g_prof_mu);
   for (size_t i = 0; i < g_prof_used; i++) {
     float t = 0.f;
-    if (cudaEventElapsedTime(&t, g_prof_recs[i].e0, g_prof_recs[i].e1) == cudaSuccess) {
+    if (g_prof_recs[i].closed && cudaEventElapsedTime(&t, g_prof_recs[i].e0, g_prof_recs[i].e1) == cudaSuccess) {
       ms[g_prof_recs[i].phase] += t; count[g_prof_recs[i].phase]++;
     }
   }
@@ -129,7 +189,9 @@ int tdvp_profile_read(double *ms, long long *count) {
 
 int tdvp_sync(tdvp_handle *h) {
   tdvp_handle *hh = h ? h : default_handle();
-  return check_cuda(h, cudaStreamSynchronize(hh->stream), "tdvp_sync");
+  const int rc = finish_blocking(hh, "tdvp_sync");
+  if (rc && !h) set_err(nullptr, rc, hh->err);
+  return rc;
 }
 
 static int bad_dims(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr) {
@@ -321,6 +383,7 @@ int tdvp_qr_gauge(tdvp_handle *h, int side, int Ml, int d, int Mr, const tdvp_c1
   long long tall = side == 0 ? (long long)Ml * d : (long long)d * Mr;
   int thin = side == 0 ? Mr : Ml;
   if (tall < thin) return set_err(h, TDVP_EINVAL, "gauge move needs a tall or square matrix");
+  if (tall > QR_MAX_TALL) return set_err(h, TDVP_EINVAL, "gauge move: tall side above 12800 rows is not supported");
   size_t qb = qr_ws_bytes((int)tall, thin);
   if (int rc = check_cuda(h, hh->arena.reserve(qb + 1024, hh->stream), "workspace")) return rc;
   hh->arena.reset();

@@ -24,22 +24,26 @@ LanczosOp bond_op(const tdvp_handle *h, int b) {
 
 __global__ void set_one_kernel(c128 *p) { p[0] = make_double2(1.0, 0.0); }
 
-// max |G - I| over an n x n matrix -> out[0] (single block)
+// fmax drops a NaN operand; the canonical check must not (a tensor with NaN / Inf entries has no
+// defect of zero): NaN if either is NaN, else the larger.
+__device__ __forceinline__ double nan_max(double a, double b) { return (a != a || b != b) ? a + b : fmax(a, b); }
+
+// max |G - I| over an n x n matrix -> out[0] (single block); NaN if G holds a non-finite entry
 __global__ void max_dev_identity_kernel(const c128 *G, int n, double *out) {
   __shared__ double red[256];
   double m = 0.0;
   for (int e = threadIdx.x; e < n * n; e += blockDim.x) {
     int i = e / n, j = e % n;
     double dx = G[e].x - (i == j ? 1.0 : 0.0), dy = G[e].y;
-    m = fmax(m, fmax(fabs(dx), fabs(dy)));
+    m = nan_max(m, nan_max(fabs(dx), fabs(dy)));           // Inf - Inf and 0 * Inf in the Gram matrix give NaN
   }
   red[threadIdx.x] = m;
   __syncthreads();
   for (int s = blockDim.x / 2; s > 0; s >>= 1) {
-    if (threadIdx.x < s) red[threadIdx.x] = fmax(red[threadIdx.x], red[threadIdx.x + s]);
+    if (threadIdx.x < s) red[threadIdx.x] = nan_max(red[threadIdx.x], red[threadIdx.x + s]);
     __syncthreads();
   }
-  if (threadIdx.x == 0) out[0] = fmax(out[0], red[0]);
+  if (threadIdx.x == 0) out[0] = nan_max(out[0], red[0]);
 }
 
 }  // namespace
@@ -91,8 +95,7 @@ int chain_canonical_defect(tdvp_handle *h, int side, int lo, int hi, double *def
       g.M = Mr; g.N = Mr; g.K = Ml * d;
       g.a_ms = 1; g.a_ks = Mr; g.conjA = 1; g.b_ks = Mr; g.b_ns = 1; g.ldc = Mr;
     }
-    g.splitk = 1;
-    zgemm(h->stream, g, nullptr);
+    zgemm(h->stream, g);
     TDVP_LAUNCH(max_dev_identity_kernel, 1, 256, 0, h->stream, G, g.M, dev);
   }
   if (int rc = check_cuda(h, cudaMemcpyAsync(defect, dev, sizeof(double), cudaMemcpyDeviceToHost, h->stream), "memcpy")) return rc;
@@ -126,6 +129,8 @@ int tdvp_destroy(tdvp_handle *h) {
   if (!h) return TDVP_OK;
   cudaStreamSynchronize(h->stream);
   free_chain(h);
+  if (h->status_dev) cudaFree(h->status_dev);
+  if (h->owns_zgemm_ctx) zgemm_release_stream(h->stream);   // the last handle on the stream frees the context
   if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
   if (h->ev_first) cudaEventDestroy(h->ev_first);
   if (h->ev_w) cudaEventDestroy(h->ev_w);
@@ -147,6 +152,8 @@ int tdvp_create(tdvp_handle **out, int n_sites, const int *phys_dim, const int *
       return set_err(nullptr, TDVP_EINVAL, "bad dimension or null tensor");
     if ((long long)mps_bond[i] * phys_dim[i] < mps_bond[i + 1] || (long long)mps_bond[i + 1] * phys_dim[i] < mps_bond[i])
       return set_err(nullptr, TDVP_EINVAL, "MPS bonds must satisfy M_i*d_i >= M_{i+1} and M_{i+1}*d_i >= M_i");
+    if ((long long)mps_bond[i] * phys_dim[i] > QR_MAX_TALL || (long long)mps_bond[i + 1] * phys_dim[i] > QR_MAX_TALL)
+      return set_err(nullptr, TDVP_EINVAL, "M_i * d_i above 12800 is not supported (QR gauge move, SURVEY.md 8(a) a7)");
   }
   tdvp_handle *h = nullptr;
   if (int rc = tdvp_create_context(&h, opt, cuda_stream)) return rc;
@@ -158,7 +165,7 @@ int tdvp_create(tdvp_handle **out, int n_sites, const int *phys_dim, const int *
   h->W.assign(n, nullptr); h->Wsp.resize(n); h->Wsp_mem.assign(n, nullptr);
   h->A.assign(n, nullptr); h->Lenv.assign(n, nullptr); h->Renv.assign(n, nullptr);
   const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
-  auto fail = [&](int rc) { std::string e = h->err; free_chain(h); delete h; return set_err(nullptr, rc, e); };
+  auto fail = [&](int rc) { std::string e = h->err; tdvp_destroy(h); return set_err(nullptr, rc, e); };
   long long max_site = 0, max_bond = 0;
   for (int i = 0; i < n; i++) {
     size_t wn = (size_t)h->Dw[i] * h->d[i] * h->d[i] * h->Dw[i + 1];

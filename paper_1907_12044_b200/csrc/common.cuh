@@ -16,18 +16,28 @@ extern thread_local long long *g_capture_tally;
 
 // Phase profiler (tdvp_profile_enable / tdvp_profile_read): CUDA-event pairs around the launches
 // of a kernel class, recorded on the launching stream; off by default, skipped during capture.
-enum { PH_ZGEMM = 0, PH_SPLITK = 1, PH_WSTAGE = 2, PH_VEC = 3, PH_QR = 4, PH_SVD = 5, PH_COUNT = 6 };
-void prof_begin(cudaStream_t st, int phase);
-void prof_end(cudaStream_t st);
-extern bool g_prof_on;
-extern int g_prof_depth;          // nested scopes: only the outermost one records
+enum { PH_ZGEMM = 0, PH_WSTAGE = 1, PH_VEC = 2, PH_QR = 3, PH_SVD = 4, PH_COUNT = 5 };
+static_assert(PH_COUNT == TDVP_PROFILE_PHASES, "phase list of include/tdvp.h");
+// Process-wide, guarded by a mutex (several handles / host threads may enqueue at once); the nesting
+// depth is per host thread.  prof_begin returns the record it opened, or -1.
+int prof_begin(cudaStream_t st, int phase);
+void prof_end(cudaStream_t st, int rec);
+extern std::atomic<bool> g_prof_on;
+extern thread_local int g_prof_depth;   // nested scopes: only the outermost one records
 struct ProfScope {
-  cudaStream_t st; bool counted, live;
-  ProfScope(cudaStream_t s, int phase) : st(s), counted(g_prof_on && !g_capture_tally), live(false) {
-    if (counted) { live = (g_prof_depth++ == 0); if (live) prof_begin(st, phase); }
+  cudaStream_t st; bool counted; int rec;
+  ProfScope(cudaStream_t s, int phase) : st(s), counted(g_prof_on.load(std::memory_order_relaxed) && !g_capture_tally), rec(-1) {
+    if (counted && g_prof_depth++ == 0) rec = prof_begin(st, phase);
   }
-  ~ProfScope() { if (counted) { g_prof_depth--; if (live) prof_end(st); } }
+  ~ProfScope() { if (counted) { g_prof_depth--; if (rec >= 0) prof_end(st, rec); } }
 };
+
+// Errors of internal stages whose call chain returns void (a GEMM that cannot get its scheduling
+// context or tensor maps): recorded per host thread, FIRST error wins, reported -- and cleared -- by
+// the next check_cuda() of the API layer, so that every public call still returns a TDVP_E* code
+// (include/tdvp.h: no signal or exception crosses the boundary).
+void sticky_error(int code, const std::string &msg);
+int sticky_take(std::string *msg);   // returns the pending code (0 = none) and clears it
 
 static inline void count_launch() {
   if (g_capture_tally) ++*g_capture_tally; else g_launch_count.fetch_add(1, std::memory_order_relaxed);
@@ -70,15 +80,14 @@ struct ZGemm {
   long long a_bsi = 0, b_bsi = 0, c_bsi = 0;   // inner batch strides
   long long a_bso = 0, b_bso = 0, c_bso = 0;   // outer batch strides
   int conjA = 0, conjB = 0;
-  int splitk = 0;                               // unused (the schedule is chosen by zgemm)
 };
 // The kernel is a persistent stream-K schedule; its partial-tile slots and flags belong to the
-// stream (one context per stream, made by zgemm_prepare_stream outside any capture; a private
-// capture stream is aliased to the stream the graph will be replayed on).  ws is unused (kept for
-// the call sites); zgemm_ws_elems returns 0.
-size_t zgemm_ws_elems(const ZGemm &p);
-void zgemm(cudaStream_t st, const ZGemm &p, c128 *ws);
-void zgemm_prepare_stream(cudaStream_t st);
+// stream (one reference-counted context per stream, made by zgemm_prepare_stream outside any capture
+// and dropped by zgemm_release_stream; a private capture stream is aliased to the stream the graph
+// will be replayed on).  Returns TDVP_OK or a TDVP_E* code, which is also left as the thread's sticky
+// error (callers with a void chain need not look at it).
+int zgemm(cudaStream_t st, const ZGemm &p);
+int zgemm_prepare_stream(cudaStream_t st);
 void zgemm_set_mode(int products);   // 3 or 4 real DMMA products per complex product
 int zgemm_get_mode();
 void zgemm_alias_stream(cudaStream_t alias, cudaStream_t of);
@@ -163,6 +172,9 @@ void lanczos_expm(cudaStream_t st, const LanczosOp &op, int k, double z_re, doub
 
 // ---------------------------------------------------------------------------------------------
 // qr.cu : Householder QR gauge move on the device.
+// Tallest matrix the panel kernels take: beyond 20 * 256 rows a one-column panel must still fit in
+// 200 KB of shared memory.  The API layer rejects taller gauge moves / unfoldings with TDVP_EINVAL.
+constexpr int QR_MAX_TALL = 12800;
 size_t qr_ws_bytes(int rows, int cols);
 // side 0: C (rows x cols, row-major, rows = Ml*d, cols = Mr) = Q D, Q rows x cols, D cols x cols
 // side 1: C (Ml x (d*Mr)) = D Q, i.e. QR of C^T: tall = d*Mr, thin = Ml; Q [Ml, d*Mr], D [Ml, Ml]
@@ -172,7 +184,11 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
 // ---------------------------------------------------------------------------------------------
 // svd.cu : matrix unfolding C[Ml, d*Mr] = U diag(lam) Vh (Eq. 36) on the device, Ml <= d*Mr.
 size_t svd_ws_bytes(int Ml, int d, int Mr);
-void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, double *lam, c128 *Vh, void *ws);
+// status: DEVICE int of the handle (nullable); bit TDVP_STATUS_SVD_UNCONVERGED is set when the Jacobi
+// iteration used up its sweeps with columns still rotating (reported by the next blocking call).
+constexpr int TDVP_STATUS_SVD_UNCONVERGED = 1;
+void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, double *lam, c128 *Vh, void *ws,
+              int *status);
 
 // ---------------------------------------------------------------------------------------------
 // small vector kernels shared by the drivers (vecops.cu)

@@ -78,10 +78,7 @@ ZGemm g_bond2(int Ml, int Mr, int Dw, const c128 *T, const c128 *R, c128 *out) {
 
 size_t heff_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr) {
   size_t t1 = (size_t)Ml * Dl * d * Mr, t2 = (size_t)Ml * d * Dr * Mr;
-  size_t s1 = zgemm_ws_elems(g_stage1_left(Ml, Mr, d, Dl, nullptr, nullptr, nullptr));
-  size_t s3 = zgemm_ws_elems(g_stage3_heff(Ml, Mr, d, Dr, nullptr, nullptr, nullptr));
-  size_t sk = s1 > s3 ? s1 : s3;
-  return up256(t1 * 16) + up256(t2 * 16) + up256(sk * 16) + 256;
+  return up256(t1 * 16) + up256(t2 * 16) + 256;
 }
 
 void heff_apply(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c128 *L,
@@ -89,12 +86,11 @@ void heff_apply(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c1
   size_t t1 = (size_t)Ml * Dl * d * Mr, t2 = (size_t)Ml * d * Dr * Mr;
   char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
   c128 *T1 = reinterpret_cast<c128 *>(p); p += up256(t1 * 16);
-  c128 *T2 = reinterpret_cast<c128 *>(p); p += up256(t2 * 16);
-  c128 *sk = reinterpret_cast<c128 *>(p);
-  zgemm(st, g_stage1_left(Ml, Mr, d, Dl, L, A, T1), sk);
+  c128 *T2 = reinterpret_cast<c128 *>(p);
+  zgemm(st, g_stage1_left(Ml, Mr, d, Dl, L, A, T1));
   if (w_ready) cudaStreamWaitEvent(st, w_ready, 0);
   wstage_left(st, W, Ml, Mr, T1, T2);
-  zgemm(st, g_stage3_heff(Ml, Mr, d, Dr, T2, R, out), sk);
+  zgemm(st, g_stage3_heff(Ml, Mr, d, Dr, T2, R, out));
 }
 
 void heff_apply_staged(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c128 *L, const c128 *W_dense,
@@ -103,33 +99,27 @@ void heff_apply_staged(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, c
   size_t t1 = (size_t)Ml * Dl * d * Mr, t2 = (size_t)Ml * d * Dr * Mr;
   char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
   c128 *T1 = reinterpret_cast<c128 *>(p); p += up256(t1 * 16);
-  c128 *T2 = reinterpret_cast<c128 *>(p); p += up256(t2 * 16);
-  c128 *sk = reinterpret_cast<c128 *>(p);
+  c128 *T2 = reinterpret_cast<c128 *>(p);
   for (int s = 0; s < nsl; s++) {
     const int a0 = (int)((long long)Ml * s / nsl), a1 = (int)((long long)Ml * (s + 1) / nsl);
     cudaStreamWaitEvent(st, ev_l[s], 0);
     if (a1 == a0) continue;
     ZGemm g = g_stage1_left(Ml, Mr, d, Dl, L + (size_t)a0 * Dl * Ml, A, T1 + (size_t)a0 * Dl * d * Mr);
     g.M = (a1 - a0) * Dl;
-    zgemm(st, g, sk);
+    zgemm(st, g);
   }
   cudaStreamWaitEvent(st, ev_w, 0);
   WSparse W;
   wsparse_build(st, W, wmem, Dl, d, Dr, W_dense, zero_tol);
   wstage_left(st, W, Ml, Mr, T1, T2);
   cudaStreamWaitEvent(st, ev_r, 0);
-  zgemm(st, g_stage3_heff(Ml, Mr, d, Dr, T2, R, out), sk);
+  zgemm(st, g_stage3_heff(Ml, Mr, d, Dr, T2, R, out));
 }
 
 size_t env_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr) {
   size_t t1 = (size_t)Ml * Dl * d * Mr, t2 = (size_t)Ml * d * Dr * Mr;
   size_t big = t1 > t2 ? t1 : t2;
-  size_t sk = 0, s;
-  s = zgemm_ws_elems(g_stage1_left(Ml, Mr, d, Dl, nullptr, nullptr, nullptr)); sk = s > sk ? s : sk;
-  s = zgemm_ws_elems(g_stage3_envL(Ml, Mr, d, Dr, nullptr, nullptr, nullptr)); sk = s > sk ? s : sk;
-  s = zgemm_ws_elems(g_stage1_right(Ml, Mr, d, Dr, nullptr, nullptr, nullptr)); sk = s > sk ? s : sk;
-  s = zgemm_ws_elems(g_stage3_envR(Ml, Mr, d, Dl, nullptr, nullptr, nullptr)); sk = s > sk ? s : sk;
-  return 2 * up256(big * 16) + up256(sk * 16) + 256;
+  return 2 * up256(big * 16) + 256;
 }
 
 void env_update(cudaStream_t st, int side, int Ml, int Mr, int d, int Dl, int Dr,
@@ -138,35 +128,30 @@ void env_update(cudaStream_t st, int side, int Ml, int Mr, int d, int Dl, int Dr
   size_t big = t1 > t2 ? t1 : t2;
   char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
   c128 *T1 = reinterpret_cast<c128 *>(p); p += up256(big * 16);
-  c128 *T2 = reinterpret_cast<c128 *>(p); p += up256(big * 16);
-  c128 *sk = reinterpret_cast<c128 *>(p);
+  c128 *T2 = reinterpret_cast<c128 *>(p);
   if (side == 0) {
-    zgemm(st, g_stage1_left(Ml, Mr, d, Dl, env_in, A, T1), sk);
+    zgemm(st, g_stage1_left(Ml, Mr, d, Dl, env_in, A, T1));
     if (w_ready) cudaStreamWaitEvent(st, w_ready, 0);
     wstage_left(st, W, Ml, Mr, T1, T2);
-    zgemm(st, g_stage3_envL(Ml, Mr, d, Dr, A, T2, env_out), sk);
+    zgemm(st, g_stage3_envL(Ml, Mr, d, Dr, A, T2, env_out));
   } else {
-    zgemm(st, g_stage1_right(Ml, Mr, d, Dr, A, env_in, T1), sk);
+    zgemm(st, g_stage1_right(Ml, Mr, d, Dr, A, env_in, T1));
     if (w_ready) cudaStreamWaitEvent(st, w_ready, 0);
     wstage_right(st, W, Ml, Mr, T1, T2);
-    zgemm(st, g_stage3_envR(Ml, Mr, d, Dl, A, T2, env_out), sk);
+    zgemm(st, g_stage3_envR(Ml, Mr, d, Dl, A, T2, env_out));
   }
 }
 
 size_t bond_ws_bytes(int Ml, int Mr, int Dw) {
   size_t t = (size_t)Ml * Dw * Mr;
-  size_t s1 = zgemm_ws_elems(g_bond1(Ml, Mr, Dw, nullptr, nullptr, nullptr));
-  size_t s2 = zgemm_ws_elems(g_bond2(Ml, Mr, Dw, nullptr, nullptr, nullptr));
-  size_t sk = s1 > s2 ? s1 : s2;
-  return up256(t * 16) + up256(sk * 16) + 256;
+  return up256(t * 16) + 256;
 }
 
 void bond_apply(cudaStream_t st, int Ml, int Mr, int Dw, const c128 *L, const c128 *D,
                 const c128 *R, c128 *out, void *ws) {
   size_t t = (size_t)Ml * Dw * Mr;
   char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
-  c128 *T = reinterpret_cast<c128 *>(p); p += up256(t * 16);
-  c128 *sk = reinterpret_cast<c128 *>(p);
-  zgemm(st, g_bond1(Ml, Mr, Dw, L, D, T), sk);
-  zgemm(st, g_bond2(Ml, Mr, Dw, T, R, out), sk);
+  c128 *T = reinterpret_cast<c128 *>(p);
+  zgemm(st, g_bond1(Ml, Mr, Dw, L, D, T));
+  zgemm(st, g_bond2(Ml, Mr, Dw, T, R, out));
 }

@@ -14,6 +14,8 @@ struct tdvp_handle {
   cudaStream_t stream = nullptr;
   tdvp_options opt;
   std::string err;
+  bool owns_zgemm_ctx = false;     // holds a reference on its stream's GEMM scheduling context
+  int *status_dev = nullptr;       // DEVICE: sticky TDVP_STATUS_* bits set by kernels, read by blocking calls
   Arena arena;                     // scratch for the current call (reset per call)
   cudaStream_t copy_stream = nullptr;   // host-entry calls: second H2D queue (created on first use)
   cudaEvent_t ev_first = nullptr, ev_w = nullptr, ev_r = nullptr, ev_l[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -52,4 +54,7 @@ struct tdvp_handle {
 
 int set_err(tdvp_handle *h, int code, const std::string &msg);
 int check_cuda(tdvp_handle *h, cudaError_t e, const char *what);
+// Blocks until the handle's stream is idle, then reports (and clears) what kernels left in status_dev:
+// TDVP_ESTATE if a bond SVD did not converge.  Every blocking public call ends here.
+int finish_blocking(tdvp_handle *h, const char *what);
 tdvp_handle *default_handle();

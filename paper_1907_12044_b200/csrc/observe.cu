@@ -37,7 +37,7 @@ __global__ void rdm_kernel(const c128 *T2, const c128 *A, int Ml, int d, int Mr,
   if (threadIdx.x == 0) rho[blockIdx.x] = make_double2(rx[0], ry[0]);
 }
 
-void gemm1(tdvp_handle *h, const ZGemm &g) { ZGemm q = g; q.splitk = 1; zgemm(h->stream, q, nullptr); }
+void gemm1(tdvp_handle *h, const ZGemm &g) { zgemm(h->stream, g); }
 
 // E'[b][y] = sum_{a,x,s} conj(A[a,s,b]) E[a][x] A[x,s,y]
 void transfer_left(tdvp_handle *h, int i, const c128 *E, c128 *Eout, c128 *T) {
@@ -94,7 +94,7 @@ int site_rdm(tdvp_handle *h, int site, std::vector<c128> &rho) {
   TDVP_LAUNCH(rdm_kernel, d * d, 256, 0, st, T2, h->A[site], Ml, d, Mr, rho_dev);
   rho.resize((size_t)d * d);
   if (int rc = check_cuda(h, cudaMemcpyAsync(rho.data(), rho_dev, (size_t)d * d * 16, cudaMemcpyDeviceToHost, st), "memcpy")) return rc;
-  return check_cuda(h, cudaStreamSynchronize(st), "site_rdm");
+  return finish_blocking(h, "site observable");
 }
 
 }  // namespace
@@ -153,7 +153,7 @@ int tdvp_norm_energy(tdvp_handle *h, double *norm_sq, double *energy) {
     }
     c128 e;
     if (int rc = check_cuda(h, cudaMemcpyAsync(&e, E0, 16, cudaMemcpyDeviceToHost, h->stream), "memcpy")) return rc;
-    if (int rc = check_cuda(h, cudaStreamSynchronize(h->stream), "tdvp_norm_energy")) return rc;
+    if (int rc = finish_blocking(h, "tdvp_norm_energy")) return rc;
     *energy = e.x;
   }
   return TDVP_OK;
@@ -167,7 +167,7 @@ int tdvp_get_mps(tdvp_handle *h, int site, tdvp_c128 *out_host, int *Ml, int *Mr
   if (!out_host) return TDVP_OK;
   size_t n = (size_t)h->M[site] * h->d[site] * h->M[site + 1];
   if (int rc = check_cuda(h, cudaMemcpyAsync(out_host, h->A[site], n * 16, cudaMemcpyDeviceToHost, h->stream), "memcpy")) return rc;
-  return check_cuda(h, cudaStreamSynchronize(h->stream), "tdvp_get_mps");
+  return finish_blocking(h, "tdvp_get_mps");
 }
 
 int tdvp_set_mps(tdvp_handle *h, const tdvp_c128 *const *mps_host, int centre) {

@@ -628,6 +628,7 @@ int panel_width(int rows) {
   long long budget = 200 * 1024;
   int nb = (int)(budget / ((long long)rows * 16));
   if (nb > NB_MAX) nb = NB_MAX;
+  if (nb < 1) nb = 1;                                     // rows > QR_MAX_TALL are rejected by the API layer
   return nb;
 }
 

@@ -100,7 +100,7 @@ MuScratch mu_scratch(tdvp_handle *h) {
   return mu_carve(h, h->mu_scratch);
 }
 
-void gemm1(cudaStream_t st, ZGemm g) { g.splitk = 1; zgemm(st, g, nullptr); }
+void gemm1(cudaStream_t st, const ZGemm &g) { zgemm(st, g); }
 
 // K = F(Y): the TDVP-MU right-hand side.  Uses the handle's Lenv / Renv storage as scratch caches.
 int mu_rhs(tdvp_handle *h, const std::vector<c128 *> &Y, const std::vector<c128 *> &K) {
@@ -124,7 +124,7 @@ int mu_rhs(tdvp_handle *h, const std::vector<c128 *> &Y, const std::vector<c128 
   c128 *Cnext = s.C0;
   for (int i = n - 1; i >= 1; i--) {
     const int Ml = h->M[i], Mr = h->M[i + 1], d = h->d[i];
-    svd_bond(st, Ml, d, Mr, C, s.U, s.lam, s.Vh, ws);                                    // Eq. 36
+    svd_bond(st, Ml, d, Mr, C, s.U, s.lam, s.Vh, ws, h->status_dev);                                    // Eq. 36
     env_update(st, 1, Ml, Mr, d, h->Dw[i], h->Dw[i + 1], h->Renv[i], h->Wsp[i], s.Vh, h->Renv[i - 1], ws);
     // site i-1: centre form C' = L (U Lambda)
     const int j = i - 1, Jl = h->M[j], Jr = h->M[j + 1], dj = h->d[j];                    // Jr == Ml
@@ -266,7 +266,7 @@ int cmf_mean_fields(tdvp_handle *h, const std::vector<c128 *> &Y) {
     const int Ml = h->M[i], Mr = h->M[i + 1], d = h->d[i];
     c128 *U = reinterpret_cast<c128 *>(h->cmf_mem[3 * i]), *UL = reinterpret_cast<c128 *>(h->cmf_mem[3 * i + 1]);
     double *lam = reinterpret_cast<double *>(h->cmf_mem[3 * i + 2]);
-    svd_bond(st, Ml, d, Mr, C, U, lam, s.Vh, ws);                                        // Eq. 36
+    svd_bond(st, Ml, d, Mr, C, U, lam, s.Vh, ws, h->status_dev);                                        // Eq. 36
     env_update(st, 1, Ml, Mr, d, h->Dw[i], h->Dw[i + 1], h->Renv[i], h->Wsp[i], s.Vh, h->Renv[i - 1], ws);
     vec_copy(st, UL, U, (long long)Ml * Ml);
     TDVP_LAUNCH(scale_cols_kernel, grid_for((long long)Ml * Ml), VT, 0, st, UL, (long long)Ml, Ml, lam, 0, 0.0);
@@ -412,7 +412,7 @@ int tdvp_step_mu(tdvp_handle *h, double dt, double *err_est) {
   if (int rc = enqueue_mu_step(h, dt)) return rc;
   if (err_est) {
     if (int rc = check_cuda(h, cudaMemcpyAsync(err_est, h->mu_err_dev, sizeof(double), cudaMemcpyDeviceToHost, h->stream), "memcpy")) return rc;
-    return check_cuda(h, cudaStreamSynchronize(h->stream), "tdvp_step_mu sync");
+    return finish_blocking(h, "tdvp_step_mu");
   }
   return TDVP_OK;
 }
@@ -437,7 +437,7 @@ int tdvp_mu_derivative(tdvp_handle *h, tdvp_c128 *const *out_host) {
     if (!out_host[i]) return set_err(h, TDVP_EINVAL, "null output tensor");
     if (int rc = check_cuda(h, cudaMemcpyAsync(out_host[i], h->mu_k[0][i], site_elems(h, i) * 16, cudaMemcpyDeviceToHost, h->stream), "memcpy")) return rc;
   }
-  return check_cuda(h, cudaStreamSynchronize(h->stream), "tdvp_mu_derivative");
+  return finish_blocking(h, "tdvp_mu_derivative");
 }
 
 int tdvp_svd_bond(tdvp_handle *h, int Ml, int d, int Mr, const tdvp_c128 *C, tdvp_c128 *U, double *lam, tdvp_c128 *Vh) {
@@ -445,12 +445,13 @@ int tdvp_svd_bond(tdvp_handle *h, int Ml, int d, int Mr, const tdvp_c128 *C, tdv
   if (!C || !U || !lam || !Vh) return set_err(h, TDVP_EINVAL, "null pointer");
   if (Ml < 1 || d < 1 || Mr < 1) return set_err(h, TDVP_EINVAL, "dimensions must be >= 1");
   if ((long long)d * Mr < Ml) return set_err(h, TDVP_EINVAL, "matrix unfolding needs Ml <= d*Mr");
+  if ((long long)d * Mr > QR_MAX_TALL) return set_err(h, TDVP_EINVAL, "matrix unfolding: d*Mr above 12800 is not supported");
   size_t sb = svd_ws_bytes(Ml, d, Mr);
   if (int rc = check_cuda(h, hh->arena.reserve(sb + 1024, hh->stream), "workspace")) return rc;
   hh->arena.reset();
   void *ws = hh->arena.take(sb);
   svd_bond(hh->stream, Ml, d, Mr, reinterpret_cast<const c128 *>(C), reinterpret_cast<c128 *>(U), lam,
-           reinterpret_cast<c128 *>(Vh), ws);
+           reinterpret_cast<c128 *>(Vh), ws, hh->status_dev);
   return check_cuda(h, cudaGetLastError(), "tdvp_svd_bond");
 }
 

@@ -26,8 +26,7 @@ void absorb_right(tdvp_handle *h, int i, const c128 *D, const c128 *A, c128 *out
   g.A = D; g.B = A; g.C = out;
   g.M = h->M[i]; g.K = h->M[i]; g.N = h->d[i] * h->M[i + 1];
   g.a_ms = h->M[i]; g.a_ks = 1; g.b_ks = g.N; g.b_ns = 1; g.ldc = g.N;
-  g.splitk = 1;
-  zgemm(h->stream, g, nullptr);
+  zgemm(h->stream, g);
 }
 // out[(a,s)][c] = sum_b A[(a,s)][b] D[b][c]     (C_{i-1} = A_{i-1} D)
 void absorb_left(tdvp_handle *h, int i, const c128 *A, const c128 *D, c128 *out) {
@@ -35,8 +34,7 @@ void absorb_left(tdvp_handle *h, int i, const c128 *A, const c128 *D, c128 *out)
   g.A = A; g.B = D; g.C = out;
   g.M = h->M[i] * h->d[i]; g.K = h->M[i + 1]; g.N = h->M[i + 1];
   g.a_ms = h->M[i + 1]; g.a_ks = 1; g.b_ks = g.N; g.b_ns = 1; g.ldc = g.N;
-  g.splitk = 1;
-  zgemm(h->stream, g, nullptr);
+  zgemm(h->stream, g);
 }
 
 // Eq. 42: one symmetric sweep pair.  The centre tensor travels through tmpA / tmpB.

@@ -14,6 +14,8 @@
 // deterministic, capturable in the step graph.
 #include <cooperative_groups.h>
 
+#include <cstdlib>
+
 #include "common.cuh"
 
 namespace cg = cooperative_groups;
@@ -50,7 +52,7 @@ constexpr int JW = 8;               // warps per CTA
 
 template <int NPL>
 __global__ void __cluster_dims__(JC, 1, 1) __launch_bounds__(JW * 32)
-svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/) {
+svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/, int max_sweeps, int *status) {
   cg::cluster_group cluster = cg::this_cluster();
   const int lane = threadIdx.x & 31;
   const int gwarp = blockIdx.x * JW + (threadIdx.x >> 5), nwarps = JC * JW;
@@ -58,7 +60,8 @@ svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/)
   const int npairs = np / 2;
   const double tol = 2.220446049250313e-16 * sqrt((double)n);   // LAPACK zgesvj: sqrt(m) * eps
   const double tol2 = tol * tol;
-  for (int sweep = 0; sweep < MAX_SWEEPS; sweep++) {
+  int sweep = 0;
+  for (; sweep < max_sweeps; sweep++) {
     bool any = false;
     for (int round = 0; round < np - 1; round++) {
       for (int k = gwarp; k < npairs; k += nwarps) {
@@ -138,6 +141,8 @@ svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/)
     if (np < 2) break;
     if (__ldcg(flags + sweep) == 0) break;                          // nobody rotated in this sweep
   }
+  // every sweep allowed still rotated: the columns are NOT orthogonal to tolerance -- tell the host
+  if (sweep == max_sweeps && np >= 2 && status && gwarp == 0 && lane == 0) atomicOr(status, TDVP_STATUS_SVD_UNCONVERGED);
 }
 
 // Block variant for n <= 128: the same rotations, but the cluster barrier is paid once per BLOCK pair
@@ -195,7 +200,7 @@ __device__ __forceinline__ bool jacobi_pair_smem(c128 *xp, c128 *xq, c128 *jp, c
 
 template <int NPL>
 __global__ void __cluster_dims__(JC, 1, 1) __launch_bounds__(JW * 32)
-svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/) {
+svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/, int max_sweeps, int *status) {
   cg::cluster_group cluster = cg::this_cluster();
   extern __shared__ __align__(16) unsigned char jsm[];
   const int bw = (n + JB - 1) / JB;                       // columns per block (<= 8 for n <= 128)
@@ -222,7 +227,8 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
     }
   };
   const int bwp = (bw + 1) & ~1;                          // players of the in-block tournament
-  for (int sweep = 0; sweep < MAX_SWEEPS; sweep++) {
+  int sweep = 0;
+  for (; sweep < max_sweeps; sweep++) {
     bool any = false;
     // (i) pairs inside blocks 2 cta and 2 cta + 1: warps 0-3 take the first block, 4-7 the second
     {
@@ -269,6 +275,7 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
     }
     if (__ldcg(flags + sweep) == 0) break;                          // nobody rotated in this sweep
   }
+  if (sweep == max_sweeps && status && cta == 0 && tid == 0) atomicOr(status, TDVP_STATUS_SVD_UNCONVERGED);
 }
 
 // lam (descending), U and the permuted J from X = U' R' (Qp = U'^T, Dp = R'^T as qr_gauge side 1 returns them).
@@ -318,8 +325,11 @@ size_t svd_ws_bytes(int Ml, int d, int Mr) {
 }
 
 // C [Ml, d, Mr] -> U [Ml, Ml], lam [Ml], Vh [Ml, d, Mr]
-void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, double *lam, c128 *Vh, void *ws) {
+void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, double *lam, c128 *Vh, void *ws, int *status) {
   ProfScope ps(st, PH_SVD);
+  // sweeps allowed (diagnostic switch TDVP_SVD_MAX_SWEEPS, read at every call: the error-path test lowers it)
+  int max_sweeps = MAX_SWEEPS;
+  if (const char *e = getenv("TDVP_SVD_MAX_SWEEPS")) { const int v = atoi(e); if (v >= 1 && v <= MAX_SWEEPS) max_sweeps = v; }
   const int n = Ml;
   const size_t nn = up256((size_t)n * n * 16);
   char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
@@ -337,11 +347,11 @@ void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, do
   TDVP_LAUNCH(svd_init_kernel, g, 256, 0, st, D, Xt, Jt, n);
   cudaMemsetAsync(flags, 0, MAX_SWEEPS * sizeof(int), st);
   const size_t bsm = (size_t)4 * ((n + JB - 1) / JB) * n * sizeof(c128);      // X and J of two blocks
-  if (n <= 16) TDVP_LAUNCH(svd_jacobi_kernel<1>, JC, JW * 32, 0, st, Xt, Jt, n, flags);
-  else if (n <= 32) TDVP_LAUNCH(svd_jacobi_block_kernel<1>, JC, JW * 32, bsm, st, Xt, Jt, n, flags);
-  else if (n <= 64) TDVP_LAUNCH(svd_jacobi_block_kernel<2>, JC, JW * 32, bsm, st, Xt, Jt, n, flags);
-  else if (n <= 128) TDVP_LAUNCH(svd_jacobi_block_kernel<4>, JC, JW * 32, bsm, st, Xt, Jt, n, flags);
-  else TDVP_LAUNCH(svd_jacobi_kernel<0>, JC, JW * 32, 0, st, Xt, Jt, n, flags);
+  if (n <= 16) TDVP_LAUNCH(svd_jacobi_kernel<1>, JC, JW * 32, 0, st, Xt, Jt, n, flags, max_sweeps, status);
+  else if (n <= 32) TDVP_LAUNCH(svd_jacobi_block_kernel<1>, JC, JW * 32, bsm, st, Xt, Jt, n, flags, max_sweeps, status);
+  else if (n <= 64) TDVP_LAUNCH(svd_jacobi_block_kernel<2>, JC, JW * 32, bsm, st, Xt, Jt, n, flags, max_sweeps, status);
+  else if (n <= 128) TDVP_LAUNCH(svd_jacobi_block_kernel<4>, JC, JW * 32, bsm, st, Xt, Jt, n, flags, max_sweeps, status);
+  else TDVP_LAUNCH(svd_jacobi_kernel<0>, JC, JW * 32, 0, st, Xt, Jt, n, flags, max_sweeps, status);
   // X = U' R'  <=>  Xt = R'^T U'^T: "side 1" factorisation of the n x n matrix Xt (d = 1)
   qr_gauge(st, 1, n, 1, n, Xt, Qp, Dp, qws);
   TDVP_LAUNCH(svd_finish_kernel, n < 148 ? n : 148, 128, n * sizeof(double), st, Qp, Dp, Jt, n, U, lam, JtP);
@@ -349,6 +359,5 @@ void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, do
   gm.A = JtP; gm.B = Q; gm.C = Vh;
   gm.M = n; gm.K = n; gm.N = d * Mr;
   gm.a_ms = n; gm.a_ks = 1; gm.conjA = 1; gm.b_ks = gm.N; gm.b_ns = 1; gm.ldc = gm.N;
-  gm.splitk = 1;
-  zgemm(st, gm, nullptr);
+  zgemm(st, gm);
 }

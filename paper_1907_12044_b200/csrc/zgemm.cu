@@ -5,9 +5,10 @@
 // sm_100a the FP64 tensor path is the warp-level DMMA; it issues at 64 FMA/clk/SM (measured:
 // 37.15 TFLOP/s), slow enough that shared-memory and L2 bandwidth are never the limit -- the
 // kernel is designed around keeping all four SMSPs issuing DMMA back to back:
-//   * CTA tile 64x64 complex, 4 warps, each warp a 32x32 complex tile = 4x4 m8n8 blocks, real and
-//     imaginary accumulators (64 f64 per thread); the complex product is 4 real MMAs per block
-//     pair, with -Im(A) made by a sign-bit XOR on the ALU pipe (no FP64 pipe work);
+//   * CTA tile 64x64 complex, 4 warps, each warp a 32x32 complex tile = 4x4 m8n8 blocks; the complex
+//     product is formed from THREE real MMAs per block pair by default (X1 = Ar Br, X2 = Ai Bi,
+//     X3 = (Ar + Ai)(Br + Bi): 96 f64 accumulators per thread, combined once per tile segment;
+//     DESIGN.md reading c15) or from four (64 accumulators, -Im(A) by a sign-bit XOR on the ALU pipe);
 //   * operands stay in their global layout (complex interleaved) in shared memory, staged by TMA
 //     (cp.async.bulk.tensor, dense boxes, zero fill at ragged edges) into a 3-slot ring guarded by
 //     full/empty mbarriers; one thread issues the loads.  Measured: every non-DMMA instruction a
@@ -423,8 +424,9 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
 }
 
 // Complex product as three real DMMA products per k-step (default) or four (TDVP_ZGEMM_4M=1 in the
-// environment, or zgemm_set_mode(4)): see DESIGN.md 5, reading c15.
-int g_mode3m = 1;
+// environment, or zgemm_set_mode(4)): see DESIGN.md 5, reading c15.  Process-wide by contract
+// (include/tdvp.h, tdvp_set_gemm_products); atomic because handles on other host threads read it.
+std::atomic<int> g_mode3m{1};
 
 template <bool AK, bool BK_, bool CJ, bool M3>
 void launch2(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, const KParams &kp) {
@@ -441,7 +443,7 @@ void launch2(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, cons
 }
 template <bool AK, bool BK_, bool CJ>
 void launch1(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, const KParams &kp) {
-  if (g_mode3m) launch2<AK, BK_, CJ, true>(st, ta, tb, kp);
+  if (g_mode3m.load(std::memory_order_relaxed)) launch2<AK, BK_, CJ, true>(st, ta, tb, kp);
   else launch2<AK, BK_, CJ, false>(st, ta, tb, kp);
 }
 template <bool AK, bool BK_>
@@ -485,10 +487,12 @@ bool encode_operand(CUtensorMap *tm, const c128 *base, bool kmajor, long long ro
                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
-    fprintf(stderr, "libtdvp: cuTensorMapEncodeTiled failed (%d): dims %llu %llu %llu %llu strides %llu %llu %llu box %u %u\n",
-            (int)r, (unsigned long long)dims[0], (unsigned long long)dims[1], (unsigned long long)dims[2],
-            (unsigned long long)dims[3], (unsigned long long)strides[0], (unsigned long long)strides[1],
-            (unsigned long long)strides[2], box[0], box[1]);
+    char buf[320];
+    snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (%d) for an operand at %p (must be 16-byte aligned): dims %llu %llu "
+             "%llu %llu strides %llu %llu %llu box %u %u", (int)r, (const void *)base, (unsigned long long)dims[0],
+             (unsigned long long)dims[1], (unsigned long long)dims[2], (unsigned long long)dims[3],
+             (unsigned long long)strides[0], (unsigned long long)strides[1], (unsigned long long)strides[2], box[0], box[1]);
+    sticky_error(TDVP_EINVAL, buf);
     return false;
   }
   return true;
@@ -524,22 +528,38 @@ bool encode_operand_5d(CUtensorMap *tm, const c128 *base, long long rows, long l
 // Per-stream scheduling state: partial-tile slots and the two counter arrays.  Kernels of one
 // stream run one after the other, so one context per stream is enough; it is created outside any
 // stream capture (zgemm_prepare_stream) because cudaMalloc is not allowed while capturing.
-struct StreamCtx { c128 *slots = nullptr; int *cnt = nullptr; int *done = nullptr; };
+struct StreamCtx { c128 *slots = nullptr; int *cnt = nullptr; int *done = nullptr; int refs = 0; bool alias = false; };
 std::mutex g_ctx_mu;
 std::unordered_map<cudaStream_t, StreamCtx> g_ctx;
 int g_slots = 0;      // resident CTAs of zgemm_kernel on this device (2 per SM)
 int g_sms = 0;
 
-StreamCtx *get_ctx(cudaStream_t st, bool create) {
+// Looks the context of a stream up; `create` makes it if missing (cudaMalloc: not inside a capture),
+// `add_ref` counts one more owner (a handle).  Failures leave the thread's sticky error.
+StreamCtx *get_ctx(cudaStream_t st, bool create, bool add_ref = false) {
   std::lock_guard<std::mutex> lk(g_ctx_mu);
   auto it = g_ctx.find(st);
-  if (it != g_ctx.end()) return &it->second;
+  if (it != g_ctx.end()) { if (add_ref) it->second.refs++; return &it->second; }
   if (!create) return nullptr;
   StreamCtx c;
-  if (cudaMalloc(&c.slots, (size_t)2 * g_slots * BM * BN * sizeof(c128)) != cudaSuccess) return nullptr;
-  if (cudaMalloc(&c.cnt, (size_t)2 * g_slots * sizeof(int)) != cudaSuccess) { cudaFree(c.slots); return nullptr; }
-  cudaMemset(c.cnt, 0, (size_t)2 * g_slots * sizeof(int));
+  cudaError_t e = cudaMalloc(&c.slots, (size_t)2 * g_slots * BM * BN * sizeof(c128));
+  if (e == cudaSuccess) {
+    e = cudaMalloc(&c.cnt, (size_t)2 * g_slots * sizeof(int));
+    if (e != cudaSuccess) cudaFree(c.slots);
+  }
+  if (e == cudaSuccess) {
+    e = cudaMemset(c.cnt, 0, (size_t)2 * g_slots * sizeof(int));
+    if (e != cudaSuccess) { cudaFree(c.slots); cudaFree(c.cnt); }
+  }
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    sticky_error(e == cudaErrorMemoryAllocation ? TDVP_ENOMEM : TDVP_ECUDA,
+                 std::string("GEMM scheduling context of the stream (first use must be outside a stream capture): ") +
+                     cudaGetErrorString(e));
+    return nullptr;
+  }
   c.done = c.cnt + g_slots;
+  c.refs = add_ref ? 1 : 0;
   return &(g_ctx[st] = c);
 }
 
@@ -575,7 +595,7 @@ void zgemm_configure() {
   if (const char *es = getenv("TDVP_ZGEMM_SPLIT_COST")) g_split_cost = atof(es);
   if (const char *e5 = getenv("TDVP_ZGEMM_NO_5D")) g_no_5d = e5[0] == '1';
   const char *e4 = getenv("TDVP_ZGEMM_4M");
-  if (e4 && e4[0] == '1') g_mode3m = 0;
+  if (e4 && e4[0] == '1') g_mode3m.store(0);
   if (per_sm < 1) per_sm = 1;
   if (per_sm > 2) per_sm = 2;
   if (g_sms < 1) g_sms = 1;
@@ -587,17 +607,23 @@ void zgemm_configure() {
     g_encode = reinterpret_cast<EncodeTiledFn>(fn);
 }
 
-void zgemm_set_mode(int products) { configure_kernels_once(); g_mode3m = products == 4 ? 0 : 1; }
-int zgemm_get_mode() { configure_kernels_once(); return g_mode3m ? 3 : 4; }
+void zgemm_set_mode(int products) { configure_kernels_once(); g_mode3m.store(products == 4 ? 0 : 1); }
+int zgemm_get_mode() { configure_kernels_once(); return g_mode3m.load() ? 3 : 4; }
 
-void zgemm_prepare_stream(cudaStream_t st) { configure_kernels_once(); get_ctx(st, true); }
+// One more owner (a handle) of the stream's context; created if missing.
+int zgemm_prepare_stream(cudaStream_t st) {
+  configure_kernels_once();
+  return get_ctx(st, true, true) ? TDVP_OK : TDVP_ECUDA;  // on failure the sticky error says why
+}
 
 void zgemm_alias_stream(cudaStream_t alias, cudaStream_t of) {
   configure_kernels_once();
   StreamCtx *c = get_ctx(of, true);
   if (!c) return;
   std::lock_guard<std::mutex> lk(g_ctx_mu);
-  g_ctx[alias] = *c;
+  StreamCtx a = *c;
+  a.alias = true; a.refs = 0;
+  g_ctx[alias] = a;
 }
 
 void zgemm_forget_stream(cudaStream_t alias) {
@@ -605,30 +631,35 @@ void zgemm_forget_stream(cudaStream_t alias) {
   g_ctx.erase(alias);
 }
 
-void zgemm_release_stream(cudaStream_t st) {           // a queue the caller owned: free its context
+// An owner of the stream's context is gone; the last one frees it (the caller has synchronised the
+// stream).  Contexts made implicitly by a handle-less call keep refs == 0 and live until exit.
+void zgemm_release_stream(cudaStream_t st) {
   std::lock_guard<std::mutex> lk(g_ctx_mu);
   auto it = g_ctx.find(st);
-  if (it == g_ctx.end()) return;
+  if (it == g_ctx.end() || it->second.alias) return;
+  if (--it->second.refs > 0) return;
   cudaFree(it->second.slots);
   cudaFree(it->second.cnt);
   g_ctx.erase(it);
 }
 
-size_t zgemm_ws_elems(const ZGemm &) { return 0; }   // the scheduling workspace belongs to the stream
-
-void zgemm(cudaStream_t st, const ZGemm &p, c128 *) {
-  if (p.M <= 0 || p.N <= 0) return;
-  StreamCtx *ctx = get_ctx(st, true);
-  if (!ctx || !g_encode) {
-    fprintf(stderr, "libtdvp: zgemm has no scheduling context for this stream (allocation failed, first use inside a "
-                    "capture) or no cuTensorMapEncodeTiled entry point\n");
-    abort();
+int zgemm(cudaStream_t st, const ZGemm &p) {
+  if (p.M <= 0 || p.N <= 0) return TDVP_OK;
+  if (!g_encode) {
+    sticky_error(TDVP_ECUDA, "no cuTensorMapEncodeTiled driver entry point (CUDA driver too old for TMA)");
+    return TDVP_ECUDA;
   }
+  StreamCtx *ctx = get_ctx(st, true);
+  if (!ctx) return TDVP_ECUDA;                            // the sticky error says why
   const bool ak = (p.a_ks == 1), bk = (p.b_ks == 1);
   CUtensorMap ta, tb;
   if (!encode_operand(&ta, p.A, ak, p.M, p.K, ak ? p.a_ms : p.a_ks, p.batch_inner, p.a_bsi, p.batch_outer, p.a_bso) ||
       !encode_operand(&tb, p.B, bk, p.N, p.K, bk ? p.b_ns : p.b_ks, p.batch_inner, p.b_bsi, p.batch_outer, p.b_bso))
-    abort();
+    return TDVP_EINVAL;
+  if ((reinterpret_cast<size_t>(p.C) & 15) != 0) {
+    sticky_error(TDVP_EINVAL, "GEMM output is not 16-byte aligned");
+    return TDVP_EINVAL;
+  }
   KParams kp;
   kp.a5 = ak && encode_operand_5d(&ta, p.A, p.M, p.K, p.a_ms, p.batch_inner, p.a_bsi, p.batch_outer, p.a_bso) ? 1 : 0;
   kp.b5 = bk && encode_operand_5d(&tb, p.B, p.N, p.K, p.b_ns, p.batch_inner, p.b_bsi, p.batch_outer, p.b_bso) ? 1 : 0;
@@ -658,4 +689,5 @@ void zgemm(cudaStream_t st, const ZGemm &p, c128 *) {
   else if (ak && !bk) launch<true, false>(st, ta, tb, kp);
   else if (!ak && bk) launch<false, true>(st, ta, tb, kp);
   else launch<false, false>(st, ta, tb, kp);
+  return TDVP_OK;
 }

@@ -373,7 +373,9 @@ def test_errors_are_reported(T):
 
 
 # ---- TDVP-MU: matrix unfolding (Eq. 36), derivative (Eq. 27, 37, 38), Dormand-Prince step ------
-@pytest.mark.parametrize("shape", [(1, 3, 4), (4, 3, 4), (12, 4, 16), (37, 5, 29), (64, 10, 64), (70, 3, 130)])
+# the last three shapes (Ml > 128) reach the generic looped Jacobi kernel, the path of TDVP-MU at M = 256
+@pytest.mark.parametrize("shape", [(1, 3, 4), (4, 3, 4), (12, 4, 16), (37, 5, 29), (64, 10, 64), (70, 3, 130),
+                                   (128, 10, 128), (160, 4, 160), (256, 2, 256)])
 @pytest.mark.parametrize("deficient", [False, True])
 def test_svd_bond(T, shape, deficient):
     Ml, d, Mr = shape

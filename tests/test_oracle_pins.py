@@ -296,3 +296,113 @@ def test_p13_cmf_is_second_order_and_agrees_with_ps(warmed_up):
     slopes = [np.log2(errs[i] / errs[i + 1]) for i in range(2)]
     assert all(1.7 < s < 2.5 for s in slopes), (errs, slopes)
     assert errs[-1] < 1e-5
+
+
+# ---------------------------------------------------------------- Dormand-Prince tableau and error estimate
+def _dp_tableau():
+    n = 7
+    A = np.zeros((n, n))
+    for i, row in enumerate(tdvp_mu._A):
+        A[i, :len(row)] = row
+    return A, np.array(tdvp_mu._C), np.array(tdvp_mu._B5), np.array(tdvp_mu._B4)
+
+
+def _order_conditions(A, c, b, order):
+    """Residuals of the Runge-Kutta order conditions (one per rooted tree, Butcher / Hairer-Norsett-
+    Wanner vol. I table II.2.1) up to `order`."""
+    Ac, Ac2, Ac3 = A @ c, A @ c ** 2, A @ c ** 3
+    AAc = A @ Ac
+    res = [b.sum() - 1.0]
+    if order >= 2:
+        res += [b @ c - 1 / 2]
+    if order >= 3:
+        res += [b @ c ** 2 - 1 / 3, b @ Ac - 1 / 6]
+    if order >= 4:
+        res += [b @ c ** 3 - 1 / 4, b @ (c * Ac) - 1 / 8, b @ Ac2 - 1 / 12, b @ AAc - 1 / 24]
+    if order >= 5:
+        res += [b @ c ** 4 - 1 / 5, b @ (c ** 2 * Ac) - 1 / 10, b @ (c * Ac2) - 1 / 15, b @ (c * AAc) - 1 / 30,
+                b @ (Ac * Ac) - 1 / 20, b @ Ac3 - 1 / 20, b @ (A @ (c * Ac)) - 1 / 40, b @ (A @ Ac2) - 1 / 60,
+                b @ (A @ AAc) - 1 / 120]
+    return np.array(res)
+
+
+def test_dormand_prince_tableau_order_conditions():
+    """oracle/tdvp_mu.py's tableau (the RK45 of PAPER.md:224): the propagated weights _B5 satisfy all 17
+    order conditions through order 5, the embedded weights _B4 all 8 through order 4 and NOT those of
+    order 5 (else the difference would not estimate the error); row sums give the nodes; stage 7 is
+    evaluated at the new state (first-same-as-last)."""
+    A, c, b5, b4 = _dp_tableau()
+    assert np.abs(A.sum(axis=1) - c).max() < 1e-15
+    assert np.abs(_order_conditions(A, c, b5, 5)).max() < 1e-15
+    assert np.abs(_order_conditions(A, c, b4, 4)).max() < 1e-15
+    assert np.abs(_order_conditions(A, c, b4, 5)[8:]).max() > 1e-4
+    assert np.array_equal(A[6, :6], b5[:6]) and b5[6] == 0.0 and c[6] == 1.0
+
+
+def test_mu_err_est_scales_as_h5(warmed_up):
+    """err_est of oracle step_mu is the norm of the (5th - 4th order) difference: it falls as h^5
+    (slope 4.5-5.5 per halving) on the warmed tiny chain, inside the smooth regime h <= 0.1 fs
+    (SURVEY.md 8(c) c12), and the 5th-order solution's own one-step error falls faster still."""
+    mpo, warm = warmed_up
+    lc = tdvp_mu.to_left_canonical(warm)
+    errs = []
+    for h in (0.1, 0.05, 0.025):
+        _, e = tdvp_mu.step_mu(mpo, lc, h)
+        errs.append(e)
+    slopes = [np.log2(errs[i] / errs[i + 1]) for i in range(2)]
+    assert all(4.5 < s < 5.5 for s in slopes), (errs, slopes)
+    # one step of h against two steps of h/2 (Richardson): the propagated solution is 5th order, local
+    # error O(h^6) -> the ratio between h = 0.2 and h = 0.1 is >= 2^6 = 64 (measured 112: Dormand-Prince
+    # minimises the h^6 coefficient, so the h^7 term still shows); a 4th-order weight row would give 32
+    def one_vs_two(h):
+        y1, _ = tdvp_mu.step_mu(mpo, lc, h)
+        y2, _ = tdvp_mu.step_mu(mpo, lc, h / 2)
+        y2, _ = tdvp_mu.step_mu(mpo, y2, h / 2)
+        return np.linalg.norm(obs.mps_to_vector(y1) - obs.mps_to_vector(y2))
+    r = one_vs_two(0.2) / one_vs_two(0.1)
+    assert 45 < r < 260, r
+
+
+# ---------------------------------------------------------------- observables: the full one-site RDM
+@pytest.mark.parametrize("site", [0, 2, 3])
+def test_one_site_rdm_all_entries_vs_full_vector(site):
+    """rho[s,t] = sum_rest psi[..s..] conj(psi[..t..]) INCLUDING the off-diagonals (a transposed or
+    conjugated rho passes every population check), on a random complex MPS that is NOT canonical
+    (the contraction is gauge-agnostic); <psi|op|psi> = trace(op^T rho) = sum_st op[s,t]... is fixed
+    by the full vector too, for a non-Hermitian op with `row = bra` (include/tdvp.h:190)."""
+    dims = [3, 2, 4, 3, 2]
+    rng = np.random.default_rng(31)
+    bonds = [1, 3, 4, 5, 2, 1]
+    mps = [si.complex_normal(rng, (bonds[i], dims[i], bonds[i + 1])) for i in range(5)]
+    psi = obs.mps_to_vector(mps).reshape(dims)
+    T = np.moveaxis(psi, site, 0).reshape(dims[site], -1)
+    brute = T @ T.conj().T                                      # rho[s,t] = sum_rest psi_s conj(psi_t)
+    rho = obs.one_site_rdm(mps, site)
+    assert np.abs(rho - brute).max() < 1e-12 * np.abs(brute).max()
+    assert np.abs(rho - rho.conj().T).max() < 1e-12 * np.abs(brute).max()
+    assert np.abs(brute - brute.T).max() > 1e-2 * np.abs(brute).max()       # the case is not symmetric
+    # <psi| O_site |psi> with O[s,t] = <s|O|t> (row = bra): sum_{s,t} conj(psi_s) O[s,t] psi_t = sum O[s,t] rho[t,s]
+    op = si.complex_normal(rng, (dims[site], dims[site]))
+    full = np.einsum("sr,st,tr->", T.conj(), op, T)
+    assert abs(np.trace(op @ rho) - full) < 1e-12 * abs(full)
+    assert abs(np.trace(op.T @ rho) - full) > 1e-3 * abs(full)
+
+
+# ---------------------------------------------------------------- gauge sweeps without evolution
+def test_to_right_canonical_keeps_the_state(warmed_up):
+    """RQ sweep (Eq. 9): every site but the first satisfies Eq. 8
+    to 1e-13 and the state is unchanged (overlap 1, same vector up to nothing at all: the sweep is
+    a pure gauge change, so the VECTORS agree, not only their overlap)."""
+    mpo, warm = warmed_up
+    lc = tdvp_mu.to_left_canonical(warm)
+    for A in lc[:-1]:                                          # Eq. 7
+        m = A.reshape(-1, A.shape[2])
+        assert np.abs(m.conj().T @ m - np.eye(A.shape[2])).max() < 1e-13
+    rc = tdvp_mu.to_right_canonical(lc)
+    for A in rc[1:]:                                           # Eq. 8
+        m = A.reshape(A.shape[0], -1)
+        assert np.abs(m @ m.conj().T - np.eye(A.shape[0])).max() < 1e-13
+    v0, v1, v2 = (obs.mps_to_vector(x) for x in (warm, lc, rc))
+    assert np.linalg.norm(v1 - v0) < 1e-12 and np.linalg.norm(v2 - v0) < 1e-12
+    assert abs(np.vdot(v2, v0) - 1.0) < 1e-12
+    assert [a.shape for a in rc] == [a.shape for a in warm]
