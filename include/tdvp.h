@@ -46,8 +46,12 @@ typedef struct tdvp_handle tdvp_handle;            /* opaque; owns all device st
 typedef struct { double re, im; } tdvp_c128;       /* interleaved complex128                    */
 
 typedef struct {
-  int    krylov_dim;   /* k of the Lanczos exponential; default 10; <= 64     */
-  double krylov_tol;   /* reserved for the adaptive rule (paper gives no formula); must be 0     */
+  int    krylov_dim;   /* k of the Lanczos exponential: the dimension used when
+                          krylov_tol = 0, the largest allowed when > 0; default 10; <= 64        */
+  double krylov_tol;   /* 0 (default): fixed dimension.  > 0: adaptive dimension (PAPER.md:292,
+                          "continues until |Psi(t+tau)> converges"; the paper gives no criterion,
+                          reading c11): stop at the first j with beta_j |[exp(z T_j) e_1]_j| < tol,
+                          decided on the device; applies to purely imaginary z only             */
   double mu_eps;       /* epsilon of Eq. 38; default 1e-10                    */
   double w_zero_tol;   /* |W| <= tol is a structural zero of the MPO; default 0 (exact zeros)    */
   int    flags;        /* TDVP_FLAG_* below                                                      */
@@ -117,9 +121,11 @@ int tdvp_apply_bond(tdvp_handle *h, int Ml, int Mr, int Dw,
                     const tdvp_c128 *L /*DEVICE*/, const tdvp_c128 *D /*DEVICE*/,
                     const tdvp_c128 *R /*DEVICE*/, tdvp_c128 *out /*DEVICE*/);
 
-/* y = exp(z * H[i]) v by the Lanczos / Krylov method with fixed dimension k = opt.krylov_dim,
-   full re-orthogonalisation, real alpha_j, breakdown rule beta_j < 1e-14 * max(1, |alpha_j|)
-   (SURVEY.md 8(c) O3/c11).  H[i] is the (Hermitian) operator of
+/* y = exp(z * H[i]) v by the Lanczos / Krylov method with dimension k = opt.krylov_dim (fixed, or
+   the cap of the adaptive rule if opt.krylov_tol > 0 and z_re = 0), full re-orthogonalisation, real
+   alpha_j, breakdown rule beta_j < 1e-14 * max(1, |alpha_j|).
+   For z_re = 0 the coefficients exp(z T) e_1 of the tridiagonal matrix come from a Chebyshev expansion,
+   which covers |z| * (spectral width of T) up to ~1850 (beyond: TDVP_ESTATE at the next blocking call).  H[i] is the (Hermitian) operator of
    tdvp_apply_heff with the given L, W, R.  All scalars of the recurrence stay on the device.
    krylov_used: HOST, nullable; if non-NULL the call blocks on the stream and returns the Krylov
    dimension actually used. */

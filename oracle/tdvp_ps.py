@@ -27,25 +27,26 @@ class PSState:
         self.krylov_dims = []
 
 
-def step_ps(st, dt, k):
-    """Advance st by one TDVP-PS step of size dt (Eq. 42) with fixed Krylov dimension k."""
+def step_ps(st, dt, k, tol=0.0):
+    """Advance st by one TDVP-PS step of size dt (Eq. 42) with Krylov dimension k (fixed if tol = 0,
+    else the cap of the adaptive rule of lanczos.py)."""
     n = st.n
     st.krylov_dims = []
     for i in range(n - 1):
         # forward evolution of the centre, Eq. 43
         C, m = lanczos_expm(lambda x: heff(st.Lenv[i], st.mpo[i], x, st.Renv[i]),
-                            st.mps[i], -1j * dt / 2, k)
+                            st.mps[i], -1j * dt / 2, k, tol)
         st.krylov_dims.append(m)
         Ml, d, Mr = C.shape
         Q, D = np.linalg.qr(C.reshape(Ml * d, Mr))                 # Eq. 9
         st.mps[i] = Q.reshape(Ml, d, Q.shape[1])
         st.Lenv[i + 1] = envL(st.Lenv[i], st.mpo[i], st.mps[i])    # Eq. 30-32
         # backward evolution of the bond matrix, Eq. 44
-        D, m = lanczos_expm(lambda x: bond(st.Lenv[i + 1], x, st.Renv[i]), D, +1j * dt / 2, k)
+        D, m = lanczos_expm(lambda x: bond(st.Lenv[i + 1], x, st.Renv[i]), D, +1j * dt / 2, k, tol)
         st.krylov_dims.append(m)
         st.mps[i + 1] = np.einsum("ab,bsc->asc", D, st.mps[i + 1])
     C, m = lanczos_expm(lambda x: heff(st.Lenv[n - 1], st.mpo[n - 1], x, st.Renv[n - 1]),
-                        st.mps[n - 1], -1j * dt, k)
+                        st.mps[n - 1], -1j * dt, k, tol)
     st.krylov_dims.append(m)
     st.mps[n - 1] = C
     for i in range(n - 1, 0, -1):
@@ -55,11 +56,11 @@ def step_ps(st, dt, k):
         D = Rt.T                                                   # C = D . B
         st.mps[i] = Q.T.reshape(Q.shape[1], d, Mr)
         st.Renv[i - 1] = envR(st.Renv[i], st.mpo[i], st.mps[i])
-        D, m = lanczos_expm(lambda x: bond(st.Lenv[i], x, st.Renv[i - 1]), D, +1j * dt / 2, k)
+        D, m = lanczos_expm(lambda x: bond(st.Lenv[i], x, st.Renv[i - 1]), D, +1j * dt / 2, k, tol)
         st.krylov_dims.append(m)
         C = np.einsum("asb,bc->asc", st.mps[i - 1], D)
         C, m = lanczos_expm(lambda x: heff(st.Lenv[i - 1], st.mpo[i - 1], x, st.Renv[i - 1]),
-                            C, -1j * dt / 2, k)
+                            C, -1j * dt / 2, k, tol)
         st.krylov_dims.append(m)
         st.mps[i - 1] = C
     return st

@@ -80,6 +80,9 @@ int finish_blocking(tdvp_handle *h, const char *what) {
   if (int rc = check_cuda(h, cudaMemcpy(&bits, h->status_dev, sizeof(int), cudaMemcpyDeviceToHost), what)) return rc;
   if (!bits) return TDVP_OK;
   cudaMemset(h->status_dev, 0, sizeof(int));
+  if (bits & TDVP_STATUS_KRYLOV_RANGE)
+    return set_err(h, TDVP_ESTATE, std::string(what) + ": a Krylov exponential had |z| * (spectral width of the tridiagonal matrix) above "
+                                                       "the ~1850 the coefficient series covers; use a smaller step");
   if (bits & TDVP_STATUS_SVD_UNCONVERGED)
     return set_err(h, TDVP_ESTATE, std::string(what) + ": a bond SVD (Eq. 36) used up its Jacobi sweeps without converging; "
                                                        "results since the last blocking call are not to tolerance");
@@ -122,7 +125,7 @@ tdvp_handle *default_handle() {
 static int check_opts(tdvp_handle *h, const tdvp_options &o) {
   if (o.krylov_dim < 1 || o.krylov_dim > TDVP_MAX_KRYLOV)
     return set_err(h, TDVP_EINVAL, "krylov_dim must be in [1, 64]");
-  if (o.krylov_tol != 0.0) return set_err(h, TDVP_EINVAL, "krylov_tol must be 0 (fixed-k contract mode)");
+  if (!(o.krylov_tol >= 0.0)) return set_err(h, TDVP_EINVAL, "krylov_tol must be >= 0 (0 = fixed Krylov dimension)");
   if (!(o.mu_eps > 0.0)) return set_err(h, TDVP_EINVAL, "mu_eps must be > 0");
   if (o.w_zero_tol < 0.0) return set_err(h, TDVP_EINVAL, "w_zero_tol must be >= 0");
   return TDVP_OK;
@@ -342,8 +345,8 @@ int tdvp_expm_heff(tdvp_handle *h, int Ml, int Mr, int d, int Dl, int Dr, const 
   WSparse wsp;
   wsparse_build(hh->stream, wsp, wmem, Dl, d, Dr, reinterpret_cast<const c128 *>(W), hh->opt.w_zero_tol);
   op.W = &wsp;
-  lanczos_expm(hh->stream, op, k, z_re, z_im, reinterpret_cast<const c128 *>(v),
-               reinterpret_cast<c128 *>(y), ws, m_dev);
+  lanczos_expm(hh->stream, op, k, hh->opt.krylov_tol, z_re, z_im, reinterpret_cast<const c128 *>(v),
+               reinterpret_cast<c128 *>(y), ws, m_dev, hh->status_dev);
   if (int rc = check_cuda(h, cudaGetLastError(), "tdvp_expm_heff")) return rc;
   if (krylov_used) {
     if (int rc = check_cuda(h, cudaMemcpyAsync(krylov_used, m_dev, sizeof(int), cudaMemcpyDeviceToHost, hh->stream), "memcpy")) return rc;
@@ -364,8 +367,8 @@ int tdvp_expm_bond(tdvp_handle *h, int Ml, int Mr, int Dw, const tdvp_c128 *L, c
   hh->arena.reset();
   void *ws = hh->arena.take(lb);
   int *m_dev = reinterpret_cast<int *>(hh->arena.take(256));
-  lanczos_expm(hh->stream, op, k, z_re, z_im, reinterpret_cast<const c128 *>(v),
-               reinterpret_cast<c128 *>(y), ws, m_dev);
+  lanczos_expm(hh->stream, op, k, hh->opt.krylov_tol, z_re, z_im, reinterpret_cast<const c128 *>(v),
+               reinterpret_cast<c128 *>(y), ws, m_dev, hh->status_dev);
   if (int rc = check_cuda(h, cudaGetLastError(), "tdvp_expm_bond")) return rc;
   if (krylov_used) {
     if (int rc = check_cuda(h, cudaMemcpyAsync(krylov_used, m_dev, sizeof(int), cudaMemcpyDeviceToHost, hh->stream), "memcpy")) return rc;

@@ -80,6 +80,7 @@ struct ZGemm {
   long long a_bsi = 0, b_bsi = 0, c_bsi = 0;   // inner batch strides
   long long a_bso = 0, b_bso = 0, c_bso = 0;   // outer batch strides
   int conjA = 0, conjB = 0;
+  const int *skip = nullptr;     // DEVICE, nullable: if *skip != 0 when the kernel starts, every CTA returns at once
 };
 // The kernel is a persistent stream-K schedule; its partial-tile slots and flags belong to the
 // stream (one reference-counted context per stream, made by zgemm_prepare_stream outside any capture
@@ -121,9 +122,9 @@ void wsparse_build(cudaStream_t st, WSparse &ws, void *mem, int Dl, int d, int D
                    const c128 *W, double zero_tol, bool want_order = true);
 constexpr int W_QUAD_MIN_PANELS = 48;   // fewer (a, 64-y) panels than this: the long-row kernel is not considered
 // T2[a,s,v,y] = sum_{w,t} W[w,s,t,v] T1[a,w,t,y];  T1 [Ml,Dl,d,Mr] -> T2 [Ml,d,Dr,Mr]
-void wstage_left(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2);
+void wstage_left(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2, const int *skip = nullptr);
 // T2[w,x,s,b] = sum_{t,v} W[w,s,t,v] T1[x,t,v,b];  T1 [Ml,d,Dr,Mr] -> T2 [Dl,Ml,d,Mr]
-void wstage_right(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2);
+void wstage_right(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2, const int *skip = nullptr);
 
 // ---------------------------------------------------------------------------------------------
 // Workspace: one growable device arena per handle (cudaMalloc only when it has to grow).
@@ -144,7 +145,8 @@ struct Arena {
 size_t heff_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr);
 void heff_apply(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c128 *L,
                 const WSparse &W, const c128 *A, const c128 *R, c128 *out, void *ws,
-                cudaEvent_t w_ready = nullptr);   // if set: the W stage waits for it (W built on a side queue)
+                cudaEvent_t w_ready = nullptr,    // if set: the W stage waits for it (W built on a side queue)
+                const int *skip = nullptr);       // DEVICE flag: non-zero turns the three kernels into no-ops
 // The same for the host-entry path, whose inputs are still arriving on a copy queue: stage 1 runs in
 // nsl slices of the bond index a, slice s after ev_l[s] (A and rows [s*Ml/nsl, (s+1)*Ml/nsl) of L
 // have landed); the sparse form of W is built after ev_w, stage 3 waits for ev_r (R).
@@ -156,7 +158,7 @@ void env_update(cudaStream_t st, int side, int Ml, int Mr, int d, int Dl, int Dr
                 const c128 *env_in, const WSparse &W, const c128 *A, c128 *env_out, void *ws, cudaEvent_t w_ready = nullptr);
 size_t bond_ws_bytes(int Ml, int Mr, int Dw);
 void bond_apply(cudaStream_t st, int Ml, int Mr, int Dw, const c128 *L, const c128 *D,
-                const c128 *R, c128 *out, void *ws);
+                const c128 *R, c128 *out, void *ws, const int *skip = nullptr);
 
 // ---------------------------------------------------------------------------------------------
 // lanczos.cu : Krylov exponential with all scalars on the device.
@@ -166,9 +168,12 @@ struct LanczosOp {           // which operator: heff (site) or bond
   const c128 *L; const c128 *R; const WSparse *W;
 };
 size_t lanczos_ws_bytes(const LanczosOp &op, int k);
-// y = exp(z H) v.  m_used_dev: DEVICE int (nullable) receiving the Krylov dimension used.
-void lanczos_expm(cudaStream_t st, const LanczosOp &op, int k, double z_re, double z_im,
-                  const c128 *v, c128 *y, void *ws, int *m_used_dev);
+// y = exp(z H) v with at most k Krylov vectors; tol > 0 (and z purely imaginary): stop at the first j with
+// beta_j |[exp(z T_j) e_1]_j| < tol.  m_used_dev: DEVICE int (nullable) receiving the Krylov dimension used;
+// status_dev: the handle's sticky device status (nullable).
+constexpr int TDVP_STATUS_KRYLOV_RANGE = 2;   // |z| * spectral width of T beyond the Chebyshev series kept
+void lanczos_expm(cudaStream_t st, const LanczosOp &op, int k, double tol, double z_re, double z_im,
+                  const c128 *v, c128 *y, void *ws, int *m_used_dev, int *status_dev);
 
 // ---------------------------------------------------------------------------------------------
 // qr.cu : Householder QR gauge move on the device.

@@ -82,15 +82,17 @@ size_t heff_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr) {
 }
 
 void heff_apply(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c128 *L,
-                const WSparse &W, const c128 *A, const c128 *R, c128 *out, void *ws, cudaEvent_t w_ready) {
+                const WSparse &W, const c128 *A, const c128 *R, c128 *out, void *ws, cudaEvent_t w_ready, const int *skip) {
   size_t t1 = (size_t)Ml * Dl * d * Mr, t2 = (size_t)Ml * d * Dr * Mr;
   char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
   c128 *T1 = reinterpret_cast<c128 *>(p); p += up256(t1 * 16);
   c128 *T2 = reinterpret_cast<c128 *>(p);
-  zgemm(st, g_stage1_left(Ml, Mr, d, Dl, L, A, T1));
+  ZGemm g1 = g_stage1_left(Ml, Mr, d, Dl, L, A, T1), g3 = g_stage3_heff(Ml, Mr, d, Dr, T2, R, out);
+  g1.skip = g3.skip = skip;
+  zgemm(st, g1);
   if (w_ready) cudaStreamWaitEvent(st, w_ready, 0);
-  wstage_left(st, W, Ml, Mr, T1, T2);
-  zgemm(st, g_stage3_heff(Ml, Mr, d, Dr, T2, R, out));
+  wstage_left(st, W, Ml, Mr, T1, T2, skip);
+  zgemm(st, g3);
 }
 
 void heff_apply_staged(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c128 *L, const c128 *W_dense,
@@ -148,10 +150,12 @@ size_t bond_ws_bytes(int Ml, int Mr, int Dw) {
 }
 
 void bond_apply(cudaStream_t st, int Ml, int Mr, int Dw, const c128 *L, const c128 *D,
-                const c128 *R, c128 *out, void *ws) {
+                const c128 *R, c128 *out, void *ws, const int *skip) {
   size_t t = (size_t)Ml * Dw * Mr;
   char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
   c128 *T = reinterpret_cast<c128 *>(p);
-  zgemm(st, g_bond1(Ml, Mr, Dw, L, D, T));
-  zgemm(st, g_bond2(Ml, Mr, Dw, T, R, out));
+  ZGemm g1 = g_bond1(Ml, Mr, Dw, L, D, T), g2 = g_bond2(Ml, Mr, Dw, T, R, out);
+  g1.skip = g2.skip = skip;
+  zgemm(st, g1);
+  zgemm(st, g2);
 }

@@ -374,7 +374,7 @@ int cmf_propagate(tdvp_handle *h, const std::vector<c128 *> &X, const std::vecto
     LanczosOp op{};
     op.kind = 0; op.Ml = h->M[i]; op.Mr = h->M[i + 1]; op.d = h->d[i]; op.Dl = h->Dw[i]; op.Dr = h->Dw[i + 1];
     op.L = h->Lenv[i]; op.R = h->Renv[i]; op.W = &h->Wsp[i];
-    lanczos_expm(st, op, h->opt.krylov_dim, 0.0, -t, X[i], Z[i], h->step_ws, nullptr);
+    lanczos_expm(st, op, h->opt.krylov_dim, h->opt.krylov_tol, 0.0, -t, X[i], Z[i], h->step_ws, nullptr, h->status_dev);
   }
   for (int q = 0; q < nq; q++) {
     cudaEventRecord(h->cmf_join[q], h->cmf_streams[q]);

@@ -41,25 +41,26 @@ void absorb_left(tdvp_handle *h, int i, const c128 *A, const c128 *D, c128 *out)
 void enqueue_ps_step(tdvp_handle *h, double dt) {
   cudaStream_t st = h->stream;
   const int n = h->n, k = h->opt.krylov_dim;
+  const double ktol = h->opt.krylov_tol;
   void *ws = h->step_ws;
   const c128 *cur = h->A[0];
   for (int i = 0; i < n - 1; i++) {
-    lanczos_expm(st, heff_op(h, i), k, 0.0, -0.5 * dt, cur, h->tmpA, ws, nullptr);            // Eq. 43
+    lanczos_expm(st, heff_op(h, i), k, ktol, 0.0, -0.5 * dt, cur, h->tmpA, ws, nullptr, h->status_dev);            // Eq. 43
     qr_gauge(st, 0, h->M[i], h->d[i], h->M[i + 1], h->tmpA, h->A[i], h->bondD, ws);            // Eq. 9
     env_update(st, 0, h->M[i], h->M[i + 1], h->d[i], h->Dw[i], h->Dw[i + 1], h->Lenv[i], h->Wsp[i], h->A[i],
                h->Lenv[i + 1], ws);                                                             // Eq. 30-32
-    lanczos_expm(st, bond_op(h, i + 1), k, 0.0, +0.5 * dt, h->bondD, h->bondD2, ws, nullptr);  // Eq. 44
+    lanczos_expm(st, bond_op(h, i + 1), k, ktol, 0.0, +0.5 * dt, h->bondD, h->bondD2, ws, nullptr, h->status_dev);  // Eq. 44
     absorb_right(h, i + 1, h->bondD2, h->A[i + 1], h->tmpB);
     cur = h->tmpB;
   }
-  lanczos_expm(st, heff_op(h, n - 1), k, 0.0, -dt, cur, h->tmpA, ws, nullptr);                 // last site, full step
+  lanczos_expm(st, heff_op(h, n - 1), k, ktol, 0.0, -dt, cur, h->tmpA, ws, nullptr, h->status_dev);                 // last site, full step
   for (int i = n - 1; i >= 1; i--) {
     qr_gauge(st, 1, h->M[i], h->d[i], h->M[i + 1], h->tmpA, h->A[i], h->bondD, ws);
     env_update(st, 1, h->M[i], h->M[i + 1], h->d[i], h->Dw[i], h->Dw[i + 1], h->Renv[i], h->Wsp[i], h->A[i],
                h->Renv[i - 1], ws);
-    lanczos_expm(st, bond_op(h, i), k, 0.0, +0.5 * dt, h->bondD, h->bondD2, ws, nullptr);
+    lanczos_expm(st, bond_op(h, i), k, ktol, 0.0, +0.5 * dt, h->bondD, h->bondD2, ws, nullptr, h->status_dev);
     absorb_left(h, i - 1, h->A[i - 1], h->bondD2, h->tmpB);
-    lanczos_expm(st, heff_op(h, i - 1), k, 0.0, -0.5 * dt, h->tmpB, h->tmpA, ws, nullptr);
+    lanczos_expm(st, heff_op(h, i - 1), k, ktol, 0.0, -0.5 * dt, h->tmpB, h->tmpA, ws, nullptr, h->status_dev);
   }
   vec_copy(st, h->A[0], h->tmpA, site_elems(h, 0));
 }

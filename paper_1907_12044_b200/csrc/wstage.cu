@@ -56,6 +56,7 @@ struct WStageParams {
   const int *cnt; const int *col; const c128 *val;   // row-padded sparse W (see csr_build_kernel)
   const int *order;                // rows by entry count, longest first
   int long_rows;                   // -1 unknown on the host, 0, 1
+  const int *skip;                 // nullable: non-zero at kernel start = nothing to do (see ZGemm::skip)
 };
 
 __device__ __forceinline__ void cfma(double &sx, double &sy, c128 w, c128 t) {
@@ -126,6 +127,7 @@ __device__ __forceinline__ void wp_rows(const WStageParams &p, const c128 *tile,
 __global__ void __launch_bounds__(WP_THREADS, 1) wstage_persistent_kernel(WStageParams p, int ntile, int npanels, int quad_follows) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ int s_next_row;
+  if (p.skip && *reinterpret_cast<const volatile int *>(p.skip)) return;
   c128 *tile = reinterpret_cast<c128 *>(smem_raw);                        // [ncols][YT]
   const int tile_elems = p.ncols * YT;
   int *rbeg = reinterpret_cast<int *>(smem_raw + (size_t)tile_elems * 16);   // [nrows]
@@ -234,6 +236,7 @@ __global__ void __launch_bounds__(WQ_THREADS, 1) wstage_quad_kernel(WStageParams
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ int s_next, s_nnz;
   __shared__ __align__(8) unsigned long long s_bar;       // completion barrier of the bulk panel copies
+  if (p.skip && *reinterpret_cast<const volatile int *>(p.skip)) return;
   c128 *tile = reinterpret_cast<c128 *>(smem_raw);                        // [ncols][YT]
   const int tile_elems = p.ncols * YT;
   int *scnt = reinterpret_cast<int *>(smem_raw + (size_t)tile_elems * 16);    // [nrows], in sorted order
@@ -350,6 +353,7 @@ __global__ void __launch_bounds__(WQ_THREADS, 1) wstage_quad_kernel(WStageParams
 // Fallback for panels that do not fit in shared memory (ncols * 1 KB > ~220 KB): one warp per
 // (a, 32 y, row), panel and entries read through L1/L2.
 __global__ void __launch_bounds__(256) wstage_direct_kernel(WStageParams p) {
+  if (p.skip && *reinterpret_cast<const volatile int *>(p.skip)) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int a = blockIdx.y, y = blockIdx.x * 32 + lane;
   const bool yok = y < p.Mr;
@@ -451,9 +455,9 @@ void wsparse_classify(WSparse &ws, cudaStream_t st) {
   ws.long_rows_r = t1 >= 8LL * n1 ? 1 : 0;
 }
 
-void wstage_left(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2) {
+void wstage_left(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2, const int *skip) {
   WStageParams p;
-  p.in = T1; p.out = T2;
+  p.in = T1; p.out = T2; p.skip = skip;
   p.nrows = ws.d * ws.Dr; p.ncols = ws.Dl * ws.d; p.Mr = Mr;
   p.in_bs = (long long)ws.Dl * ws.d * Mr;
   p.rdiv = p.nrows > 0 ? p.nrows : 1; p.o_s1 = 0; p.o_s2 = Mr;
@@ -462,9 +466,9 @@ void wstage_left(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 
   launch_wstage(st, p, Ml);
 }
 
-void wstage_right(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2) {
+void wstage_right(cudaStream_t st, const WSparse &ws, int Ml, int Mr, const c128 *T1, c128 *T2, const int *skip) {
   WStageParams p;
-  p.in = T1; p.out = T2;
+  p.in = T1; p.out = T2; p.skip = skip;
   p.nrows = ws.Dl * ws.d; p.ncols = ws.d * ws.Dr; p.Mr = Mr;
   p.in_bs = (long long)ws.d * ws.Dr * Mr;
   p.rdiv = ws.d; p.o_s1 = (long long)Ml * ws.d * Mr; p.o_s2 = Mr;

@@ -57,6 +57,7 @@ struct KParams {
   int tiles_m, tiles_n, ktiles;
   int G;                // CTAs of this launch (cooperative: all resident)
   int upc_base, upc_rem;// units (tile, k-tile) per CTA: base, +1 for the first upc_rem CTAs
+  const int *skip;      // nullable: non-zero at kernel start = the caller no longer needs this product
   c128 *slots;          // [2 G][BM*BN] partial tiles of segments that do not cover their tile's whole K
   int *cnt;             // [G] partial segments published for the cut tile whose LAST unit CTA j holds
   int *done;            // [G] contributors that have finished reducing it (the last one zeroes both)
@@ -126,8 +127,7 @@ __device__ __forceinline__ int cta_of_unit(int u, int base, int rem) {
 }
 
 template <bool A_KMAJOR, bool B_KMAJOR, bool CONJ, bool M3>
-__global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constant__ CUtensorMap tmA,
-                                                            const __grid_constant__ CUtensorMap tmB, KParams p) {
+__device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtensorMap &tmB, const KParams &p) {
   extern __shared__ __align__(128) unsigned char smem_dyn[];
   __shared__ int s_fix_tile[2];
   __shared__ __align__(8) unsigned long long s_full[STAGES], s_empty[STAGES];
@@ -423,6 +423,27 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constan
   }
 }
 
+// The kernel proper.  SKIP = false: the body inlined, no test (every fixed-k launch: the headline path).
+// SKIP = true (launches that carry a skip flag: the applies of an adaptive Krylov recurrence): the flag is
+// tested first and the body is a function of its own -- with the test inlined in front of it ptxas spilled
+// ~270 bytes in the 3-product instances, which sit at 244 of 255 registers; outlined it costs ~5 % instead.
+template <bool A_KMAJOR, bool B_KMAJOR, bool CONJ, bool M3>
+__device__ __noinline__ void zgemm_body_outlined(const CUtensorMap &tmA, const CUtensorMap &tmB, const KParams &p) {
+  zgemm_body<A_KMAJOR, B_KMAJOR, CONJ, M3>(tmA, tmB, p);
+}
+template <bool A_KMAJOR, bool B_KMAJOR, bool CONJ, bool M3, bool SKIP>
+__global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constant__ CUtensorMap tmA,
+                                                            const __grid_constant__ CUtensorMap tmB,
+                                                            const __grid_constant__ KParams p) {
+  if (SKIP) {
+    // written by an earlier kernel of the stream, so every CTA reads the same value: all return or none does
+    if (p.skip != nullptr && __ldcg(p.skip) != 0) return;
+    zgemm_body_outlined<A_KMAJOR, B_KMAJOR, CONJ, M3>(tmA, tmB, p);
+  } else {
+    zgemm_body<A_KMAJOR, B_KMAJOR, CONJ, M3>(tmA, tmB, p);
+  }
+}
+
 // Complex product as three real DMMA products per k-step (default) or four (TDVP_ZGEMM_4M=1 in the
 // environment, or zgemm_set_mode(4)): see DESIGN.md 5, reading c15.  Process-wide by contract
 // (include/tdvp.h, tdvp_set_gemm_products); atomic because handles on other host threads read it.
@@ -438,7 +459,8 @@ void launch2(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, cons
   // no tile is cut when the ranges are whole tiles: nobody waits for anybody, a plain launch will do
   const bool cut = kp.upc_rem != 0 || (kp.upc_base % kp.ktiles) != 0;
   cfg.attrs = attr; cfg.numAttrs = cut ? 1 : 0;
-  cudaLaunchKernelEx(&cfg, zgemm_kernel<AK, BK_, CJ, M3>, ta, tb, kp);
+  if (kp.skip) cudaLaunchKernelEx(&cfg, zgemm_kernel<AK, BK_, CJ, M3, true>, ta, tb, kp);
+  else cudaLaunchKernelEx(&cfg, zgemm_kernel<AK, BK_, CJ, M3, false>, ta, tb, kp);
   count_launch();
 }
 template <bool AK, bool BK_, bool CJ>
@@ -453,10 +475,14 @@ void launch(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, const
 }
 template <bool AK, bool BK_>
 void set_smem_attr() {
-  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda).
@@ -589,8 +615,8 @@ void zgemm_configure() {
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev);
   int per_sm4 = 0;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, zgemm_kernel<true, true, true, true>, NTHREADS, SMEM_BYTES);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm4, zgemm_kernel<true, true, true, false>, NTHREADS, SMEM_BYTES);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, zgemm_kernel<true, true, true, true, false>, NTHREADS, SMEM_BYTES);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm4, zgemm_kernel<true, true, true, false, false>, NTHREADS, SMEM_BYTES);
   if (per_sm4 < per_sm) per_sm = per_sm4;
   if (const char *es = getenv("TDVP_ZGEMM_SPLIT_COST")) g_split_cost = atof(es);
   if (const char *e5 = getenv("TDVP_ZGEMM_NO_5D")) g_no_5d = e5[0] == '1';
@@ -684,6 +710,7 @@ int zgemm(cudaStream_t st, const ZGemm &p) {
   kp.upc_base = (int)(units / kp.G);
   kp.upc_rem = (int)(units % kp.G);
   kp.slots = ctx->slots; kp.cnt = ctx->cnt; kp.done = ctx->done;
+  kp.skip = p.skip;
   ProfScope ps(st, PH_ZGEMM);
   if (ak && bk) launch<true, true>(st, ta, tb, kp);
   else if (ak && !bk) launch<true, false>(st, ta, tb, kp);

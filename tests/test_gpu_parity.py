@@ -259,6 +259,81 @@ def test_expm_breakdown_small_space(T):
     assert rel(host(got), want) <= 1e-10
 
 
+def _hermitian_product_operator(Ml, d, Mr, seed):
+    """L, W, R with D_W = 1 and Hermitian factors: H = L (x) h (x) R^T is Hermitian, cheap at any size."""
+    rng = np.random.default_rng(seed)
+    def herm(n):
+        g = si.complex_normal(rng, (n, n))
+        return (g + g.conj().T) / (2.0 * np.sqrt(2.0 * n))
+    L = herm(Ml).reshape(Ml, 1, Ml)
+    R = herm(Mr).reshape(Mr, 1, Mr)
+    W = herm(d).reshape(1, d, d, 1) * 3.0
+    v = si.complex_normal(rng, (Ml, d, Mr))
+    return np.ascontiguousarray(L), np.ascontiguousarray(W), np.ascontiguousarray(R), v
+
+
+@pytest.mark.parametrize("case", [(100, 6, 100, 40, -0.9j),     # 41 vectors of 60 000: the basis does not fit in shared memory
+                                  (450, 10, 450, 4, 1.3j),       # 2 M elements: not even the chunk of w fits
+                                  (33, 3, 29, 64, -2.0j),        # k = 64: both halves of the coefficient warp
+                                  (16, 2, 16, 7, -0.4 + 0.3j)])  # z with a real part: eigen-decomposition path
+def test_expm_large_and_general(T, case):
+    Ml, d, Mr, k, z = case
+    L, W, R, v = _hermitian_product_operator(Ml, d, Mr, seed=70 + Ml)
+    want, m = lanczos.lanczos_expm(lambda x: oc.heff(L, W, x, R), v, z, k)
+    ctx = T.tdvp_create_context(T.make_options(krylov_dim=k))
+    got, mg = T.tdvp_expm_heff(dev(L), dev(W), dev(R), z, dev(v), handle=ctx, want_dim=True)
+    assert mg == m
+    assert rel(host(got), want) <= REL_TOL
+    ctx.close()
+
+
+@pytest.mark.parametrize("tol", [1e-6, 1e-10])
+def test_expm_adaptive_krylov_dimension(T, tol):
+    """opt.krylov_tol > 0 (reading c11): the device stops at the same Krylov
+    dimension as the oracle's rule, the result agrees to 1e-11, and the error against the dense
+    exponential is of the order of tol."""
+    import scipy.linalg
+    Ml, d, Mr = 12, 3, 10
+    L, W, R, v = _hermitian_product_operator(Ml, d, Mr, seed=5)
+    z = -4.0j
+    want, m = lanczos.lanczos_expm(lambda x: oc.heff(L, W, x, R), v, z, 48, tol=tol)
+    assert 4 < m < 48
+    ctx = T.tdvp_create_context(T.make_options(krylov_dim=48, krylov_tol=tol))
+    got, mg = T.tdvp_expm_heff(dev(L), dev(W), dev(R), z, dev(v), handle=ctx, want_dim=True)
+    assert mg == m
+    assert rel(host(got), want) <= REL_TOL
+    Hd = np.einsum("ax,st,by->asbxty", L[:, 0, :], W[0, :, :, 0], R[:, 0, :]).reshape(Ml * d * Mr, -1)
+    ref = scipy.linalg.expm(z * Hd) @ v.reshape(-1)
+    assert np.linalg.norm(host(got).reshape(-1) - ref) <= 20 * tol * np.linalg.norm(v)
+    # the bond operator through the same rule
+    rng = np.random.default_rng(6)
+    Dm = si.complex_normal(rng, (Ml, Mr))
+    want, m = lanczos.lanczos_expm(lambda x: oc.bond(L, x, R), Dm, -z, 48, tol=tol)
+    got, mg = T.tdvp_expm_bond(dev(L), dev(R), -z, dev(Dm), handle=ctx, want_dim=True)
+    assert mg == m and rel(host(got), want) <= REL_TOL
+    ctx.close()
+
+
+def test_tiny_chain_adaptive_krylov(T):
+    """TDVP-PS with the adaptive Krylov dimension (cap 30, tol 1e-9) against the oracle running the same
+    rule: 10 steps of configs[0], populations 1e-8; the converged dimension beats the fixed k = 10 run
+    against exact propagation (k = 10 costs 4e-6 there)."""
+    cfg = si.CONFIGS["tiny"]
+    params = si.draw_vibronic_params(cfg)
+    mpo = model.build_mpo(params)
+    mps = si.padded_product_mps(si.site_dims(params), si.initial_occupations(params), cfg.M, cfg.pad_seed)
+    st = tdvp_ps.PSState(mpo, mps)
+    ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=30, krylov_tol=1e-9))
+    for s in range(10):
+        tdvp_ps.step_ps(st, cfg.dt_fs, 30, tol=1e-9)
+        ch.tdvp_step_ps(cfg.dt_fs)
+        assert np.abs(ch.tdvp_populations(0) - obs.populations(st.mps)).max() <= 1e-8
+    assert 4 < max(st.krylov_dims) < 30 and len(set(st.krylov_dims)) > 1      # the rule, not the cap, stopped every exponential
+    nrm, _ = ch.tdvp_norm_energy()
+    assert abs(nrm - 1.0) < 1e-8                               # unitary up to the tolerance of the rule
+    ch.close()
+
+
 # ---- whole trajectories ---------------------------------------------------------------------
 @pytest.mark.parametrize("graph", [True, False])
 def test_tiny_chain_20_steps(T, graph):

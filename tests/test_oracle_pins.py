@@ -153,6 +153,32 @@ def test_p8_lanczos_truncated_is_unitary_and_accurate():
     assert np.abs(y - ref).max() < 1e-9
 
 
+@pytest.mark.parametrize("tol", [1e-6, 1e-10])
+def test_lanczos_adaptive_rule_meets_its_tolerance(tol):
+    """Reading c11 (the paper gives no criterion): stopping at the first j with
+    beta_j |[exp(z T_j) e_1]_j| < tol leaves an error of the order of tol * |v| against the dense
+    exponential, with far fewer than the allowed vectors, and a tighter tol uses more of them."""
+    rng = np.random.default_rng(10)
+    n = 200
+    G = si.complex_normal(rng, (n, n))
+    Hm = (G + G.conj().T) / 2 / np.sqrt(n)                    # spectrum in about [-2, 2]
+    v = si.complex_normal(rng, (n,))
+    z = -3.0j
+    y, m = lanczos.lanczos_expm(lambda x: Hm @ x, v, z, 64, tol=tol)
+    ref = scipy.linalg.expm(z * Hm) @ v
+    err = np.linalg.norm(y - ref) / np.linalg.norm(v)
+    assert err < 20 * tol, (err, m)
+    assert 8 < m < 40
+    y1, m1 = lanczos.lanczos_expm(lambda x: Hm @ x, v, z, m - 2, tol=0.0)     # two vectors fewer: not yet converged
+    assert np.linalg.norm(y1 - ref) / np.linalg.norm(v) > tol / 20
+    if tol == 1e-10:
+        _, m6 = lanczos.lanczos_expm(lambda x: Hm @ x, v, z, 64, tol=1e-6)
+        assert m6 < m
+    # tol = 0 is the fixed-k contract mode, unchanged
+    y0, m0 = lanczos.lanczos_expm(lambda x: Hm @ x, v, z, 12)
+    assert m0 == 12
+
+
 # ---------------------------------------------------------------- p3: TDVP-PS closed form
 def test_p3_ps_untruncated_equals_exact_propagation(tiny_model):
     """With complete bonds every backward step cancels a forward step and Eq. 42 reduces to
