@@ -263,6 +263,8 @@ long long tdvp_launch_count(void);
                               before (bit-identical by construction; read at every step);
      TDVP_CMF_QUEUES=n        side queues of the CMF local propagation (1..8, default 4; results are
                               bit-identical for any n), read when a handle first runs tdvp_step_mu_cmf;
+     TDVP_QR_CLUSTER=0        QR gauge moves of up to 1280 rows with one launch per panel and per trailing update
+                              instead of the single 16-CTA cluster kernel, read once;
      TDVP_SVD_MAX_SWEEPS=n    Jacobi sweeps a bond SVD may use (1..40, default 40; lowering it forces the
                               TDVP_ESTATE "did not converge" report: used by the error-path test), read at
                               every SVD. */

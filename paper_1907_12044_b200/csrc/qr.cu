@@ -13,6 +13,8 @@
 //                  (zlarfg-style reflectors), builds the compact-WY factor T, emits R entries
 //   trail kernel : X[:, c] <- (I - V T^H V^H) X[:, c] for the trailing columns (a few columns/CTA)
 //   the same kernel with T instead of T^H applied to identity columns, panels in reverse, forms Q.
+#include <cstdlib>
+
 #include "common.cuh"
 
 namespace {
@@ -286,6 +288,361 @@ __global__ void __maxnreg__(RP_THREADS <= 256 ? 255 : 128) qr_panel_reg_kernel(c
   }
   __syncthreads();
   if (tid < 32) build_T(Gs, tau_s, Ts, Tm, w);
+}
+
+// ---- cluster panel factorisation ---------------------------------------------------------------
+// The same column-by-column Householder elimination (one combined reduction per column, see above), with
+// the panel's rows spread over a thread-block CLUSTER of QC CTAs (QC SMs): a column step is bound by the
+// FP64 and shuffle throughput of the SM(s) that hold the panel -- 2.9 us per column for 1280 rows on one
+// SM -- and by the reduction's latency.  Here every CTA reduces its rows (warp level: a transposed
+// butterfly, 16 values in 16 shuffle steps instead of 75), pushes its 16 partial sums into the shared
+// memory of ALL CTAs of the cluster (st.shared::cluster), and after ONE cluster barrier every CTA adds
+// the QC partials in the same order, so all hold bit-identical scalars.  The pivot row (alpha and the
+// pivot entries of the other columns) travels in the same message from the CTA that owns it.  Exchange
+// slots are double-buffered by column parity, which makes one barrier per column enough.
+// Rows are dealt round-robin: local row i = r * (QC * QT) + cta * QT + tid.
+constexpr int QC = 16;                // CTAs per cluster (non-portable size: allowed explicitly in qr_configure)
+constexpr int QT = 256;               // threads per CTA
+constexpr int QW = QT / 32;
+
+__device__ __forceinline__ unsigned cluster_ctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_barrier() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n" ::: "memory");
+  asm volatile("barrier.cluster.wait.acquire.aligned;\n" ::: "memory");
+}
+__device__ __forceinline__ void st_cluster_f64(const double *local_addr, unsigned cta, double v) {
+  const unsigned la = (unsigned)__cvta_generic_to_shared(local_addr);
+  unsigned ra;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(la), "r"(cta));
+  asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(ra), "d"(v) : "memory");
+}
+// Sum 16 values per lane over the warp: afterwards lane l holds the total of value index
+// 8 b4 + 4 b3 + 2 b2 + b1 (b_k = bit k of l), in a fixed order.  16 shuffle steps.
+__device__ __forceinline__ double warp_reduce16(double (&v)[16], int lane, int &index) {
+#pragma unroll
+  for (int o = 16, half = 8; o >= 2; o >>= 1, half >>= 1) {
+    const bool bit = (lane & o) != 0;
+#pragma unroll
+    for (int i = 0; i < half; i++) {
+      const double send = bit ? v[i] : v[i + half];
+      const double keep = bit ? v[i + half] : v[i];
+      v[i] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+    }
+  }
+  index = ((lane >> 4) & 1) * 8 + ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1);
+  return v[0] + __shfl_xor_sync(0xffffffffu, v[0], 1);
+}
+
+// Exchange: every CTA contributes `n` doubles (n <= 64; loc[] in its own shared memory; entries >= n_sum are
+// taken from CTA `owner` only); afterwards tot[t] = sum over CTAs (t < n_sum) or owner's value, in all CTAs.
+__device__ __forceinline__ void cluster_exchange(const double *loc, int n, int n_sum, unsigned owner, double *exch /*[QC][64]*/,
+                                                 double *tot /*[64]*/, unsigned me) {
+  const int t = threadIdx.x;
+  if (t < n && (t < n_sum || me == owner)) {
+    const double v = loc[t];
+#pragma unroll
+    for (unsigned c = 0; c < QC; c++) st_cluster_f64(exch + me * 64 + t, c, v);
+  }
+  cluster_barrier();
+  if (t < n) {
+    double a;
+    if (t < n_sum) {
+      a = 0.0;
+#pragma unroll
+      for (int c = 0; c < QC; c++) a += exch[c * 64 + t];
+    } else {
+      a = exch[owner * 64 + t];
+    }
+    tot[t] = a;
+  }
+  __syncthreads();
+}
+
+// The WHOLE factorisation in one kernel, by one cluster: for every panel (1) the column-by-column
+// elimination above with the panel's rows spread over the cluster, (2) the compact-WY factor T, built by
+// every CTA for itself from the exchanged Gram sums, (3) the trailing update X[:, c] <- (I - V T^H V^H) X[:, c]
+// with the COLUMNS dealt round-robin to the CTAs (all rows of a column in one CTA: its reductions stay
+// inside the CTA, V is read back from global memory / L2 into registers once per panel and CTA).  Cluster
+// barriers separate the phases (their release / acquire covers global memory).  Against one launch per
+// panel and per update (2 x 16 launches for 128 columns) this removes the launch gaps and the cold
+// instruction fetch of every launch -- the panel kernel's stall profile was dominated by both -- and the
+// per-column reduction no longer waits on one SM's FP64 and shuffle throughput.
+// RA = rows per thread in the update (rows <= RA * QT), NB = panel width; rows per thread in the panel
+// phase RPT = ceil(RA / QC).  Forming Q stays a kernel of its own (one CTA per column, all SMs).
+template <int RA, int NB>
+__global__ void __cluster_dims__(QC, 1, 1) __launch_bounds__(QT, 1)
+qr_factor_cluster_kernel(c128 *X, int rows, int cols, c128 *Rm, c128 *Tm /*[npanels][NB_MAX][NB_MAX]*/) {
+  constexpr int RPT = (RA + QC - 1) / QC;
+  constexpr int NGRAM = NB * (NB - 1);                   // re / im of the strictly upper Gram entries (<= 56)
+  constexpr int NGB = (NGRAM + 15) / 16;                 // 16-value reduction rounds for them
+  extern __shared__ __align__(16) unsigned char qr_dyn_smem[];
+  c128 *vsm = reinterpret_cast<c128 *>(qr_dyn_smem);     // [NB][RA * QT]: the reflector block during the update
+  __shared__ double exch[2][QC * 64];
+  __shared__ double loc[64], tot[64];
+  __shared__ double wpart[QW][64];
+  __shared__ c128 tau_s[NB_MAX];
+  __shared__ c128 Ts[NB_MAX * NB_MAX];
+  __shared__ c128 Tl[NB_MAX * NB_MAX];
+  __shared__ c128 Gs[NB_MAX * NB_MAX];
+  const unsigned me = cluster_ctarank();
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int gthread = (int)me * QT + tid;
+  unsigned par = 0;                                         // parity of the exchange slots
+  cluster_barrier();                                        // every CTA of the cluster is running: its shared memory may be written
+  const int npanels = (cols + NB - 1) / NB;
+  for (int pz = 0; pz < npanels; pz++) {
+    const int j0 = pz * NB, w = cols - j0 < NB ? cols - j0 : NB;
+    const int len = rows - j0;
+    c128 *Tp = Tm + (size_t)pz * NB_MAX * NB_MAX;
+    auto row_of = [&](int r) { return r * (QC * QT) + gthread; };
+    // ---- (1) panel: rows round-robin over the cluster, in registers ----
+    c128 x[RPT][NB];
+#pragma unroll
+    for (int r = 0; r < RPT; r++) {
+      const int i = row_of(r);
+#pragma unroll
+      for (int c = 0; c < NB; c++)
+        x[r][c] = (i < len && c < w) ? __ldcg(X + (long long)(j0 + c) * rows + j0 + i) : make_double2(0.0, 0.0);
+    }
+    for (int i = gthread; i < j0; i += QC * QT)               // R entries above the panel rows are final
+      for (int c = 0; c < w; c++) Rm[(long long)i * cols + j0 + c] = __ldcg(X + (long long)(j0 + c) * rows + i);
+    for (int i = j0 + 1 + gthread; i < cols; i += QC * QT)    // zeros below the diagonal of R
+      for (int c = 0; c < w; c++)
+        if (i > j0 + c) Rm[(long long)i * cols + j0 + c] = make_double2(0.0, 0.0);
+    for (int jj = 0; jj < w; jj++) {
+      double red[16];
+#pragma unroll
+      for (int q = 0; q < 16; q++) red[q] = 0.0;
+#pragma unroll
+      for (int r = 0; r < RPT; r++) {
+        const int i = row_of(r);
+        if (i >= jj && i < len) {
+          const c128 u = x[r][0];
+          red[0] = fma(u.x, u.x, fma(u.y, u.y, red[0]));
+#pragma unroll
+          for (int c = 1; c < NB; c++) {
+            const c128 yv = x[r][c];
+            red[1 + 2 * (c - 1)] = fma(u.x, yv.x, fma(u.y, yv.y, red[1 + 2 * (c - 1)]));
+            red[2 + 2 * (c - 1)] = fma(u.x, yv.y, fma(-u.y, yv.x, red[2 + 2 * (c - 1)]));
+          }
+          if (i == jj) {                                      // pivot row: owner is CTA 0, thread jj (jj < NB <= QT)
+#pragma unroll
+            for (int c = 0; c < NB; c++) { loc[16 + 2 * c] = x[r][c].x; loc[17 + 2 * c] = x[r][c].y; }
+          }
+        }
+      }
+      int idx;
+      const double part = warp_reduce16(red, lane, idx);
+      if ((lane & 1) == 0) wpart[warp][idx] = part;
+      __syncthreads();
+      if (tid < 16) { double a = 0.0; for (int k = 0; k < QW; k++) a += wpart[k][tid]; loc[tid] = a; }
+      __syncthreads();
+      cluster_exchange(loc, 16 + 2 * NB, 16, 0u, exch[par], tot, me);
+      par ^= 1u;
+      const c128 alpha = make_double2(tot[16], tot[17]);
+      double xn2 = tot[0] - (alpha.x * alpha.x + alpha.y * alpha.y);
+      if (xn2 < 0.0) xn2 = 0.0;
+      c128 tau, scal;
+      double beta;
+      if (xn2 == 0.0 && alpha.y == 0.0) {
+        tau = make_double2(0.0, 0.0); scal = make_double2(0.0, 0.0); beta = alpha.x;
+      } else {
+        const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xn2);
+        beta = alpha.x >= 0.0 ? -nrm : nrm;
+        const double ib = 1.0 / beta;
+        tau = make_double2((beta - alpha.x) * ib, -alpha.y * ib);
+        const double dr = alpha.x - beta, di = alpha.y, idn = 1.0 / (dr * dr + di * di);
+        scal = make_double2(dr * idn, -di * idn);
+      }
+      if (tid == 0) {
+        tau_s[jj] = tau;                                    // every CTA keeps the taus: it builds T itself
+        if (me == 0) Rm[(long long)(j0 + jj) * cols + j0 + jj] = make_double2(beta, 0.0);
+      }
+      c128 g[NB];                                            // conj(tau) * (v^H y_c)
+#pragma unroll
+      for (int c = 1; c < NB; c++) {
+        const c128 dc = make_double2(tot[1 + 2 * (c - 1)], tot[2 + 2 * (c - 1)]);
+        const c128 yj = make_double2(tot[16 + 2 * c], tot[17 + 2 * c]);
+        const c128 t1 = cmul(cconj(alpha), yj);
+        const c128 t2 = cmul(cconj(scal), make_double2(dc.x - t1.x, dc.y - t1.y));
+        g[c] = cmul(cconj(tau), make_double2(yj.x + t2.x, yj.y + t2.y));
+        if (c >= NB - jj) g[c] = make_double2(0.0, 0.0);     // slots at the back hold finished reflectors: not columns
+      }
+      c128 *Xc = X + (long long)(j0 + jj) * rows + j0;
+#pragma unroll
+      for (int r = 0; r < RPT; r++) {
+        const int i = row_of(r);
+        if (i < len) {
+          if (i < jj) {                                      // above the diagonal: an R entry, zero in V
+            Rm[(long long)(j0 + i) * cols + j0 + jj] = x[r][0];
+            Xc[i] = make_double2(0.0, 0.0);
+          } else {
+            const c128 v = (i == jj) ? make_double2(1.0, 0.0) : cmul(x[r][0], scal);
+            Xc[i] = v;
+            x[r][0] = v;                                     // kept (rotated to the back below) for the Gram matrix
+#pragma unroll
+            for (int c = 1; c < NB; c++) {
+              x[r][c].x = fma(g[c].y, v.y, fma(-g[c].x, v.x, x[r][c].x));
+              x[r][c].y = fma(-g[c].y, v.x, fma(-g[c].x, v.y, x[r][c].y));
+            }
+          }
+        }
+        if (i >= len || i < jj) x[r][0] = make_double2(0.0, 0.0);
+        // rotate: the finished reflector goes to the back, so after w steps x[r][NB - w + a] = v_a[row]
+        const c128 fin = x[r][0];
+#pragma unroll
+        for (int c = 0; c < NB - 1; c++) x[r][c] = x[r][c + 1];
+        x[r][NB - 1] = fin;
+      }
+    }
+    // ---- (2) compact WY factor from the strictly upper Gram entries v_a^H v_b (reflector a sits in x[.][NB - w + a]) ----
+    if (NB > 1 && w > 1) {
+      double gr[NGB * 16];
+#pragma unroll
+      for (int q = 0; q < NGB * 16; q++) gr[q] = 0.0;
+      if (w == NB) {                                        // full panel: reflector a sits in slot a (static indexing)
+#pragma unroll
+        for (int r = 0; r < RPT; r++) {
+          int q = 0;
+#pragma unroll
+          for (int a = 0; a < NB - 1; a++) {
+            const c128 u = x[r][a];
+#pragma unroll
+            for (int b = a + 1; b < NB; b++) {
+              const c128 v = x[r][b];
+              gr[q] = fma(u.x, v.x, fma(u.y, v.y, gr[q]));
+              gr[q + 1] = fma(u.x, v.y, fma(-u.y, v.x, gr[q + 1]));
+              q += 2;
+            }
+          }
+        }
+      } else {                                              // the ragged last panel: slots NB - w + a, selected at run time
+#pragma unroll 1
+        for (int r = 0; r < RPT; r++) {
+          int q = 0;
+#pragma unroll
+          for (int a = 0; a < NB - 1; a++) {
+#pragma unroll
+            for (int b = a + 1; b < NB; b++) {
+              const int sa = NB - w + a, sb = NB - w + b;
+              if (b < w) {
+                c128 u = make_double2(0.0, 0.0), v = make_double2(0.0, 0.0);
+#pragma unroll
+                for (int c = 0; c < NB; c++) { if (c == sa) u = x[r][c]; if (c == sb) v = x[r][c]; }
+                gr[q] = fma(u.x, v.x, fma(u.y, v.y, gr[q]));
+                gr[q + 1] = fma(u.x, v.y, fma(-u.y, v.x, gr[q + 1]));
+              }
+              q += 2;
+            }
+          }
+        }
+      }
+#pragma unroll
+      for (int blk = 0; blk < NGB; blk++) {
+        double v16[16];
+#pragma unroll
+        for (int q = 0; q < 16; q++) v16[q] = gr[blk * 16 + q];
+        int idx;
+        const double part = warp_reduce16(v16, lane, idx);
+        if ((lane & 1) == 0) wpart[warp][blk * 16 + idx] = part;
+      }
+      __syncthreads();
+      if (tid < NGB * 16) { double a = 0.0; for (int k = 0; k < QW; k++) a += wpart[k][tid]; loc[tid] = a; }
+      __syncthreads();
+      cluster_exchange(loc, NGB * 16, NGB * 16, 0u, exch[par], tot, me);
+      par ^= 1u;
+      if (tid == 0) {
+        int q = 0;
+        for (int a = 0; a < NB - 1; a++)
+          for (int b = a + 1; b < NB; b++) { Gs[a * NB_MAX + b] = make_double2(tot[q], tot[q + 1]); q += 2; }
+      }
+    }
+    __syncthreads();
+    if (tid < 32) build_T(Gs, tau_s, Ts, me == 0 ? Tp : Tl, w);
+    cluster_barrier();                                      // V (global) complete and visible; Ts ready in every CTA
+    // ---- (3) trailing update: column c to CTA (c - c_begin) % QC, all its rows >= j0 in this CTA ----
+    const int c_begin = j0 + w;
+    if (c_begin + (int)me < cols) {
+      // the reflector block V of this panel: global memory / L2 -> shared memory, [q][row - j0] (its registers
+      // are needed for two columns in flight and the prefetch of the next two)
+#pragma unroll
+      for (int r = 0; r < RA; r++) {
+        const int i = j0 + tid + r * QT;
+#pragma unroll
+        for (int q = 0; q < NB; q++)
+          vsm[q * (RA * QT) + tid + r * QT] = (i < rows && q < w) ? __ldcg(X + (long long)(j0 + q) * rows + i) : make_double2(0.0, 0.0);
+      }
+      // (each thread reads back only what it wrote: no barrier needed)
+      auto v = [&](int r, int q) -> c128 { return vsm[q * (RA * QT) + tid + r * QT]; };
+      // two columns per pass (one pair of block barriers for both), the next pair's loads issued before the
+      // reductions of this one: a pass is a chain of latencies (L2 load, shuffles, barriers), not of flops
+      auto load_col = [&](int c, c128 (&y)[RA]) {
+#pragma unroll
+        for (int r = 0; r < RA; r++) {
+          const int i = j0 + tid + r * QT;
+          y[r] = (c < cols && i < rows) ? __ldcg(X + (long long)c * rows + i) : make_double2(0.0, 0.0);
+        }
+      };
+      c128 ya[RA], yb[RA];
+      int c = c_begin + (int)me;
+      load_col(c, ya); load_col(c + QC, yb);
+      for (; c < cols; c += 2 * QC) {
+        double acc[16], acc2[16];
+#pragma unroll
+        for (int q = 0; q < 16; q++) acc[q] = acc2[q] = 0.0;
+#pragma unroll
+        for (int r = 0; r < RA; r++)
+#pragma unroll
+          for (int q = 0; q < NB; q++) {
+            const c128 vv = v(r, q);
+            acc[2 * q] = fma(vv.x, ya[r].x, fma(vv.y, ya[r].y, acc[2 * q]));
+            acc[2 * q + 1] = fma(vv.x, ya[r].y, fma(-vv.y, ya[r].x, acc[2 * q + 1]));
+            acc2[2 * q] = fma(vv.x, yb[r].x, fma(vv.y, yb[r].y, acc2[2 * q]));
+            acc2[2 * q + 1] = fma(vv.x, yb[r].y, fma(-vv.y, yb[r].x, acc2[2 * q + 1]));
+          }
+        int idx;
+        const double part = warp_reduce16(acc, lane, idx);
+        const double part2 = warp_reduce16(acc2, lane, idx);
+        if ((lane & 1) == 0) { wpart[warp][idx] = part; wpart[warp][16 + idx] = part2; }
+        __syncthreads();
+        if (tid < 32) { double a = 0.0; for (int k = 0; k < QW; k++) a += wpart[k][tid]; loc[tid] = a; }
+        __syncthreads();
+        if (tid < 2 * NB) {                                 // T^H (V^H y): one component of one column per thread, then shared
+          const int col = tid / NB, q = tid % NB;
+          c128 a = make_double2(0.0, 0.0);
+#pragma unroll
+          for (int r = 0; r < NB; r++) {
+            const c128 pr = cmul(cconj(Ts[r * NB_MAX + q]), make_double2(loc[16 * col + 2 * r], loc[16 * col + 2 * r + 1]));
+            a.x += pr.x; a.y += pr.y;
+          }
+          tot[16 * col + 2 * q] = a.x; tot[16 * col + 2 * q + 1] = a.y;
+        }
+        __syncthreads();
+        c128 na[RA], nb2[RA];
+        load_col(c + 2 * QC, na); load_col(c + 3 * QC, nb2);    // next pair: in flight during the update below
+#pragma unroll
+        for (int r = 0; r < RA; r++) {
+#pragma unroll
+          for (int q = 0; q < NB; q++) {
+            const c128 s1 = make_double2(tot[2 * q], tot[2 * q + 1]), s2 = make_double2(tot[16 + 2 * q], tot[17 + 2 * q]);
+            const c128 vv = v(r, q);
+            ya[r].x = fma(vv.y, s1.y, fma(-vv.x, s1.x, ya[r].x));
+            ya[r].y = fma(-vv.y, s1.x, fma(-vv.x, s1.y, ya[r].y));
+            yb[r].x = fma(vv.y, s2.y, fma(-vv.x, s2.x, yb[r].x));
+            yb[r].y = fma(-vv.y, s2.x, fma(-vv.x, s2.y, yb[r].y));
+          }
+          const int i = j0 + tid + r * QT;
+          if (i < rows) {
+            X[(long long)c * rows + i] = ya[r];
+            if (c + QC < cols) X[(long long)(c + QC) * rows + i] = yb[r];
+          }
+          ya[r] = na[r]; yb[r] = nb2[r];
+        }
+        // wpart / loc / tot are rewritten only after the next pass's first barrier ... tot after its second
+      }
+    }
+    cluster_barrier();                                      // the updated columns are visible before the next panel is read
+  }
 }
 
 // Factor the panel of columns [j0, j0+w) on rows [j0, rows).  Writes reflectors back into X (unit
@@ -634,7 +991,27 @@ int panel_width(int rows) {
 
 }  // namespace
 
+constexpr int QF_SMEM = 40 * QT * 16;   // RA * NB = 40 reflector entries per thread in every mode
+int g_qr_cluster = 1;            // TDVP_QR_CLUSTER=0: one launch per panel and per trailing update (diagnostic switch)
+int g_qr_cluster_min = 0;        // matrices with more rows than this use the cluster kernel (TDVP_QR_CLUSTER_MIN)
+
 void qr_configure() {
+  cudaFuncSetAttribute(qr_factor_cluster_kernel<5, 8>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+  cudaFuncSetAttribute(qr_factor_cluster_kernel<5, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, QF_SMEM);
+  {                                                       // can a 16-CTA cluster of this kernel be resident at all?
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(QC); cfg.blockDim = dim3(QT); cfg.dynamicSmemBytes = QF_SMEM;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = QC; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    int nclusters = 0;
+    if (cudaOccupancyMaxActiveClusters(&nclusters, qr_factor_cluster_kernel<5, 8>, &cfg) != cudaSuccess || nclusters < 1) {
+      cudaGetLastError();
+      g_qr_cluster = 0;
+    }
+  }
+  if (const char *e = getenv("TDVP_QR_CLUSTER")) g_qr_cluster = g_qr_cluster && e[0] != '0';
+  if (const char *e = getenv("TDVP_QR_CLUSTER_MIN")) g_qr_cluster_min = atoi(e);
   cudaFuncSetAttribute(qr_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024 + 1024);
 }
 
@@ -675,6 +1052,13 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
   if (side == 0) TDVP_LAUNCH(transpose_in_kernel, tg, tb, 0, st, C, X, rows, cols);
   else TDVP_LAUNCH(copy_kernel, gcopy, 256, 0, st, X, C, n);
   const int npanels = (cols + nb - 1) / nb;
+  if (g_qr_cluster && mode == 1 && rows > g_qr_cluster_min) {
+    // up to 1280 rows: the whole factorisation (panels + trailing updates) in ONE cluster kernel.  Measured
+    // (B200, 1280 x 128): 580 us against 698 us with one launch per panel and per update; at 2560 x 256 the
+    // 16 SMs of the cluster are too few for the trailing updates (2170 against 1924 us), so taller matrices
+    // keep the launch-per-panel path below.
+    TDVP_LAUNCH((qr_factor_cluster_kernel<5, 8>), QC, QT, QF_SMEM, st, X, rows, cols, Rm, Tm);
+  } else
   for (int pz = 0; pz < npanels; pz++) {
     int j0 = pz * nb, w = cols - j0 < nb ? cols - j0 : nb;
     size_t smem = (size_t)w * (rows - j0) * 16;

@@ -432,3 +432,113 @@ def test_to_right_canonical_keeps_the_state(warmed_up):
     assert np.linalg.norm(v1 - v0) < 1e-12 and np.linalg.norm(v2 - v0) < 1e-12
     assert abs(np.vdot(v2, v0) - 1.0) < 1e-12
     assert [a.shape for a in rc] == [a.shape for a in warm]
+
+
+# ---------------------------------------------------------------- P&C-RK4 building blocks (Eq. 10, 13, 15, 16)
+def _random_mps(dims, bonds, seed):
+    rng = np.random.default_rng(seed)
+    return [si.complex_normal(rng, (bonds[i], dims[i], bonds[i + 1])) for i in range(len(dims))]
+
+
+def test_pc_mpo_times_mps_and_add_against_dense_vectors():
+    """Eq. 13: the MPS of H|Psi> contracts to H_dense @ psi and has bond dimension M_O * M_S (PAPER.md:105);
+    Eq. 15: the merged MPS contracts to the linear combination and has bond M_A + M_B."""
+    from oracle import pc_rk4
+    p = _small_params("A", n_el=3, n_modes=1, n_ph=3)
+    H, dims = model.kronecker_sum_hamiltonian(p)
+    mpo = model.build_mpo(p)
+    a = _random_mps(dims, [1, 3, 4, 2, 1], 41)
+    b = _random_mps(dims, [1, 2, 5, 3, 1], 42)
+    c = _random_mps(dims, [1, 1, 1, 1, 1], 43)
+    va, vb, vc = (obs.mps_to_vector(x) for x in (a, b, c))
+    ha = pc_rk4.mpo_times_mps(mpo, a)
+    assert np.abs(obs.mps_to_vector(ha) - H @ va).max() < 1e-12 * np.abs(H @ va).max()
+    assert [t.shape[2] for t in ha] == [mpo[i].shape[3] * a[i].shape[2] for i in range(len(a))]
+    s = pc_rk4.mps_add([(1.0, a), (0.5 - 2.0j, b), (-3.0, c)])
+    want = va + (0.5 - 2.0j) * vb - 3.0 * vc
+    assert np.abs(obs.mps_to_vector(s) - want).max() < 1e-13 * np.abs(want).max()
+    assert [t.shape[2] for t in s] == [3 + 2 + 1, 4 + 5 + 1, 2 + 3 + 1, 1]
+    assert s[0].shape[0] == 1
+
+
+def test_pc_compress_is_the_truncated_svd():
+    """Eq. 10.  Two sites: the compressed state is the best rank-M approximation of the coefficient matrix
+    (Eckart-Young: same singular values kept, error^2 = discarded weight).  Four sites: no truncation leaves
+    the vector unchanged and returns a right-canonical MPS (Eq. 8) with the bond dimensions capped by the
+    shapes; with truncation, max(discarded) <= |Psi - Psi~|^2 <= sum(discarded)."""
+    from oracle import pc_rk4
+    two = _random_mps([5, 6], [1, 9, 1], 51)                 # bond 9 > min(5, 6): canonicalisation caps it at 5
+    v = obs.mps_to_vector(two).reshape(5, 6)
+    sv = np.linalg.svd(v, compute_uv=False)
+    for M in (5, 3, 1):
+        comp, disc = pc_rk4.compress(two, M)
+        vc = obs.mps_to_vector(comp).reshape(5, 6)
+        assert comp[0].shape == (1, 5, M) and comp[1].shape == (M, 6, 1)
+        assert abs(np.linalg.norm(v - vc) ** 2 - np.sum(sv[M:] ** 2)) < 1e-12
+        assert abs(disc[0] - np.sum(sv[M:] ** 2)) < 1e-12
+        assert np.abs(np.linalg.svd(vc, compute_uv=False)[:M] - sv[:M]).max() < 1e-12
+    dims = [3, 4, 2, 5]
+    four = _random_mps(dims, [1, 7, 9, 6, 1], 52)
+    v = obs.mps_to_vector(four)
+    comp, disc = pc_rk4.compress(four, 64)
+    assert [t.shape[2] for t in comp] == [3, 9, 5, 1] and sum(disc) < 1e-24     # min(raw bond, left cap, right cap)
+    assert np.linalg.norm(obs.mps_to_vector(comp) - v) < 1e-12 * np.linalg.norm(v)
+    for A in comp[1:]:
+        m = A.reshape(A.shape[0], -1)
+        assert np.abs(m @ m.conj().T - np.eye(A.shape[0])).max() < 1e-13
+    comp, disc = pc_rk4.compress(four, 3)
+    err2 = np.linalg.norm(obs.mps_to_vector(comp) - v) ** 2
+    assert max(disc) * (1 - 1e-12) <= err2 <= sum(disc) * (1 + 1e-12)
+    assert [t.shape[2] for t in comp] == [3, 3, 3, 1]
+
+
+def test_pc_rk4_is_dense_rk4_and_fourth_order(tiny_model):
+    """Eq. 16.  Without truncation (M_max = 64 holds every state of config 1's chain) P&C-RK4 is the classical
+    RK4 of i d/dt psi = H psi on the full vector, to round-off; against exact propagation its global error
+    falls as tau^4 (slope 3.5-4.5)."""
+    from oracle import pc_rk4
+    cfg, params, mpo, dims, occ = tiny_model
+    H, _ = model.kronecker_sum_hamiltonian(params)
+    prod = [np.zeros((1, d, 1), dtype=np.complex128) for d in dims]
+    for t, o in zip(prod, occ):
+        t[0, o, 0] = 1.0
+    psi0 = obs.mps_to_vector(prod)
+    tau = 0.5
+    f = lambda y: -1j * (H @ y)
+    k1 = f(psi0); k2 = f(psi0 + 0.5 * tau * k1); k3 = f(psi0 + 0.5 * tau * k2); k4 = f(psi0 + tau * k3)
+    dense = psi0 + tau / 6.0 * (k1 + 2 * k2 + 2 * k3 + k4)
+    got = pc_rk4.rk4_step(mpo, prod, tau, 64)
+    assert np.linalg.norm(obs.mps_to_vector(got) - dense) < 1e-13
+    T = 4.0
+    exact_T = list(exact.propagate(H, psi0, T, 1))[-1]
+    errs = []
+    for n in (4, 8, 16):
+        psi = prod
+        for _ in range(n):
+            psi = pc_rk4.rk4_step(mpo, psi, T / n, 64)
+        errs.append(np.linalg.norm(obs.mps_to_vector(psi) - exact_T))
+    slopes = [np.log2(errs[i] / errs[i + 1]) for i in range(2)]
+    assert all(3.5 < s < 4.5 for s in slopes), (errs, slopes)
+
+
+def test_pc_warmup_fills_the_bonds(tiny_model):
+    """after the P&C-RK4 warm-up and the compression to M_S the state is right-canonical
+    with the bond dimensions the shapes allow, close to the exactly propagated state, and its bonds are
+    numerically full rank (what one-site TDVP needs) -- unlike the padded product state."""
+    from oracle import pc_rk4
+    cfg, params, mpo, dims, occ = tiny_model
+    H, _ = model.kronecker_sum_hamiltonian(params)
+    prod = [np.zeros((1, d, 1), dtype=np.complex128) for d in dims]
+    for t, o in zip(prod, occ):
+        t[0, o, 0] = 1.0
+    tau, n = 80 * 0.0241888, 10                               # the paper's 80 a.u., in fs
+    warm = pc_rk4.warmup(mpo, prod, tau, n, 32, cfg.M)
+    assert [t.shape[2] for t in warm] == si.capped_bonds(dims, cfg.M)[1:]
+    for A in warm[1:]:
+        m = A.reshape(A.shape[0], -1)
+        assert np.abs(m @ m.conj().T - np.eye(A.shape[0])).max() < 1e-13
+    psi = list(exact.propagate(H, obs.mps_to_vector(prod), tau * n, 1))[-1]
+    assert np.linalg.norm(obs.mps_to_vector(warm) - psi) < 1e-3
+    lc = tdvp_mu.to_left_canonical(warm)
+    sv = np.linalg.svd(lc[-1].reshape(lc[-1].shape[0], -1), compute_uv=False)
+    assert sv[-1] > 1e-9 * sv[0]                              # the last bond carries weight in every state
