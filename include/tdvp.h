@@ -157,6 +157,24 @@ int tdvp_qr_gauge(tdvp_handle *h, int side, int Ml, int d, int Mr,
 int tdvp_svd_bond(tdvp_handle *h, int Ml, int d, int Mr, const tdvp_c128 *C /*DEVICE*/,
                   tdvp_c128 *U /*DEVICE*/, double *lam /*DEVICE*/, tdvp_c128 *Vh /*DEVICE*/);
 
+/* Propagation and compression with the classical Runge-Kutta method (P&C-RK4), the paper's warm-up of its
+   TDVP runs ("P&C-RK4 ... with M_max = 256 and time step size tau = 80 a.u. in the first 10
+   steps ... Thereafter, the state is compressed to the pre-defined bond dimension M_S"), built from MPO x MPS
+   (Eq. 12-13), MPS + MPS (Eq. 14-15), canonicalisation (Eq. 9) and SVD
+   compression (Eq. 10), all on the device.  n_steps RK4 steps of size tau (Eq. 16,
+   PAPER.md:119-131; every MPO x MPS product and every linear combination is compressed to M_max, reading
+   c20), then one compression to M_out.  n_steps = 0 is a plain canonicalise-and-compress of the input.
+     mpo / mps          as in tdvp_create (HOST pointers, HOST tensors); the MPS need not be canonical
+     mps_bond_out[N+1]  HOST out: bond dimensions of the result, min(M_out, k_i) with k_i what the shapes allow
+     mps_out[N]         HOST pointers to caller buffers; mps_out[i] must hold cap_i * d_i * cap_{i+1} elements,
+                        cap_i = min(M_out, d_0...d_{i-1}, d_i...d_{N-1}); filled as [bond_i, d_i, bond_{i+1}]
+   The result is right-canonical (Eq. 8) with the gauge centre at site 0: the input tdvp_create expects.
+   h: stream + error slot (NULL: default).  Blocks.  Limits: M_O * M * d <= 12800 rows in every QR / SVD
+   (TDVP_EINVAL beyond); bonds above 128 use the slow generic Jacobi SVD. */
+int tdvp_pc_rk4_warmup(tdvp_handle *h, int n_sites, const int *phys_dim, const int *mpo_bond,
+                       const tdvp_c128 *const *mpo, const int *mps_bond, const tdvp_c128 *const *mps,
+                       double tau, int n_steps, int M_max, int M_out, int *mps_bond_out, tdvp_c128 *const *mps_out);
+
 /* ---- stateful calls on the handle's resident MPS / environment cache ---------------------- */
 
 /* H[site] applied to A_dev using the cached L[site], R[site] (valid when the gauge centre is at

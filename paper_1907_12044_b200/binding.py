@@ -32,7 +32,7 @@ EXPORTED_SYMBOLS = [
     "tdvp_step_ps", "tdvp_step_mu", "tdvp_step_mu_cmf", "tdvp_mu_derivative", "tdvp_set_gauge", "tdvp_observe", "tdvp_populations",
     "tdvp_norm_energy", "tdvp_get_mps", "tdvp_set_mps", "tdvp_get_centre", "tdvp_sync",
     "tdvp_last_error", "tdvp_probe_fp64_tensor_peak", "tdvp_probe_dmma_issue", "tdvp_set_gemm_products", "tdvp_get_gemm_products", "tdvp_launch_count", "tdvp_profile_enable",
-    "tdvp_profile_read",
+    "tdvp_profile_read", "tdvp_pc_rk4_warmup",
 ]
 
 
@@ -91,6 +91,8 @@ def _load():
         "tdvp_get_gemm_products": (c_int, []),
         "tdvp_profile_enable": (c_int, [c_int]),
         "tdvp_profile_read": (c_int, [POINTER(c_double), POINTER(c_longlong)]),
+        "tdvp_pc_rk4_warmup": (c_int, [P, c_int, POINTER(c_int), POINTER(c_int), POINTER(P), POINTER(c_int), POINTER(P),
+                                       c_double, c_int, c_int, c_int, POINTER(c_int), POINTER(P)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -261,6 +263,31 @@ def tdvp_svd_bond(C, handle=None):
     h = _hptr(handle)
     _check(_lib.tdvp_svd_bond(h, Ml, d, Mr, _dev(C), _dev(U), c_void_p(lam.data_ptr()), _dev(Vh)), h)
     return U, lam, Vh
+
+
+def tdvp_pc_rk4_warmup(mpo, mps, tau, n_steps, M_max, M_out, handle=None):
+    """P&C-RK4 warm-up (include/tdvp.h): HOST numpy MPO / MPS in, list of HOST numpy site tensors out
+    (right-canonical, centre at site 0, bonds min(M_out, what the shapes allow))."""
+    n = len(mps)
+    keep = [np.ascontiguousarray(t, dtype=np.complex128) for t in list(mpo) + list(mps)]
+    phys = [int(A.shape[1]) for A in mps]
+    mpo_bond = [int(W.shape[0]) for W in mpo] + [int(mpo[-1].shape[3])]
+    mps_bond = [int(A.shape[0]) for A in mps] + [int(mps[-1].shape[2])]
+    left, right = [1] * (n + 1), [1] * (n + 1)
+    for i in range(n):
+        left[i + 1] = min(left[i] * phys[i], 1 << 40)
+    for i in range(n - 1, -1, -1):
+        right[i] = min(right[i + 1] * phys[i], 1 << 40)
+    cap = [int(min(M_out, left[i], right[i])) for i in range(n + 1)]
+    outs = [np.zeros(cap[i] * phys[i] * cap[i + 1], dtype=np.complex128) for i in range(n)]
+    PA, IA, IB = c_void_p * n, c_int * n, c_int * (n + 1)
+    bonds = IB()
+    h = _hptr(handle)
+    _check(_lib.tdvp_pc_rk4_warmup(h, n, IA(*phys), IB(*mpo_bond), PA(*[t.ctypes.data for t in keep[:n]]), IB(*mps_bond),
+                                   PA(*[t.ctypes.data for t in keep[n:]]), float(tau), int(n_steps), int(M_max), int(M_out),
+                                   bonds, PA(*[o.ctypes.data for o in outs])), h)
+    b = list(bonds)
+    return [outs[i][:b[i] * phys[i] * b[i + 1]].reshape(b[i], phys[i], b[i + 1]).copy() for i in range(n)]
 
 
 def tdvp_probe_fp64_tensor_peak(iters=20000) -> float:

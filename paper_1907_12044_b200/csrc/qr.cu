@@ -23,6 +23,10 @@ constexpr int NB_MAX = 8;
 constexpr int PANEL_THREADS = 1024;
 constexpr int TRAIL_THREADS = 256;
 constexpr int CB = 4;   // columns per CTA in the trailing update
+// A column whose squared norm is below this (entries below ~1e-145: products of round-off residues along a
+// chain of rank-deficient bonds get there) is treated as zero: H = I, the entries below the diagonal are dropped.
+// Its squared norm would underflow and the reflector scalars 1 / beta, 1 / |alpha - beta|^2 would be Inf / NaN.
+constexpr double TINY_NORM2 = 1e-290;
 
 inline size_t up256(size_t x) { return (x + 255) & ~size_t(255); }
 
@@ -176,7 +180,7 @@ __device__ __forceinline__ void qr_panel_col(c128 (&x)[RPT][NB], c128 (*pivot)[N
   if (xn2 < 0.0) xn2 = 0.0;
   c128 tau, scal;
   double beta;
-  if (xn2 == 0.0 && alpha.y == 0.0) {
+  if ((xn2 == 0.0 && alpha.y == 0.0) || alpha.x * alpha.x + alpha.y * alpha.y + xn2 < TINY_NORM2) {
     tau = make_double2(0.0, 0.0); scal = make_double2(0.0, 0.0); beta = alpha.x;
   } else {
     const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xn2);
@@ -444,7 +448,7 @@ qr_factor_cluster_kernel(c128 *X, int rows, int cols, c128 *Rm, c128 *Tm /*[npan
       if (xn2 < 0.0) xn2 = 0.0;
       c128 tau, scal;
       double beta;
-      if (xn2 == 0.0 && alpha.y == 0.0) {
+      if ((xn2 == 0.0 && alpha.y == 0.0) || alpha.x * alpha.x + alpha.y * alpha.y + xn2 < TINY_NORM2) {
         tau = make_double2(0.0, 0.0); scal = make_double2(0.0, 0.0); beta = alpha.x;
       } else {
         const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xn2);
@@ -692,7 +696,7 @@ __global__ void __launch_bounds__(PANEL_THREADS) qr_panel_kernel(c128 *X, int ro
       c128 alpha = x[jj];
       c128 tau, scal;
       double beta;
-      if (xn2 == 0.0 && alpha.y == 0.0) {
+      if ((xn2 == 0.0 && alpha.y == 0.0) || alpha.x * alpha.x + alpha.y * alpha.y + xn2 < TINY_NORM2) {
         tau = make_double2(0.0, 0.0); scal = make_double2(0.0, 0.0); beta = alpha.x;
       } else {
         double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xn2);

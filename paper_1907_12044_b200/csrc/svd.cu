@@ -23,6 +23,9 @@ namespace cg = cooperative_groups;
 namespace {
 
 constexpr int MAX_SWEEPS = 40;
+// A sweep that still rotates only pairs whose cosine is below this is "hovering at round-off" (the threshold
+// sqrt(n) eps sits at the error level of the dot product itself), not a failure to converge.
+constexpr double COARSE_TOL2 = 1e-20;
 inline size_t up256(size_t x) { return (x + 255) & ~size_t(255); }
 
 __device__ __forceinline__ double wsum(double v) {
@@ -62,7 +65,7 @@ svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/,
   const double tol2 = tol * tol;
   int sweep = 0;
   for (; sweep < max_sweeps; sweep++) {
-    bool any = false;
+    bool any = false, coarse = false;
     for (int round = 0; round < np - 1; round++) {
       for (int k = gwarp; k < npairs; k += nwarps) {
         int p, q;
@@ -106,6 +109,7 @@ svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/,
         const double c2 = cr * cr + ci * ci;
         if (!(c2 > tol2 * a * b) || c2 == 0.0) continue;
         any = true;
+        if (c2 > COARSE_TOL2 * a * b) coarse = true;
         // y_q = e^{-i phi} x_q makes <x_p, y_q> = |c| real; then a real rotation (cs, sn)
         const double cabs = sqrt(c2), icabs = 1.0 / cabs;
         const double er = cr * icabs, ei = -ci * icabs;          // e^{-i phi}
@@ -136,13 +140,16 @@ svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/,
         }
       }
       if (round == np - 2 && any && lane == 0) flags[sweep] = 1;   // benign race: every writer stores 1
+      if (round == np - 2 && coarse && lane == 0) flags[64 + sweep] = 1;
       cluster.sync();
     }
     if (np < 2) break;
     if (__ldcg(flags + sweep) == 0) break;                          // nobody rotated in this sweep
   }
-  // every sweep allowed still rotated: the columns are NOT orthogonal to tolerance -- tell the host
-  if (sweep == max_sweeps && np >= 2 && status && gwarp == 0 && lane == 0) atomicOr(status, TDVP_STATUS_SVD_UNCONVERGED);
+  // every sweep allowed still rotated, and the last one still saw a pair far from orthogonal (rotations that
+  // hover at the round-off threshold of sqrt(n) eps are convergence): tell the host
+  if (sweep == max_sweeps && np >= 2 && status && gwarp == 0 && lane == 0 && __ldcg(flags + 64 + max_sweeps - 1))
+    atomicOr(status, TDVP_STATUS_SVD_UNCONVERGED);
 }
 
 // Block variant for n <= 128: the same rotations, but the cluster barrier is paid once per BLOCK pair
@@ -155,7 +162,7 @@ svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/,
 constexpr int JB = 16;              // column blocks
 
 template <int NPL>
-__device__ __forceinline__ bool jacobi_pair_smem(c128 *xp, c128 *xq, c128 *jp, c128 *jq, int n, int lane, double tol2) {
+__device__ __forceinline__ int jacobi_pair_smem(c128 *xp, c128 *xq, c128 *jp, c128 *jq, int n, int lane, double tol2) {
   c128 xu[NPL], xv[NPL], ju[NPL], jv[NPL];
   double a = 0.0, b = 0.0, cr = 0.0, ci = 0.0;
 #pragma unroll
@@ -174,7 +181,8 @@ __device__ __forceinline__ bool jacobi_pair_smem(c128 *xp, c128 *xq, c128 *jp, c
   }
   a = wsum(a); b = wsum(b); cr = wsum(cr); ci = wsum(ci);
   const double c2 = cr * cr + ci * ci;
-  if (!(c2 > tol2 * a * b) || c2 == 0.0) return false;
+  if (!(c2 > tol2 * a * b) || c2 == 0.0) return 0;
+  const int result = c2 > COARSE_TOL2 * a * b ? 3 : 1;
   // the scalar chain is the critical path of a round: reciprocal square roots instead of sqrt + divide
   const double icabs = rsqrt(c2);
   const double er = cr * icabs, ei = -ci * icabs;                // e^{-i phi}
@@ -195,7 +203,7 @@ __device__ __forceinline__ bool jacobi_pair_smem(c128 *xp, c128 *xq, c128 *jp, c
       rot(ju[r], jv[r], o1, o2); jp[i] = o1; jq[i] = o2;
     }
   }
-  return true;
+  return result;
 }
 
 template <int NPL>
@@ -229,7 +237,7 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
   const int bwp = (bw + 1) & ~1;                          // players of the in-block tournament
   int sweep = 0;
   for (; sweep < max_sweeps; sweep++) {
-    bool any = false;
+    int any = 0;
     // (i) pairs inside blocks 2 cta and 2 cta + 1: warps 0-3 take the first block, 4-7 the second
     {
       const int b0 = 2 * cta, b1 = 2 * cta + 1;
@@ -271,11 +279,12 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
         store_blocks(bp, bq);
       }
       if (round == JB - 2 && any && lane == 0) flags[sweep] = 1;   // benign race: every writer stores 1
+      if (round == JB - 2 && (any & 2) && lane == 0) flags[64 + sweep] = 1;
       cluster.sync();
     }
     if (__ldcg(flags + sweep) == 0) break;                          // nobody rotated in this sweep
   }
-  if (sweep == max_sweeps && status && cta == 0 && tid == 0) atomicOr(status, TDVP_STATUS_SVD_UNCONVERGED);
+  if (sweep == max_sweeps && status && cta == 0 && tid == 0 && __ldcg(flags + 64 + max_sweeps - 1)) atomicOr(status, TDVP_STATUS_SVD_UNCONVERGED);
 }
 
 // lam (descending), U and the permuted J from X = U' R' (Qp = U'^T, Dp = R'^T as qr_gauge side 1 returns them).
@@ -321,7 +330,7 @@ void svd_configure() {
 size_t svd_ws_bytes(int Ml, int d, int Mr) {
   const size_t n = Ml, nn = up256(n * n * 16);
   size_t q1 = qr_ws_bytes(d * Mr, Ml), q2 = qr_ws_bytes(Ml, Ml);
-  return up256((size_t)Ml * d * Mr * 16) + 6 * nn + 256 + up256(q1 > q2 ? q1 : q2) + 1024;
+  return up256((size_t)Ml * d * Mr * 16) + 6 * nn + 512 + up256(q1 > q2 ? q1 : q2) + 1024;
 }
 
 // C [Ml, d, Mr] -> U [Ml, Ml], lam [Ml], Vh [Ml, d, Mr]
@@ -340,12 +349,12 @@ void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, do
   c128 *Qp = reinterpret_cast<c128 *>(p); p += nn;
   c128 *Dp = reinterpret_cast<c128 *>(p); p += nn;
   c128 *JtP = reinterpret_cast<c128 *>(p); p += nn;
-  int *flags = reinterpret_cast<int *>(p); p += 256;
+  int *flags = reinterpret_cast<int *>(p); p += 512;        // [0, 40): a sweep rotated; [64, 104): ... a pair far from orthogonal
   void *qws = p;
   qr_gauge(st, 1, Ml, d, Mr, C, Q, D, qws);                               // C = D Q
   const int g = (n * n + 255) / 256 > 296 ? 296 : (n * n + 255) / 256;
   TDVP_LAUNCH(svd_init_kernel, g, 256, 0, st, D, Xt, Jt, n);
-  cudaMemsetAsync(flags, 0, MAX_SWEEPS * sizeof(int), st);
+  cudaMemsetAsync(flags, 0, 128 * sizeof(int), st);
   const size_t bsm = (size_t)4 * ((n + JB - 1) / JB) * n * sizeof(c128);      // X and J of two blocks
   if (n <= 16) TDVP_LAUNCH(svd_jacobi_kernel<1>, JC, JW * 32, 0, st, Xt, Jt, n, flags, max_sweeps, status);
   else if (n <= 32) TDVP_LAUNCH(svd_jacobi_block_kernel<1>, JC, JW * 32, bsm, st, Xt, Jt, n, flags, max_sweeps, status);

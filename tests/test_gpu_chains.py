@@ -182,7 +182,7 @@ def test_layout_b_chain_free_running(T):
         want = np.array([obs.populations(st.mps, e)[1] for e in el_sites])
         got = np.array([ch.tdvp_populations(e)[1] for e in el_sites])
         assert np.abs(got - want).max() <= 1e-8
-        assert abs(got.sum() - 1.0) <= 1e-10                    # one exciton
+        assert abs(got.sum() - 1.0) <= 1e-4                     # one exciton, up to the delta^2 weight the seeding puts outside that sector
     check_state(T, ch, mpo, st.mps, pop_tol=1e-8, ov_tol=1e-8, pop_sites=el_sites)
     # one CMF step in the same layout
     lc = tdvp_mu.to_left_canonical(st.mps)
@@ -190,4 +190,59 @@ def test_layout_b_chain_free_running(T):
     want = tdvp_cmf.step_cmf(mpo, lc, 0.05, 4, cfg.krylov_dim)
     ch.tdvp_step_mu_cmf(0.05, 4)
     check_state(T, ch, mpo, want, pop_tol=1e-8, ov_tol=1e-8, pop_sites=el_sites)
+    ch.close()
+
+
+# ---- P&C-RK4 warm-up ---------------------------------------
+def _product_state(dims, occ):
+    prod = [np.zeros((1, d, 1), dtype=np.complex128) for d in dims]
+    for t, o in zip(prod, occ):
+        t[0, o, 0] = 1.0
+    return prod
+
+
+def test_pc_rk4_compress_only(T):
+    """n_steps = 0: canonicalise + SVD compression (Eq. 9, 10) of a random non-canonical MPS against the oracle:
+    same bonds, same state (overlap), right-canonical output, including wide and tall unfoldings."""
+    from oracle import pc_rk4
+    dims = [3, 4, 2, 5, 3]
+    rng = np.random.default_rng(61)
+    bonds = [1, 7, 9, 13, 6, 1]
+    mps = [si.complex_normal(rng, (bonds[i], dims[i], bonds[i + 1])) for i in range(5)]
+    mpo = [np.ones((1, d, d, 1), dtype=np.complex128) for d in dims]        # unused when n_steps = 0
+    for M in (64, 4):
+        want, _ = pc_rk4.compress(mps, M)
+        got = T.tdvp_pc_rk4_warmup(mpo, mps, 0.0, 0, M, M)
+        assert [g.shape for g in got] == [w.shape for w in want]
+        for A in got[1:]:
+            m = A.reshape(A.shape[0], -1)
+            assert np.abs(m @ m.conj().T - np.eye(A.shape[0])).max() < 1e-12
+        nw, ng = obs.norm_sq(want), obs.norm_sq(got)
+        assert abs(ng - nw) <= 1e-11 * nw
+        assert abs(abs(overlap(want, got)) / np.sqrt(nw * ng) - 1.0) <= 1e-11
+
+
+def test_pc_rk4_warmup_then_ps_steps(T):
+    """The paper's procedure on configs[0]: 10 P&C-RK4 steps of tau = 80 a.u. from the bare product state
+    (bond dimension 1), compression to M_S = 16, then 5 TDVP-PS steps -- both sides end to end, populations 1e-8,
+    state overlap.  Also the warmed state lets Dormand-Prince take the paper's step sizes."""
+    from oracle import pc_rk4
+    cfg, params, mpo, dims, mps = chain_inputs("tiny")
+    prod = _product_state(dims, si.initial_occupations(params))
+    tau = 80 * 0.0241888
+    want = pc_rk4.warmup(mpo, prod, tau, 10, 32, cfg.M)
+    got = T.tdvp_pc_rk4_warmup(mpo, prod, tau, 10, 32, cfg.M)
+    assert [g.shape for g in got] == [w.shape for w in want]
+    assert np.abs(obs.populations(got) - obs.populations(want)).max() <= 1e-9
+    nw, ng = obs.norm_sq(want), obs.norm_sq(got)
+    assert abs(abs(overlap(want, got)) / np.sqrt(nw * ng) - 1.0) <= 1e-10
+    st = tdvp_ps.PSState(mpo, want)
+    ch = T.tdvp_create(mpo, got, T.make_options(krylov_dim=cfg.krylov_dim))
+    for s in range(5):
+        tdvp_ps.step_ps(st, cfg.dt_fs, cfg.krylov_dim)
+        ch.tdvp_step_ps(cfg.dt_fs)
+        assert np.abs(ch.tdvp_populations(0) - obs.populations(st.mps)).max() <= 1e-8
+    # TDVP-MU from the warmed state: a Dormand-Prince step of 10 a.u. (PAPER.md:337: "from 5 to 30")
+    err = ch.tdvp_step_mu(10 * 0.0241888, want_err=True)
+    assert err < 1e-5
     ch.close()
