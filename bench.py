@@ -318,15 +318,15 @@ def sweep_point(torch, T, M, peak_tflops):
 
 
 def build_chain(name, M=None):
-    """MPO (built by the oracle's model builder: host-side input construction) and the
+    """MPO (built by the library's own host-side builder, tdvp_build_vibronic_mpo: SURVEY.md A21) and the
     seeded delta-padded initial MPS of one of BASELINE.json's chain configs."""
     import dataclasses
-    from oracle import model
+    import paper_1907_12044_b200 as T
     cfg = si.CONFIGS[name]
     if M is not None:
         cfg = dataclasses.replace(cfg, M=M)
     params = si.draw_vibronic_params(cfg)
-    mpo = model.build_mpo(params)
+    mpo = T.tdvp_build_vibronic_mpo(params.E, params.J, params.omega, params.S, params.n_ph, params.layout)
     dims = si.site_dims(params)
     mps = si.padded_product_mps(dims, si.initial_occupations(params), cfg.M, cfg.pad_seed, cfg.delta, cfg.delta_seed)
     return cfg, mpo, mps
@@ -551,6 +551,70 @@ def run_ours(args):
         out["ps_step"]["phase_ms"] = {k: round(v[0], 3) for k, v in ph.items()}
         out["ps_step"]["phase_brackets"] = {k: v[1] for k, v in ph.items()}
         ch.close()
+        # (f)3: the same step with the adaptive Krylov dimension (device-side rule, cap 40, tol 1e-8): the configured
+        # k = 10 is far from converged at this dt, so both are reported side by side
+        try:
+            KCAP, KTOL = 40, 1e-8
+            ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=KCAP, krylov_tol=KTOL))
+            ch.tdvp_step_ps(cfg.dt_fs)
+            ch.tdvp_sync()
+            e0.record()
+            for _ in range(2):
+                ch.tdvp_step_ps(cfg.dt_fs)
+            e1.record()
+            ch.tdvp_sync()
+            torch.cuda.synchronize()
+            nrm, en = ch.tdvp_norm_energy()
+            out["ps_step_adaptive_krylov"] = {"krylov_cap": KCAP, "krylov_tol": KTOL, "ms_per_step": e0.elapsed_time(e1) / 2,
+                                              "norm_sq": nrm, "energy": en,
+                                              "note": "stop at the first j with beta_j |[exp(z T_j) e_1]_j| < tol, decided on the device; "
+                                                      "applies after the stop return at once (skip flag)"}
+            ch.close()
+        except Exception as ex:                      # noqa: BLE001 -- a bench extra must not take the headline down
+            out["ps_step_adaptive_krylov"] = {"error": str(ex)}
+        # (f)2: the paper's warm-up: 10 P&C-RK4 steps of 80 a.u. from the bare product state, on the
+        # device, then compression -- at M = 14 (M_O M <= 128 keeps every SVD on the fast Jacobi path; at M = 128 the
+        # compression SVDs are 1152 x 1152: DESIGN.md 6).  Then: the largest Dormand-Prince step h that keeps
+        # err_est <= 1e-7 from the WARMED start against the delta-seeded padded start after 5 PS steps (both M = 14)
+        try:
+            import dataclasses
+            M_W, AU = 14, 0.0241888
+            cfgw = dataclasses.replace(si.CONFIGS["fmo128"], M=M_W)
+            params = si.draw_vibronic_params(cfgw)
+            dims = si.site_dims(params)
+            prod = []
+            for dd, oo in zip(dims, si.initial_occupations(params)):
+                a = np.zeros((1, dd, 1), dtype=np.complex128)
+                a[0, oo, 0] = 1.0
+                prod.append(a)
+            t0 = time.perf_counter()
+            warm = T.tdvp_pc_rk4_warmup(mpo, prod, 80 * AU, 10, M_W, M_W)
+            warm_s = time.perf_counter() - t0
+            H_LIST = [30 * AU, 15 * AU, 5 * AU, 0.05, 0.02, 0.01, 0.004]
+
+            def mu_errs(start_mps, n_ps):
+                chw = T.tdvp_create(mpo, start_mps, T.make_options(krylov_dim=cfg.krylov_dim))
+                for _ in range(n_ps):
+                    chw.tdvp_step_ps(cfg.dt_fs)
+                base = chw.tdvp_get_mps()
+                errs = {}
+                for h in H_LIST:
+                    chw.tdvp_set_mps(base, 0)
+                    errs["%.4f" % h] = chw.tdvp_step_mu(h, want_err=True)
+                chw.close()
+                ok = [h for h in H_LIST if np.isfinite(errs["%.4f" % h]) and errs["%.4f" % h] <= 1e-7]
+                return errs, (max(ok) if ok else None)
+
+            errs_w, h_w = mu_errs(warm, 0)
+            padded = si.padded_product_mps(dims, si.initial_occupations(params), M_W, cfgw.pad_seed, cfgw.delta, cfgw.delta_seed)
+            errs_p, h_p = mu_errs(padded, 5)
+            out["pc_rk4_warmup"] = {"workload": "configs[3] chain (71 sites), 10 P&C-RK4 steps of 80 a.u. at M_max = %d, compressed to %d" % (M_W, M_W),
+                                    "seconds": warm_s, "bonds_max": max(a.shape[2] for a in warm),
+                                    "dp5_err_est_by_h_fs": {"warmed": errs_w, "padded_delta_seeded_after_5_ps_steps": errs_p},
+                                    "largest_h_fs_with_err_below_1e-7": {"warmed": h_w, "padded": h_p},
+                                    "paper_step_range_fs": [5 * AU, 30 * AU]}
+        except Exception as ex:                      # noqa: BLE001
+            out["pc_rk4_warmup"] = {"error": str(ex)}
         # TDVP-MU on the same chain (configs[3]): five PS steps of warm-up (the MU right-hand side needs
         # full-rank bonds, DESIGN.md c18), then Dormand-Prince steps of h = 0.004 fs: with eps = 1e-10 the
         # right-hand side is stiff (1 / sqrt(eps) = 1e5 on the weakly occupied bonds of this chain), the

@@ -236,6 +236,24 @@ int tdvp_get_centre(tdvp_handle *h);               /* current gauge centre, or a
 int tdvp_sync(tdvp_handle *h);                     /* block until the handle's stream is idle    */
 const char *tdvp_last_error(const tdvp_handle *h);
 
+/* ---- workload construction (host only, no GPU work) ------------------------------------------- */
+/* The Frenkel-Holstein Hamiltonian of the paper (Eq. 45), single-exciton sector,
+       H = sum_m E_m a+_m a_m + sum_{m != n} J_mn a+_m a_n + sum_{m,l} w_ml (b+ b + 1/2) + sum_{m,l} g_ml w_ml (b+ + b) a+_m a_m,
+   as an MPO (Eq. 11), W_i[w, s, t, v] with s = bra, t = ket as everywhere in this header.
+     layout       0: one electronic site of dimension n_el, then all modes, state-major (BASELINE configs 1, 3, 4)
+                  1: the paper's own order: a two-level site per electronic state followed by its modes
+     E[n_el], J[n_el * n_el] (symmetric, zero diagonal), omega[n_el * n_modes], huang_rhys[n_el * n_modes]
+                  HOST; g_ml = sqrt(huang_rhys_ml) (reading c4); phonon modes truncated to n_ph number states
+     energy_unit  factor applied to E, J, omega (2 pi c = 1.8836515673e-4 turns cm^-1 into rad/fs, reading c5)
+     n_sites      HOST out; phys_dim[n_sites], mpo_bond[n_sites + 1]: HOST out, nullable
+     mpo[n_sites] HOST pointers to caller buffers [mpo_bond[i], d_i, d_i, mpo_bond[i+1]], or NULL for a size query
+                  (call once with mpo = NULL to learn n_sites, phys_dim and mpo_bond, allocate, call again).
+   Bond dimensions: at most n_el + 2 (layout 0) / 2 n_el + 1 (layout 1); the tensors are real and a few per cent
+   dense.  Returns TDVP_EINVAL on bad arguments; the error text is that of handle-less calls. */
+int tdvp_build_vibronic_mpo(int layout, int n_el, int n_modes, int n_ph, const double *E, const double *J,
+                            const double *omega, const double *huang_rhys, double energy_unit,
+                            int *n_sites, int *phys_dim, int *mpo_bond, tdvp_c128 *const *mpo);
+
 /* ---- measurement helpers ------------------------------------------------------------------- */
 /* Issue-rate probe of the FP64 tensor pipe (DMMA m8n8k4 in registers, no memory traffic): runs on
    the legacy default stream, blocks, returns TFLOP/s.  This is the denominator bench.py uses for

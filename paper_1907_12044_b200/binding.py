@@ -32,7 +32,7 @@ EXPORTED_SYMBOLS = [
     "tdvp_step_ps", "tdvp_step_mu", "tdvp_step_mu_cmf", "tdvp_mu_derivative", "tdvp_set_gauge", "tdvp_observe", "tdvp_populations",
     "tdvp_norm_energy", "tdvp_get_mps", "tdvp_set_mps", "tdvp_get_centre", "tdvp_sync",
     "tdvp_last_error", "tdvp_probe_fp64_tensor_peak", "tdvp_probe_dmma_issue", "tdvp_set_gemm_products", "tdvp_get_gemm_products", "tdvp_launch_count", "tdvp_profile_enable",
-    "tdvp_profile_read", "tdvp_pc_rk4_warmup",
+    "tdvp_profile_read", "tdvp_pc_rk4_warmup", "tdvp_build_vibronic_mpo",
 ]
 
 
@@ -91,6 +91,8 @@ def _load():
         "tdvp_get_gemm_products": (c_int, []),
         "tdvp_profile_enable": (c_int, [c_int]),
         "tdvp_profile_read": (c_int, [POINTER(c_double), POINTER(c_longlong)]),
+        "tdvp_build_vibronic_mpo": (c_int, [c_int, c_int, c_int, c_int, POINTER(c_double), POINTER(c_double), POINTER(c_double),
+                                            POINTER(c_double), c_double, POINTER(c_int), POINTER(c_int), POINTER(c_int), POINTER(P)]),
         "tdvp_pc_rk4_warmup": (c_int, [P, c_int, POINTER(c_int), POINTER(c_int), POINTER(P), POINTER(c_int), POINTER(P),
                                        c_double, c_int, c_int, c_int, POINTER(c_int), POINTER(P)]),
     }
@@ -263,6 +265,33 @@ def tdvp_svd_bond(C, handle=None):
     h = _hptr(handle)
     _check(_lib.tdvp_svd_bond(h, Ml, d, Mr, _dev(C), _dev(U), c_void_p(lam.data_ptr()), _dev(Vh)), h)
     return U, lam, Vh
+
+
+CM1_TO_RAD_PER_FS = 1.8836515673e-4        # 2 pi c: energies in cm^-1 -> angular frequencies in rad/fs (reading c5)
+
+
+def tdvp_build_vibronic_mpo(E, J, omega, huang_rhys, n_ph, layout="A", energy_unit=CM1_TO_RAD_PER_FS):
+    """Frenkel-Holstein Hamiltonian (Eq. 45) -> list of HOST numpy MPO site tensors W_i[Dl, d, d, Dr]
+    (include/tdvp.h).  Host-only: needs no GPU."""
+    E = np.ascontiguousarray(E, dtype=np.float64)
+    J = np.ascontiguousarray(J, dtype=np.float64)
+    om = np.ascontiguousarray(omega, dtype=np.float64)
+    S = np.ascontiguousarray(huang_rhys, dtype=np.float64)
+    n_el = E.shape[0]
+    n_modes = om.shape[1] if om.ndim == 2 else 0
+    lay = {"A": 0, "B": 1}[layout]
+    dp = lambda a: a.ctypes.data_as(POINTER(c_double))
+    n = c_int(0)
+    cap = n_el * (1 + max(n_modes, 0)) + 1
+    phys, bond = (c_int * cap)(), (c_int * (cap + 1))()
+    _check(_lib.tdvp_build_vibronic_mpo(lay, n_el, n_modes, int(n_ph), dp(E), dp(J), dp(om), dp(S), float(energy_unit),
+                                        byref(n), phys, bond, None))
+    ns = n.value
+    out = [np.empty((bond[i], phys[i], phys[i], bond[i + 1]), dtype=np.complex128) for i in range(ns)]
+    PA = c_void_p * ns
+    _check(_lib.tdvp_build_vibronic_mpo(lay, n_el, n_modes, int(n_ph), dp(E), dp(J), dp(om), dp(S), float(energy_unit),
+                                        byref(n), phys, bond, PA(*[o.ctypes.data for o in out])))
+    return out
 
 
 def tdvp_pc_rk4_warmup(mpo, mps, tau, n_steps, M_max, M_out, handle=None):

@@ -154,7 +154,10 @@ def test_fmo128_ps_step_from_full_rank_state(T):
     needs a few minutes for it (one heff at M = 128 is ~50 ms, ~1600 of them)."""
     cfg, params, mpo, dims, mps = chain_inputs("fmo128", start="random")
     assert len(mps) == 71 and max(a.shape[2] for a in mps) == 128
-    ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=cfg.krylov_dim))
+    # the CUDA side runs on the MPO of the library's own builder (tdvp_build_vibronic_mpo), the oracle on its own:
+    # two independent constructions of Eq. 45 (both pinned against the Kronecker-sum Hamiltonian)
+    mpo_lib = T.tdvp_build_vibronic_mpo(params.E, params.J, params.omega, params.S, params.n_ph, params.layout)
+    ch = T.tdvp_create(mpo_lib, mps, T.make_options(krylov_dim=cfg.krylov_dim))
     st = tdvp_ps.PSState(mpo, mps)
     tdvp_ps.step_ps(st, cfg.dt_fs, cfg.krylov_dim)
     ch.tdvp_step_ps(cfg.dt_fs)

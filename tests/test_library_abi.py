@@ -44,3 +44,31 @@ def test_default_options_roundtrip():
     import paper_1907_12044_b200 as t
     o = t.make_options()
     assert (o.krylov_dim, o.krylov_tol, o.mu_eps, o.w_zero_tol, o.flags) == (10, 0.0, 1e-10, 0.0, 0)
+
+
+def test_vibronic_mpo_builder_matches_the_kronecker_sum_hamiltonian():
+    """tdvp_build_vibronic_mpo is host code (no GPU): its MPO, contracted to a dense matrix, is Eq. 45 written
+    out term by term (the oracle's Kronecker-sum Hamiltonian, which shares nothing with either MPO builder),
+    for both layouts; the bond dimensions stay within the bounds include/tdvp.h states; full-size shapes."""
+    import dataclasses
+    import numpy as np
+    import synthetic_inputs as si
+    import paper_1907_12044_b200 as t
+    from oracle import model
+    for layout in ("A", "B"):
+        cfg = dataclasses.replace(si.CONFIGS["tiny"], model_seed=11, n_el=3, n_modes=2, n_ph=2, nearest_neighbour=False, layout=layout)
+        p = si.draw_vibronic_params(cfg)
+        H, dims = model.kronecker_sum_hamiltonian(p)
+        mpo = t.tdvp_build_vibronic_mpo(p.E, p.J, p.omega, p.S, p.n_ph, layout)
+        assert [W.shape[1] for W in mpo] == dims
+        Hd = model.mpo_to_dense(mpo)
+        assert np.abs(Hd - H.toarray()).max() < 1e-15
+        assert max(W.shape[3] for W in mpo) <= (3 + 2 if layout == "A" else 2 * 3 + 1)
+        assert all(np.all(W.imag == 0.0) for W in mpo)
+    for name, n_sites, dmax in (("fmo128", 71, 9), ("fmo256", 147, 15)):
+        p = si.draw_vibronic_params(si.CONFIGS[name])
+        mpo = t.tdvp_build_vibronic_mpo(p.E, p.J, p.omega, p.S, p.n_ph, p.layout)
+        assert len(mpo) == n_sites and max(W.shape[3] for W in mpo) <= dmax
+        assert mpo[0].shape[0] == 1 and mpo[-1].shape[3] == 1
+        dens = [np.count_nonzero(W) / W.size for W in mpo[1:-1]]
+        assert max(dens) < 0.2 and np.mean(dens) < 0.06
