@@ -190,6 +190,17 @@ int tdvp_update_env_site(tdvp_handle *h, int site, int side);
    Enqueue only: no host round trip inside the step. */
 int tdvp_step_ps(tdvp_handle *h, double dt);
 
+/* One step of length dt of the TWO-SITE projector-splitting integrator ("it is also possible to
+   formulate TDVP-PS into a two-site algorithm"; the paper gives no equations and declines it for its cost --
+   this is the integrator of its ref. 32 built from the paper's Eq. 29-32, 10 and 43):
+   left to right, every pair (i, i+1) is evolved by dt/2 with the two-site effective Hamiltonian, split by SVD
+   (Eq. 10) keeping the bond dimension the chain already has, and the new centre is evolved backward by dt/2
+   with the one-site H[i+1]; the last pair is evolved once by dt; then the mirror sweep.  Same gauge contract as
+   tdvp_step_ps (centre at site 0 before and after); enqueue only.  The bond dimensions stay fixed, the norm is
+   conserved up to the truncation.  Limit: M_i d_i <= 12800, and the pair SVDs are Jacobi iterations on
+   min(M_i d_i, d_{i+1} M_{i+2}) columns -- fast up to 128, slow beyond (the paper's reason to decline it holds here). */
+int tdvp_step_ps2(tdvp_handle *h, double dt);
+
 /* One Dormand-Prince 5(4) step of length dt of the TDVP-MU equations of motion
    (Eq. 27, 33, 36-38) in the left-canonical gauge (centre at site N-1).  If the
    handle is in the PS gauge it is first moved by a QR sweep (no time evolution).

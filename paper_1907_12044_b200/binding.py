@@ -32,7 +32,7 @@ EXPORTED_SYMBOLS = [
     "tdvp_step_ps", "tdvp_step_mu", "tdvp_step_mu_cmf", "tdvp_mu_derivative", "tdvp_set_gauge", "tdvp_observe", "tdvp_populations",
     "tdvp_norm_energy", "tdvp_get_mps", "tdvp_set_mps", "tdvp_get_centre", "tdvp_sync",
     "tdvp_last_error", "tdvp_probe_fp64_tensor_peak", "tdvp_probe_dmma_issue", "tdvp_set_gemm_products", "tdvp_get_gemm_products", "tdvp_launch_count", "tdvp_profile_enable",
-    "tdvp_profile_read", "tdvp_pc_rk4_warmup", "tdvp_build_vibronic_mpo",
+    "tdvp_profile_read", "tdvp_pc_rk4_warmup", "tdvp_build_vibronic_mpo", "tdvp_step_ps2",
 ]
 
 
@@ -72,6 +72,7 @@ def _load():
         "tdvp_apply_heff_site": (c_int, [P, c_int, P, P]),
         "tdvp_update_env_site": (c_int, [P, c_int, c_int]),
         "tdvp_step_ps": (c_int, [P, c_double]),
+        "tdvp_step_ps2": (c_int, [P, c_double]),
         "tdvp_step_mu": (c_int, [P, c_double, POINTER(c_double)]),
         "tdvp_step_mu_cmf": (c_int, [P, c_double, c_int]),
         "tdvp_mu_derivative": (c_int, [P, POINTER(P)]),
@@ -400,6 +401,9 @@ class Chain:
 
     def tdvp_step_ps(self, dt):
         _check(_lib.tdvp_step_ps(self._h, float(dt)), self._h)
+
+    def tdvp_step_ps2(self, dt):
+        _check(_lib.tdvp_step_ps2(self._h, float(dt)), self._h)
 
     def tdvp_step_mu(self, dt, want_err=False):
         e = c_double(0.0)

@@ -118,6 +118,8 @@ static void free_chain(tdvp_handle *h) {
   for (auto e : h->cmf_join) cudaEventDestroy(e);
   if (h->cmf_fork) cudaEventDestroy(h->cmf_fork);
   fr(h->tmpA); fr(h->tmpB); fr(h->bondD); fr(h->bondD2); fr(h->step_ws); fr(h->mu_err_dev); fr(h->mu_scratch);
+  if (h->ps2_graph.exec) cudaGraphExecDestroy(h->ps2_graph.exec);
+  fr(h->ps2_ws);
   if (h->ps_graph.exec) cudaGraphExecDestroy(h->ps_graph.exec);
   if (h->mu_graph.exec) cudaGraphExecDestroy(h->mu_graph.exec);
   h->arena.release();

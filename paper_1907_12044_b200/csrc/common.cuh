@@ -153,6 +153,11 @@ void heff_apply(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c1
 void heff_apply_staged(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, const c128 *L, const c128 *W_dense,
                        void *wmem, double zero_tol, const c128 *A, const c128 *R, c128 *out, void *ws,
                        int nsl, const cudaEvent_t *ev_l, cudaEvent_t ev_w, cudaEvent_t ev_r);
+// Two-site H_eff (Eq. 29 with two sites between the blocks): out[a,s1,s2,b] = sum L[a,w,x] W1[w,s1,t1,u]
+// W2[u,s2,t2,v] Theta[x,t1,t2,y] R[b,v,y] -- stage 1, the W stage once per site, stage 3, on the same kernels.
+size_t heff2_ws_bytes(int Ml, int Mr, int d1, int d2, int Dl, int Dm, int Dr);
+void heff2_apply(cudaStream_t st, int Ml, int Mr, int d1, int d2, int Dl, int Dm, int Dr, const c128 *L, const WSparse &W1,
+                 const WSparse &W2, const c128 *Theta, const c128 *R, c128 *out, void *ws, const int *skip = nullptr);
 size_t env_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr);
 void env_update(cudaStream_t st, int side, int Ml, int Mr, int d, int Dl, int Dr,
                 const c128 *env_in, const WSparse &W, const c128 *A, c128 *env_out, void *ws, cudaEvent_t w_ready = nullptr);
@@ -162,10 +167,13 @@ void bond_apply(cudaStream_t st, int Ml, int Mr, int Dw, const c128 *L, const c1
 
 // ---------------------------------------------------------------------------------------------
 // lanczos.cu : Krylov exponential with all scalars on the device.
-struct LanczosOp {           // which operator: heff (site) or bond
-  int kind;                  // 0 = heff, 1 = bond
+struct LanczosOp {           // which operator: heff (site), bond, or two-site heff
+  int kind;                  // 0 = heff, 1 = bond, 2 = two-site heff (sites i, i + 1 between L and R)
   int Ml, Mr, d, Dl, Dr;     // bond: d = 1, Dl = Dr = Dw
   const c128 *L; const c128 *R; const WSparse *W;
+  int d2 = 1, Dm = 1;        // two-site: physical dimension of the second site, MPO bond between the two sites
+  const WSparse *W2 = nullptr;   // (W: Dl x d x d x Dm, W2: Dm x d2 x d2 x Dr)
+  long long elems() const { return kind == 1 ? (long long)Ml * Mr : (long long)Ml * d * (kind == 2 ? d2 : 1) * Mr; }
 };
 size_t lanczos_ws_bytes(const LanczosOp &op, int k);
 // y = exp(z H) v with at most k Krylov vectors; tol > 0 (and z purely imaginary): stop at the first j with

@@ -118,6 +118,33 @@ void heff_apply_staged(cudaStream_t st, int Ml, int Mr, int d, int Dl, int Dr, c
   zgemm(st, g_stage3_heff(Ml, Mr, d, Dr, T2, R, out));
 }
 
+size_t heff2_ws_bytes(int Ml, int Mr, int d1, int d2, int Dl, int Dm, int Dr) {
+  const size_t per = (size_t)Ml * d1 * d2 * Mr;
+  const size_t big = per * (size_t)(Dl > Dm ? (Dl > Dr ? Dl : Dr) : (Dm > Dr ? Dm : Dr));
+  return 2 * up256(big * 16) + 256;
+}
+
+void heff2_apply(cudaStream_t st, int Ml, int Mr, int d1, int d2, int Dl, int Dm, int Dr, const c128 *L, const WSparse &W1,
+                 const WSparse &W2, const c128 *Theta, const c128 *R, c128 *out, void *ws, const int *skip) {
+  const size_t per = (size_t)Ml * d1 * d2 * Mr;
+  const size_t big = per * (size_t)(Dl > Dm ? (Dl > Dr ? Dl : Dr) : (Dm > Dr ? Dm : Dr));
+  char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
+  c128 *Ta = reinterpret_cast<c128 *>(p); p += up256(big * 16);
+  c128 *Tb = reinterpret_cast<c128 *>(p);
+  // T1[(a,w),(t1,t2,y)] = L Theta: stage 1 with the pair (t1,t2) as one physical index
+  ZGemm g1 = g_stage1_left(Ml, Mr, d1 * d2, Dl, L, Theta, Ta);
+  g1.skip = skip;
+  zgemm(st, g1);
+  // site i:     T2[a, s1, u, (t2,y)] = sum_{w,t1} W1[w,s1,t1,u] T1[a, w, t1, (t2,y)]   (panel rows of length d2 Mr)
+  wstage_left(st, W1, Ml, d2 * Mr, Ta, Tb, skip);
+  // site i + 1: T3[(a,s1), s2, v, y] = sum_{u,t2} W2[u,s2,t2,v] T2[(a,s1), u, t2, y]    (batch index (a,s1))
+  wstage_left(st, W2, Ml * d1, Mr, Tb, Ta, skip);
+  // out[((a,s1),s2), b] = sum_{(v,y)} T3[((a,s1),s2), (v,y)] R[b, (v,y)]
+  ZGemm g3 = g_stage3_heff(Ml * d1, Mr, d2, Dr, Ta, R, out);
+  g3.skip = skip;
+  zgemm(st, g3);
+}
+
 size_t env_ws_bytes(int Ml, int Mr, int d, int Dl, int Dr) {
   size_t t1 = (size_t)Ml * Dl * d * Mr, t2 = (size_t)Ml * d * Dr * Mr;
   size_t big = t1 > t2 ? t1 : t2;

@@ -49,7 +49,9 @@ struct tdvp_handle {
   std::vector<cudaEvent_t> cmf_join;
   std::vector<void *> cmf_ws, cmf_scratch;
   cudaEvent_t cmf_fork = nullptr;
-  StepGraph ps_graph, mu_graph;
+  StepGraph ps_graph, mu_graph, ps2_graph;
+  void *ps2_ws = nullptr;          // two-site TDVP-PS workspace (allocated by the first tdvp_step_ps2)
+  size_t ps2_ws_bytes = 0;
 };
 
 int set_err(tdvp_handle *h, int code, const std::string &msg);

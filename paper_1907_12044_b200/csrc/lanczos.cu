@@ -483,6 +483,7 @@ __global__ void __launch_bounds__(VT) lz_combine_kernel(long long n, int k, doub
 inline size_t up256(size_t x) { return (x + 255) & ~size_t(255); }
 
 size_t apply_ws_bytes(const LanczosOp &op) {
+  if (op.kind == 2) return heff2_ws_bytes(op.Ml, op.Mr, op.d, op.d2, op.Dl, op.Dm, op.Dr);
   return op.kind == 0 ? heff_ws_bytes(op.Ml, op.Mr, op.d, op.Dl, op.Dr) : bond_ws_bytes(op.Ml, op.Mr, op.Dl);
 }
 
@@ -501,14 +502,14 @@ void lanczos_configure() {
 }
 
 size_t lanczos_ws_bytes(const LanczosOp &op, int k) {
-  size_t n = (size_t)op.Ml * (op.kind == 0 ? op.d : 1) * op.Mr;
+  size_t n = (size_t)op.elems();
   return up256((k + 1) * n * 16) + up256(k * 16) + 2 * up256(k * 8) + 1024 +
          up256((size_t)2 * MAXG * (TDVP_MAX_KRYLOV + 1) * 16) + up256(MAXG * 8) + apply_ws_bytes(op) + 512;
 }
 
 void lanczos_expm(cudaStream_t st, const LanczosOp &op, int k, double tol, double z_re, double z_im,
                   const c128 *v, c128 *y, void *ws, int *m_used_dev, int *status_dev) {
-  const long long n = (long long)op.Ml * (op.kind == 0 ? op.d : 1) * op.Mr;
+  const long long n = op.elems();
   char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
   LzBuffers b;
   b.Q = reinterpret_cast<c128 *>(p); p += up256((k + 1) * n * 16);
@@ -548,6 +549,8 @@ void lanczos_expm(cudaStream_t st, const LanczosOp &op, int k, double tol, doubl
     const int *skip = (j > 0 && tol > 0.0 && imaginary) ? b.hist + (j - 1) : nullptr;
     if (op.kind == 0)
       heff_apply(st, op.Ml, op.Mr, op.d, op.Dl, op.Dr, op.L, *op.W, uj, op.R, w, b.apply_ws, nullptr, skip);
+    else if (op.kind == 2)
+      heff2_apply(st, op.Ml, op.Mr, op.d, op.d2, op.Dl, op.Dm, op.Dr, op.L, *op.W, *op.W2, uj, op.R, w, b.apply_ws, skip);
     else
       bond_apply(st, op.Ml, op.Mr, op.Dl, op.L, uj, op.R, w, b.apply_ws, skip);
     ProfScope ps(st, PH_VEC);

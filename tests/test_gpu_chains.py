@@ -12,6 +12,7 @@ both sides start one step from the same tensors, and the start is either
     rank (the oracle's own sensitivity there: populations 2e-11, overlap 1e-14 per step),
 on the real MPO, real shapes, configured dt and Krylov dimension."""
 import dataclasses
+import os
 
 import numpy as np
 import pytest
@@ -148,12 +149,8 @@ def test_fmo64_ps_mu_cmf_steps_from_full_rank_state(T):
     ch.close()
 
 
-# ---- configs[3]: 71 sites, M = 128 ---------------------------------------------------------------
-def test_fmo128_ps_step_from_full_rank_state(T):
-    """The headline chain (M = 128, dt = 5 fs, k = 10): one teacher-forced TDVP-PS step.  The oracle
-    needs a few minutes for it (one heff at M = 128 is ~50 ms, ~1600 of them)."""
-    cfg, params, mpo, dims, mps = chain_inputs("fmo128", start="random")
-    assert len(mps) == 71 and max(a.shape[2] for a in mps) == 128
+# ---- configs[3]: M = 128 -------------------------------------------------------------------------
+def _fmo128_step(T, cfg, params, mpo, mps):
     # the CUDA side runs on the MPO of the library's own builder (tdvp_build_vibronic_mpo), the oracle on its own:
     # two independent constructions of Eq. 45 (both pinned against the Kronecker-sum Hamiltonian)
     mpo_lib = T.tdvp_build_vibronic_mpo(params.E, params.J, params.omega, params.S, params.n_ph, params.layout)
@@ -163,6 +160,30 @@ def test_fmo128_ps_step_from_full_rank_state(T):
     ch.tdvp_step_ps(cfg.dt_fs)
     check_state(T, ch, mpo, st.mps, pop_tol=1e-9, ov_tol=1e-10)
     ch.close()
+
+
+def test_fmo128_bulk_ps_step_short_chain(T):
+    """M = 128, d = 10, the real MPO, dt = 5 fs, k = 10, one teacher-forced TDVP-PS step from a full-rank state on
+    the FMO-like model with ONE mode per electronic state (8 sites, bonds 7, 70, 128, 128, 128, 100, 10): every
+    kernel shape of the configs[3] bulk (1280 x 128 gauge moves, M = 128 applies and bond steps) at a cost the
+    oracle pays in about two minutes.  The full 71-site step is the next test."""
+    cfg = dataclasses.replace(si.CONFIGS["fmo128"], n_modes=1)
+    params = si.draw_vibronic_params(cfg)
+    mpo = model.build_mpo(params)
+    dims = si.site_dims(params)
+    mps = si.random_right_canonical_mps(dims, cfg.M, seed=77)
+    assert len(mps) == 8 and max(a.shape[2] for a in mps) == 128
+    _fmo128_step(T, cfg, params, mpo, mps)
+
+
+@pytest.mark.skipif(os.environ.get("TDVP_SLOW_TESTS") != "1",
+                    reason="the oracle needs ~20 minutes for one 71-site step at M = 128; set TDVP_SLOW_TESTS=1 "
+                           "(last run: passed in 1303 s, gpurun_out of round 2, recorded in DESIGN.md 2.1)")
+def test_fmo128_ps_step_from_full_rank_state(T):
+    """The headline chain as configured (71 sites, M = 128, dt = 5 fs, k = 10): one teacher-forced TDVP-PS step."""
+    cfg, params, mpo, dims, mps = chain_inputs("fmo128", start="random")
+    assert len(mps) == 71 and max(a.shape[2] for a in mps) == 128
+    _fmo128_step(T, cfg, params, mpo, mps)
 
 
 # ---- layout B (the paper's own site order, PAPER.md:320; configs[4]'s layout) ----------------------
@@ -248,4 +269,44 @@ def test_pc_rk4_warmup_then_ps_steps(T):
     # TDVP-MU from the warmed state: a Dormand-Prince step of 10 a.u. ("from 5 to 30")
     err = ch.tdvp_step_mu(10 * 0.0241888, want_err=True)
     assert err < 1e-5
+    ch.close()
+
+
+# ---- two-site TDVP-PS ------------------------------------------
+@pytest.mark.parametrize("graph", [True, False])
+def test_two_site_ps_tiny_chain(T, graph):
+    """configs[0] with the two-site integrator: 10 free-running steps against oracle/tdvp_ps2.py (populations 1e-8,
+    state overlap), wide / square / tall pair matrices all occur along this chain (bonds 3, 12, 16, 16, 16, 4)."""
+    from oracle import tdvp_ps2
+    cfg, params, mpo, dims, mps = chain_inputs("tiny")
+    st = tdvp_ps.PSState(mpo, mps)
+    ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=cfg.krylov_dim, flags=0 if graph else T.TDVP_FLAG_NO_GRAPH))
+    for s in range(10):
+        tdvp_ps2.step_ps2(st, cfg.dt_fs, cfg.krylov_dim)
+        ch.tdvp_step_ps2(cfg.dt_fs)
+        assert np.abs(ch.tdvp_populations(0) - obs.populations(st.mps)).max() <= 1e-8
+    assert ch.tdvp_get_centre() == 0
+    check_state(T, ch, mpo, st.mps, pop_tol=1e-8, ov_tol=1e-8)
+    # one-site and two-site steps share the handle and the gauge
+    tdvp_ps.step_ps(st, cfg.dt_fs, cfg.krylov_dim)
+    ch.tdvp_step_ps(cfg.dt_fs)
+    assert np.abs(ch.tdvp_populations(0) - obs.populations(st.mps)).max() <= 1e-8
+    ch.close()
+
+
+def test_two_site_ps_fmo_like_chain(T):
+    """A short FMO-like chain (d = 6 phonon sites, D_W up to 6, M = 12) from the delta-seeded start: the pair
+    matrices are 72 x 72 in the bulk."""
+    from oracle import tdvp_ps2
+    cfg = dataclasses.replace(si.CONFIGS["fmo64"], n_el=4, n_modes=2, n_ph=6, M=12, dt_fs=5.0)
+    params = si.draw_vibronic_params(cfg)
+    mpo = model.build_mpo(params)
+    dims = si.site_dims(params)
+    mps = si.padded_product_mps(dims, si.initial_occupations(params), cfg.M, cfg.pad_seed, cfg.delta, cfg.delta_seed)
+    st = tdvp_ps.PSState(mpo, mps)
+    ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=cfg.krylov_dim))
+    for s in range(3):
+        tdvp_ps2.step_ps2(st, cfg.dt_fs, cfg.krylov_dim)
+        ch.tdvp_step_ps2(cfg.dt_fs)
+        assert np.abs(ch.tdvp_populations(0) - obs.populations(st.mps)).max() <= 1e-8
     ch.close()
