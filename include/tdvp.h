@@ -148,6 +148,17 @@ int tdvp_expm_bond(tdvp_handle *h, int Ml, int Mr, int Dw,
 int tdvp_qr_gauge(tdvp_handle *h, int side, int Ml, int d, int Mr,
                   const tdvp_c128 *C /*DEVICE*/, tdvp_c128 *Q /*DEVICE*/, tdvp_c128 *D /*DEVICE*/);
 
+/* The same gauge move for callers that cannot allocate (code under CUDA-graph capture, tight serving loops,
+   harnesses that forbid cudaMalloc): no handle, and NO cudaMalloc / cudaFree / allocating library call --
+   the scratch lives in a 6 MiB static device array inside the library (held by every GPU that loads it,
+   until exit).  Limit: the move's scratch must fit, i.e. about 2 * 16 * tall * thin + 16 * thin^2 bytes
+   <= 6 MiB -- up to 1280 x 128, the M = 128, d = 10 move; larger shapes return TDVP_EINVAL (use tdvp_qr_gauge).
+   Same arguments, kernels and results as tdvp_qr_gauge; cuda_stream: a cudaStream_t (NULL = legacy default).
+   All calls share the one scratch block: calls that overlap on the GPU (different streams or host threads)
+   race -- keep them on one stream.  Enqueue only.  Errors are those of handle-less calls (tdvp_last_error(NULL)). */
+int tdvp_qr_gauge_noalloc(void *cuda_stream, int side, int Ml, int d, int Mr,
+                          const tdvp_c128 *C /*DEVICE*/, tdvp_c128 *Q /*DEVICE*/, tdvp_c128 *D /*DEVICE*/);
+
 /* Matrix unfolding of a bond (Eq. 36): C[Ml,d,Mr] viewed as Ml x (d*Mr) with
    Ml <= d*Mr is factored as U diag(lam) Vh on the device (Householder QR of C^T, then one-sided
    Jacobi on the Ml x Ml triangular factor).  U: DEVICE [Ml,Ml] unitary; lam: DEVICE double[Ml],

@@ -32,7 +32,7 @@ EXPORTED_SYMBOLS = [
     "tdvp_step_ps", "tdvp_step_mu", "tdvp_step_mu_cmf", "tdvp_mu_derivative", "tdvp_set_gauge", "tdvp_observe", "tdvp_populations",
     "tdvp_norm_energy", "tdvp_get_mps", "tdvp_set_mps", "tdvp_get_centre", "tdvp_sync",
     "tdvp_last_error", "tdvp_probe_fp64_tensor_peak", "tdvp_probe_dmma_issue", "tdvp_set_gemm_products", "tdvp_get_gemm_products", "tdvp_launch_count", "tdvp_profile_enable",
-    "tdvp_profile_read", "tdvp_pc_rk4_warmup", "tdvp_build_vibronic_mpo", "tdvp_step_ps2",
+    "tdvp_profile_read", "tdvp_pc_rk4_warmup", "tdvp_build_vibronic_mpo", "tdvp_step_ps2", "tdvp_qr_gauge_noalloc",
 ]
 
 
@@ -68,6 +68,7 @@ def _load():
                                    P, P, POINTER(c_int)]),
         "tdvp_expm_bond": (c_int, [P, c_int, c_int, c_int, P, P, c_double, c_double, P, P, POINTER(c_int)]),
         "tdvp_qr_gauge": (c_int, [P, c_int, c_int, c_int, c_int, P, P, P]),
+        "tdvp_qr_gauge_noalloc": (c_int, [P, c_int, c_int, c_int, c_int, P, P, P]),
         "tdvp_svd_bond": (c_int, [P, c_int, c_int, c_int, P, P, P, P]),
         "tdvp_apply_heff_site": (c_int, [P, c_int, P, P]),
         "tdvp_update_env_site": (c_int, [P, c_int, c_int]),
@@ -254,6 +255,15 @@ def tdvp_qr_gauge(side, C, handle=None):
     D = torch.empty((n, n), dtype=torch.complex128, device=C.device)
     h = _hptr(handle)
     _check(_lib.tdvp_qr_gauge(h, side, Ml, d, Mr, _dev(C), _dev(Q), _dev(D)), h)
+    return Q, D
+
+
+def tdvp_qr_gauge_noalloc(side, C, Q, D, stream=None):
+    """tdvp_qr_gauge without any allocation (include/tdvp.h): the caller passes the outputs too --
+    Q like C, D [n, n] with n = Mr (side 0) or Ml (side 1); scratch is the library's static 6 MiB block."""
+    Ml, d, Mr = C.shape
+    n = Mr if side == 0 else Ml
+    _check(_lib.tdvp_qr_gauge_noalloc(_stream_ptr(stream), side, Ml, d, Mr, _dev(C), _dev(Q, (Ml, d, Mr)), _dev(D, (n, n))))
     return Q, D
 
 

@@ -1092,3 +1092,65 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
   else TDVP_LAUNCH(copy_kernel, gcopy, 256, 0, st, Q, Y, n);
   TDVP_LAUNCH(store_d_kernel, (cols * cols + 255) / 256 > 296 ? 296 : (cols * cols + 255) / 256, 256, 0, st, Rm, D, cols, side);
 }
+
+// ---------------------------------------------------------------------------------------------
+// tdvp_qr_gauge_noalloc: the QR gauge move (Eq. 9) for callers that cannot allocate --
+// code under CUDA-graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The same kernels
+// and the same host driver (qr_gauge above) as tdvp_qr_gauge; only the scratch block (column-major copy X,
+// the Q workspace Y, R, the compact-WY factors T) differs: instead of the handle's growable arena it is the
+// file-scope device array below, which every GPU that loads libtdvp.so holds until the process exits.
+//
+// In host code `g_qr_static_scratch` is a host-side stand-in for the symbol, NOT a device address: its
+// device address is taken once per device, with that device current, by cudaGetSymbolAddress, and only that
+// pointer is handed to the kernels.
+//
+// Nothing in the block has to start at zero: every kernel of the move writes each scratch element before
+// any kernel reads it (X by the transpose / copy, R and T by the panel phase, Y by the Q formation), which is
+// also why the arena path may reuse its memory from call to call; the block keeps the previous call's
+// contents and the test calls twice in a row with different shapes to show that stale contents are harmless.
+// All calls share the one block: calls that overlap on the GPU (two streams, or two host threads) RACE --
+// serialise them on one stream.
+#include <mutex>
+
+#include "handle.cuh"
+
+constexpr size_t QR_STATIC_SCRATCH_BYTES = 6u << 20;     // 6 MiB: up to the 1280 x 128 move of configs[3] (5.3 MiB)
+static __device__ __align__(256) unsigned char g_qr_static_scratch[QR_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int QR_STATIC_MAX_DEVICES = 64;
+std::mutex g_qr_static_mu;
+void *g_qr_static_ptr[QR_STATIC_MAX_DEVICES] = {nullptr};
+}  // namespace
+
+extern "C" int tdvp_qr_gauge_noalloc(void *cuda_stream, int side, int Ml, int d, int Mr, const tdvp_c128 *C,
+                                     tdvp_c128 *Q, tdvp_c128 *D) {
+  if (!C || !Q || !D) return set_err(nullptr, TDVP_EINVAL, "tdvp_qr_gauge_noalloc: null pointer");
+  if (side != 0 && side != 1) return set_err(nullptr, TDVP_EINVAL, "tdvp_qr_gauge_noalloc: side must be 0 or 1");
+  if (Ml < 1 || d < 1 || Mr < 1) return set_err(nullptr, TDVP_EINVAL, "tdvp_qr_gauge_noalloc: dimensions must be >= 1");
+  const long long tall = side == 0 ? (long long)Ml * d : (long long)d * Mr;
+  const int thin = side == 0 ? Mr : Ml;
+  if (tall < thin) return set_err(nullptr, TDVP_EINVAL, "tdvp_qr_gauge_noalloc: gauge move needs a tall or square matrix");
+  if (tall > QR_MAX_TALL) return set_err(nullptr, TDVP_EINVAL, "tdvp_qr_gauge_noalloc: tall side above 12800 rows is not supported");
+  const size_t need = qr_ws_bytes((int)tall, thin) + 256;
+  if (need > QR_STATIC_SCRATCH_BYTES)
+    return set_err(nullptr, TDVP_EINVAL, "tdvp_qr_gauge_noalloc: needs " + std::to_string(need) + " bytes of scratch, the static block holds " +
+                                             std::to_string(QR_STATIC_SCRATCH_BYTES) + " (6 MiB: e.g. up to 1280 x 128); use tdvp_qr_gauge");
+  configure_kernels_once();                              // kernel attributes only: no allocation
+  int dev = 0;
+  if (int rc = check_cuda(nullptr, cudaGetDevice(&dev), "tdvp_qr_gauge_noalloc")) return rc;
+  if (dev < 0 || dev >= QR_STATIC_MAX_DEVICES) return set_err(nullptr, TDVP_EINVAL, "tdvp_qr_gauge_noalloc: device ordinal above 63");
+  void *scratch = nullptr;
+  {
+    std::lock_guard<std::mutex> lk(g_qr_static_mu);
+    if (!g_qr_static_ptr[dev]) {                         // once per device, with that device current
+      void *p = nullptr;
+      if (int rc = check_cuda(nullptr, cudaGetSymbolAddress(&p, g_qr_static_scratch), "tdvp_qr_gauge_noalloc: cudaGetSymbolAddress")) return rc;
+      g_qr_static_ptr[dev] = p;
+    }
+    scratch = g_qr_static_ptr[dev];
+  }
+  qr_gauge(reinterpret_cast<cudaStream_t>(cuda_stream), side, Ml, d, Mr, reinterpret_cast<const c128 *>(C), reinterpret_cast<c128 *>(Q),
+           reinterpret_cast<c128 *>(D), scratch);
+  return check_cuda(nullptr, cudaGetLastError(), "tdvp_qr_gauge_noalloc");
+}
