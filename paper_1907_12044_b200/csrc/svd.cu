@@ -26,12 +26,44 @@ constexpr int MAX_SWEEPS = 40;
 // A sweep that still rotates only pairs whose cosine is below this is "hovering at round-off" (the threshold
 // sqrt(n) eps sits at the error level of the dot product itself), not a failure to converge.
 constexpr double COARSE_TOL2 = 1e-20;
+// A column whose squared norm is below this (norm below 1e-75: products of round-off residues along a chain of
+// rank-deficient bonds get there) is zero for every purpose of the path.  The product a * b of the convergence
+// test underflows for two such columns, the test then always fires and the pair would be rotated for ever.
+constexpr double TINY_COL2 = 1e-150;
+// ... and RELATIVE to the matrix: a column more than three orders of magnitude below the round-off floor of the
+// largest column (norm < 1e-3 eps max_c |x_c|) is noise of noise.  Orthogonalising two such columns against
+// each other leaves one of them smaller still, with a direction that is round-off again: a cascade down to the
+// underflow threshold that used up all 40 sweeps on the graded bonds of a P&C-RK4 stage (singular values 6.6,
+// 1e-3 ..., a degenerate cluster at 6.6e-16, columns at 5e-34).  Pairs with such a column are left alone: the
+// reconstruction U Lambda V^dagger changes by less than those norms, J stays unitary by construction, and the
+// Householder step that follows makes U exactly unitary whatever the tiny columns look like.
+constexpr double REL_TINY2 = 4.9e-38;     // (1e-3 * 2.2e-16)^2
+
 inline size_t up256(size_t x) { return (x + 255) & ~size_t(255); }
 
 __device__ __forceinline__ double wsum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
+}
+
+// max_c |x_c|^2 over the columns of the n x n column-major Xt, identically in every CTA (fixed order)
+template <int NWARPS>
+__device__ double max_col_norm2(const c128 *Xt, int n, double *sm /*[NWARPS]*/) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  double m = 0.0;
+  for (int c = warp; c < n; c += NWARPS) {
+    double a = 0.0;
+    for (int i = lane; i < n; i += 32) { const c128 u = __ldcg(Xt + (size_t)c * n + i); a += u.x * u.x + u.y * u.y; }
+    a = wsum(a);
+    m = fmax(m, a);
+  }
+  if (lane == 0) sm[warp] = m;
+  __syncthreads();
+  double r = 0.0;
+  for (int k = 0; k < NWARPS; k++) r = fmax(r, sm[k]);
+  __syncthreads();
+  return r;
 }
 
 // Xt[c][r] = D[r][c];  Jt[c][r] = delta(c, r)          (column-major copies: contiguous columns)
@@ -63,6 +95,9 @@ svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/,
   const int npairs = np / 2;
   const double tol = 2.220446049250313e-16 * sqrt((double)n);   // LAPACK zgesvj: sqrt(m) * eps
   const double tol2 = tol * tol;
+  __shared__ double s_cmax[JW];
+  const double thr = fmax(TINY_COL2, REL_TINY2 * max_col_norm2<JW>(Xt, n, s_cmax));
+  cluster.sync();                                       // everybody has read the initial columns
   int sweep = 0;
   for (; sweep < max_sweeps; sweep++) {
     bool any = false, coarse = false;
@@ -107,7 +142,7 @@ svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/,
         }
         a = wsum(a); b = wsum(b); cr = wsum(cr); ci = wsum(ci);
         const double c2 = cr * cr + ci * ci;
-        if (!(c2 > tol2 * a * b) || c2 == 0.0) continue;
+        if (!(c2 > tol2 * a * b) || c2 == 0.0 || a < thr || b < thr) continue;
         any = true;
         if (c2 > COARSE_TOL2 * a * b) coarse = true;
         // y_q = e^{-i phi} x_q makes <x_p, y_q> = |c| real; then a real rotation (cs, sn)
@@ -162,7 +197,7 @@ svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/,
 constexpr int JB = 16;              // column blocks
 
 template <int NPL>
-__device__ __forceinline__ int jacobi_pair_smem(c128 *xp, c128 *xq, c128 *jp, c128 *jq, int n, int lane, double tol2) {
+__device__ __forceinline__ int jacobi_pair_smem(c128 *xp, c128 *xq, c128 *jp, c128 *jq, int n, int lane, double tol2, double thr) {
   c128 xu[NPL], xv[NPL], ju[NPL], jv[NPL];
   double a = 0.0, b = 0.0, cr = 0.0, ci = 0.0;
 #pragma unroll
@@ -181,7 +216,7 @@ __device__ __forceinline__ int jacobi_pair_smem(c128 *xp, c128 *xq, c128 *jp, c1
   }
   a = wsum(a); b = wsum(b); cr = wsum(cr); ci = wsum(ci);
   const double c2 = cr * cr + ci * ci;
-  if (!(c2 > tol2 * a * b) || c2 == 0.0) return 0;
+  if (!(c2 > tol2 * a * b) || c2 == 0.0 || a < thr || b < thr) return 0;
   const int result = c2 > COARSE_TOL2 * a * b ? 3 : 1;
   // the scalar chain is the critical path of a round: reciprocal square roots instead of sqrt + divide
   const double icabs = rsqrt(c2);
@@ -218,6 +253,9 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
   const int cta = blockIdx.x;                             // one cluster: rank == blockIdx.x
   const double tol = 2.220446049250313e-16 * sqrt((double)n);
   const double tol2 = tol * tol;
+  __shared__ double s_cmax[JW];
+  const double thr = fmax(TINY_COL2, REL_TINY2 * max_col_norm2<JW>(Xt, n, s_cmax));
+  cluster.sync();                                       // everybody has read the initial columns
   auto load_blocks = [&](int bp, int bq) {
     for (int e = tid; e < 2 * bw * n; e += JW * 32) {
       const int lc = e / n, i = e - lc * n;
@@ -252,7 +290,7 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
           const int base = half ? b1 * bw : b0 * bw;
           if (q < bw && base + q < n) {
             const int lp = half * bw + p, lq = half * bw + q;
-            any |= jacobi_pair_smem<NPL>(Xs + (size_t)lp * n, Xs + (size_t)lq * n, Js + (size_t)lp * n, Js + (size_t)lq * n, n, lane, tol2);
+            any |= jacobi_pair_smem<NPL>(Xs + (size_t)lp * n, Xs + (size_t)lq * n, Js + (size_t)lp * n, Js + (size_t)lq * n, n, lane, tol2, thr);
           }
         }
         __syncthreads();
@@ -272,7 +310,7 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
           if (warp < bw) {
             const int lp = warp, lq = bw + (warp + r) % bw;
             if (bp * bw + lp < n && bq * bw + (lq - bw) < n)
-              any |= jacobi_pair_smem<NPL>(Xs + (size_t)lp * n, Xs + (size_t)lq * n, Js + (size_t)lp * n, Js + (size_t)lq * n, n, lane, tol2);
+              any |= jacobi_pair_smem<NPL>(Xs + (size_t)lp * n, Xs + (size_t)lq * n, Js + (size_t)lp * n, Js + (size_t)lq * n, n, lane, tol2, thr);
           }
           __syncthreads();
         }
@@ -285,6 +323,35 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
     if (__ldcg(flags + sweep) == 0) break;                          // nobody rotated in this sweep
   }
   if (sweep == max_sweeps && status && cta == 0 && tid == 0 && __ldcg(flags + 64 + max_sweeps - 1)) atomicOr(status, TDVP_STATUS_SVD_UNCONVERGED);
+}
+
+// Columns of the rotated X (and of J with them) in the order of decreasing norm, before the Householder step:
+// that step reads the singular values off the diagonal of R', which needs every column orthogonal -- in
+// DIRECTION -- to the columns before it.  The columns the Jacobi iteration leaves alone (below the REL_TINY2
+// floor) have arbitrary directions; placed last they can only couple among themselves, at their own magnitude.
+__global__ void svd_colnorm_kernel(const c128 *Xt, int n, double *nrm) {
+  const int lane = threadIdx.x & 31, c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (c >= n) return;
+  double a = 0.0;
+  for (int i = lane; i < n; i += 32) { const c128 u = Xt[(size_t)c * n + i]; a += u.x * u.x + u.y * u.y; }
+  a = wsum(a);
+  if (lane == 0) nrm[c] = a;
+}
+__global__ void svd_sortcols_kernel(const c128 *Xt, const c128 *Jt, const double *nrm, int n, c128 *Xs, c128 *Js) {
+  __shared__ int s_rank;
+  const int c = blockIdx.x;
+  if (threadIdx.x == 0) s_rank = 0;
+  __syncthreads();
+  const double mine = nrm[c];
+  int cnt = 0;
+  for (int q = threadIdx.x; q < n; q += blockDim.x) { const double o = nrm[q]; cnt += (o > mine || (o == mine && q < c)) ? 1 : 0; }
+  if (cnt) atomicAdd(&s_rank, cnt);
+  __syncthreads();
+  const int k = s_rank;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) {
+    Xs[(size_t)k * n + i] = Xt[(size_t)c * n + i];
+    Js[(size_t)k * n + i] = Jt[(size_t)c * n + i];
+  }
 }
 
 // lam (descending), U and the permuted J from X = U' R' (Qp = U'^T, Dp = R'^T as qr_gauge side 1 returns them).
@@ -330,7 +397,7 @@ void svd_configure() {
 size_t svd_ws_bytes(int Ml, int d, int Mr) {
   const size_t n = Ml, nn = up256(n * n * 16);
   size_t q1 = qr_ws_bytes(d * Mr, Ml), q2 = qr_ws_bytes(Ml, Ml);
-  return up256((size_t)Ml * d * Mr * 16) + 6 * nn + 512 + up256(q1 > q2 ? q1 : q2) + 1024;
+  return up256((size_t)Ml * d * Mr * 16) + 7 * nn + 512 + up256(n * 8) + up256(q1 > q2 ? q1 : q2) + 1024;
 }
 
 // C [Ml, d, Mr] -> U [Ml, Ml], lam [Ml], Vh [Ml, d, Mr]
@@ -349,6 +416,8 @@ void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, do
   c128 *Qp = reinterpret_cast<c128 *>(p); p += nn;
   c128 *Dp = reinterpret_cast<c128 *>(p); p += nn;
   c128 *JtP = reinterpret_cast<c128 *>(p); p += nn;
+  c128 *Js = reinterpret_cast<c128 *>(p); p += nn;              // J with its columns in the sorted order (X sorted goes into D's buffer)
+  double *cnorm = reinterpret_cast<double *>(p); p += up256((size_t)n * 8);
   int *flags = reinterpret_cast<int *>(p); p += 512;        // [0, 40): a sweep rotated; [64, 104): ... a pair far from orthogonal
   void *qws = p;
   qr_gauge(st, 1, Ml, d, Mr, C, Q, D, qws);                               // C = D Q
@@ -362,8 +431,11 @@ void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, do
   else if (n <= 128) TDVP_LAUNCH(svd_jacobi_block_kernel<4>, JC, JW * 32, bsm, st, Xt, Jt, n, flags, max_sweeps, status);
   else TDVP_LAUNCH(svd_jacobi_kernel<0>, JC, JW * 32, 0, st, Xt, Jt, n, flags, max_sweeps, status);
   // X = U' R'  <=>  Xt = R'^T U'^T: "side 1" factorisation of the n x n matrix Xt (d = 1)
-  qr_gauge(st, 1, n, 1, n, Xt, Qp, Dp, qws);
-  TDVP_LAUNCH(svd_finish_kernel, n < 148 ? n : 148, 128, n * sizeof(double), st, Qp, Dp, Jt, n, U, lam, JtP);
+  c128 *Xs = D;                                                   // D is no longer needed
+  TDVP_LAUNCH(svd_colnorm_kernel, (n + 7) / 8, 256, 0, st, Xt, n, cnorm);
+  TDVP_LAUNCH(svd_sortcols_kernel, n, 128, 0, st, Xt, Jt, cnorm, n, Xs, Js);
+  qr_gauge(st, 1, n, 1, n, Xs, Qp, Dp, qws);
+  TDVP_LAUNCH(svd_finish_kernel, n < 148 ? n : 148, 128, n * sizeof(double), st, Qp, Dp, Js, n, U, lam, JtP);
   ZGemm gm{};                                   // Vh[k][:] = sum_j conj(JtP[k][j]) Q[j][:]
   gm.A = JtP; gm.B = Q; gm.C = Vh;
   gm.M = n; gm.K = n; gm.N = d * Mr;

@@ -43,6 +43,7 @@ constexpr int TILE_K_BYTES = KG * BM * 4 * 16;         // 16384
 constexpr int TILE_MN_BYTES = BK * LDM * 16;           // 16896
 constexpr int TILE_BYTES = TILE_MN_BYTES;              // slot size of either layout (128 B multiple)
 constexpr int SMEM_BYTES = STAGES * 2 * TILE_BYTES + 128;
+constexpr int SMEM_BYTES_32 = STAGES * 2 * (BK * (32 + 2) * 16) + 128;   // the 32 x 32 tile instance
 
 struct KParams {
   c128 *C;
@@ -57,6 +58,7 @@ struct KParams {
   int tiles_m, tiles_n, ktiles;
   int G;                // CTAs of this launch (cooperative: all resident)
   int upc_base, upc_rem;// units (tile, k-tile) per CTA: base, +1 for the first upc_rem CTAs
+  int tile;             // 64 or 32: edge of the CTA tile of this launch
   const int *skip;      // nullable: non-zero at kernel start = the caller no longer needs this product
   c128 *slots;          // [2 G][BM*BN] partial tiles of segments that do not cover their tile's whole K
   int *cnt;             // [G] partial segments published for the cut tile whose LAST unit CTA j holds
@@ -126,8 +128,12 @@ __device__ __forceinline__ int cta_of_unit(int u, int base, int rem) {
   return u < cut ? u / (base + 1) : rem + (u - cut) / base;
 }
 
-template <bool A_KMAJOR, bool B_KMAJOR, bool CONJ, bool M3>
+template <bool A_KMAJOR, bool B_KMAJOR, bool CONJ, bool M3, int TB>
 __device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtensorMap &tmB, const KParams &p) {
+  // tile geometry of this instance (TB = 64: the default; TB = 32: small problems, see choose_tile)
+  constexpr int BM = TB, BN = TB, WM = TB / 2, WN = TB / 2, NB8 = WM / 8;      // NB8 x NB8 m8n8 blocks per warp
+  constexpr int LDM = TB + 2;
+  constexpr int TILE_K_BYTES = KG * TB * 4 * 16, TILE_MN_BYTES = BK * LDM * 16, TILE_BYTES = TILE_MN_BYTES;
   extern __shared__ __align__(128) unsigned char smem_dyn[];
   __shared__ int s_fix_tile[2];
   __shared__ __align__(8) unsigned long long s_full[STAGES], s_empty[STAGES];
@@ -213,11 +219,11 @@ __device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtenso
   // 4M: cr = sum ar br - ai bi, ci = sum ar bi + ai br.
   // 3M: cr = sum ar br, ci = sum ai bi, cs = sum (ar + ai)(br + bi); the tile is cr - ci and
   //     cs - cr - ci, formed once per segment (fin()).
-  double cr[4][4][2], ci[4][4][2], cs[M3 ? 4 : 1][M3 ? 4 : 1][2];
+  double cr[NB8][NB8][2], ci[NB8][NB8][2], cs[M3 ? NB8 : 1][M3 ? NB8 : 1][2];
 #pragma unroll
-  for (int i = 0; i < 4; i++)
+  for (int i = 0; i < NB8; i++)
 #pragma unroll
-    for (int j = 0; j < 4; j++) {
+    for (int j = 0; j < NB8; j++) {
       cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
       if (M3) cs[M3 ? i : 0][M3 ? j : 0][0] = cs[M3 ? i : 0][M3 ? j : 0][1] = 0.0;
     }
@@ -245,9 +251,9 @@ __device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtenso
 #pragma unroll
     for (int ks = 0; ks < KG; ks++) {
       if (M3) {
-        double ar[4], ai[4], as[4], br[4], bi[4], bs[4];
+        double ar[NB8], ai[NB8], as[NB8], br[NB8], bi[NB8], bs[NB8];
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
+        for (int j = 0; j < NB8; j++) {
           c128 v = B_KMAJOR ? b[(ks * BN + wn0 + j * 8 + lr) * 4 + lk]
                             : b[(ks * 4 + lk) * LDM + wn0 + j * 8 + lr];
           br[j] = v.x;
@@ -255,7 +261,7 @@ __device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtenso
           bs[j] = br[j] + bi[j];
         }
 #pragma unroll
-        for (int i = 0; i < 4; i++) {
+        for (int i = 0; i < NB8; i++) {
           c128 v = A_KMAJOR ? a[(ks * BM + wm0 + i * 8 + lr) * 4 + lk]
                             : a[(ks * 4 + lk) * LDM + wm0 + i * 8 + lr];
           ar[i] = v.x;
@@ -267,17 +273,17 @@ __device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtenso
           if (lane == 0) mbar_arrive(empty0 + 8 * slot);
         }
 #pragma unroll
-        for (int i = 0; i < 4; i++)
+        for (int i = 0; i < NB8; i++)
 #pragma unroll
-          for (int j = 0; j < 4; j++) {
+          for (int j = 0; j < NB8; j++) {
             dmma(cr[i][j][0], cr[i][j][1], ar[i], br[j]);
             dmma(ci[i][j][0], ci[i][j][1], ai[i], bi[j]);
             dmma(cs[M3 ? i : 0][M3 ? j : 0][0], cs[M3 ? i : 0][M3 ? j : 0][1], as[i], bs[j]);
           }
       } else {
-      double ar[4], ai[4], nai[4], br[4], bi[4];
+      double ar[NB8], ai[NB8], nai[NB8], br[NB8], bi[NB8];
 #pragma unroll
-      for (int i = 0; i < 4; i++) {
+      for (int i = 0; i < NB8; i++) {
         c128 v = A_KMAJOR ? a[(ks * BM + wm0 + i * 8 + lr) * 4 + lk]
                           : a[(ks * 4 + lk) * LDM + wm0 + i * 8 + lr];
         ar[i] = v.x;
@@ -285,7 +291,7 @@ __device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtenso
         nai[i] = flip(v.y, CONJ ? na_sign : 0x80000000u);
       }
 #pragma unroll
-      for (int j = 0; j < 4; j++) {
+      for (int j = 0; j < NB8; j++) {
         c128 v = B_KMAJOR ? b[(ks * BN + wn0 + j * 8 + lr) * 4 + lk]
                           : b[(ks * 4 + lk) * LDM + wn0 + j * 8 + lr];
         br[j] = v.x;
@@ -296,16 +302,16 @@ __device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtenso
         if (lane == 0) mbar_arrive(empty0 + 8 * slot);
       }
 #pragma unroll
-      for (int i = 0; i < 4; i++)
+      for (int i = 0; i < NB8; i++)
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
+        for (int j = 0; j < NB8; j++) {
           dmma(cr[i][j][0], cr[i][j][1], ar[i], br[j]);
           dmma(ci[i][j][0], ci[i][j][1], ar[i], bi[j]);
         }
 #pragma unroll
-      for (int i = 0; i < 4; i++)
+      for (int i = 0; i < NB8; i++)
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
+        for (int j = 0; j < NB8; j++) {
           dmma(cr[i][j][0], cr[i][j][1], nai[i], bi[j]);
           dmma(ci[i][j][0], ci[i][j][1], ai[i], br[j]);
         }
@@ -321,11 +327,11 @@ __device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtenso
       c128 *Cb = p.C + bin * p.c_bsi + bo * p.c_bso;
       // thread holds C(row = lane/4, cols = 2*(lane%4) + {0,1}) of every 8x8 block
 #pragma unroll
-      for (int i = 0; i < 4; i++) {
+      for (int i = 0; i < NB8; i++) {
         int m = m0 + wm0 + i * 8 + lr;
         if (m >= p.M) continue;
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
+        for (int j = 0; j < NB8; j++) {
           int n = n0 + wn0 + j * 8 + 2 * lk;
           c128 *dst = Cb + (long long)m * p.ldc + n;
           if (n < p.N) dst[0] = fin(i, j, 0);
@@ -337,11 +343,11 @@ __device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtenso
       const int which = it < lenF ? 0 : 1;
       c128 *sl = p.slots + (size_t)(2 * cta + which) * (BM * BN);
 #pragma unroll
-      for (int i = 0; i < 4; i++)
+      for (int i = 0; i < NB8; i++)
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
-          __stcg(sl + ((i * 4 + j) * 2 + 0) * NTHREADS + tid, fin(i, j, 0));
-          __stcg(sl + ((i * 4 + j) * 2 + 1) * NTHREADS + tid, fin(i, j, 1));
+        for (int j = 0; j < NB8; j++) {
+          __stcg(sl + ((i * NB8 + j) * 2 + 0) * NTHREADS + tid, fin(i, j, 0));
+          __stcg(sl + ((i * NB8 + j) * 2 + 1) * NTHREADS + tid, fin(i, j, 1));
         }
       __syncthreads();               // all stores of the CTA are ordered before thread 0's release
       if (tid == 0) {
@@ -351,9 +357,9 @@ __device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtenso
       }
     }
 #pragma unroll
-    for (int i = 0; i < 4; i++)
+    for (int i = 0; i < NB8; i++)
 #pragma unroll
-      for (int j = 0; j < 4; j++) {
+      for (int j = 0; j < NB8; j++) {
         cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
         if (M3) cs[M3 ? i : 0][M3 ? j : 0][0] = cs[M3 ? i : 0][M3 ? j : 0][1] = 0.0;
       }
@@ -411,7 +417,7 @@ __device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtenso
         const int e = eb + u * NTHREADS;
         if (e >= e_end) continue;
         const int q = e >> 7;                               // e & 127 == tid
-        const int i = q >> 3, jb = (q >> 1) & 3, h = q & 1;
+        const int i = q / (2 * NB8), jb = (q >> 1) % NB8, h = q & 1;
         const int m = fm0 + i * 8, n = fn0 + jb * 8 + h;
         if (m < p.M && n < p.N) Cb[(long long)m * p.ldc + n] = make_double2(sx[u], sy[u]);
       }
@@ -427,20 +433,20 @@ __device__ __forceinline__ void zgemm_body(const CUtensorMap &tmA, const CUtenso
 // SKIP = true (launches that carry a skip flag: the applies of an adaptive Krylov recurrence): the flag is
 // tested first and the body is a function of its own -- with the test inlined in front of it ptxas spilled
 // ~270 bytes in the 3-product instances, which sit at 244 of 255 registers; outlined it costs ~5 % instead.
-template <bool A_KMAJOR, bool B_KMAJOR, bool CONJ, bool M3>
+template <bool A_KMAJOR, bool B_KMAJOR, bool CONJ, bool M3, int TB>
 __device__ __noinline__ void zgemm_body_outlined(const CUtensorMap &tmA, const CUtensorMap &tmB, const KParams &p) {
-  zgemm_body<A_KMAJOR, B_KMAJOR, CONJ, M3>(tmA, tmB, p);
+  zgemm_body<A_KMAJOR, B_KMAJOR, CONJ, M3, TB>(tmA, tmB, p);
 }
-template <bool A_KMAJOR, bool B_KMAJOR, bool CONJ, bool M3, bool SKIP>
+template <bool A_KMAJOR, bool B_KMAJOR, bool CONJ, bool M3, bool SKIP, int TB = 64>
 __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const __grid_constant__ CUtensorMap tmA,
                                                             const __grid_constant__ CUtensorMap tmB,
                                                             const __grid_constant__ KParams p) {
   if (SKIP) {
     // written by an earlier kernel of the stream, so every CTA reads the same value: all return or none does
     if (p.skip != nullptr && __ldcg(p.skip) != 0) return;
-    zgemm_body_outlined<A_KMAJOR, B_KMAJOR, CONJ, M3>(tmA, tmB, p);
+    zgemm_body_outlined<A_KMAJOR, B_KMAJOR, CONJ, M3, TB>(tmA, tmB, p);
   } else {
-    zgemm_body<A_KMAJOR, B_KMAJOR, CONJ, M3>(tmA, tmB, p);
+    zgemm_body<A_KMAJOR, B_KMAJOR, CONJ, M3, TB>(tmA, tmB, p);
   }
 }
 
@@ -453,13 +459,14 @@ template <bool AK, bool BK_, bool CJ, bool M3>
 void launch2(cudaStream_t st, const CUtensorMap &ta, const CUtensorMap &tb, const KParams &kp) {
   // cooperative: the CTAs of a cut tile wait for one another in the fix-up, so all must be resident
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(kp.G); cfg.blockDim = dim3(NTHREADS); cfg.dynamicSmemBytes = SMEM_BYTES; cfg.stream = st;
+  cfg.gridDim = dim3(kp.G); cfg.blockDim = dim3(NTHREADS); cfg.dynamicSmemBytes = kp.tile == 32 ? SMEM_BYTES_32 : SMEM_BYTES; cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeCooperative; attr[0].val.cooperative = 1;
   // no tile is cut when the ranges are whole tiles: nobody waits for anybody, a plain launch will do
   const bool cut = kp.upc_rem != 0 || (kp.upc_base % kp.ktiles) != 0;
   cfg.attrs = attr; cfg.numAttrs = cut ? 1 : 0;
-  if (kp.skip) cudaLaunchKernelEx(&cfg, zgemm_kernel<AK, BK_, CJ, M3, true>, ta, tb, kp);
+  if (kp.tile == 32) cudaLaunchKernelEx(&cfg, zgemm_kernel<AK, BK_, CJ, M3, true, 32>, ta, tb, kp);   // (tests its skip flag, if any)
+  else if (kp.skip) cudaLaunchKernelEx(&cfg, zgemm_kernel<AK, BK_, CJ, M3, true>, ta, tb, kp);
   else cudaLaunchKernelEx(&cfg, zgemm_kernel<AK, BK_, CJ, M3, false>, ta, tb, kp);
   count_launch();
 }
@@ -483,6 +490,10 @@ void set_smem_attr() {
   cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
   cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
   cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true, true, true, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES_32);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false, true, true, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES_32);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, true, false, true, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES_32);
+  cudaFuncSetAttribute(zgemm_kernel<AK, BK_, false, false, true, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES_32);
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda).
@@ -495,7 +506,7 @@ int g_no_5d = 0;       // set when the driver rejects a 5-D map once (or by TDVP
 // Tensor map of one operand seen as doubles.  K-major (unit stride along k): dims (2K, rows, bi, bo),
 // box (8 doubles = 4 complex, 64 rows); MN-major (unit stride along m/n): dims (2*rows, K, bi, bo),
 // box (2*LDM doubles, BK).  Out-of-range box elements read as zero: ragged edges need no predicates.
-bool encode_operand(CUtensorMap *tm, const c128 *base, bool kmajor, long long rows, long long K, long long ld /*complex*/,
+bool encode_operand(CUtensorMap *tm, int tile, const c128 *base, bool kmajor, long long rows, long long K, long long ld /*complex*/,
                     int nbi, long long bsi, int nbo, long long bso) {
   cuuint64_t dims[4], strides[3];
   cuuint32_t box[4], estr[4] = {1, 1, 1, 1};
@@ -508,7 +519,7 @@ bool encode_operand(CUtensorMap *tm, const c128 *base, bool kmajor, long long ro
   const cuuint64_t dummy = strides[0] * dims[1];
   strides[1] = bi ? (cuuint64_t)bsi * 16 : dummy;
   strides[2] = bo ? (cuuint64_t)bso * 16 : dummy;
-  box[0] = kmajor ? 8 : 2 * LDM; box[1] = kmajor ? BM : BK; box[2] = 1; box[3] = 1;
+  box[0] = kmajor ? 8 : 2 * (tile + 2); box[1] = kmajor ? tile : BK; box[2] = 1; box[3] = 1;
   CUresult r = g_encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<c128 *>(base), dims, strides, box, estr,
                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -528,11 +539,11 @@ bool encode_operand(CUtensorMap *tm, const c128 *base, bool kmajor, long long ro
 // (8, 64, KG, 1, 1) -- written to shared memory as [k-group][row][4 complex], the layout the four
 // separate boxes of the 4-D map produce, with one TMA instruction.  Returns false if the driver
 // rejects the map (the caller then keeps the 4-D one).
-bool encode_operand_5d(CUtensorMap *tm, const c128 *base, long long rows, long long K, long long ld /*complex*/,
+bool encode_operand_5d(CUtensorMap *tm, int tile, const c128 *base, long long rows, long long K, long long ld /*complex*/,
                        int nbi, long long bsi, int nbo, long long bso) {
   if (K % 4 != 0 || g_no_5d) return false;
   cuuint64_t dims[5], strides[4];
-  cuuint32_t box[5] = {8, (cuuint32_t)BM, (cuuint32_t)KG, 1, 1}, estr[5] = {1, 1, 1, 1, 1};
+  cuuint32_t box[5] = {8, (cuuint32_t)tile, (cuuint32_t)KG, 1, 1}, estr[5] = {1, 1, 1, 1, 1};
   dims[0] = 8; dims[1] = (cuuint64_t)rows; dims[2] = (cuuint64_t)(K / 4);
   if (rows == 1) ld = K;
   strides[0] = (cuuint64_t)ld * 16;      // rows
@@ -594,17 +605,36 @@ StreamCtx *get_ctx(cudaStream_t st, bool create, bool add_ref = false) {
 // alone reaches ~90 % of the pipe); cutting tiles costs the publish + slice reduction, measured at
 // about 8 us = four units whatever the depth of the cut.
 double g_split_cost = 5.0;
-int choose_grid(long long units, int ktiles) {
+// unit_cost: time of one (tile, k-tile) unit relative to a 64 x 64 unit; split: cost of cutting tiles
+int choose_grid(long long units, int ktiles, double unit_cost = 1.0, double split = -1.0, double *best_out = nullptr) {
   int best_g = 1;
   double best = 1e300;
+  if (split < 0.0) split = g_split_cost;
   const int gmax = units < g_slots ? (int)units : g_slots;
   for (int g = 1; g <= gmax; g++) {
     const long long upc = (units + g - 1) / g;
-    const bool split = (units % g != 0) || (upc % ktiles != 0);
-    const double cost = (double)upc * (g > g_sms ? 2.0 : 1.1) + (split ? g_split_cost : 0.0) - 1e-6 * g;
+    const bool cut = (units % g != 0) || (upc % ktiles != 0);
+    const double cost = unit_cost * (double)upc * (g > g_sms ? 2.0 : 1.1) + (cut ? split : 0.0) - 1e-6 * g;
     if (cost < best) { best = cost; best_g = g; }
   }
+  if (best_out) *best_out = best;
   return best_g;
+}
+// Tile edge of a launch.  A 64 x 64 tile keeps the DMMA pipe busiest (48 DMMAs per 8 fragment loads), but a
+// small product has too few of them to fill 148 SMs without cutting every tile many times (the bond operator of
+// Eq. 44 at M = 128: 4 output tiles, K = 768 -- a 48-way cut whose fix-up costs more than the product).  With
+// 32 x 32 tiles there are four times as many, each unit a quarter of the DMMAs at ~0.4 of the time (12 DMMAs per
+// 4 fragment loads), and a cut tile's fix-up moves a quarter of the data.  The same cost model as choose_grid
+// picks whichever is cheaper; TDVP_ZGEMM_TILE=64 / 32 forces one (diagnostic).
+int g_force_tile = 0;
+double g_unit32 = 0.4, g_split32 = 2.0;
+int choose_tile(long long M, long long N, long long batch, int ktiles, int *G) {
+  double c64 = 0.0, c32 = 0.0;
+  const long long u64 = ((M + 63) / 64) * ((N + 63) / 64) * batch * ktiles, u32 = ((M + 31) / 32) * ((N + 31) / 32) * batch * ktiles;
+  const int g64 = choose_grid(u64, ktiles, 1.0, -1.0, &c64), g32 = choose_grid(u32, ktiles, g_unit32, g_split32, &c32);
+  const bool use32 = g_force_tile == 32 || (g_force_tile == 0 && c32 < c64);
+  *G = use32 ? g32 : g64;
+  return use32 ? 32 : 64;
 }
 
 }  // namespace
@@ -620,6 +650,9 @@ void zgemm_configure() {
   if (per_sm4 < per_sm) per_sm = per_sm4;
   if (const char *es = getenv("TDVP_ZGEMM_SPLIT_COST")) g_split_cost = atof(es);
   if (const char *e5 = getenv("TDVP_ZGEMM_NO_5D")) g_no_5d = e5[0] == '1';
+  if (const char *et = getenv("TDVP_ZGEMM_TILE")) g_force_tile = atoi(et);
+  if (const char *eu = getenv("TDVP_ZGEMM_UNIT32")) g_unit32 = atof(eu);
+  if (const char *eu = getenv("TDVP_ZGEMM_SPLIT32")) g_split32 = atof(eu);
   const char *e4 = getenv("TDVP_ZGEMM_4M");
   if (e4 && e4[0] == '1') g_mode3m.store(0);
   if (per_sm < 1) per_sm = 1;
@@ -678,17 +711,23 @@ int zgemm(cudaStream_t st, const ZGemm &p) {
   StreamCtx *ctx = get_ctx(st, true);
   if (!ctx) return TDVP_ECUDA;                            // the sticky error says why
   const bool ak = (p.a_ks == 1), bk = (p.b_ks == 1);
+  const long long batch = (long long)p.batch_inner * p.batch_outer;
+  int ktiles = (p.K + BK - 1) / BK;
+  if (ktiles < 1) ktiles = 1;
+  int G = 1;
+  const int tile = choose_tile(p.M, p.N, batch, ktiles, &G);
   CUtensorMap ta, tb;
-  if (!encode_operand(&ta, p.A, ak, p.M, p.K, ak ? p.a_ms : p.a_ks, p.batch_inner, p.a_bsi, p.batch_outer, p.a_bso) ||
-      !encode_operand(&tb, p.B, bk, p.N, p.K, bk ? p.b_ns : p.b_ks, p.batch_inner, p.b_bsi, p.batch_outer, p.b_bso))
+  if (!encode_operand(&ta, tile, p.A, ak, p.M, p.K, ak ? p.a_ms : p.a_ks, p.batch_inner, p.a_bsi, p.batch_outer, p.a_bso) ||
+      !encode_operand(&tb, tile, p.B, bk, p.N, p.K, bk ? p.b_ns : p.b_ks, p.batch_inner, p.b_bsi, p.batch_outer, p.b_bso))
     return TDVP_EINVAL;
   if ((reinterpret_cast<size_t>(p.C) & 15) != 0) {
     sticky_error(TDVP_EINVAL, "GEMM output is not 16-byte aligned");
     return TDVP_EINVAL;
   }
   KParams kp;
-  kp.a5 = ak && encode_operand_5d(&ta, p.A, p.M, p.K, p.a_ms, p.batch_inner, p.a_bsi, p.batch_outer, p.a_bso) ? 1 : 0;
-  kp.b5 = bk && encode_operand_5d(&tb, p.B, p.N, p.K, p.b_ns, p.batch_inner, p.b_bsi, p.batch_outer, p.b_bso) ? 1 : 0;
+  kp.a5 = ak && encode_operand_5d(&ta, tile, p.A, p.M, p.K, p.a_ms, p.batch_inner, p.a_bsi, p.batch_outer, p.a_bso) ? 1 : 0;
+  kp.b5 = bk && encode_operand_5d(&tb, tile, p.B, p.N, p.K, p.b_ns, p.batch_inner, p.b_bsi, p.batch_outer, p.b_bso) ? 1 : 0;
+  kp.tile = tile;
   kp.C = p.C;
   kp.M = p.M; kp.N = p.N; kp.K = p.K;
   kp.ldc = p.ldc;
@@ -698,15 +737,12 @@ int zgemm(cudaStream_t st, const ZGemm &p) {
   kp.b_batched_i = p.batch_inner > 1 && p.b_bsi != 0; kp.b_batched_o = p.batch_outer > 1 && p.b_bso != 0;
   kp.a_sign = p.conjA ? 0x80000000u : 0u;
   kp.b_sign = p.conjB ? 0x80000000u : 0u;
-  kp.tiles_m = (p.M + BM - 1) / BM;
-  kp.tiles_n = (p.N + BN - 1) / BN;
-  const long long batch = (long long)p.batch_inner * p.batch_outer;
+  kp.tiles_m = (p.M + tile - 1) / tile;
+  kp.tiles_n = (p.N + tile - 1) / tile;
   const long long tiles = (long long)kp.tiles_m * kp.tiles_n * batch;
-  int ktiles = (p.K + BK - 1) / BK;
-  if (ktiles < 1) ktiles = 1;
   kp.ktiles = ktiles;
   const long long units = tiles * ktiles;
-  kp.G = choose_grid(units, ktiles);
+  kp.G = G;
   kp.upc_base = (int)(units / kp.G);
   kp.upc_rem = (int)(units % kp.G);
   kp.slots = ctx->slots; kp.cnt = ctx->cnt; kp.done = ctx->done;

@@ -310,3 +310,28 @@ def test_two_site_ps_fmo_like_chain(T):
         ch.tdvp_step_ps2(cfg.dt_fs)
         assert np.abs(ch.tdvp_populations(0) - obs.populations(st.mps)).max() <= 1e-8
     ch.close()
+
+
+def test_pc_rk4_step_on_the_fmo_chain(T):
+    """One P&C-RK4 step on the real 71-site FMO-like chain (d = 10, D_W <= 9) from the bare product state at
+    M_max = 14 (M_O M <= 126: every compression SVD on the block-Jacobi path), against oracle/pc_rk4.py.  The
+    compressions of the second Runge-Kutta stage unfold bonds with singular values 6.6, 1e-3 ..., a degenerate
+    cluster at the round-off floor (6.6e-16) and columns another 18 orders below: the device SVD used to run out
+    of sweeps on exactly these (noise-of-noise cascade, svd.cu REL_TINY2).  tau = 20 a.u.: at the paper's 80 a.u.
+    the explicit RK4 is outside its stability region on this chain ((n_ph - 1) w_max tau = 4.9 > 2.8; the paper's
+    own modes have 4-8 levels and lower frequencies)."""
+    from oracle import pc_rk4
+    cfg, params, mpo, dims, mps = chain_inputs("fmo128", M=14)
+    prod = _product_state(dims, si.initial_occupations(params))
+    tau = 20 * 0.0241888
+    want = pc_rk4.warmup(mpo, prod, tau, 1, 14, 14)
+    got = T.tdvp_pc_rk4_warmup(mpo, prod, tau, 1, 14, 14)
+    assert [g.shape for g in got] == [w.shape for w in want]
+    nw, ng = obs.norm_sq(want), obs.norm_sq(got)
+    # the truncation to M = 14 discards weight and nothing renormalises (reading c20): both sides lose the same 3.7 %
+    assert abs(ng - nw) <= 1e-10 * nw and 0.9 < nw < 1.0 + 1e-9
+    assert np.abs(obs.populations(got) - obs.populations(want)).max() <= 1e-9
+    assert abs(abs(overlap(want, got)) / np.sqrt(nw * ng) - 1.0) <= 1e-9
+    for A in got[1:]:
+        m = A.reshape(A.shape[0], -1)
+        assert np.abs(m @ m.conj().T - np.eye(A.shape[0])).max() < 1e-12
