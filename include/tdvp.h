@@ -227,7 +227,9 @@ int tdvp_step_mu(tdvp_handle *h, double dt, double *err_est);
    propagation (readings, DESIGN.md c19): L_i by n_sub classical Runge-Kutta (RK4) sub-steps of
    Eq. 37/33/38 (ceil(n_sub/2) over the half step), C_N by the Lanczos exponential of Eq. 27 with
    the handle's krylov_dim.  SVDs and environment updates therefore run twice per step whatever
-   n_sub is.  Same gauge handling as tdvp_step_mu; enqueue only.  TDVP_EINVAL if n_sub < 1. */
+   n_sub is.  Same gauge handling as tdvp_step_mu; enqueue only; like tdvp_step_ps the step is captured into a
+   CUDA graph once per (dt, n_sub) and replayed (not with TDVP_FLAG_NO_GRAPH, and not while the phase profiler is
+   enabled: a replayed graph carries no brackets).  TDVP_EINVAL if n_sub < 1. */
 int tdvp_step_mu_cmf(tdvp_handle *h, double dt, int n_sub);
 
 /* One evaluation of the TDVP-MU right-hand side (Eq. 27 and Eq. 37-38) on the resident MPS, which

@@ -122,6 +122,7 @@ static void free_chain(tdvp_handle *h) {
   fr(h->ps2_ws);
   if (h->ps_graph.exec) cudaGraphExecDestroy(h->ps_graph.exec);
   if (h->mu_graph.exec) cudaGraphExecDestroy(h->mu_graph.exec);
+  if (h->cmf_graph.exec) cudaGraphExecDestroy(h->cmf_graph.exec);
   h->arena.release();
 }
 

@@ -4,9 +4,10 @@
 
 #include "common.cuh"
 
-struct StepGraph {                 // a captured TDVP step (CUDA graph), keyed by dt
+struct StepGraph {                 // a captured TDVP step (CUDA graph), keyed by dt (and one integer: CMF sub-steps)
   cudaGraphExec_t exec = nullptr;
   double dt = 0.0;
+  int key = 0;
   long long launches = 0;          // kernels inside the graph (for tdvp_launch_count)
 };
 
@@ -49,7 +50,7 @@ struct tdvp_handle {
   std::vector<cudaEvent_t> cmf_join;
   std::vector<void *> cmf_ws, cmf_scratch;
   cudaEvent_t cmf_fork = nullptr;
-  StepGraph ps_graph, mu_graph, ps2_graph;
+  StepGraph ps_graph, mu_graph, ps2_graph, cmf_graph;
   void *ps2_ws = nullptr;          // two-site TDVP-PS workspace (allocated by the first tdvp_step_ps2)
   size_t ps2_ws_bytes = 0;
 };
@@ -60,3 +61,47 @@ int check_cuda(tdvp_handle *h, cudaError_t e, const char *what);
 // TDVP_ESTATE if a bond SVD did not converge.  Every blocking public call ends here.
 int finish_blocking(tdvp_handle *h, const char *what);
 tdvp_handle *default_handle();
+
+// Capture `enqueue` into a graph (once per dt and key) and launch it; falls back to direct enqueue when graphs are
+// disabled.  Side queues that `enqueue` forks from h->stream by an event and joins again before it returns (the CMF
+// local propagation) become parallel branches of the graph.  `enqueue` returns void or a TDVP_E* code.
+template <class F>
+static inline int run_step(tdvp_handle *h, StepGraph &sg, double dt, F enqueue, const char *what, int key = 0) {
+  // (a replayed graph carries no phase brackets: while the phase profiler is on, steps are enqueued directly)
+  if ((h->opt.flags & TDVP_FLAG_NO_GRAPH) || g_prof_on.load(std::memory_order_relaxed)) {
+    enqueue();
+    return check_cuda(h, cudaGetLastError(), what);
+  }
+  if (!sg.exec || sg.dt != dt || sg.key != key) {
+    if (sg.exec) { cudaGraphExecDestroy(sg.exec); sg.exec = nullptr; }
+    cudaStream_t cap = h->stream;
+    cudaStream_t own = nullptr;
+    if (cap == nullptr || cap == cudaStreamLegacy || cap == cudaStreamPerThread) {
+      // the legacy default stream cannot be captured: record on a private stream, replay on h->stream
+      if (int rc = check_cuda(h, cudaStreamCreateWithFlags(&own, cudaStreamNonBlocking), "stream")) return rc;
+      cap = own;
+      zgemm_alias_stream(own, h->stream);
+    }
+    cudaStream_t saved = h->stream;
+    h->stream = cap;
+    long long tally = 0;
+    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    cudaGraph_t graph = nullptr;
+    if (e == cudaSuccess) {
+      g_capture_tally = &tally;
+      enqueue();
+      g_capture_tally = nullptr;
+      e = cudaStreamEndCapture(cap, &graph);
+    }
+    h->stream = saved;
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&sg.exec, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    if (own) { zgemm_forget_stream(own); cudaStreamDestroy(own); }
+    if (e != cudaSuccess) { sg.exec = nullptr; cudaGetLastError(); return check_cuda(h, e, what); }
+    sg.dt = dt; sg.key = key; sg.launches = tally;
+  }
+  if (int rc = check_cuda(h, cudaGraphLaunch(sg.exec, h->stream), what)) return rc;
+  g_launch_count.fetch_add(sg.launches);
+  return TDVP_OK;
+}
+

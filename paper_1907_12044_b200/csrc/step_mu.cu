@@ -425,7 +425,13 @@ int tdvp_step_mu_cmf(tdvp_handle *h, double dt, int n_sub) {
   if (h->centre != h->n - 1) {
     if (int rc = move_gauge(h, h->n - 1)) return rc;
   }
-  return enqueue_cmf_step(h, dt, n_sub);
+  // one CUDA graph per (dt, n_sub): the ~46 000 launches of a step of the 71-site chain, the four side queues of the
+  // local propagation as parallel branches, cost one graph launch on the host
+  if (!mu_scratch(h).U) return set_err(h, TDVP_ENOMEM, "TDVP-MU scratch allocation failed");   // (allocates on first use: not inside a capture)
+  int rc_enq = TDVP_OK;
+  h->mu_fsal = false;
+  const int rc = run_step(h, h->cmf_graph, dt, [&] { rc_enq = enqueue_cmf_step(h, dt, n_sub); }, "tdvp_step_mu_cmf", n_sub);
+  return rc_enq != TDVP_OK ? rc_enq : rc;
 }
 
 int tdvp_mu_derivative(tdvp_handle *h, tdvp_c128 *const *out_host) {

@@ -181,47 +181,6 @@ void enqueue_ps2_step(tdvp_handle *h, double dt) {
 
 }  // namespace
 
-// Capture `enqueue` into a graph (once per dt) and launch it; falls back to direct enqueue when
-// graphs are disabled.
-template <class F>
-static int run_step(tdvp_handle *h, StepGraph &sg, double dt, F enqueue, const char *what) {
-  if (h->opt.flags & TDVP_FLAG_NO_GRAPH) {
-    enqueue();
-    return check_cuda(h, cudaGetLastError(), what);
-  }
-  if (!sg.exec || sg.dt != dt) {
-    if (sg.exec) { cudaGraphExecDestroy(sg.exec); sg.exec = nullptr; }
-    cudaStream_t cap = h->stream;
-    cudaStream_t own = nullptr;
-    if (cap == nullptr || cap == cudaStreamLegacy || cap == cudaStreamPerThread) {
-      // the legacy default stream cannot be captured: record on a private stream, replay on h->stream
-      if (int rc = check_cuda(h, cudaStreamCreateWithFlags(&own, cudaStreamNonBlocking), "stream")) return rc;
-      cap = own;
-      zgemm_alias_stream(own, h->stream);
-    }
-    cudaStream_t saved = h->stream;
-    h->stream = cap;
-    long long tally = 0;
-    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
-    cudaGraph_t graph = nullptr;
-    if (e == cudaSuccess) {
-      g_capture_tally = &tally;
-      enqueue();
-      g_capture_tally = nullptr;
-      e = cudaStreamEndCapture(cap, &graph);
-    }
-    h->stream = saved;
-    if (e == cudaSuccess) e = cudaGraphInstantiate(&sg.exec, graph, 0);
-    if (graph) cudaGraphDestroy(graph);
-    if (own) { zgemm_forget_stream(own); cudaStreamDestroy(own); }
-    if (e != cudaSuccess) { sg.exec = nullptr; cudaGetLastError(); return check_cuda(h, e, what); }
-    sg.dt = dt; sg.launches = tally;
-  }
-  if (int rc = check_cuda(h, cudaGraphLaunch(sg.exec, h->stream), what)) return rc;
-  g_launch_count.fetch_add(sg.launches);
-  return TDVP_OK;
-}
-
 int move_gauge(tdvp_handle *h, int centre);
 
 extern "C" {
