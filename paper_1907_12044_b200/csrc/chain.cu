@@ -116,7 +116,10 @@ static void free_chain(tdvp_handle *h) {
   for (auto p : h->cmf_scratch) fr(p);
   for (auto q : h->cmf_streams) { cudaStreamSynchronize(q); zgemm_release_stream(q); cudaStreamDestroy(q); }
   for (auto e : h->cmf_join) cudaEventDestroy(e);
+  for (auto e : h->cmf_rel) cudaEventDestroy(e);
   if (h->cmf_fork) cudaEventDestroy(h->cmf_fork);
+  if (h->cmf_hi) { cudaStreamSynchronize(h->cmf_hi); zgemm_release_stream(h->cmf_hi); cudaStreamDestroy(h->cmf_hi); }
+  if (h->cmf_hi_done) cudaEventDestroy(h->cmf_hi_done);
   fr(h->tmpA); fr(h->tmpB); fr(h->bondD); fr(h->bondD2); fr(h->step_ws); fr(h->mu_err_dev); fr(h->mu_scratch);
   if (h->ps2_graph.exec) cudaGraphExecDestroy(h->ps2_graph.exec);
   fr(h->ps2_ws);

@@ -89,6 +89,8 @@ struct ZGemm {
 // error (callers with a void chain need not look at it).
 int zgemm(cudaStream_t st, const ZGemm &p);
 int zgemm_prepare_stream(cudaStream_t st);
+void zgemm_set_stream_cap(cudaStream_t st, int max_ctas);   // GEMMs on st use at most this many CTAs (0: no limit)
+int zgemm_device_sms();
 void zgemm_set_mode(int products);   // 3 or 4 real DMMA products per complex product
 int zgemm_get_mode();
 void zgemm_alias_stream(cudaStream_t alias, cudaStream_t of);
@@ -191,8 +193,11 @@ constexpr int QR_MAX_TALL = 12800;
 size_t qr_ws_bytes(int rows, int cols);
 // side 0: C (rows x cols, row-major, rows = Ml*d, cols = Mr) = Q D, Q rows x cols, D cols x cols
 // side 1: C (Ml x (d*Mr)) = D Q, i.e. QR of C^T: tall = d*Mr, thin = Ml; Q [Ml, d*Mr], D [Ml, Ml]
+// gate (DEVICE, nullable): if it points at zero when the kernels start, the two expensive ones (cluster factorisation
+// and Q formation, matrices of up to 1280 rows) return at once and Q, D are left undefined -- for callers that decide
+// on the device whether the factorisation is needed at all (svd.cu)
 void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c128 *Q, c128 *D,
-              void *ws);
+              void *ws, const int *gate = nullptr);
 
 // ---------------------------------------------------------------------------------------------
 // svd.cu : matrix unfolding C[Ml, d*Mr] = U diag(lam) Vh (Eq. 36) on the device, Ml <= d*Mr.

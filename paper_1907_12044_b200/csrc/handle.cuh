@@ -47,9 +47,10 @@ struct tdvp_handle {
   void *mu_scratch = nullptr;      // U, Lambda, V^dagger, centre forms ... of one derivative evaluation
   std::vector<void *> cmf_mem;     // CMF mean fields per bond b: [3b] U, [3b+1] U Lambda, [3b+2] Lambda (first use)
   std::vector<cudaStream_t> cmf_streams;   // side queues of the CMF local propagation, each with scratch
-  std::vector<cudaEvent_t> cmf_join;
+  std::vector<cudaEvent_t> cmf_join, cmf_rel;   // queue q has finished; mean fields of site j are ready
   std::vector<void *> cmf_ws, cmf_scratch;
-  cudaEvent_t cmf_fork = nullptr;
+  cudaEvent_t cmf_fork = nullptr, cmf_hi_done = nullptr;
+  cudaStream_t cmf_hi = nullptr;   // highest-priority queue of the CMF mean-field (bond unfolding) chain
   StepGraph ps_graph, mu_graph, ps2_graph, cmf_graph;
   void *ps2_ws = nullptr;          // two-site TDVP-PS workspace (allocated by the first tdvp_step_ps2)
   size_t ps2_ws_bytes = 0;

@@ -375,7 +375,9 @@ __device__ __forceinline__ void cluster_exchange(const double *loc, int n, int n
 // phase RPT = ceil(RA / QC).  Forming Q stays a kernel of its own (one CTA per column, all SMs).
 template <int RA, int NB>
 __global__ void __cluster_dims__(QC, 1, 1) __launch_bounds__(QT, 1)
-qr_factor_cluster_kernel(c128 *X, int rows, int cols, c128 *Rm, c128 *Tm /*[npanels][NB_MAX][NB_MAX]*/) {
+qr_factor_cluster_kernel(c128 *X, int rows, int cols, c128 *Rm, c128 *Tm /*[npanels][NB_MAX][NB_MAX]*/,
+                         const int *gate /*DEVICE, nullable: run only if non-zero (written by an earlier kernel of the stream)*/) {
+  if (gate && __ldcg(gate) == 0) return;                   // every CTA of the cluster reads the same value
   constexpr int RPT = (RA + QC - 1) / QC;
   constexpr int NGRAM = NB * (NB - 1);                   // re / im of the strictly upper Gram entries (<= 56)
   constexpr int NGB = (NGRAM + 15) / 16;                 // 16-value reduction rounds for them
@@ -890,7 +892,9 @@ __global__ void __launch_bounds__(TRAIL_THREADS) qr_apply_kernel(const c128 *X, 
 //                  for the whole Q instead of one per panel.
 template <int AT, int RA, int NBW, bool FORMQ>
 __global__ void __launch_bounds__(AT) qr_apply1_kernel(const c128 *__restrict__ X, c128 *Y, int rows, int j0_in, int w_in,
-                                                        const c128 *__restrict__ Tm, int nb, int cols, int c_begin) {
+                                                        const c128 *__restrict__ Tm, int nb, int cols, int c_begin,
+                                                        const int *gate = nullptr /*DEVICE, nullable: run only if non-zero*/) {
+  if (gate && __ldcg(gate) == 0) return;
   __shared__ double sm[(AT / 32 + 1) * 2 * NBW];
   __shared__ c128 Tsm[NB_MAX * NB_MAX];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -1038,7 +1042,7 @@ size_t qr_ws_bytes(int rows, int cols) {
   return 2 * mat + up256((size_t)cols * cols * 16) + up256(npanels * NB_MAX * NB_MAX * 16) + 512;
 }
 
-void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c128 *Q, c128 *D, void *ws) {
+void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c128 *Q, c128 *D, void *ws, const int *gate) {
   const int rows = side == 0 ? Ml * d : d * Mr;
   const int cols = side == 0 ? Mr : Ml;
   int nb = 1;
@@ -1061,7 +1065,7 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
     // (B200, 1280 x 128): 580 us against 698 us with one launch per panel and per update; at 2560 x 256 the
     // 16 SMs of the cluster are too few for the trailing updates (2170 against 1924 us), so taller matrices
     // keep the launch-per-panel path below.
-    TDVP_LAUNCH((qr_factor_cluster_kernel<5, 8>), QC, QT, QF_SMEM, st, X, rows, cols, Rm, Tm);
+    TDVP_LAUNCH((qr_factor_cluster_kernel<5, 8>), QC, QT, QF_SMEM, st, X, rows, cols, Rm, Tm, gate);
   } else
   for (int pz = 0; pz < npanels; pz++) {
     int j0 = pz * nb, w = cols - j0 < nb ? cols - j0 : nb;
@@ -1078,7 +1082,7 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
     int c_begin = j0 + w;
     launch_apply(st, mode, X, X, rows, j0, w, Tp, 1, c_begin, cols);
   }
-  if (mode == 1) TDVP_LAUNCH((qr_apply1_kernel<256, 5, 8, true>), cols, 256, 0, st, X, Y, rows, 0, 0, Tm, nb, cols, 0);
+  if (mode == 1) TDVP_LAUNCH((qr_apply1_kernel<256, 5, 8, true>), cols, 256, 0, st, X, Y, rows, 0, 0, Tm, nb, cols, 0, gate);
   else if (mode == 2) TDVP_LAUNCH((qr_apply1_kernel<256, 10, 4, true>), cols, 256, 0, st, X, Y, rows, 0, 0, Tm, nb, cols, 0);
   else if (mode == 3) TDVP_LAUNCH((qr_apply1_kernel<256, 20, 2, true>), cols, 256, 0, st, X, Y, rows, 0, 0, Tm, nb, cols, 0);
   else {

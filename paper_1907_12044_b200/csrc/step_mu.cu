@@ -15,6 +15,8 @@
 #include <cstdlib>
 #include <utility>
 
+#include <functional>
+
 #include "handle.cuh"
 
 int move_gauge(tdvp_handle *h, int centre);
@@ -251,7 +253,10 @@ int cmf_alloc(tdvp_handle *h) {
 }
 
 // Mean fields of the left-canonical state Y: Lenv[i] for every site, Renv[j] / U / Lambda for j < n-1.
-int cmf_mean_fields(tdvp_handle *h, const std::vector<c128 *> &Y) {
+// `released(j)` (optional) is called as soon as everything the local problem of site j reads has been enqueued on
+// h->stream -- L[j] from the forward pass, R[j] and U, Lambda of the bond to its right from the backward pass at bond
+// j + 1 -- i.e. while the unfoldings of the bonds further left are still to come: the caller starts site j there.
+int cmf_mean_fields(tdvp_handle *h, const std::vector<c128 *> &Y, const std::function<void(int)> &released = nullptr) {
   cudaStream_t st = h->stream;
   const int n = h->n;
   MuScratch s = mu_scratch(h);
@@ -270,6 +275,7 @@ int cmf_mean_fields(tdvp_handle *h, const std::vector<c128 *> &Y) {
     env_update(st, 1, Ml, Mr, d, h->Dw[i], h->Dw[i + 1], h->Renv[i], h->Wsp[i], s.Vh, h->Renv[i - 1], ws);
     vec_copy(st, UL, U, (long long)Ml * Ml);
     TDVP_LAUNCH(scale_cols_kernel, grid_for((long long)Ml * Ml), VT, 0, st, UL, (long long)Ml, Ml, lam, 0, 0.0);
+    if (released) released(i - 1);
     if (i > 1) {                                           // centre form of site i-1, unfolded next
       const int j = i - 1;
       ZGemm g{};
@@ -322,6 +328,20 @@ int cmf_queues(tdvp_handle *h) {
   if (nq < 1) nq = 1;
   if (nq > 8) nq = 8;
   if (int rc = check_cuda(h, cudaEventCreateWithFlags(&h->cmf_fork, cudaEventDisableTiming), "event")) return rc;
+  {
+    static const bool hi = [] { const char *e = getenv("TDVP_CMF_PRIORITY"); return !(e && e[0] == '0'); }();
+    int least = 0, greatest = 0;
+    if (hi && cudaDeviceGetStreamPriorityRange(&least, &greatest) == cudaSuccess && greatest != least) {
+      if (int rc = check_cuda(h, cudaStreamCreateWithPriority(&h->cmf_hi, cudaStreamNonBlocking, greatest), "CMF mean-field queue")) return rc;
+      if (int rc = check_cuda(h, cudaEventCreateWithFlags(&h->cmf_hi_done, cudaEventDisableTiming), "event")) return rc;
+      zgemm_prepare_stream(h->cmf_hi);
+    }
+  }
+  for (int j = 0; j < h->n; j++) {                           // "mean fields of site j are ready"
+    cudaEvent_t ev = nullptr;
+    if (int rc = check_cuda(h, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming), "event")) return rc;
+    h->cmf_rel.push_back(ev);
+  }
   for (int q = 0; q < nq; q++) {
     cudaStream_t st = nullptr; cudaEvent_t ev = nullptr; void *ws = nullptr, *sc = nullptr;
     if (int rc = check_cuda(h, cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking), "CMF queue")) return rc;
@@ -329,6 +349,13 @@ int cmf_queues(tdvp_handle *h) {
     if (int rc = check_cuda(h, cudaMalloc(&ws, h->step_ws_bytes), "cudaMalloc CMF workspace")) return rc;
     if (int rc = check_cuda(h, cudaMalloc(&sc, mu_scratch_bytes(h, nullptr, nullptr)), "cudaMalloc CMF scratch")) return rc;
     zgemm_prepare_stream(st);
+    // the side queues run beside the unfolding chain's cluster kernels (16 SMs for a QR, 8 for the Jacobi sweeps, up
+    // to 2 ms each): their GEMMs leave those SMs out of their grids, or every cut (cooperative) launch would wait
+    {
+      static const int spare = [] { const char *e = getenv("TDVP_CMF_SPARE_SMS"); return e ? atoi(e) : 24; }();
+      const int sms = zgemm_device_sms();
+      if (spare > 0 && sms > 2 * spare) zgemm_set_stream_cap(st, 2 * (sms - spare));
+    }
     h->cmf_streams.push_back(st); h->cmf_join.push_back(ev); h->cmf_ws.push_back(ws); h->cmf_scratch.push_back(sc);
   }
   return TDVP_OK;
@@ -358,16 +385,41 @@ void cmf_site(tdvp_handle *h, int j, const c128 *Xj, c128 *y, double t, int n_su
   }
 }
 
-// Z[i] = every local matrix of X propagated over time t with the handle's mean fields.
-int cmf_propagate(tdvp_handle *h, const std::vector<c128 *> &X, const std::vector<c128 *> &Z, double t, int n_sub) {
+// Mean fields of the state Y, then Z[i] = every local matrix of X propagated over time t with them.  The two are
+// pipelined: the backward pass of the mean-field build is a chain of bond unfoldings (one 8-SM cluster kernel at a
+// time, ~2.5 ms per bond at M = 128), and site j's local problem needs nothing left of bond j + 1 -- so site j starts
+// on its side queue the moment that bond is done (an event per site), and the local propagation, which is where the
+// step's GEMM work is, fills the SMs the unfolding chain leaves idle.  Same kernels in the same order on every
+// queue: bit-identical to running the two phases one after the other (TDVP_CMF_PIPELINE=0).
+int cmf_fields_and_propagate(tdvp_handle *h, const std::vector<c128 *> &Y, const std::vector<c128 *> &X, const std::vector<c128 *> &Z,
+                             double t, int n_sub) {
   cudaStream_t st = h->stream;
   const int n = h->n;
   const int nq = (int)h->cmf_streams.size();
-  cudaEventRecord(h->cmf_fork, st);                          // the mean fields are ready
-  for (int q = 0; q < nq; q++) cudaStreamWaitEvent(h->cmf_streams[q], h->cmf_fork, 0);
-  for (int j = 0; j < n - 1; j++) {
+  static const bool pipeline = [] { const char *e = getenv("TDVP_CMF_PIPELINE"); return !(e && e[0] == '0'); }();
+  auto start_site = [&](int j) {
     const int q = j % nq;
     cmf_site(h, j, X[j], Z[j], t, n_sub, mu_carve(h, h->cmf_scratch[q]), h->cmf_streams[q], h->cmf_ws[q]);
+  };
+  if (pipeline) {
+    // the unfolding chain is the critical path: it runs on a queue of its own with the highest priority, so that its
+    // short cluster kernels are scheduled ahead of the side queues' GEMM CTAs whenever SMs come free
+    cudaStream_t mf = h->cmf_hi ? h->cmf_hi : st;
+    if (mf != st) { cudaEventRecord(h->cmf_fork, st); cudaStreamWaitEvent(mf, h->cmf_fork, 0); }
+    h->stream = mf;
+    const int rc = cmf_mean_fields(h, Y, [&](int j) {
+      cudaEventRecord(h->cmf_rel[j], mf);                    // mean fields of site j are ready
+      cudaStreamWaitEvent(h->cmf_streams[j % nq], h->cmf_rel[j], 0);
+      start_site(j);
+    });
+    h->stream = st;
+    if (mf != st) { cudaEventRecord(h->cmf_hi_done, mf); cudaStreamWaitEvent(st, h->cmf_hi_done, 0); }
+    if (rc) return rc;
+  } else {
+    if (int rc = cmf_mean_fields(h, Y)) return rc;
+    cudaEventRecord(h->cmf_fork, st);
+    for (int q = 0; q < nq && q < n - 1; q++) cudaStreamWaitEvent(h->cmf_streams[q], h->cmf_fork, 0);
+    for (int j = 0; j < n - 1; j++) start_site(j);
   }
   {                                                        // Eq. 27 by the Krylov exponential
     const int i = n - 1;
@@ -376,7 +428,7 @@ int cmf_propagate(tdvp_handle *h, const std::vector<c128 *> &X, const std::vecto
     op.L = h->Lenv[i]; op.R = h->Renv[i]; op.W = &h->Wsp[i];
     lanczos_expm(st, op, h->opt.krylov_dim, h->opt.krylov_tol, 0.0, -t, X[i], Z[i], h->step_ws, nullptr, h->status_dev);
   }
-  for (int q = 0; q < nq; q++) {
+  for (int q = 0; q < nq && q < n - 1; q++) {
     cudaEventRecord(h->cmf_join[q], h->cmf_streams[q]);
     cudaStreamWaitEvent(st, h->cmf_join[q], 0);
   }
@@ -385,10 +437,8 @@ int cmf_propagate(tdvp_handle *h, const std::vector<c128 *> &X, const std::vecto
 
 int enqueue_cmf_step(tdvp_handle *h, double dt, int n_sub) {
   h->mu_fsal = false;
-  if (int rc = cmf_mean_fields(h, h->A)) return rc;
-  if (int rc = cmf_propagate(h, h->A, h->mu_k[4], 0.5 * dt, (n_sub + 1) / 2)) return rc;
-  if (int rc = cmf_mean_fields(h, h->mu_k[4])) return rc;
-  if (int rc = cmf_propagate(h, h->A, h->mu_k[5], dt, n_sub)) return rc;
+  if (int rc = cmf_fields_and_propagate(h, h->A, h->A, h->mu_k[4], 0.5 * dt, (n_sub + 1) / 2)) return rc;
+  if (int rc = cmf_fields_and_propagate(h, h->mu_k[4], h->A, h->mu_k[5], dt, n_sub)) return rc;
   for (int i = 0; i < h->n; i++) vec_copy(h->stream, h->A[i], h->mu_k[5][i], site_elems(h, i));
   return check_cuda(h, cudaGetLastError(), "tdvp_step_mu_cmf");
 }

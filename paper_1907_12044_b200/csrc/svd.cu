@@ -84,6 +84,9 @@ __global__ void svd_init_kernel(const c128 *D, c128 *Xt, c128 *Jt, int n) {
 // NPL = rows per lane held in registers (n <= 32 * NPL); NPL = 0 is the generic looped variant.
 constexpr int JC = 8;               // CTAs per cluster
 constexpr int JW = 8;               // warps per CTA
+// flags[] of one unfolding (ints, zeroed): [0, 40) a sweep rotated, [64, 104) ... a pair far from orthogonal, and
+constexpr int FLAG_FORCE_QR = 120;  // the Jacobi kernel ran out of sweeps
+constexpr int FLAG_NEED_QR = 121;   // decided by svd_sortcols_kernel: the Householder step has to make U unitary
 
 template <int NPL>
 __global__ void __cluster_dims__(JC, 1, 1) __launch_bounds__(JW * 32)
@@ -183,8 +186,10 @@ svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/,
   }
   // every sweep allowed still rotated, and the last one still saw a pair far from orthogonal (rotations that
   // hover at the round-off threshold of sqrt(n) eps are convergence): tell the host
-  if (sweep == max_sweeps && np >= 2 && status && gwarp == 0 && lane == 0 && __ldcg(flags + 64 + max_sweeps - 1))
-    atomicOr(status, TDVP_STATUS_SVD_UNCONVERGED);
+  if (sweep == max_sweeps && np >= 2 && gwarp == 0 && lane == 0) {
+    flags[FLAG_FORCE_QR] = 1;                           // columns may still be far from orthogonal: U comes from the Householder step
+    if (status && __ldcg(flags + 64 + max_sweeps - 1)) atomicOr(status, TDVP_STATUS_SVD_UNCONVERGED);
+  }
 }
 
 // Block variant for n <= 128: the same rotations, but the cluster barrier is paid once per BLOCK pair
@@ -322,7 +327,10 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
     }
     if (__ldcg(flags + sweep) == 0) break;                          // nobody rotated in this sweep
   }
-  if (sweep == max_sweeps && status && cta == 0 && tid == 0 && __ldcg(flags + 64 + max_sweeps - 1)) atomicOr(status, TDVP_STATUS_SVD_UNCONVERGED);
+  if (sweep == max_sweeps && cta == 0 && tid == 0) {
+    flags[FLAG_FORCE_QR] = 1;
+    if (status && __ldcg(flags + 64 + max_sweeps - 1)) atomicOr(status, TDVP_STATUS_SVD_UNCONVERGED);
+  }
 }
 
 // Columns of the rotated X (and of J with them) in the order of decreasing norm, before the Householder step:
@@ -337,11 +345,27 @@ __global__ void svd_colnorm_kernel(const c128 *Xt, int n, double *nrm) {
   a = wsum(a);
   if (lane == 0) nrm[c] = a;
 }
-__global__ void svd_sortcols_kernel(const c128 *Xt, const c128 *Jt, const double *nrm, int n, c128 *Xs, c128 *Js) {
+// It also decides (CTA 0) whether the Householder step is needed: the rotated columns are mutually orthogonal to
+// sqrt(n) eps RELATIVE to their norms -- U = X diag(1 / |x_c|) is then unitary to round-off as it stands -- unless the
+// iteration left columns alone (below the REL_TINY2 / TINY_COL2 floors: their directions are arbitrary) or ran out of
+// sweeps.  Only then does the factorisation X = U' R' run (flags[FLAG_NEED_QR] gates its kernels).
+__global__ void svd_sortcols_kernel(const c128 *Xt, const c128 *Jt, const double *nrm, int n, c128 *Xs, c128 *Js, int *flags, int always_qr) {
   __shared__ int s_rank;
   const int c = blockIdx.x;
   if (threadIdx.x == 0) s_rank = 0;
   __syncthreads();
+  if (c == 0 && threadIdx.x < 32) {
+    double mx = 0.0, mn = 1e308;
+    for (int q = threadIdx.x; q < n; q += 32) { const double o = nrm[q]; mx = fmax(mx, o); mn = (o < mn || o != o) ? o : mn; }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+      const double t = __shfl_xor_sync(0xffffffffu, mn, o);
+      mn = (t < mn || t != t) ? t : mn;
+    }
+    if (threadIdx.x == 0)
+      flags[FLAG_NEED_QR] = (always_qr || flags[FLAG_FORCE_QR] || !(mn >= fmax(TINY_COL2, REL_TINY2 * mx)) || !(mx < 1e300)) ? 1 : 0;
+  }
   const double mine = nrm[c];
   int cnt = 0;
   for (int q = threadIdx.x; q < n; q += blockDim.x) { const double o = nrm[q]; cnt += (o > mine || (o == mine && q < c)) ? 1 : 0; }
@@ -356,9 +380,30 @@ __global__ void svd_sortcols_kernel(const c128 *Xt, const c128 *Jt, const double
 
 // lam (descending), U and the permuted J from X = U' R' (Qp = U'^T, Dp = R'^T as qr_gauge side 1 returns them).
 // U[i][k] = Qp[r][i] * sgn(Dp[r][r]),  JtP[k][j] = Jt[r][j]   with k = rank of r.
+// Without the Householder step (flags[FLAG_NEED_QR] == 0): column k of the sorted X is sigma_k u_k as it stands.
 __global__ void svd_finish_kernel(const c128 *Qp, const c128 *Dp, const c128 *Jt, int n, c128 *U, double *lam,
-                                  c128 *JtP) {
+                                  c128 *JtP, const c128 *Xs, const double *nrm_unused, const int *flags) {
   extern __shared__ double sl[];                                  // [n] |R'_rr|
+  if (__ldcg(flags + FLAG_NEED_QR) == 0) {
+    __shared__ double s_part[4];
+    for (int k = blockIdx.x; k < n; k += gridDim.x) {
+      double a = 0.0;
+      for (int i = threadIdx.x; i < n; i += blockDim.x) { const c128 u = Xs[(long long)k * n + i]; a += u.x * u.x + u.y * u.y; }
+      a = wsum(a);
+      if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = a;
+      __syncthreads();
+      const double nrm2 = s_part[0] + s_part[1] + s_part[2] + s_part[3];      // (128 threads: four warps, fixed order)
+      const double nr = sqrt(nrm2), inv = 1.0 / nr;
+      if (threadIdx.x == 0) lam[k] = nr;
+      for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const c128 u = Xs[(long long)k * n + i];
+        U[(long long)i * n + k] = make_double2(u.x * inv, u.y * inv);
+        JtP[(long long)k * n + i] = Jt[(long long)k * n + i];
+      }
+      __syncthreads();
+    }
+    return;
+  }
   for (int r = threadIdx.x; r < n; r += blockDim.x) {
     c128 v = Dp[(long long)r * n + r];
     sl[r] = sqrt(v.x * v.x + v.y * v.y);
@@ -433,9 +478,11 @@ void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, do
   // X = U' R'  <=>  Xt = R'^T U'^T: "side 1" factorisation of the n x n matrix Xt (d = 1)
   c128 *Xs = D;                                                   // D is no longer needed
   TDVP_LAUNCH(svd_colnorm_kernel, (n + 7) / 8, 256, 0, st, Xt, n, cnorm);
-  TDVP_LAUNCH(svd_sortcols_kernel, n, 128, 0, st, Xt, Jt, cnorm, n, Xs, Js);
-  qr_gauge(st, 1, n, 1, n, Xs, Qp, Dp, qws);
-  TDVP_LAUNCH(svd_finish_kernel, n < 148 ? n : 148, 128, n * sizeof(double), st, Qp, Dp, Js, n, U, lam, JtP);
+  // TDVP_SVD_ALWAYS_QR=1: the Householder step runs whatever the columns look like (diagnostic switch)
+  static const int always_qr = [] { const char *e = getenv("TDVP_SVD_ALWAYS_QR"); return (e && e[0] == '1') ? 1 : 0; }();
+  TDVP_LAUNCH(svd_sortcols_kernel, n, 128, 0, st, Xt, Jt, cnorm, n, Xs, Js, flags, always_qr);
+  qr_gauge(st, 1, n, 1, n, Xs, Qp, Dp, qws, flags + FLAG_NEED_QR);
+  TDVP_LAUNCH(svd_finish_kernel, n < 148 ? n : 148, 128, n * sizeof(double), st, Qp, Dp, Js, n, U, lam, JtP, Xs, cnorm, flags);
   ZGemm gm{};                                   // Vh[k][:] = sum_j conj(JtP[k][j]) Q[j][:]
   gm.A = JtP; gm.B = Q; gm.C = Vh;
   gm.M = n; gm.K = n; gm.N = d * Mr;

@@ -565,7 +565,7 @@ bool encode_operand_5d(CUtensorMap *tm, int tile, const c128 *base, long long ro
 // Per-stream scheduling state: partial-tile slots and the two counter arrays.  Kernels of one
 // stream run one after the other, so one context per stream is enough; it is created outside any
 // stream capture (zgemm_prepare_stream) because cudaMalloc is not allowed while capturing.
-struct StreamCtx { c128 *slots = nullptr; int *cnt = nullptr; int *done = nullptr; int refs = 0; bool alias = false; };
+struct StreamCtx { c128 *slots = nullptr; int *cnt = nullptr; int *done = nullptr; int refs = 0; bool alias = false; int cap = 0; };
 std::mutex g_ctx_mu;
 std::unordered_map<cudaStream_t, StreamCtx> g_ctx;
 int g_slots = 0;      // resident CTAs of zgemm_kernel on this device (2 per SM)
@@ -606,11 +606,12 @@ StreamCtx *get_ctx(cudaStream_t st, bool create, bool add_ref = false) {
 // about 8 us = four units whatever the depth of the cut.
 double g_split_cost = 5.0;
 // unit_cost: time of one (tile, k-tile) unit relative to a 64 x 64 unit; split: cost of cutting tiles
-int choose_grid(long long units, int ktiles, double unit_cost = 1.0, double split = -1.0, double *best_out = nullptr) {
+int choose_grid(long long units, int ktiles, double unit_cost = 1.0, double split = -1.0, double *best_out = nullptr, int cap = 0) {
   int best_g = 1;
   double best = 1e300;
   if (split < 0.0) split = g_split_cost;
-  const int gmax = units < g_slots ? (int)units : g_slots;
+  const int slots = cap > 0 && cap < g_slots ? cap : g_slots;
+  const int gmax = units < slots ? (int)units : slots;
   for (int g = 1; g <= gmax; g++) {
     const long long upc = (units + g - 1) / g;
     const bool cut = (units % g != 0) || (upc % ktiles != 0);
@@ -628,10 +629,10 @@ int choose_grid(long long units, int ktiles, double unit_cost = 1.0, double spli
 // picks whichever is cheaper; TDVP_ZGEMM_TILE=64 / 32 forces one (diagnostic).
 int g_force_tile = 0;
 double g_unit32 = 0.4, g_split32 = 2.0;
-int choose_tile(long long M, long long N, long long batch, int ktiles, int *G) {
+int choose_tile(long long M, long long N, long long batch, int ktiles, int *G, int cap) {
   double c64 = 0.0, c32 = 0.0;
   const long long u64 = ((M + 63) / 64) * ((N + 63) / 64) * batch * ktiles, u32 = ((M + 31) / 32) * ((N + 31) / 32) * batch * ktiles;
-  const int g64 = choose_grid(u64, ktiles, 1.0, -1.0, &c64), g32 = choose_grid(u32, ktiles, g_unit32, g_split32, &c32);
+  const int g64 = choose_grid(u64, ktiles, 1.0, -1.0, &c64, cap), g32 = choose_grid(u32, ktiles, g_unit32, g_split32, &c32, cap);
   const bool use32 = g_force_tile == 32 || (g_force_tile == 0 && c32 < c64);
   *G = use32 ? g32 : g64;
   return use32 ? 32 : 64;
@@ -668,6 +669,16 @@ void zgemm_configure() {
 
 void zgemm_set_mode(int products) { configure_kernels_once(); g_mode3m.store(products == 4 ? 0 : 1); }
 int zgemm_get_mode() { configure_kernels_once(); return g_mode3m.load() ? 3 : 4; }
+
+// Launches on `st` use at most `max_ctas` CTAs (0 = all the device holds).  For queues that run beside long cluster
+// kernels: a cut GEMM is a cooperative launch, which starts only when ALL its CTAs fit at once -- with every slot of
+// the device in its grid it would wait for a 2 ms bond-unfolding kernel on 8 SMs to end.
+void zgemm_set_stream_cap(cudaStream_t st, int max_ctas) {
+  std::lock_guard<std::mutex> lk(g_ctx_mu);
+  auto it = g_ctx.find(st);
+  if (it != g_ctx.end()) it->second.cap = max_ctas;
+}
+int zgemm_device_sms() { configure_kernels_once(); return g_sms; }
 
 // One more owner (a handle) of the stream's context; created if missing.
 int zgemm_prepare_stream(cudaStream_t st) {
@@ -715,7 +726,7 @@ int zgemm(cudaStream_t st, const ZGemm &p) {
   int ktiles = (p.K + BK - 1) / BK;
   if (ktiles < 1) ktiles = 1;
   int G = 1;
-  const int tile = choose_tile(p.M, p.N, batch, ktiles, &G);
+  const int tile = choose_tile(p.M, p.N, batch, ktiles, &G, ctx->cap);
   CUtensorMap ta, tb;
   if (!encode_operand(&ta, tile, p.A, ak, p.M, p.K, ak ? p.a_ms : p.a_ks, p.batch_inner, p.a_bsi, p.batch_outer, p.a_bso) ||
       !encode_operand(&tb, tile, p.B, bk, p.N, p.K, bk ? p.b_ns : p.b_ks, p.batch_inner, p.b_bsi, p.batch_outer, p.b_bso))
