@@ -321,8 +321,16 @@ long long tdvp_launch_count(void);
                               Lanczos iteration, read once;
      TDVP_NO_FSAL=1           tdvp_step_mu recomputes stage 1 instead of reusing stage 7 of the step
                               before (bit-identical by construction; read at every step);
-     TDVP_CMF_QUEUES=n        side queues of the CMF local propagation (1..8, default 4; results are
-                              bit-identical for any n), read when a handle first runs tdvp_step_mu_cmf;
+     TDVP_CMF_QUEUES=n        side queues of the local problems of TDVP-MU (1..8, default 4), read when a handle
+                              first runs tdvp_step_mu / tdvp_step_mu_cmf / tdvp_mu_derivative;
+     TDVP_CMF_PIPELINE=0      CMF step: build all mean fields first, then propagate all sites (default: site j starts
+                              on its side queue as soon as the bond to its right is unfolded), read once;
+     TDVP_MU_PIPELINE=0       the same switch for the right-hand side of tdvp_step_mu / tdvp_mu_derivative, read once;
+     TDVP_CMF_PRIORITY=0      no separate highest-priority queue for the chain of bond unfoldings, read once;
+     TDVP_CMF_SPARE_SMS=n     SMs the GEMMs of the side queues leave out of their grids, for the cluster kernels of
+                              the unfolding chain that run beside them (default 24; 0 = none), read once;
+     TDVP_SVD_ALWAYS_QR=1     a bond SVD always runs its final Householder step (default: only when the Jacobi
+                              iteration left columns alone or ran out of sweeps; decided on the device), read once;
      TDVP_QR_CLUSTER=0        QR gauge moves of up to 1280 rows with one launch per panel and per trailing update
                               instead of the single 16-CTA cluster kernel, read once;
      TDVP_SVD_MAX_SWEEPS=n    Jacobi sweeps a bond SVD may use (1..40, default 40; lowering it forces the

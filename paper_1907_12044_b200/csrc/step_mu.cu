@@ -104,8 +104,11 @@ MuScratch mu_scratch(tdvp_handle *h) {
 
 void gemm1(cudaStream_t st, const ZGemm &g) { zgemm(st, g); }
 
+int mu_rhs_pipelined(tdvp_handle *h, const std::vector<c128 *> &Y, const std::vector<c128 *> &K);
+
 // K = F(Y): the TDVP-MU right-hand side.  Uses the handle's Lenv / Renv storage as scratch caches.
-int mu_rhs(tdvp_handle *h, const std::vector<c128 *> &Y, const std::vector<c128 *> &K) {
+// (One queue, everything in sequence: kept as the reference order, TDVP_MU_PIPELINE=0; mu_rhs below is what runs.)
+int mu_rhs_serial(tdvp_handle *h, const std::vector<c128 *> &Y, const std::vector<c128 *> &K) {
   cudaStream_t st = h->stream;
   const int n = h->n;
   MuScratch s = mu_scratch(h);
@@ -156,6 +159,12 @@ int mu_rhs(tdvp_handle *h, const std::vector<c128 *> &Y, const std::vector<c128 
     Cnext = (Cnext == s.C0) ? s.C1 : s.C0;
   }
   return check_cuda(h, cudaGetLastError(), "TDVP-MU derivative");
+}
+
+int mu_rhs(tdvp_handle *h, const std::vector<c128 *> &Y, const std::vector<c128 *> &K) {
+  static const bool pipeline = [] { const char *e = getenv("TDVP_MU_PIPELINE"); return !(e && e[0] == '0'); }();
+  if (pipeline && !h->cmf_streams.empty() && !h->cmf_mem.empty()) return mu_rhs_pipelined(h, Y, K);
+  return mu_rhs_serial(h, Y, K);
 }
 
 int mu_alloc(tdvp_handle *h) {
@@ -385,6 +394,41 @@ void cmf_site(tdvp_handle *h, int j, const c128 *Xj, c128 *y, double t, int n_su
   }
 }
 
+// The right-hand side with the same pipeline as the CMF step below: the bond unfoldings (Eq. 36) are a sequential
+// chain, site j's share of Eq. 37 (the H_eff apply and four GEMMs) needs only the bond to its right -- it runs on a
+// side queue as soon as that bond is done, with the per-bond U, Lambda kept in the handle (cmf_mem) instead of one
+// scratch copy the next unfolding overwrites.  Same kernels on the same data as mu_rhs_serial.
+int mu_rhs_pipelined(tdvp_handle *h, const std::vector<c128 *> &Y, const std::vector<c128 *> &K) {
+  cudaStream_t st = h->stream;
+  const int n = h->n;
+  const int nq = (int)h->cmf_streams.size();
+  cudaStream_t mf = h->cmf_hi ? h->cmf_hi : st;
+  if (mf != st) { cudaEventRecord(h->cmf_fork, st); cudaStreamWaitEvent(mf, h->cmf_fork, 0); }
+  h->stream = mf;
+  const int rc = cmf_mean_fields(h, Y, [&](int j) {
+    const int q = j % nq;
+    cudaEventRecord(h->cmf_rel[j], mf);
+    cudaStreamWaitEvent(h->cmf_streams[q], h->cmf_rel[j], 0);
+    cmf_local_rhs(h, j, Y[j], K[j], mu_carve(h, h->cmf_scratch[q]), h->cmf_streams[q], h->cmf_ws[q]);
+  });
+  h->stream = st;
+  if (mf != st) { cudaEventRecord(h->cmf_hi_done, mf); cudaStreamWaitEvent(st, h->cmf_hi_done, 0); }
+  if (rc) return rc;
+  {                                                                                      // Eq. 27
+    const int i = n - 1;
+    MuScratch s = mu_scratch(h);
+    heff_apply(st, h->M[i], h->M[i + 1], h->d[i], h->Dw[i], h->Dw[i + 1], h->Lenv[i], h->Wsp[i], Y[i], h->Renv[i],
+               s.HC, h->step_ws);
+    TDVP_LAUNCH(minus_i_diff_kernel, grid_for(site_elems(h, i)), VT, 0, st, K[i], s.HC, (const c128 *)nullptr,
+                site_elems(h, i));
+  }
+  for (int q = 0; q < nq && q < n - 1; q++) {
+    cudaEventRecord(h->cmf_join[q], h->cmf_streams[q]);
+    cudaStreamWaitEvent(st, h->cmf_join[q], 0);
+  }
+  return check_cuda(h, cudaGetLastError(), "TDVP-MU derivative");
+}
+
 // Mean fields of the state Y, then Z[i] = every local matrix of X propagated over time t with them.  The two are
 // pipelined: the backward pass of the mean-field build is a chain of bond unfoldings (one 8-SM cluster kernel at a
 // time, ~2.5 ms per bond at M = 128), and site j's local problem needs nothing left of bond j + 1 -- so site j starts
@@ -447,6 +491,10 @@ int prepare_mu(tdvp_handle *h) {
   if (!h || h->n < 1) return set_err(h, TDVP_EINVAL, "handle has no chain");
   if (h->n < 2) return set_err(h, TDVP_EINVAL, "TDVP-MU needs at least two sites");
   if (int rc = mu_alloc(h)) return rc;
+  if (!getenv("TDVP_MU_PIPELINE") || getenv("TDVP_MU_PIPELINE")[0] != '0') {   // per-bond U, Lambda and the side queues of mu_rhs
+    if (int rc = cmf_alloc(h)) return rc;
+    if (int rc = cmf_queues(h)) return rc;
+  }
   return TDVP_OK;
 }
 
