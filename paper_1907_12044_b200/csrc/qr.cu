@@ -362,6 +362,134 @@ __device__ __forceinline__ void cluster_exchange(const double *loc, int n, int n
   __syncthreads();
 }
 
+
+// ---- fast panel: the column steps' reductions predicted from ONE Gram matrix -------------------------
+// The column-by-column elimination pays one cluster-wide reduction per COLUMN (2.2 us each: 17 us per panel of
+// eight).  What a column step jj reduces -- s = sum_{i>=jj} |x_i,jj|^2 and d_c = sum_{i>=jj} conj(x_i,jj) x_i,c over
+// the CURRENT (partly eliminated) panel -- follows from the panel's Gram matrix G = P^H P and its top 8 x 8 block
+// alone: a reflector is unitary on the rows it acts on, so the sums over rows >= jj of the updated columns equal
+// those of the columns before the update, and leaving out row jj afterwards subtracts conj(R[jj][a]) R[jj][b] -- the
+// Cholesky downdate with the new row of R.  One warp runs that 8-step recurrence on 8 x 8 data (lane = column, in
+// registers, neighbours by shuffles) and writes, for every step, the reflector's scalars and its products with the
+// columns to its right (what every thread otherwise derives, redundantly, from the exchanged sums: a square root,
+// two divisions and seven complex products per thread and column, about half of a column step's 2.2 us on its
+// own); all threads then run the eight column updates back to back, without a barrier.  One cluster reduction per
+// panel instead of eight.
+// The predicted sums are differences: s loses log10(G_jj / s) digits.  A panel in which some column keeps less than
+// FAST_TAIL_MIN of its squared norm after the columns before it have been eliminated (nearly dependent or zero
+// columns: the padded / delta-seeded centres this file's header is about; typically also the first panel of a
+// centre dominated by one singular vector) is left to the exact column-by-column path, untouched.  With the
+// threshold at 1e-2 the reflectors' scalars carry at most ~100 eps: isometry and reconstruction stay at 1e-15
+// (tests/test_gpu_parity.py::test_qr_gauge).  The decision is taken from the exchanged sums, which are
+// bit-identical in every CTA.  TDVP_QR_FAST=0 switches the path off.
+constexpr double FAST_TAIL_MIN = 1e-2;
+
+// 64 Gram sums of one row's eight entries, added to acc: acc[c] += |x_c|^2, acc[8 + 2 q], acc[9 + 2 q] += conj(x_a) x_b
+// (q = index of the pair a < b in row-major order)
+__device__ __forceinline__ void gram8_accumulate(double (&acc)[64], const c128 (&x)[NB_MAX]) {
+  int q = 0;
+#pragma unroll
+  for (int a = 0; a < NB_MAX; a++) {
+    acc[a] = fma(x[a].x, x[a].x, fma(x[a].y, x[a].y, acc[a]));
+#pragma unroll
+    for (int b = a + 1; b < NB_MAX; b++) {
+      acc[8 + 2 * q] = fma(x[a].x, x[b].x, fma(x[a].y, x[b].y, acc[8 + 2 * q]));
+      acc[9 + 2 * q] = fma(x[a].x, x[b].y, fma(-x[a].y, x[b].x, acc[9 + 2 * q]));
+      q++;
+    }
+  }
+}
+__device__ __forceinline__ c128 shfl_c(c128 v, int src) {
+  return make_double2(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src));
+}
+// The reflector of a column with pivot alpha and squared norm xn2 below it (the scalars of the column step)
+__device__ __forceinline__ void house_scalars(c128 alpha, double xn2, c128 &tau, c128 &scal, double &beta) {
+  if ((xn2 == 0.0 && alpha.y == 0.0) || alpha.x * alpha.x + alpha.y * alpha.y + xn2 < TINY_NORM2) {
+    tau = make_double2(0.0, 0.0); scal = make_double2(0.0, 0.0); beta = alpha.x;
+  } else {
+    const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xn2);
+    beta = alpha.x >= 0.0 ? -nrm : nrm;
+    const double ib = 1.0 / beta;
+    tau = make_double2((beta - alpha.x) * ib, -alpha.y * ib);
+    const double dr = alpha.x - beta, di = alpha.y, idn = 1.0 / (dr * dr + di * di);
+    scal = make_double2(dr * idn, -di * idn);
+  }
+}
+// One warp, lane c < 8 = column c of the panel: g = the 64 Gram sums (layout of gram8_accumulate), B[i] = entry
+// (row i, column c) of the panel's top block.  Writes tab[jj][.] = what column step jj applies: [0], [1] scal, [2], [3]
+// tau, [4] beta, [8 + 2 c'], [9 + 2 c'] g = conj(tau) v^H y for the column c' = c - jj places to the right (the kernel
+// keeps the current column in slot 0), and returns whether every column kept FAST_TAIL_MIN of its norm (all lanes).
+__device__ __forceinline__ bool predict_panel(const double *g, c128 (&B)[NB_MAX], double (*tab)[32], int lane) {
+  constexpr int N = NB_MAX;
+  c128 G[N];                                              // G[a] = Gram entry (a, lane)
+  {
+    int q = 0;
+#pragma unroll
+    for (int a = 0; a < N; a++) {
+      G[a] = make_double2(0.0, 0.0);
+#pragma unroll
+      for (int b = a + 1; b < N; b++) {
+        if (lane < N) {
+          if (b == lane) G[a] = make_double2(g[8 + 2 * q], g[9 + 2 * q]);
+        }
+        q++;
+      }
+    }
+    q = 0;
+#pragma unroll
+    for (int a = 0; a < N; a++)
+#pragma unroll
+      for (int b = a + 1; b < N; b++) { if (a == lane) G[b] = make_double2(g[8 + 2 * q], -g[9 + 2 * q]); q++; }
+#pragma unroll
+    for (int a = 0; a < N; a++) if (a == lane) G[a] = make_double2(g[a], 0.0);
+  }
+  const double g0 = lane < N ? g[lane] : 0.0;
+  if (lane >= N) {
+#pragma unroll
+    for (int i = 0; i < N; i++) B[i] = make_double2(0.0, 0.0);
+  }
+  bool ok = true;
+#pragma unroll
+  for (int jj = 0; jj < N; jj++) {
+    const c128 alpha = shfl_c(B[jj], jj);
+    const double s = __shfl_sync(0xffffffffu, G[jj].x, jj);
+    const double g0j = __shfl_sync(0xffffffffu, g0, jj);
+    if (!(s >= FAST_TAIL_MIN * g0j) || !(g0j > 0.0) || !(g0j < 1e300)) ok = false;
+    double xn2 = s - (alpha.x * alpha.x + alpha.y * alpha.y);
+    if (xn2 < 0.0) xn2 = 0.0;
+    c128 tau, scal;
+    double beta;
+    house_scalars(alpha, xn2, tau, scal, beta);
+    const c128 dc = G[jj], yj = B[jj];
+    c128 gg = make_double2(0.0, 0.0);
+    if (lane > jj && lane < N) {
+      const c128 t1 = cmul(cconj(alpha), yj);
+      const c128 t2 = cmul(cconj(scal), make_double2(dc.x - t1.x, dc.y - t1.y));
+      gg = cmul(cconj(tau), make_double2(yj.x + t2.x, yj.y + t2.y));
+      const int cp = lane - jj;
+      tab[jj][8 + 2 * cp] = gg.x; tab[jj][9 + 2 * cp] = gg.y;
+    } else if (lane == jj) {
+      tab[jj][0] = scal.x; tab[jj][1] = scal.y; tab[jj][2] = tau.x; tab[jj][3] = tau.y; tab[jj][4] = beta;
+    } else if (lane < jj) {                                // slots of finished reflectors at the back: no column there
+      const int cp = N - jj + lane;
+      tab[jj][8 + 2 * cp] = 0.0; tab[jj][9 + 2 * cp] = 0.0;
+    }
+    // row jj of R as this step leaves it (this lane's entry), the top block's rows below it, the Gram downdate
+    const c128 rrow = lane == jj ? make_double2(beta, 0.0) : make_double2(yj.x - gg.x, yj.y - gg.y);
+#pragma unroll
+    for (int i = jj + 1; i < N; i++) {
+      const c128 v = cmul(shfl_c(B[i], jj), scal);
+      if (lane > jj) { const c128 u = cmul(gg, v); B[i].x -= u.x; B[i].y -= u.y; }
+    }
+#pragma unroll
+    for (int a = jj + 1; a < N; a++) {
+      const c128 ra = shfl_c(rrow, a);
+      if (lane > jj) { const c128 u = cmul(cconj(ra), rrow); G[a].x -= u.x; G[a].y -= u.y; }
+    }
+  }
+  return ok;
+}
+
 // The WHOLE factorisation in one kernel, by one cluster: for every panel (1) the column-by-column
 // elimination above with the panel's rows spread over the cluster, (2) the compact-WY factor T, built by
 // every CTA for itself from the exchanged Gram sums, (3) the trailing update X[:, c] <- (I - V T^H V^H) X[:, c]
@@ -376,7 +504,8 @@ __device__ __forceinline__ void cluster_exchange(const double *loc, int n, int n
 template <int RA, int NB>
 __global__ void __cluster_dims__(QC, 1, 1) __launch_bounds__(QT, 1)
 qr_factor_cluster_kernel(c128 *X, int rows, int cols, c128 *Rm, c128 *Tm /*[npanels][NB_MAX][NB_MAX]*/,
-                         const int *gate /*DEVICE, nullable: run only if non-zero (written by an earlier kernel of the stream)*/) {
+                         const int *gate /*DEVICE, nullable: run only if non-zero (written by an earlier kernel of the stream)*/,
+                         int fast /*try the one-reduction panel (predict_panel) first*/) {
   if (gate && __ldcg(gate) == 0) return;                   // every CTA of the cluster reads the same value
   constexpr int RPT = (RA + QC - 1) / QC;
   constexpr int NGRAM = NB * (NB - 1);                   // re / im of the strictly upper Gram entries (<= 56)
@@ -390,6 +519,8 @@ qr_factor_cluster_kernel(c128 *X, int rows, int cols, c128 *Rm, c128 *Tm /*[npan
   __shared__ c128 Ts[NB_MAX * NB_MAX];
   __shared__ c128 Tl[NB_MAX * NB_MAX];
   __shared__ c128 Gs[NB_MAX * NB_MAX];
+  __shared__ double ftab[NB_MAX][32];                     // fast panel: the predicted sums of every column step
+  __shared__ int fOk;
   const unsigned me = cluster_ctarank();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int gthread = (int)me * QT + tid;
@@ -415,7 +546,46 @@ qr_factor_cluster_kernel(c128 *X, int rows, int cols, c128 *Rm, c128 *Tm /*[npan
     for (int i = j0 + 1 + gthread; i < cols; i += QC * QT)    // zeros below the diagonal of R
       for (int c = 0; c < w; c++)
         if (i > j0 + c) Rm[(long long)i * cols + j0 + c] = make_double2(0.0, 0.0);
+    // ---- fast panel: one Gram reduction, then the column steps' sums by recurrence (predict_panel) ----
+    bool predicted = false;
+    if (fast && RPT == 1 && NB == NB_MAX && w == NB) {
+      c128 ptop[NB_MAX];                                    // top block, lane = column (warp 0 of every CTA)
+      if (tid < NB_MAX) {
+#pragma unroll
+        for (int i = 0; i < NB_MAX; i++) ptop[i] = __ldcg(X + (long long)(j0 + tid) * rows + j0 + i);
+      }
+      double acc[64];
+#pragma unroll
+      for (int t = 0; t < 64; t++) acc[t] = 0.0;
+      if (row_of(0) < len) {
+        c128 xr[NB_MAX];
+#pragma unroll
+        for (int c = 0; c < NB_MAX; c++) xr[c] = x[0][c < NB ? c : 0];
+        gram8_accumulate(acc, xr);
+      }
+#pragma unroll
+      for (int blk = 0; blk < 4; blk++) {
+        double v16[16];
+#pragma unroll
+        for (int q = 0; q < 16; q++) v16[q] = acc[blk * 16 + q];
+        int idx;
+        const double part = warp_reduce16(v16, lane, idx);
+        if ((lane & 1) == 0) wpart[warp][blk * 16 + idx] = part;
+      }
+      __syncthreads();
+      if (tid < 64) { double a = 0.0; for (int k = 0; k < QW; k++) a += wpart[k][tid]; loc[tid] = a; }
+      __syncthreads();
+      cluster_exchange(loc, 64, 64, 0u, exch[par], tot, me);
+      par ^= 1u;
+      if (warp == 0) { const bool ok = predict_panel(tot, ptop, ftab, lane); if (lane == 0) fOk = ok ? 1 : 0; }
+      __syncthreads();
+      predicted = fOk != 0;                                 // (same sums, hence the same decision, in every CTA)
+    }
     for (int jj = 0; jj < w; jj++) {
+      const double *tt = tot;                               // where the step's sums come from
+      if (predicted) {
+        tt = ftab[jj];
+      } else {
       double red[16];
 #pragma unroll
       for (int q = 0; q < 16; q++) red[q] = 0.0;
@@ -445,20 +615,16 @@ qr_factor_cluster_kernel(c128 *X, int rows, int cols, c128 *Rm, c128 *Tm /*[npan
       __syncthreads();
       cluster_exchange(loc, 16 + 2 * NB, 16, 0u, exch[par], tot, me);
       par ^= 1u;
-      const c128 alpha = make_double2(tot[16], tot[17]);
-      double xn2 = tot[0] - (alpha.x * alpha.x + alpha.y * alpha.y);
-      if (xn2 < 0.0) xn2 = 0.0;
-      c128 tau, scal;
+      }
+      c128 tau, scal, alpha = make_double2(0.0, 0.0);
       double beta;
-      if ((xn2 == 0.0 && alpha.y == 0.0) || alpha.x * alpha.x + alpha.y * alpha.y + xn2 < TINY_NORM2) {
-        tau = make_double2(0.0, 0.0); scal = make_double2(0.0, 0.0); beta = alpha.x;
+      if (predicted) {
+        scal = make_double2(tt[0], tt[1]); tau = make_double2(tt[2], tt[3]); beta = tt[4];
       } else {
-        const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xn2);
-        beta = alpha.x >= 0.0 ? -nrm : nrm;
-        const double ib = 1.0 / beta;
-        tau = make_double2((beta - alpha.x) * ib, -alpha.y * ib);
-        const double dr = alpha.x - beta, di = alpha.y, idn = 1.0 / (dr * dr + di * di);
-        scal = make_double2(dr * idn, -di * idn);
+        alpha = make_double2(tt[16], tt[17]);
+        double xn2 = tt[0] - (alpha.x * alpha.x + alpha.y * alpha.y);
+        if (xn2 < 0.0) xn2 = 0.0;
+        house_scalars(alpha, xn2, tau, scal, beta);
       }
       if (tid == 0) {
         tau_s[jj] = tau;                                    // every CTA keeps the taus: it builds T itself
@@ -467,11 +633,15 @@ qr_factor_cluster_kernel(c128 *X, int rows, int cols, c128 *Rm, c128 *Tm /*[npan
       c128 g[NB];                                            // conj(tau) * (v^H y_c)
 #pragma unroll
       for (int c = 1; c < NB; c++) {
-        const c128 dc = make_double2(tot[1 + 2 * (c - 1)], tot[2 + 2 * (c - 1)]);
-        const c128 yj = make_double2(tot[16 + 2 * c], tot[17 + 2 * c]);
-        const c128 t1 = cmul(cconj(alpha), yj);
-        const c128 t2 = cmul(cconj(scal), make_double2(dc.x - t1.x, dc.y - t1.y));
-        g[c] = cmul(cconj(tau), make_double2(yj.x + t2.x, yj.y + t2.y));
+        if (predicted) {
+          g[c] = make_double2(tt[8 + 2 * c], tt[9 + 2 * c]);
+        } else {
+          const c128 dc = make_double2(tt[1 + 2 * (c - 1)], tt[2 + 2 * (c - 1)]);
+          const c128 yj = make_double2(tt[16 + 2 * c], tt[17 + 2 * c]);
+          const c128 t1 = cmul(cconj(alpha), yj);
+          const c128 t2 = cmul(cconj(scal), make_double2(dc.x - t1.x, dc.y - t1.y));
+          g[c] = cmul(cconj(tau), make_double2(yj.x + t2.x, yj.y + t2.y));
+        }
         if (c >= NB - jj) g[c] = make_double2(0.0, 0.0);     // slots at the back hold finished reflectors: not columns
       }
       c128 *Xc = X + (long long)(j0 + jj) * rows + j0;
@@ -1002,6 +1172,7 @@ int panel_width(int rows) {
 constexpr int QF_SMEM = 40 * QT * 16;   // RA * NB = 40 reflector entries per thread in every mode
 int g_qr_cluster = 1;            // TDVP_QR_CLUSTER=0: one launch per panel and per trailing update (diagnostic switch)
 int g_qr_cluster_min = 0;        // matrices with more rows than this use the cluster kernel (TDVP_QR_CLUSTER_MIN)
+int g_qr_fast = 1;               // TDVP_QR_FAST=0: every panel column by column with one cluster reduction per column (diagnostic switch)
 
 void qr_configure() {
   cudaFuncSetAttribute(qr_factor_cluster_kernel<5, 8>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
@@ -1020,6 +1191,7 @@ void qr_configure() {
   }
   if (const char *e = getenv("TDVP_QR_CLUSTER")) g_qr_cluster = g_qr_cluster && e[0] != '0';
   if (const char *e = getenv("TDVP_QR_CLUSTER_MIN")) g_qr_cluster_min = atoi(e);
+  if (const char *e = getenv("TDVP_QR_FAST")) g_qr_fast = e[0] != '0';
   cudaFuncSetAttribute(qr_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024 + 1024);
 }
 
@@ -1065,7 +1237,7 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
     // (B200, 1280 x 128): 580 us against 698 us with one launch per panel and per update; at 2560 x 256 the
     // 16 SMs of the cluster are too few for the trailing updates (2170 against 1924 us), so taller matrices
     // keep the launch-per-panel path below.
-    TDVP_LAUNCH((qr_factor_cluster_kernel<5, 8>), QC, QT, QF_SMEM, st, X, rows, cols, Rm, Tm, gate);
+    TDVP_LAUNCH((qr_factor_cluster_kernel<5, 8>), QC, QT, QF_SMEM, st, X, rows, cols, Rm, Tm, gate, g_qr_fast);
   } else
   for (int pz = 0; pz < npanels; pz++) {
     int j0 = pz * nb, w = cols - j0 < nb ? cols - j0 : nb;
