@@ -246,23 +246,72 @@ __device__ __forceinline__ int jacobi_pair_smem(c128 *xp, c128 *xq, c128 *jp, c1
   return result;
 }
 
+// The same rotation with the first column of the pair (X and J) held in REGISTERS by the warp across the inner
+// rounds of a block pair -- a warp keeps its column of the first block and meets a different column of the second
+// block every round -- so that a round moves one column through shared memory, not two: the inner rounds of a
+// block pair are bound by shared-memory traffic (8 warps x 8 KB each way per round).
 template <int NPL>
-__global__ void __cluster_dims__(JC, 1, 1) __launch_bounds__(JW * 32)
+__device__ __forceinline__ int jacobi_pair_preg(c128 (&xu)[NPL], c128 (&ju)[NPL], c128 *xq, c128 *jq, int n, int lane, double tol2, double thr) {
+  c128 xv[NPL], jv[NPL];
+  double a = 0.0, b = 0.0, cr = 0.0, ci = 0.0;
+#pragma unroll
+  for (int r = 0; r < NPL; r++) {
+    const int i = lane + 32 * r;
+    const bool ok = i < n;
+    xv[r] = ok ? xq[i] : make_double2(0.0, 0.0);
+    const c128 u = xu[r], v = xv[r];
+    a += u.x * u.x + u.y * u.y;
+    b += v.x * v.x + v.y * v.y;
+    cr += u.x * v.x + u.y * v.y;                                 // conj(u) * v
+    ci += u.x * v.y - u.y * v.x;
+  }
+  a = wsum(a); b = wsum(b); cr = wsum(cr); ci = wsum(ci);
+  const double c2 = cr * cr + ci * ci;
+  if (!(c2 > tol2 * a * b) || c2 == 0.0 || a < thr || b < thr) return 0;
+  const int result = c2 > COARSE_TOL2 * a * b ? 3 : 1;
+#pragma unroll
+  for (int r = 0; r < NPL; r++) { const int i = lane + 32 * r; jv[r] = i < n ? jq[i] : make_double2(0.0, 0.0); }
+  const double icabs = rsqrt(c2);
+  const double er = cr * icabs, ei = -ci * icabs;                // e^{-i phi}
+  const double zeta = 0.5 * (b - a) * icabs;
+  const double t = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+  const double cs = rsqrt(1.0 + t * t), sn = cs * t;
+  auto rot = [&](c128 u, c128 v, c128 &o1, c128 &o2) {
+    const c128 y = make_double2(er * v.x - ei * v.y, er * v.y + ei * v.x);
+    o1 = make_double2(cs * u.x - sn * y.x, cs * u.y - sn * y.y);
+    o2 = make_double2(sn * u.x + cs * y.x, sn * u.y + cs * y.y);
+  };
+#pragma unroll
+  for (int r = 0; r < NPL; r++) {
+    const int i = lane + 32 * r;
+    c128 o1, o2;
+    rot(xu[r], xv[r], o1, o2); xu[r] = o1; if (i < n) xq[i] = o2;
+    rot(ju[r], jv[r], o1, o2); ju[r] = o1; if (i < n) jq[i] = o2;
+  }
+  return result;
+}
+
+// Geometry: JB_ column blocks, JC_ = JB_ / 2 CTAs (one block pair each), JW_ warps per CTA (>= columns per block).
+// (16, 8, 8) is what runs.  (8, 4, 16) -- 8 phases of 16 inner rounds per sweep instead of 16 of 8, half the block
+// exchanges and cluster barriers -- measured SLOWER (3.04 against 2.42 ms per 128 x 128 bond): a sweep's time is in its
+// 127 inner rounds, which are bound by shared-memory traffic, and 16 warps per CTA double that traffic per round.
+template <int NPL, int JB_, int JC_, int JW_>
+__global__ void __cluster_dims__(JC_, 1, 1) __launch_bounds__(JW_ * 32)
 svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/, int max_sweeps, int *status) {
   cg::cluster_group cluster = cg::this_cluster();
   extern __shared__ __align__(16) unsigned char jsm[];
-  const int bw = (n + JB - 1) / JB;                       // columns per block (<= 8 for n <= 128)
+  const int bw = (n + JB_ - 1) / JB_;                     // columns per block (<= JW_)
   c128 *Xs = reinterpret_cast<c128 *>(jsm);               // [2 bw][n]
   c128 *Js = Xs + (size_t)2 * bw * n;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int cta = blockIdx.x;                             // one cluster: rank == blockIdx.x
   const double tol = 2.220446049250313e-16 * sqrt((double)n);
   const double tol2 = tol * tol;
-  __shared__ double s_cmax[JW];
-  const double thr = fmax(TINY_COL2, REL_TINY2 * max_col_norm2<JW>(Xt, n, s_cmax));
+  __shared__ double s_cmax[JW_];
+  const double thr = fmax(TINY_COL2, REL_TINY2 * max_col_norm2<JW_>(Xt, n, s_cmax));
   cluster.sync();                                       // everybody has read the initial columns
   auto load_blocks = [&](int bp, int bq) {
-    for (int e = tid; e < 2 * bw * n; e += JW * 32) {
+    for (int e = tid; e < 2 * bw * n; e += JW_ * 32) {
       const int lc = e / n, i = e - lc * n;
       const int g = (lc < bw ? bp * bw + lc : bq * bw + (lc - bw));
       if (g < n) { Xs[e] = __ldcg(Xt + (size_t)g * n + i); Js[e] = __ldcg(Jt + (size_t)g * n + i); }
@@ -271,7 +320,7 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
   };
   auto store_blocks = [&](int bp, int bq) {
     __syncthreads();
-    for (int e = tid; e < 2 * bw * n; e += JW * 32) {
+    for (int e = tid; e < 2 * bw * n; e += JW_ * 32) {
       const int lc = e / n, i = e - lc * n;
       const int g = (lc < bw ? bp * bw + lc : bq * bw + (lc - bw));
       if (g < n) { Xt[(size_t)g * n + i] = Xs[e]; Jt[(size_t)g * n + i] = Js[e]; }
@@ -281,12 +330,12 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
   int sweep = 0;
   for (; sweep < max_sweeps; sweep++) {
     int any = 0;
-    // (i) pairs inside blocks 2 cta and 2 cta + 1: warps 0-3 take the first block, 4-7 the second
+    // (i) pairs inside blocks 2 cta and 2 cta + 1: the first half of the warps takes the first block, the second half the other
     {
       const int b0 = 2 * cta, b1 = 2 * cta + 1;
       load_blocks(b0, b1);
       for (int round = 0; round < bwp - 1; round++) {
-        const int half = warp >> 2, k = warp & 3;
+        const int half = warp / (JW_ / 2), k = warp % (JW_ / 2);
         if (k < bwp / 2) {
           int p, q;
           if (k == 0) { p = round; q = bwp - 1; }
@@ -304,25 +353,42 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
       cluster.sync();
     }
     // (ii) tournament of the blocks: CTA k plays block pair k of the round
-    for (int round = 0; round < JB - 1; round++) {
+    for (int round = 0; round < JB_ - 1; round++) {
       int bp, bq;
-      if (cta == 0) { bp = round; bq = JB - 1; }
-      else { bp = (round + cta) % (JB - 1); bq = (round - cta + (JB - 1)) % (JB - 1); }
+      if (cta == 0) { bp = round; bq = JB_ - 1; }
+      else { bp = (round + cta) % (JB_ - 1); bq = (round - cta + (JB_ - 1)) % (JB_ - 1); }
       if (bp > bq) { const int t = bp; bp = bq; bq = t; }
       if (bq * bw < n) {                                   // both blocks hold real columns
         load_blocks(bp, bq);
+        const bool have_p = warp < bw && bp * bw + warp < n;
+        c128 xu[NPL], ju[NPL];                              // this warp's column of block bp, in registers for all bw rounds
+        if (have_p) {
+#pragma unroll
+          for (int q = 0; q < NPL; q++) {
+            const int i = lane + 32 * q;
+            xu[q] = i < n ? Xs[(size_t)warp * n + i] : make_double2(0.0, 0.0);
+            ju[q] = i < n ? Js[(size_t)warp * n + i] : make_double2(0.0, 0.0);
+          }
+        }
         for (int r = 0; r < bw; r++) {
-          if (warp < bw) {
-            const int lp = warp, lq = bw + (warp + r) % bw;
-            if (bp * bw + lp < n && bq * bw + (lq - bw) < n)
-              any |= jacobi_pair_smem<NPL>(Xs + (size_t)lp * n, Xs + (size_t)lq * n, Js + (size_t)lp * n, Js + (size_t)lq * n, n, lane, tol2, thr);
+          if (have_p) {
+            const int lq = bw + (warp + r) % bw;
+            if (bq * bw + (lq - bw) < n)
+              any |= jacobi_pair_preg<NPL>(xu, ju, Xs + (size_t)lq * n, Js + (size_t)lq * n, n, lane, tol2, thr);
           }
           __syncthreads();
         }
+        if (have_p) {
+#pragma unroll
+          for (int q = 0; q < NPL; q++) {
+            const int i = lane + 32 * q;
+            if (i < n) { Xs[(size_t)warp * n + i] = xu[q]; Js[(size_t)warp * n + i] = ju[q]; }
+          }
+        }
         store_blocks(bp, bq);
       }
-      if (round == JB - 2 && any && lane == 0) flags[sweep] = 1;   // benign race: every writer stores 1
-      if (round == JB - 2 && (any & 2) && lane == 0) flags[64 + sweep] = 1;
+      if (round == JB_ - 2 && any && lane == 0) flags[sweep] = 1;   // benign race: every writer stores 1
+      if (round == JB_ - 2 && (any & 2) && lane == 0) flags[64 + sweep] = 1;
       cluster.sync();
     }
     if (__ldcg(flags + sweep) == 0) break;                          // nobody rotated in this sweep
@@ -434,9 +500,10 @@ __global__ void svd_finish_kernel(const c128 *Qp, const c128 *Dp, const c128 *Jt
 
 void svd_configure() {
   const int bytes = 4 * 8 * 128 * (int)sizeof(c128);     // X and J of two blocks at n = 128
-  cudaFuncSetAttribute(svd_jacobi_block_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  cudaFuncSetAttribute(svd_jacobi_block_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  cudaFuncSetAttribute(svd_jacobi_block_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  cudaFuncSetAttribute(svd_jacobi_block_kernel<1, JB, JC, JW>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  cudaFuncSetAttribute(svd_jacobi_block_kernel<2, JB, JC, JW>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  cudaFuncSetAttribute(svd_jacobi_block_kernel<4, JB, JC, JW>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+
 }
 
 size_t svd_ws_bytes(int Ml, int d, int Mr) {
@@ -471,9 +538,9 @@ void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, do
   cudaMemsetAsync(flags, 0, 128 * sizeof(int), st);
   const size_t bsm = (size_t)4 * ((n + JB - 1) / JB) * n * sizeof(c128);      // X and J of two blocks
   if (n <= 16) TDVP_LAUNCH(svd_jacobi_kernel<1>, JC, JW * 32, 0, st, Xt, Jt, n, flags, max_sweeps, status);
-  else if (n <= 32) TDVP_LAUNCH(svd_jacobi_block_kernel<1>, JC, JW * 32, bsm, st, Xt, Jt, n, flags, max_sweeps, status);
-  else if (n <= 64) TDVP_LAUNCH(svd_jacobi_block_kernel<2>, JC, JW * 32, bsm, st, Xt, Jt, n, flags, max_sweeps, status);
-  else if (n <= 128) TDVP_LAUNCH(svd_jacobi_block_kernel<4>, JC, JW * 32, bsm, st, Xt, Jt, n, flags, max_sweeps, status);
+  else if (n <= 32) TDVP_LAUNCH((svd_jacobi_block_kernel<1, JB, JC, JW>), JC, JW * 32, bsm, st, Xt, Jt, n, flags, max_sweeps, status);
+  else if (n <= 64) TDVP_LAUNCH((svd_jacobi_block_kernel<2, JB, JC, JW>), JC, JW * 32, bsm, st, Xt, Jt, n, flags, max_sweeps, status);
+  else if (n <= 128) TDVP_LAUNCH((svd_jacobi_block_kernel<4, JB, JC, JW>), JC, JW * 32, bsm, st, Xt, Jt, n, flags, max_sweeps, status);
   else TDVP_LAUNCH(svd_jacobi_kernel<0>, JC, JW * 32, 0, st, Xt, Jt, n, flags, max_sweeps, status);
   // X = U' R'  <=>  Xt = R'^T U'^T: "side 1" factorisation of the n x n matrix Xt (d = 1)
   c128 *Xs = D;                                                   // D is no longer needed
