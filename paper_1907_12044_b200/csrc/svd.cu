@@ -183,6 +183,10 @@ svd_jacobi_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zeroed*/,
     }
     if (np < 2) break;
     if (__ldcg(flags + sweep) == 0) break;                          // nobody rotated in this sweep
+    // ... or every pair it met was orthogonal to 1e-10 already (no "coarse" pair): a rotation by an angle <= 1e-10
+    // disturbs the other products of its two columns by <= 1e-10 * 1e-10 each, so after this sweep every cosine is
+    // below ~2 n 1e-20 << sqrt(n) eps and the next sweep would only confirm it (a sweep is ~0.2 ms at n = 128)
+    if (__ldcg(flags + 64 + sweep) == 0) break;
   }
   // every sweep allowed still rotated, and the last one still saw a pair far from orthogonal (rotations that
   // hover at the round-off threshold of sqrt(n) eps are convergence): tell the host
@@ -392,6 +396,10 @@ svd_jacobi_block_kernel(c128 *Xt, c128 *Jt, int n, int *flags /*[MAX_SWEEPS] zer
       cluster.sync();
     }
     if (__ldcg(flags + sweep) == 0) break;                          // nobody rotated in this sweep
+    // ... or every pair it met was orthogonal to 1e-10 already (no "coarse" pair): a rotation by an angle <= 1e-10
+    // disturbs the other products of its two columns by <= 1e-10 * 1e-10 each, so after this sweep every cosine is
+    // below ~2 n 1e-20 << sqrt(n) eps and the next sweep would only confirm it (a sweep is ~0.2 ms at n = 128)
+    if (__ldcg(flags + 64 + sweep) == 0) break;
   }
   if (sweep == max_sweeps && cta == 0 && tid == 0) {
     flags[FLAG_FORCE_QR] = 1;
