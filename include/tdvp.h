@@ -327,6 +327,8 @@ long long tdvp_launch_count(void);
                               on its side queue as soon as the bond to its right is unfolded), read once;
      TDVP_MU_PIPELINE=0       the same switch for the right-hand side of tdvp_step_mu / tdvp_mu_derivative, read once;
      TDVP_CMF_PRIORITY=0      no separate highest-priority queue for the chain of bond unfoldings, read once;
+     TDVP_CMF_SPLIT_SVD=0     Vh of a bond and the right block built from it stay on the queue of the unfolding chain
+                              (default: on a queue of their own, one bond behind the chain), read once;
      TDVP_CMF_SPARE_SMS=n     SMs the GEMMs of the side queues leave out of their grids, for the cluster kernels of
                               the unfolding chain that run beside them (default 24; 0 = none), read once;
      TDVP_SVD_ALWAYS_QR=1     a bond SVD always runs its final Householder step (default: only when the Jacobi

@@ -117,6 +117,9 @@ static void free_chain(tdvp_handle *h) {
   for (auto q : h->cmf_streams) { cudaStreamSynchronize(q); zgemm_release_stream(q); cudaStreamDestroy(q); }
   for (auto e : h->cmf_join) cudaEventDestroy(e);
   for (auto e : h->cmf_rel) cudaEventDestroy(e);
+  for (auto e : h->cmf_fac) cudaEventDestroy(e);
+  if (h->cmf_env) { cudaStreamSynchronize(h->cmf_env); zgemm_release_stream(h->cmf_env); cudaStreamDestroy(h->cmf_env); }
+  fr(h->cmf_env_ws); fr(h->cmf_svd_ws[0]); fr(h->cmf_svd_ws[1]);
   if (h->cmf_fork) cudaEventDestroy(h->cmf_fork);
   if (h->cmf_hi) { cudaStreamSynchronize(h->cmf_hi); zgemm_release_stream(h->cmf_hi); cudaStreamDestroy(h->cmf_hi); }
   if (h->cmf_hi_done) cudaEventDestroy(h->cmf_hi_done);

@@ -198,6 +198,9 @@ size_t qr_ws_bytes(int rows, int cols);
 // on the device whether the factorisation is needed at all (svd.cu)
 void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c128 *Q, c128 *D,
               void *ws, const int *gate = nullptr);
+// its two halves on the same workspace: factor (writes D, leaves the reflectors in ws), then form Q from them
+void qr_factor(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c128 *D, void *ws, const int *gate = nullptr);
+void qr_form_q(cudaStream_t st, int side, int Ml, int d, int Mr, c128 *Q, void *ws, const int *gate = nullptr);
 
 // ---------------------------------------------------------------------------------------------
 // svd.cu : matrix unfolding C[Ml, d*Mr] = U diag(lam) Vh (Eq. 36) on the device, Ml <= d*Mr.
@@ -207,6 +210,9 @@ size_t svd_ws_bytes(int Ml, int d, int Mr);
 constexpr int TDVP_STATUS_SVD_UNCONVERGED = 1;
 void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, double *lam, c128 *Vh, void *ws,
               int *status);
+// its two halves on the same workspace (svd.cu): U and lam first, Vh later -- possibly on another queue
+void svd_bond_factor(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, double *lam, void *ws, int *status);
+void svd_bond_vh(cudaStream_t st, int Ml, int d, int Mr, c128 *Vh, void *ws);
 
 // ---------------------------------------------------------------------------------------------
 // small vector kernels shared by the drivers (vecops.cu)

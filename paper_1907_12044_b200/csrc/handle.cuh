@@ -51,6 +51,9 @@ struct tdvp_handle {
   std::vector<void *> cmf_ws, cmf_scratch;
   cudaEvent_t cmf_fork = nullptr, cmf_hi_done = nullptr;
   cudaStream_t cmf_hi = nullptr;   // highest-priority queue of the CMF mean-field (bond unfolding) chain
+  cudaStream_t cmf_env = nullptr;  // queue of what hangs off that chain without being on it: Vh of a bond and the R block built from it
+  void *cmf_env_ws = nullptr, *cmf_svd_ws[2] = {nullptr, nullptr};   // its workspace; unfolding workspaces of even / odd bonds
+  std::vector<cudaEvent_t> cmf_fac;   // bond i: U, Lambda are ready (the first half of its unfolding is done)
   StepGraph ps_graph, mu_graph, ps2_graph, cmf_graph;
   void *ps2_ws = nullptr;          // two-site TDVP-PS workspace (allocated by the first tdvp_step_ps2)
   size_t ps2_ws_bytes = 0;

@@ -1214,7 +1214,10 @@ size_t qr_ws_bytes(int rows, int cols) {
   return 2 * mat + up256((size_t)cols * cols * 16) + up256(npanels * NB_MAX * NB_MAX * 16) + 512;
 }
 
-void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c128 *Q, c128 *D, void *ws, const int *gate) {
+// The two halves of a gauge move on one workspace: qr_factor leaves the reflectors (X), their T factors and R in `ws`
+// and writes D; qr_form_q forms Q from them.  A caller that needs D first (the chain of bond unfoldings: svd.cu) can
+// run the second half later, on another queue, as long as nothing else uses `ws` in between.
+void qr_factor(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c128 *D, void *ws, const int *gate) {
   const int rows = side == 0 ? Ml * d : d * Mr;
   const int cols = side == 0 ? Mr : Ml;
   int nb = 1;
@@ -1229,6 +1232,7 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
   const long long n = (long long)rows * cols;
   const int gcopy = (int)((n + 255) / 256 > 592 ? 592 : (n + 255) / 256);
   dim3 tb(32, 8), tg((cols + 31) / 32, (rows + 31) / 32);
+  (void)Y;
   if (side == 0) TDVP_LAUNCH(transpose_in_kernel, tg, tb, 0, st, C, X, rows, cols);
   else TDVP_LAUNCH(copy_kernel, gcopy, 256, 0, st, X, C, n);
   const int npanels = (cols + nb - 1) / nb;
@@ -1254,6 +1258,26 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
     int c_begin = j0 + w;
     launch_apply(st, mode, X, X, rows, j0, w, Tp, 1, c_begin, cols);
   }
+  TDVP_LAUNCH(store_d_kernel, (cols * cols + 255) / 256 > 296 ? 296 : (cols * cols + 255) / 256, 256, 0, st, Rm, D, cols, side);
+}
+
+void qr_form_q(cudaStream_t st, int side, int Ml, int d, int Mr, c128 *Q, void *ws, const int *gate) {
+  const int rows = side == 0 ? Ml * d : d * Mr;
+  const int cols = side == 0 ? Mr : Ml;
+  int nb = 1;
+  const int mode = panel_mode(rows, &nb);
+  ProfScope ps(st, PH_QR);
+  char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
+  size_t mat = up256((size_t)rows * cols * 16);
+  c128 *X = reinterpret_cast<c128 *>(p); p += mat;
+  c128 *Y = reinterpret_cast<c128 *>(p); p += mat;
+  c128 *Rm = reinterpret_cast<c128 *>(p); p += up256((size_t)cols * cols * 16);
+  c128 *Tm = reinterpret_cast<c128 *>(p);
+  const long long n = (long long)rows * cols;
+  const int gcopy = (int)((n + 255) / 256 > 592 ? 592 : (n + 255) / 256);
+  dim3 tb(32, 8), tg((cols + 31) / 32, (rows + 31) / 32);
+  (void)Rm;
+  const int npanels = (cols + nb - 1) / nb;
   if (mode == 1) TDVP_LAUNCH((qr_apply1_kernel<256, 5, 8, true>), cols, 256, 0, st, X, Y, rows, 0, 0, Tm, nb, cols, 0, gate);
   else if (mode == 2) TDVP_LAUNCH((qr_apply1_kernel<256, 10, 4, true>), cols, 256, 0, st, X, Y, rows, 0, 0, Tm, nb, cols, 0);
   else if (mode == 3) TDVP_LAUNCH((qr_apply1_kernel<256, 20, 2, true>), cols, 256, 0, st, X, Y, rows, 0, 0, Tm, nb, cols, 0);
@@ -1266,7 +1290,11 @@ void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c
   }
   if (side == 0) TDVP_LAUNCH(transpose_out_kernel, tg, tb, 0, st, Y, Q, rows, cols);
   else TDVP_LAUNCH(copy_kernel, gcopy, 256, 0, st, Q, Y, n);
-  TDVP_LAUNCH(store_d_kernel, (cols * cols + 255) / 256 > 296 ? 296 : (cols * cols + 255) / 256, 256, 0, st, Rm, D, cols, side);
+}
+
+void qr_gauge(cudaStream_t st, int side, int Ml, int d, int Mr, const c128 *C, c128 *Q, c128 *D, void *ws, const int *gate) {
+  qr_factor(st, side, Ml, d, Mr, C, D, ws, gate);
+  qr_form_q(st, side, Ml, d, Mr, Q, ws, gate);
 }
 
 // ---------------------------------------------------------------------------------------------

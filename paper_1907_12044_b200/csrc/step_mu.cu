@@ -274,17 +274,30 @@ int cmf_mean_fields(tdvp_handle *h, const std::vector<c128 *> &Y, const std::fun
   for (int i = 0; i < n - 1; i++)                                                        // "Get Env"
     env_update(st, 0, h->M[i], h->M[i + 1], h->d[i], h->Dw[i], h->Dw[i + 1], h->Lenv[i], h->Wsp[i], Y[i],
                h->Lenv[i + 1], ws);
+  // The backward pass.  On the chain (queue st): R factor of the centre, Jacobi iteration, U Lambda, the next centre.
+  // Off the chain, one bond behind it on the queue cmf_env when the handle has one: Q and Vh of the bond, the R block
+  // built from Vh, and with that the release of site i - 1 (event cmf_rel[i - 1]).  The unfolding workspaces alternate
+  // with the bond's parity: bond i's first half waits until bond i + 2's second half has let go of the workspace.
+  cudaStream_t eq = (h->cmf_env && released) ? h->cmf_env : st;
+  const bool split = eq != st;
   const c128 *C = Y[n - 1];
   c128 *Cnext = s.C0;
   for (int i = n - 1; i >= 1; i--) {
     const int Ml = h->M[i], Mr = h->M[i + 1], d = h->d[i];
     c128 *U = reinterpret_cast<c128 *>(h->cmf_mem[3 * i]), *UL = reinterpret_cast<c128 *>(h->cmf_mem[3 * i + 1]);
     double *lam = reinterpret_cast<double *>(h->cmf_mem[3 * i + 2]);
-    svd_bond(st, Ml, d, Mr, C, U, lam, s.Vh, ws, h->status_dev);                                        // Eq. 36
-    env_update(st, 1, Ml, Mr, d, h->Dw[i], h->Dw[i + 1], h->Renv[i], h->Wsp[i], s.Vh, h->Renv[i - 1], ws);
+    void *sws = split ? h->cmf_svd_ws[i & 1] : ws;
+    if (split && i + 2 <= n - 1) cudaStreamWaitEvent(st, h->cmf_rel[i + 1], 0);
+    svd_bond_factor(st, Ml, d, Mr, C, U, lam, sws, h->status_dev);                                     // Eq. 36
     vec_copy(st, UL, U, (long long)Ml * Ml);
     TDVP_LAUNCH(scale_cols_kernel, grid_for((long long)Ml * Ml), VT, 0, st, UL, (long long)Ml, Ml, lam, 0, 0.0);
-    if (released) released(i - 1);
+    if (split) { cudaEventRecord(h->cmf_fac[i], st); cudaStreamWaitEvent(eq, h->cmf_fac[i], 0); }
+    svd_bond_vh(eq, Ml, d, Mr, s.Vh, sws);
+    env_update(eq, 1, Ml, Mr, d, h->Dw[i], h->Dw[i + 1], h->Renv[i], h->Wsp[i], s.Vh, h->Renv[i - 1], split ? h->cmf_env_ws : ws);
+    if (released) {
+      cudaEventRecord(h->cmf_rel[i - 1], eq);              // the mean fields of site i - 1 are ready
+      released(i - 1);
+    }
     if (i > 1) {                                           // centre form of site i-1, unfolded next
       const int j = i - 1;
       ZGemm g{};
@@ -295,6 +308,7 @@ int cmf_mean_fields(tdvp_handle *h, const std::vector<c128 *> &Y, const std::fun
       Cnext = (Cnext == s.C0) ? s.C1 : s.C0;
     }
   }
+  if (split && n >= 2) cudaStreamWaitEvent(st, h->cmf_rel[0], 0);   // the environment queue joins the chain again
   return check_cuda(h, cudaGetLastError(), "CMF mean fields");
 }
 
@@ -346,6 +360,23 @@ int cmf_queues(tdvp_handle *h) {
       zgemm_prepare_stream(h->cmf_hi);
     }
   }
+  {
+    // Vh of a bond and the R block built from it hang off the chain of unfoldings without being on it (the next
+    // unfolding needs U Lambda only): they run on a queue of their own, one bond behind the chain
+    static const bool split = [] { const char *e = getenv("TDVP_CMF_SPLIT_SVD"); return !(e && e[0] == '0'); }();
+    if (split) {
+      if (int rc = check_cuda(h, cudaStreamCreateWithFlags(&h->cmf_env, cudaStreamNonBlocking), "CMF environment queue")) return rc;
+      zgemm_prepare_stream(h->cmf_env);
+      if (int rc = check_cuda(h, cudaMalloc(&h->cmf_env_ws, h->step_ws_bytes), "cudaMalloc CMF workspace")) return rc;
+      for (int k = 0; k < 2; k++)
+        if (int rc = check_cuda(h, cudaMalloc(&h->cmf_svd_ws[k], h->step_ws_bytes), "cudaMalloc CMF workspace")) return rc;
+      for (int j = 0; j < h->n; j++) {
+        cudaEvent_t ev = nullptr;
+        if (int rc = check_cuda(h, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming), "event")) return rc;
+        h->cmf_fac.push_back(ev);
+      }
+    }
+  }
   for (int j = 0; j < h->n; j++) {                           // "mean fields of site j are ready"
     cudaEvent_t ev = nullptr;
     if (int rc = check_cuda(h, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming), "event")) return rc;
@@ -366,6 +397,11 @@ int cmf_queues(tdvp_handle *h) {
       if (spare > 0 && sms > 2 * spare) zgemm_set_stream_cap(st, 2 * (sms - spare));
     }
     h->cmf_streams.push_back(st); h->cmf_join.push_back(ev); h->cmf_ws.push_back(ws); h->cmf_scratch.push_back(sc);
+  }
+  if (h->cmf_env) {                                          // (the same grid cap as the side queues, for the same reason)
+    const char *e = getenv("TDVP_CMF_SPARE_SMS");
+    const int spare = e ? atoi(e) : 24, sms = zgemm_device_sms();
+    if (spare > 0 && sms > 2 * spare) zgemm_set_stream_cap(h->cmf_env, 2 * (sms - spare));
   }
   return TDVP_OK;
 }
@@ -407,7 +443,6 @@ int mu_rhs_pipelined(tdvp_handle *h, const std::vector<c128 *> &Y, const std::ve
   h->stream = mf;
   const int rc = cmf_mean_fields(h, Y, [&](int j) {
     const int q = j % nq;
-    cudaEventRecord(h->cmf_rel[j], mf);
     cudaStreamWaitEvent(h->cmf_streams[q], h->cmf_rel[j], 0);
     cmf_local_rhs(h, j, Y[j], K[j], mu_carve(h, h->cmf_scratch[q]), h->cmf_streams[q], h->cmf_ws[q]);
   });
@@ -451,8 +486,7 @@ int cmf_fields_and_propagate(tdvp_handle *h, const std::vector<c128 *> &Y, const
     cudaStream_t mf = h->cmf_hi ? h->cmf_hi : st;
     if (mf != st) { cudaEventRecord(h->cmf_fork, st); cudaStreamWaitEvent(mf, h->cmf_fork, 0); }
     h->stream = mf;
-    const int rc = cmf_mean_fields(h, Y, [&](int j) {
-      cudaEventRecord(h->cmf_rel[j], mf);                    // mean fields of site j are ready
+    const int rc = cmf_mean_fields(h, Y, [&](int j) {          // (cmf_rel[j] has been recorded: mean fields of site j are ready)
       cudaStreamWaitEvent(h->cmf_streams[j % nq], h->cmf_rel[j], 0);
       start_site(j);
     });

@@ -514,33 +514,49 @@ void svd_configure() {
 
 }
 
+namespace {
+struct SvdWs { c128 *Q, *D, *Xt, *Jt, *Qp, *Dp, *JtP, *Js; double *cnorm; int *flags; void *qws1, *qws2; };
+SvdWs svd_carve(int Ml, int d, int Mr, void *ws) {
+  const size_t n = Ml, nn = up256(n * n * 16);
+  char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
+  SvdWs w;
+  w.Q = reinterpret_cast<c128 *>(p); p += up256((size_t)Ml * d * Mr * 16);
+  w.D = reinterpret_cast<c128 *>(p); p += nn;
+  w.Xt = reinterpret_cast<c128 *>(p); p += nn;
+  w.Jt = reinterpret_cast<c128 *>(p); p += nn;
+  w.Qp = reinterpret_cast<c128 *>(p); p += nn;
+  w.Dp = reinterpret_cast<c128 *>(p); p += nn;
+  w.JtP = reinterpret_cast<c128 *>(p); p += nn;
+  w.Js = reinterpret_cast<c128 *>(p); p += nn;              // J with its columns in the sorted order (X sorted goes into D's buffer)
+  w.cnorm = reinterpret_cast<double *>(p); p += up256(n * 8);
+  w.flags = reinterpret_cast<int *>(p); p += 512;           // see FLAG_*
+  w.qws1 = p; p += up256(qr_ws_bytes(d * Mr, Ml));          // the RQ of C: its reflectors must survive until svd_bond_vh forms Q
+  w.qws2 = p;                                               // the (gated) Householder step on the rotated matrix
+  return w;
+}
+}  // namespace
+
 size_t svd_ws_bytes(int Ml, int d, int Mr) {
   const size_t n = Ml, nn = up256(n * n * 16);
   size_t q1 = qr_ws_bytes(d * Mr, Ml), q2 = qr_ws_bytes(Ml, Ml);
-  return up256((size_t)Ml * d * Mr * 16) + 7 * nn + 512 + up256(n * 8) + up256(q1 > q2 ? q1 : q2) + 1024;
+  return up256((size_t)Ml * d * Mr * 16) + 7 * nn + 512 + up256(n * 8) + up256(q1) + up256(q2) + 1024;
 }
 
-// C [Ml, d, Mr] -> U [Ml, Ml], lam [Ml], Vh [Ml, d, Mr]
-void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, double *lam, c128 *Vh, void *ws, int *status) {
+// The unfolding in two halves on one workspace.  svd_bond_factor: everything the NEXT bond of a chain of unfoldings
+// needs (U, lam) -- the R factor of C = D Q without forming Q, the Jacobi iteration, U.  svd_bond_vh: Q and
+// Vh = (J permuted)^H Q, which only the bond's own consumers need; it may run later and on another queue, as long as the
+// workspace is left alone in between (step_mu.cu runs it beside the next bond's factor phase).
+void svd_bond_factor(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, double *lam, void *ws, int *status) {
   ProfScope ps(st, PH_SVD);
   // sweeps allowed (diagnostic switch TDVP_SVD_MAX_SWEEPS, read at every call: the error-path test lowers it)
   int max_sweeps = MAX_SWEEPS;
   if (const char *e = getenv("TDVP_SVD_MAX_SWEEPS")) { const int v = atoi(e); if (v >= 1 && v <= MAX_SWEEPS) max_sweeps = v; }
   const int n = Ml;
-  const size_t nn = up256((size_t)n * n * 16);
-  char *p = reinterpret_cast<char *>(up256(reinterpret_cast<size_t>(ws)));
-  c128 *Q = reinterpret_cast<c128 *>(p); p += up256((size_t)Ml * d * Mr * 16);
-  c128 *D = reinterpret_cast<c128 *>(p); p += nn;
-  c128 *Xt = reinterpret_cast<c128 *>(p); p += nn;
-  c128 *Jt = reinterpret_cast<c128 *>(p); p += nn;
-  c128 *Qp = reinterpret_cast<c128 *>(p); p += nn;
-  c128 *Dp = reinterpret_cast<c128 *>(p); p += nn;
-  c128 *JtP = reinterpret_cast<c128 *>(p); p += nn;
-  c128 *Js = reinterpret_cast<c128 *>(p); p += nn;              // J with its columns in the sorted order (X sorted goes into D's buffer)
-  double *cnorm = reinterpret_cast<double *>(p); p += up256((size_t)n * 8);
-  int *flags = reinterpret_cast<int *>(p); p += 512;        // [0, 40): a sweep rotated; [64, 104): ... a pair far from orthogonal
-  void *qws = p;
-  qr_gauge(st, 1, Ml, d, Mr, C, Q, D, qws);                               // C = D Q
+  const SvdWs w = svd_carve(Ml, d, Mr, ws);
+  c128 *D = w.D, *Xt = w.Xt, *Jt = w.Jt, *Qp = w.Qp, *Dp = w.Dp, *JtP = w.JtP, *Js = w.Js;
+  double *cnorm = w.cnorm;
+  int *flags = w.flags;
+  qr_factor(st, 1, Ml, d, Mr, C, D, w.qws1);                              // C = D Q (Q formed later)
   const int g = (n * n + 255) / 256 > 296 ? 296 : (n * n + 255) / 256;
   TDVP_LAUNCH(svd_init_kernel, g, 256, 0, st, D, Xt, Jt, n);
   cudaMemsetAsync(flags, 0, 128 * sizeof(int), st);
@@ -556,11 +572,24 @@ void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, do
   // TDVP_SVD_ALWAYS_QR=1: the Householder step runs whatever the columns look like (diagnostic switch)
   static const int always_qr = [] { const char *e = getenv("TDVP_SVD_ALWAYS_QR"); return (e && e[0] == '1') ? 1 : 0; }();
   TDVP_LAUNCH(svd_sortcols_kernel, n, 128, 0, st, Xt, Jt, cnorm, n, Xs, Js, flags, always_qr);
-  qr_gauge(st, 1, n, 1, n, Xs, Qp, Dp, qws, flags + FLAG_NEED_QR);
+  qr_gauge(st, 1, n, 1, n, Xs, Qp, Dp, w.qws2, flags + FLAG_NEED_QR);
   TDVP_LAUNCH(svd_finish_kernel, n < 148 ? n : 148, 128, n * sizeof(double), st, Qp, Dp, Js, n, U, lam, JtP, Xs, cnorm, flags);
+}
+
+void svd_bond_vh(cudaStream_t st, int Ml, int d, int Mr, c128 *Vh, void *ws) {
+  ProfScope ps(st, PH_SVD);
+  const int n = Ml;
+  const SvdWs w = svd_carve(Ml, d, Mr, ws);
+  qr_form_q(st, 1, Ml, d, Mr, w.Q, w.qws1);
   ZGemm gm{};                                   // Vh[k][:] = sum_j conj(JtP[k][j]) Q[j][:]
-  gm.A = JtP; gm.B = Q; gm.C = Vh;
+  gm.A = w.JtP; gm.B = w.Q; gm.C = Vh;
   gm.M = n; gm.K = n; gm.N = d * Mr;
   gm.a_ms = n; gm.a_ks = 1; gm.conjA = 1; gm.b_ks = gm.N; gm.b_ns = 1; gm.ldc = gm.N;
   zgemm(st, gm);
+}
+
+// C [Ml, d, Mr] -> U [Ml, Ml], lam [Ml], Vh [Ml, d, Mr]
+void svd_bond(cudaStream_t st, int Ml, int d, int Mr, const c128 *C, c128 *U, double *lam, c128 *Vh, void *ws, int *status) {
+  svd_bond_factor(st, Ml, d, Mr, C, U, lam, ws, status);
+  svd_bond_vh(st, Ml, d, Mr, Vh, ws);
 }
