@@ -335,3 +335,56 @@ def test_pc_rk4_step_on_the_fmo_chain(T):
     for A in got[1:]:
         m = A.reshape(A.shape[0], -1)
         assert np.abs(m @ m.conj().T - np.eye(A.shape[0])).max() < 1e-12
+
+
+# ---- the schedules of TDVP-MU and the two QR / SVD paths compute the same thing ---------------------------------------
+_SCHEDULE_SNIPPET = r"""
+import dataclasses, json, sys
+import numpy as np
+import synthetic_inputs as si
+import paper_1907_12044_b200 as T
+cfg = dataclasses.replace(si.CONFIGS["fmo64"], n_el=4, n_modes=2, n_ph=6, M=12, dt_fs=5.0)
+params = si.draw_vibronic_params(cfg)
+mpo = T.tdvp_build_vibronic_mpo(params.E, params.J, params.omega, params.S, params.n_ph, params.layout)
+mps = si.padded_product_mps(si.site_dims(params), si.initial_occupations(params), cfg.M, cfg.pad_seed, cfg.delta, cfg.delta_seed)
+ch = T.tdvp_create(mpo, mps, T.make_options(krylov_dim=cfg.krylov_dim))
+for _ in range(4):
+    ch.tdvp_step_ps(cfg.dt_fs)
+out = {"ps": ch.tdvp_populations(0).tolist()}
+ch.tdvp_step_mu_cmf(0.05, 10)
+out["cmf"] = ch.tdvp_populations(0).tolist()
+out["err"] = ch.tdvp_step_mu(0.002, want_err=True)
+out["mu"] = ch.tdvp_populations(0).tolist()
+out["norm_energy"] = list(ch.tdvp_norm_energy())
+ch.close()
+print("RESULT " + json.dumps(out))
+"""
+
+
+def _run_schedule(env_extra):
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ)
+    env.update(env_extra)
+    r = subprocess.run([sys.executable, "-c", _SCHEDULE_SNIPPET], cwd=root, env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    line = [l for l in r.stdout.splitlines() if l.startswith("RESULT ")][-1]
+    return json.loads(line[len("RESULT "):])
+
+
+def test_mu_schedules_and_factorisation_paths_agree(T):
+    """The switches of include/tdvp.h are read once per process, so each variant runs in a process of its own: the
+    pipelined TDVP-MU schedules (side queues, split unfolding chain, capped GEMM grids) against the sequential order, and
+    the fast QR panel / gated Householder step against the exact paths -- PS warm-up, one CMF step, one Dormand-Prince
+    step on a short FMO-like chain; everything agrees to round-off (different summation orders only)."""
+    ref = _run_schedule({})
+    variants = [{"TDVP_CMF_PIPELINE": "0", "TDVP_MU_PIPELINE": "0"}, {"TDVP_CMF_SPLIT_SVD": "0"},
+                {"TDVP_QR_FAST": "0", "TDVP_SVD_ALWAYS_QR": "1"}]
+    for env in variants:
+        got = _run_schedule(env)
+        for key in ("ps", "cmf", "mu"):
+            assert np.abs(np.array(got[key]) - np.array(ref[key])).max() <= 1e-9, (env, key)
+        assert abs(got["err"] - ref["err"]) <= 1e-6 * abs(ref["err"]) + 1e-14, env
+        assert np.abs(np.array(got["norm_energy"]) - np.array(ref["norm_energy"])).max() <= 1e-9, env
