@@ -335,6 +335,8 @@ long long tdvp_launch_count(void);
                               iteration left columns alone or ran out of sweeps; decided on the device), read once;
      TDVP_QR_CLUSTER=0        QR gauge moves of up to 1280 rows with one launch per panel and per trailing update
                               instead of the single 16-CTA cluster kernel, read once;
+     TDVP_QR_FAST=0           that kernel eliminates every panel column by column, one cluster reduction per column
+                              (default: one reduction per panel where its columns are well enough conditioned), read once;
      TDVP_SVD_MAX_SWEEPS=n    Jacobi sweeps a bond SVD may use (1..40, default 40; lowering it forces the
                               TDVP_ESTATE "did not converge" report: used by the error-path test), read at
                               every SVD. */
