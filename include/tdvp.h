@@ -321,7 +321,7 @@ long long tdvp_launch_count(void);
                               Lanczos iteration, read once;
      TDVP_NO_FSAL=1           tdvp_step_mu recomputes stage 1 instead of reusing stage 7 of the step
                               before (bit-identical by construction; read at every step);
-     TDVP_CMF_QUEUES=n        side queues of the local problems of TDVP-MU (1..8, default 4), read when a handle
+     TDVP_CMF_QUEUES=n        side queues of the local problems of TDVP-MU (1..16, default 6), read when a handle
                               first runs tdvp_step_mu / tdvp_step_mu_cmf / tdvp_mu_derivative;
      TDVP_CMF_PIPELINE=0      CMF step: build all mean fields first, then propagate all sites (default: site j starts
                               on its side queue as soon as the bond to its right is unfolded), read once;
@@ -331,6 +331,8 @@ long long tdvp_launch_count(void);
                               (default: on a queue of their own, one bond behind the chain), read once;
      TDVP_CMF_SPARE_SMS=n     SMs the GEMMs of the side queues leave out of their grids, for the cluster kernels of
                               the unfolding chain that run beside them (default 24; 0 = none), read once;
+     TDVP_CMF_QUEUE_CTAS=n    CTAs a GEMM of one of those side queues may use (default: half the SM count, a quarter of
+                              the device's CTA slots; 0 = only the TDVP_CMF_SPARE_SMS limit), read once;
      TDVP_SVD_ALWAYS_QR=1     a bond SVD always runs its final Householder step (default: only when the Jacobi
                               iteration left columns alone or ran out of sweeps; decided on the device), read once;
      TDVP_QR_CLUSTER=0        QR gauge moves of up to 1280 rows with one launch per panel and per trailing update
